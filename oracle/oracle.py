@@ -1,0 +1,278 @@
+"""Python face of the fp64 CPU oracle (oracle/cc_oracle.c) -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this.  Nothing here imports or is imported by paper_1409_2065_b200 (the CUDA path).
+
+Everything is fp64.  Each function cites the PAPER.md passage (or DESIGN.md reading Sx) it follows.
+The numpy parts are plain definitions (weights eq. 8, default constants, objective eq. 1/6).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "cc_oracle.c")
+_LIB = os.path.join(_HERE, "libcc_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile cc_oracle.c with gcc (-O2, OpenMP).  Building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"])
+    return _LIB
+
+
+def _L():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB)
+        i64, i32, dbl, vp = ctypes.c_int64, ctypes.c_int, ctypes.c_double, ctypes.c_void_p
+        L.orc_num_threads.restype = i32
+        L.orc_set_threads.argtypes = [i32]
+        L.orc_row_dist2.argtypes = [i64, i64, vp, vp, i64, vp]
+        L.orc_knn.argtypes = [i64, i64, vp, vp, i32, i64, vp, vp, vp]
+        L.orc_knn.restype = i32
+        L.orc_project.argtypes = [i64, i64, i64, vp, vp, vp, vp, i32, dbl, i64, vp]
+        L.orc_project.restype = i64
+        L.orc_mm.argtypes = [i64, i64, vp, vp, i64, vp, vp, vp, dbl, dbl, dbl, i32, dbl, i32, i32, dbl, i64,
+                             vp, vp, vp, vp, vp, vp]
+        L.orc_mm.restype = i32
+        L.orc_labels.argtypes = [i64, i64, i64, vp, vp, vp, vp]
+        L.orc_labels.restype = i64
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def num_threads() -> int:
+    return int(_L().orc_num_threads())
+
+
+def set_threads(t: int) -> None:
+    _L().orc_set_threads(int(t))
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _u8(a):
+    return None if a is None else np.ascontiguousarray(a, dtype=np.uint8)
+
+
+# ----------------------------------------------------------------------------- weights (a0)
+def row_dist2(X, mask, i: int) -> np.ndarray:
+    """Squared distances from row i to all rows (masked rule: reading S11)."""
+    X = _f64(X)
+    mask = _u8(mask)
+    n, p = X.shape
+    out = np.empty(n)
+    _L().orc_row_dist2(n, p, _p(X), _p(mask), int(i), _p(out))
+    return out
+
+
+def knn(X, mask, k: int, rows=None):
+    """k nearest neighbours by brute force (S9: self excluded, ties -> smaller index)."""
+    X = _f64(X)
+    mask = _u8(mask)
+    n, p = X.shape
+    rows_a = None if rows is None else np.ascontiguousarray(rows, dtype=np.int64)
+    nr = n if rows_a is None else rows_a.size
+    nbr = np.empty((nr, k), dtype=np.int32)
+    d2 = np.empty((nr, k))
+    rc = _L().orc_knn(n, p, _p(X), _p(mask), int(k), nr, _p(rows_a), _p(nbr), _p(d2))
+    if rc:
+        raise ValueError("orc_knn: need 1 <= k <= n-1")
+    return nbr, d2
+
+
+def pair_dist2(X, mask, i, j) -> np.ndarray:
+    """Squared distances of the listed pairs, same rule as the C code (plain definition in numpy)."""
+    X = _f64(X)
+    out = np.empty(len(i))
+    step = max(1, (1 << 22) // max(1, X.shape[1]))
+    for s in range(0, len(i), step):
+        ii, jj = i[s:s + step], j[s:s + step]
+        df = X[ii] - X[jj]
+        if mask is None:
+            out[s:s + step] = np.einsum("ij,ij->i", df, df)
+        else:
+            co = (mask[ii] != 0) & (mask[jj] != 0)
+            cnt = co.sum(axis=1)
+            ss = np.einsum("ij,ij->i", df * co, df * co)
+            with np.errstate(divide="ignore", invalid="ignore"):
+                out[s:s + step] = np.where(cnt > 0, ss * X.shape[1] / np.maximum(cnt, 1), np.inf)
+    return out
+
+
+def knn_graph(X, mask, k: int, phi: float, normalize: bool = False):
+    """Weights of eq. 8: i~j iff j among the k nearest of i OR vice versa;
+    w_ij = exp(-phi d_ij^2); optional normalisation to sum 1 over pairs i<j (S8).
+    Returns (ei, ej, w, d2) with ei<ej, sorted by (ei, ej)."""
+    n = X.shape[0]
+    nbr, d2 = knn(X, mask, k)
+    i = np.repeat(np.arange(n, dtype=np.int64), k)
+    j = nbr.reshape(-1).astype(np.int64)
+    lo, hi = np.minimum(i, j), np.maximum(i, j)
+    key = lo * n + hi
+    key_u, first = np.unique(key, return_index=True)
+    ei = (key_u // n).astype(np.int32)
+    ej = (key_u % n).astype(np.int32)
+    dd = d2.reshape(-1)[first]
+    w = np.exp(-phi * dd)
+    if normalize:
+        w = w / w.sum()
+    return ei, ej, w, dd
+
+
+def complete_graph(X, mask, phi: float, normalize: bool = False):
+    """All pairs i<j with Gaussian weights (eq. 8 with k = n-1)."""
+    n = X.shape[0]
+    ei, ej = np.triu_indices(n, k=1)
+    dd = pair_dist2(X, mask, ei, ej)
+    w = np.exp(-phi * dd)
+    if normalize:
+        w = w / w.sum()
+    return ei.astype(np.int32), ej.astype(np.int32), w, dd
+
+
+def to_csr(n: int, ei, ej, w):
+    """Symmetric CSR (both directions) of the pair list: rowptr int64, col int32 (sorted), w."""
+    r = np.concatenate([ei, ej]).astype(np.int64)
+    c = np.concatenate([ej, ei]).astype(np.int64)
+    ww = np.concatenate([w, w])
+    order = np.lexsort((c, r))
+    r, c, ww = r[order], c[order], ww[order]
+    rowptr = np.zeros(n + 1, dtype=np.int64)
+    np.add.at(rowptr, r + 1, 1)
+    rowptr = np.cumsum(rowptr)
+    return rowptr, c.astype(np.int32), ww
+
+
+# ----------------------------------------------------------------------------- constants
+def column_means(X, mask):
+    """Observed column means (used by the cold start S4 and by G_bound S1)."""
+    X = _f64(X)
+    if mask is None:
+        return X.mean(axis=0)
+    mk = mask != 0
+    cnt = mk.sum(axis=0)
+    return (X * mk).sum(axis=0) / np.maximum(cnt, 1)
+
+
+def g_bound(X, mask, w, gamma: float) -> float:
+    """[reading S1] G_bound(gamma) = sqrt(sum_Gamma (x - xbar_j)^2 + gamma^2 sum_E w^2)."""
+    X = _f64(X)
+    xc = X - column_means(X, mask)[None, :]
+    if mask is not None:
+        xc = xc * (mask != 0)
+    return float(np.sqrt((xc * xc).sum() + gamma * gamma * float((np.asarray(w, dtype=np.float64) ** 2).sum())))
+
+
+def default_rho_eps(X, mask, w, gamma: float, rho_scale: float = 1.1, kappa: float = 1e-2):
+    """[readings S1, S2] rho = rho_scale * G_bound(gamma), eps = (kappa rho)^2."""
+    rho = rho_scale * g_bound(X, mask, w, gamma)
+    return rho, (kappa * rho) ** 2
+
+
+def cold_start(X, mask, ei, ej):
+    """[reading S4] U0 = X with missing entries set to the observed column mean; V0 = D U0."""
+    U = _f64(X).copy()
+    if mask is not None:
+        cm = column_means(X, mask)
+        miss = mask == 0
+        U[miss] = np.broadcast_to(cm, U.shape)[miss]
+    V = U[ei] - U[ej]
+    return U, np.ascontiguousarray(V)
+
+
+# ----------------------------------------------------------------------------- MM iteration
+def project(U, V, ei, ej, method: int = 0, tol: float = 1e-13, maxcycles: int = 100000):
+    """Projection of (U~,V~) onto C.  Returns (A, cycles); B = A[ei]-A[ej]."""
+    U = _f64(U)
+    V = _f64(V)
+    ei = np.ascontiguousarray(ei, dtype=np.int32)
+    ej = np.ascontiguousarray(ej, dtype=np.int32)
+    n, p = U.shape
+    A = np.empty_like(U)
+    cyc = _L().orc_project(n, p, ei.size, _p(ei), _p(ej), _p(U), _p(V), int(method), float(tol),
+                           int(maxcycles), _p(A))
+    if cyc < 0:
+        raise RuntimeError(f"oracle projection failed to converge (code {cyc})")
+    return A, int(cyc)
+
+
+def mm(X, mask, ei, ej, w, gamma, rho, eps, U, V, maxit, tol=0.0, min_it=10, proj_method=0,
+       proj_tol=1e-13, proj_maxcycles=100000):
+    """Run the MM iteration from state (U,V); returns a dict with the new
+    state, the Phi_m / d_m sequences and the iteration count.  Fails loudly on non-convergence of the
+    projection or on an increase of Phi (MM descent property)."""
+    X = _f64(X)
+    mask = _u8(mask)
+    ei = np.ascontiguousarray(ei, dtype=np.int32)
+    ej = np.ascontiguousarray(ej, dtype=np.int32)
+    w = _f64(w)
+    n, p = X.shape
+    U = _f64(U).copy()
+    V = _f64(V).copy()
+    phi_h = np.zeros(max(1, maxit))
+    d_h = np.zeros(max(1, maxit))
+    it = ctypes.c_int(0)
+    cyc = ctypes.c_int64(0)
+    rc = _L().orc_mm(n, p, _p(X), _p(mask), ei.size, _p(ei), _p(ej), _p(w), float(gamma), float(rho),
+                     float(eps), int(maxit), float(tol), int(min_it), int(proj_method), float(proj_tol),
+                     int(proj_maxcycles), _p(U), _p(V), _p(phi_h), _p(d_h), ctypes.byref(it),
+                     ctypes.byref(cyc))
+    if rc:
+        raise RuntimeError({-1: "projection did not converge", -2: "out of memory",
+                            -3: "Phi increased: MM descent property violated"}.get(rc, str(rc)))
+    k = it.value
+    return {"U": U, "V": V, "phi": phi_h[:k].copy(), "d": d_h[:k].copy(), "iters": k,
+            "proj_cycles": int(cyc.value)}
+
+
+def labels(V, ei, ej, n: int):
+    """[reading S16] components over pairs with v_ij == 0 exactly, canonical numbering."""
+    V = _f64(V)
+    ei = np.ascontiguousarray(ei, dtype=np.int32)
+    ej = np.ascontiguousarray(ej, dtype=np.int32)
+    lab = np.empty(n, dtype=np.int32)
+    k = _L().orc_labels(n, V.shape[1], ei.size, _p(ei), _p(ej), _p(V), _p(lab))
+    return lab, int(k)
+
+
+def objective(X, mask, ei, ej, w, gamma, U) -> float:
+    """f_gamma(U) of eq. 1 / eq. 6."""
+    X = _f64(X)
+    U = _f64(U)
+    r = X - U
+    if mask is not None:
+        r = r * (mask != 0)
+    df = U[ei] - U[ej]
+    return float(0.5 * (r * r).sum() + gamma * (np.asarray(w) * np.sqrt(np.einsum("ij,ij->i", df, df))).sum())
+
+
+def path(X, mask, ei, ej, w, gammas, maxit, tol=0.0, min_it=10, rho_scale=1.1, kappa=1e-2, proj_method=0,
+         proj_tol=1e-13):
+    """gamma path with warm starts (warm start: reading S4).  rho, eps per gamma by
+    S1/S2.  Returns a list of per-gamma dicts (U, labels, nclusters, iters, phi, d, rho, eps)."""
+    U, V = cold_start(X, mask, ei, ej)
+    out = []
+    n = X.shape[0]
+    for g in gammas:
+        rho, eps = default_rho_eps(X, mask, w, g, rho_scale, kappa)
+        r = mm(X, mask, ei, ej, w, g, rho, eps, U, V, maxit, tol, min_it, proj_method, proj_tol)
+        U, V = r["U"], r["V"]
+        lab, k = labels(V, ei, ej, n)
+        r.update(labels=lab, nclusters=k, rho=rho, eps=eps, gamma=float(g))
+        out.append(r)
+    return out

@@ -1,0 +1,156 @@
+/*
+ * cc_b200.h -- C ABI of libcc_b200.so: the data-parallel hot path of the proximal distance (MM)
+ * algorithm for convex clustering (Chen, Chi, Ranola, Lange, arXiv 1409.2065; cited below as
+ * PAPER.md:L<line>), hand-written CUDA for NVIDIA B200 (sm_100a).
+ *
+ * Problem (eq. 1; missing data L107-L110 eq. 6):
+ *     minimise_U  1/2 sum_{(i,c) observed} (x_ic - u_ic)^2  +  gamma sum_{(i,j) in E} w_ij ||u_i - u_j||_2
+ * The paper writes the penalty constant as mu; this library (like BASELINE.json) calls it gamma.
+ *
+ * Conventions
+ *   - X, U are n x p row-major fp32 (one contiguous row per case -- the same memory as the paper's
+ *     column-per-case p x n matrix, L38).  mask is n x p uint8, 1 = observed (the set Gamma, L107).
+ *   - The graph is a SYMMETRIC CSR over the n cases: both (i,j) and (j,i) are stored, no self
+ *     loops, w_ij = w_ji > 0 (L90, L125; zero-weight pairs are simply absent, L40).  rowptr is
+ *     int64[n+1], col is int32[nnz] sorted increasingly inside a row, w is fp32[nnz].
+ *   - Every array argument says HOST or DEVICE.  DEVICE pointers must belong to the current CUDA
+ *     device.  The caller owns every pointer it passes; cc_create copies what it needs into
+ *     library-owned device buffers, so inputs may be freed after it returns.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All device work
+ *     of a handle is enqueued on the stream given to cc_create.  Calls that return scalars to the
+ *     host synchronise that stream; cc_get_U / cc_clusters with DEVICE outputs do not.
+ *   - Return value: CC_OK (0) or a negative CC_E* code; cc_last_error() gives a message.  The library
+ *     never aborts, throws or prints.  There is no CPU fallback: without a CUDA device every compute
+ *     entry point fails with CC_ECUDA.
+ *   - Determinism: no floating-point atomics anywhere; all reductions run in a fixed order, so the
+ *     same inputs give bit-identical outputs on the same GPU model.
+ */
+#ifndef CC_B200_H
+#define CC_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CC_OK 0
+#define CC_EINVAL (-1) /* bad size / NULL pointer / negative gamma / NaN or Inf in observed X or in w  */
+#define CC_EGRAPH (-2) /* CSR not symmetric, w_ij != w_ji, self loop, w <= 0, col out of range/unsorted */
+#define CC_EMASK (-3)  /* a column has no observed entry at all (its fused value is undetermined)       */
+#define CC_ENOMEM (-4) /* host or device allocation failed                                              */
+#define CC_ECUDA (-5)  /* CUDA runtime error (message in cc_last_error)                                 */
+#define CC_ESTATE (-6) /* bad gamma_index, or the call needs state that does not exist yet              */
+#define CC_ENOCONV (-7)/* the inner projection solve hit proj_maxit (state is still consistent)         */
+
+typedef struct cc_handle cc_handle; /* opaque; owns all device buffers */
+
+/* Constants the paper leaves open ("rho large enough", L57 "epsilon > 0 small"; no
+ * stopping rule anywhere in L57-L103).  DESIGN.md readings S1-S5 define them; oracle and GPU take
+ * the same numbers. */
+typedef struct {
+    double rho_scale; /* S1: rho = rho_scale * sqrt(sum_obs (x - colmean)^2 + gamma^2 sum_E w^2); used when rho_abs <= 0 */
+    double rho_abs;   /*     > 0: use this rho for every gamma                                           */
+    double kappa;     /* S2: eps = (kappa * rho)^2; used when eps_abs <= 0                               */
+    double eps_abs;   /*     > 0: use this eps for every gamma                                           */
+    double proj_tol;  /* S5: the projection's linear solve (I+L) A = R stops when its
+                             residual r has sqrt(r' D^-1 r) <= proj_tol * (d_prev / rho) * sqrt(sum_obs (x-colmean)^2),
+                             D = diag(1 + |N_i|).  Default 1e-5.      */
+    int32_t proj_maxit; /*   cap on inner iterations per MM iteration (default 500); hitting it => CC_ENOCONV */
+    int32_t min_it;   /* S3: never stop before this many MM iterations (default 10)                      */
+    int32_t dense;    /* 0: graph given as CSR.  1: complete graph; `w` is an n x n row-major symmetric
+                             fp32 matrix (diagonal ignored, off-diagonal > 0), rowptr/col ignored        */
+    int32_t use_graph;/* 1 (default): one CUDA-graph launch per solve with device-side WHILE loops;
+                         0: plain stream launches with a host loop (debugging)                           */
+    int32_t hist_cap; /* capacity of the per-solve Phi_m / d_m history kept on the device (default 4096;
+                         iterations beyond it are not recorded)                                          */
+    int32_t max_snapshots; /* how many per-gamma snapshots of U cc_path may keep (default 64)            */
+    int32_t reserved0;
+} cc_params;
+
+/* Fill *prm with the defaults above.  HOST pointer. */
+int cc_default_params(cc_params* prm);
+
+/* ---- a0: one-time k-NN + Gaussian weights, PAPER.md L127-L133 (eq. 8) -------------------------------
+ * w_ij = 1{i ~_k j} exp(-phi ||x_i - x_j||^2), i ~_k j iff j is among the k nearest of i OR vice versa
+ * (L127); self excluded, ties to the smaller index (S9).  With a mask, the squared distance is taken
+ * over co-observed coordinates and scaled by p / #co-observed (S11).  normalize != 0 divides the
+ * weights by their sum over pairs i<j (L133, S8).
+ * X (DEVICE, n*p fp32), mask (DEVICE n*p uint8 or NULL).  Outputs: *rowptr (int64[n+1]), *col
+ * (int32[nnz]), *w (fp32[nnz]) are DEVICE arrays allocated by the library (cudaMalloc) and owned by
+ * the caller, to be released with cc_free_graph; *nnz (HOST) receives the directed entry count.
+ * Needs 1 <= k <= n-1.  Synchronises `stream`. */
+int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t k, float phi,
+                   int32_t normalize, int64_t** rowptr, int32_t** col, float** w, int64_t* nnz,
+                   void* stream);
+
+/* Release the three arrays cc_knn_weights returned (NULLs are ignored). */
+void cc_free_graph(int64_t* rowptr, int32_t* col, float* w);
+
+/* ---- problem set-up --------------------------------------------------------------------------------
+ * Validates the inputs once (error codes above), copies them, builds the internal layout and sets the
+ * cold start (S4): U0 = X with missing entries set to the observed column mean, V0 = D U0.
+ * X, mask, rowptr, col, w: DEVICE pointers (mask may be NULL = all observed; with prm->dense = 1,
+ * rowptr and col are ignored and w is the n x n matrix).  prm: HOST pointer or NULL for defaults.
+ * *out (HOST) receives the handle. */
+int cc_create(cc_handle** out, int64_t n, int64_t p, const float* X, const uint8_t* mask,
+              const int64_t* rowptr, const int32_t* col, const float* w, const cc_params* prm,
+              void* stream);
+
+/* ---- a1-a6: the MM iteration, PAPER.md L57-L103, L116 ---------------------------------------------
+ * Runs MM iterations at this gamma, warm-started from the handle's current state (after cc_create or
+ * cc_reset: the cold start).  Each iteration: projection onto C (L90-L103), d_m (L76), U update (L82,
+ * L116), block soft-threshold (L86-L88).  Stops after an iteration m with m+1 >= min_it, m >= 1 and
+ * Phi_{m-1} - Phi_m <= tol (1 + |Phi_{m-1}|) (S3), or after maxit iterations; tol = 0 runs exactly
+ * maxit iterations.  Phi_m = 1/2 sum_obs (x-u_m)^2 + gamma sum_E w ||v_m|| + rho d_m (L64-L66, L109).
+ * iters_out, phi_out (HOST, may be NULL): iterations done and the last recorded Phi.  Synchronises. */
+int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* iters_out,
+             double* phi_out);
+
+/* ---- a7: gamma path, PAPER.md L144 (U stays on the device between gammas, cf. L202) ---------------
+ * For each gamma in the caller's order: cc_solve warm-started from the previous gamma, then a device
+ * snapshot of U and of the cluster labels.  gammas, iters_out[ngamma], phi_out[ngamma]: HOST (outputs
+ * may be NULL).  ngamma must be <= max_snapshots.  Snapshots of an earlier path are dropped. */
+int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int32_t maxit,
+            int32_t* iters_out, double* phi_out);
+
+/* Copy U (n*p fp32 row-major) into a caller-owned buffer.  gamma_index = -1: the current state;
+ * 0..ngamma-1: the snapshot cc_path took.  U_out is DEVICE when out_on_device != 0, else HOST. */
+int cc_get_U(cc_handle* h, int32_t gamma_index, float* U_out, int32_t out_on_device);
+
+/* ---- a8: cluster read-out (S16; the paper never defines it, L154, L206) ---------------------------
+ * Connected components of the graph whose edges are the pairs with v_ij = 0 exactly, numbered in
+ * increasing order of each component's smallest member.  labels_out: int32[n], DEVICE when
+ * out_on_device != 0 else HOST; nclusters (HOST, may be NULL).  gamma_index as in cc_get_U.
+ * Synchronises. */
+int cc_clusters(cc_handle* h, int32_t gamma_index, int32_t* labels_out, int32_t out_on_device,
+                int32_t* nclusters);
+
+/* Phi_m and d_m of the last cc_solve (or of the last gamma of cc_path), up to `cap` entries each, into
+ * HOST arrays (either may be NULL); *count (HOST) = entries written. */
+int cc_get_history(cc_handle* h, double* phi_out, double* d_out, int32_t cap, int32_t* count);
+
+/* Diagnostics of the last cc_solve (HOST outputs, any may be NULL): rho and eps used, total inner
+ * (projection) iterations, f_gamma(U) of eq. 1/6 at the current U (L35, L109; costs one extra pair
+ * sweep), and the smallest relative margin | ||b_ij|| - thr_ij | / thr_ij over pairs at the last
+ * shrink (how close any pair was to flipping its fused/unfused decision). */
+int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, double* f_gamma,
+                 double* min_margin);
+
+/* Back to the cold start (S4); snapshots are dropped. */
+int cc_reset(cc_handle* h);
+
+/* Counts (HOST outputs, any may be NULL): undirected pairs |E|, directed entries nnz, and the number
+ * of kernel launches this handle has issued so far (graph kernel nodes executed are counted). */
+int cc_get_counts(cc_handle* h, int64_t* n_pairs, int64_t* nnz, int64_t* launches);
+
+/* Message of the last failing call on this handle (h = NULL: of the last failing cc_create /
+ * cc_knn_weights on this thread).  Never NULL. */
+const char* cc_last_error(const cc_handle* h);
+
+void cc_destroy(cc_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CC_B200_H */

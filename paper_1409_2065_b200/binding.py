@@ -1,0 +1,180 @@
+"""Thin Python binding of libcc_b200.so (include/cc_b200.h): argument marshalling only.
+
+Every function has the name and argument order of its C entry point; tensors are passed as
+`data_ptr()`s.  PyTorch is used for device memory and streams, nothing else.  There is no CPU
+fallback: importing this module fails loudly when the library has not been built
+(`python -m paper_1409_2065_b200.build`), and every compute call fails with CC_ECUDA without a GPU.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcc_b200.so")
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1409_2065_b200.build` "
+                      "(there is no CPU fallback)")
+_lib = ctypes.CDLL(LIB_PATH)
+
+CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
+
+SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
+           "cc_get_U", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_reset", "cc_get_counts",
+           "cc_last_error", "cc_destroy")
+
+
+class cc_params(ctypes.Structure):
+    _fields_ = [("rho_scale", ctypes.c_double), ("rho_abs", ctypes.c_double), ("kappa", ctypes.c_double),
+                ("eps_abs", ctypes.c_double), ("proj_tol", ctypes.c_double), ("proj_maxit", ctypes.c_int32),
+                ("min_it", ctypes.c_int32), ("dense", ctypes.c_int32), ("use_graph", ctypes.c_int32),
+                ("hist_cap", ctypes.c_int32), ("max_snapshots", ctypes.c_int32), ("reserved0", ctypes.c_int32)]
+
+
+_vp, _i64, _i32, _dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double
+_P = ctypes.POINTER
+_lib.cc_default_params.argtypes = [_P(cc_params)]
+_lib.cc_knn_weights.argtypes = [_i64, _i64, _vp, _vp, _i32, ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp),
+                                _P(_i64), _vp]
+_lib.cc_free_graph.argtypes = [_vp, _vp, _vp]
+_lib.cc_free_graph.restype = None
+_lib.cc_create.argtypes = [_P(_vp), _i64, _i64, _vp, _vp, _vp, _vp, _vp, _P(cc_params), _vp]
+_lib.cc_solve.argtypes = [_vp, _dbl, _dbl, _i32, _P(_i32), _P(_dbl)]
+_lib.cc_path.argtypes = [_vp, _P(_dbl), _i32, _dbl, _i32, _P(_i32), _P(_dbl)]
+_lib.cc_get_U.argtypes = [_vp, _i32, _vp, _i32]
+_lib.cc_clusters.argtypes = [_vp, _i32, _vp, _i32, _P(_i32)]
+_lib.cc_get_history.argtypes = [_vp, _vp, _vp, _i32, _P(_i32)]
+_lib.cc_get_stats.argtypes = [_vp, _P(_dbl), _P(_dbl), _P(_i64), _P(_dbl), _P(_dbl)]
+_lib.cc_reset.argtypes = [_vp]
+_lib.cc_get_counts.argtypes = [_vp, _P(_i64), _P(_i64), _P(_i64)]
+_lib.cc_last_error.argtypes = [_vp]
+_lib.cc_last_error.restype = ctypes.c_char_p
+_lib.cc_destroy.argtypes = [_vp]
+_lib.cc_destroy.restype = None
+
+
+class CCError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libcc_b200 error {code}: {msg}")
+        self.code = code
+
+
+def _check(rc, h=None, allow=()):
+    if rc != CC_OK and rc not in allow:
+        raise CCError(rc, _lib.cc_last_error(h).decode())
+    return rc
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream():
+    if not torch.cuda.is_available():   # let the library report CC_ECUDA itself
+        return None
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def cc_default_params(**overrides) -> cc_params:
+    prm = cc_params()
+    _check(_lib.cc_default_params(ctypes.byref(prm)))
+    for k, v in overrides.items():
+        if not hasattr(prm, k):
+            raise AttributeError(k)
+        setattr(prm, k, v)
+    return prm
+
+
+def cc_create(n, p, X, mask, rowptr, col, w, prm=None):
+    """Device tensors: X fp32 (n,p), mask uint8 (n,p) or None, rowptr int64, col int32, w fp32
+    (or the (n,n) matrix when prm.dense = 1).  Returns the opaque handle."""
+    h = ctypes.c_void_p()
+    rc = _lib.cc_create(ctypes.byref(h), n, p, _ptr(X), _ptr(mask), _ptr(rowptr), _ptr(col), _ptr(w),
+                        ctypes.byref(prm) if prm is not None else None, _stream())
+    _check(rc)
+    return h
+
+
+def cc_solve(h, gamma, tol, maxit, allow_noconv=False):
+    it, phi = _i32(0), _dbl(0.0)
+    rc = _check(_lib.cc_solve(h, gamma, tol, maxit, ctypes.byref(it), ctypes.byref(phi)), h,
+                allow=(CC_ENOCONV,) if allow_noconv else ())
+    return it.value, phi.value, rc
+
+
+def cc_path(h, gammas, tol, maxit):
+    g = (ctypes.c_double * len(gammas))(*[float(x) for x in gammas])
+    its = (ctypes.c_int32 * len(gammas))()
+    phis = (ctypes.c_double * len(gammas))()
+    _check(_lib.cc_path(h, g, len(gammas), tol, maxit, its, phis), h)
+    return list(its), list(phis)
+
+
+def cc_get_U(h, gamma_index, U_out):
+    """U_out: fp32 (n,p) contiguous torch tensor, on the device or on the host."""
+    _check(_lib.cc_get_U(h, gamma_index, _ptr(U_out), 1 if U_out.is_cuda else 0), h)
+    return U_out
+
+
+def cc_clusters(h, gamma_index, labels_out):
+    k = _i32(0)
+    _check(_lib.cc_clusters(h, gamma_index, _ptr(labels_out), 1 if labels_out.is_cuda else 0, ctypes.byref(k)), h)
+    return labels_out, k.value
+
+
+def cc_get_history(h, cap=4096):
+    phi = np.zeros(cap)
+    d = np.zeros(cap)
+    cnt = _i32(0)
+    _check(_lib.cc_get_history(h, phi.ctypes.data_as(_vp), d.ctypes.data_as(_vp), cap, ctypes.byref(cnt)), h)
+    return phi[:cnt.value].copy(), d[:cnt.value].copy()
+
+
+def cc_get_stats(h, f_gamma=False, min_margin=False):
+    rho, eps, fg, mm = _dbl(0), _dbl(0), _dbl(0), _dbl(0)
+    pi = _i64(0)
+    _check(_lib.cc_get_stats(h, ctypes.byref(rho), ctypes.byref(eps), ctypes.byref(pi),
+                             ctypes.byref(fg) if f_gamma else None, ctypes.byref(mm) if min_margin else None), h)
+    return {"rho": rho.value, "eps": eps.value, "proj_iters": pi.value,
+            "f_gamma": fg.value if f_gamma else None, "min_margin": mm.value if min_margin else None}
+
+
+def cc_reset(h):
+    _check(_lib.cc_reset(h), h)
+
+
+def cc_get_counts(h):
+    a, b, c = _i64(0), _i64(0), _i64(0)
+    _check(_lib.cc_get_counts(h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)), h)
+    return {"n_pairs": a.value, "nnz": b.value, "launches": c.value}
+
+
+def cc_last_error(h=None) -> str:
+    return _lib.cc_last_error(h).decode()
+
+
+def cc_destroy(h):
+    _lib.cc_destroy(h)
+
+
+def cc_knn_weights(n, p, X, mask, k, phi, normalize=False):
+    """Returns (rowptr int64, col int32, w fp32) as torch device tensors (copies; the library's
+    arrays are released with cc_free_graph before returning)."""
+    rp, cl, ww = _vp(), _vp(), _vp()
+    nnz = _i64(0)
+    _check(_lib.cc_knn_weights(n, p, _ptr(X), _ptr(mask), k, phi, 1 if normalize else 0, ctypes.byref(rp),
+                               ctypes.byref(cl), ctypes.byref(ww), ctypes.byref(nnz), _stream()))
+    dev = X.device
+    rowptr = torch.empty(n + 1, dtype=torch.int64, device=dev)
+    col = torch.empty(nnz.value, dtype=torch.int32, device=dev)
+    w = torch.empty(nnz.value, dtype=torch.float32, device=dev)
+    cudart = torch.cuda.cudart()
+    cudart.cudaMemcpy(rowptr.data_ptr(), rp.value, rowptr.numel() * 8, 3)
+    if nnz.value:
+        cudart.cudaMemcpy(col.data_ptr(), cl.value, nnz.value * 4, 3)
+        cudart.cudaMemcpy(w.data_ptr(), ww.value, nnz.value * 4, 3)
+    _lib.cc_free_graph(rp, cl, ww)
+    return rowptr, col, w

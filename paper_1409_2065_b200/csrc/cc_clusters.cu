@@ -1,0 +1,106 @@
+// cc_clusters.cu -- a8, cluster read-out (S16; the paper never defines it, PAPER.md L154,
+// L206): connected components of the graph whose edges are the pairs with v_ij = 0 exactly (s_ij = 0
+// after the block soft-threshold, L86-L88), numbered in increasing order of each component's smallest
+// member.  Integer work only: min-label hooking + pointer jumping, then a scan over the roots.
+#include <cstdio>
+
+#include "cc_internal.h"
+
+namespace {
+
+__global__ void k_lab_init(int n, int* __restrict__ lab) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) lab[i] = i;
+}
+
+// One thread per row: smallest label among the row and its fused neighbours; hook the old root to it.
+__global__ void k_lab_hook(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                           const float* __restrict__ s, int* lab, int* changed) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const int li = lab[i];
+    int m = li;
+    for (int e = rowptr[i]; e < rowptr[i + 1]; ++e)
+        if (s[e] == 0.f) m = min(m, lab[col[e]]);
+    if (m < li) {
+        atomicMin(&lab[li], m);
+        atomicMin(&lab[i], m);
+        *changed = 1;
+    }
+}
+
+__global__ void k_lab_jump(int n, int* lab) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int l = lab[i];
+    while (true) {
+        const int ll = lab[l];
+        if (ll == l) break;
+        l = ll;
+    }
+    lab[i] = l;
+}
+
+// Roots are the smallest members; canonical label = number of roots before this root.  One block.
+__global__ void k_lab_rank(int n, const int* __restrict__ lab, int* __restrict__ rank, int* nclusters) {
+    __shared__ int sm[1024];
+    __shared__ int carry;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += 1024) {
+        const int i = base + threadIdx.x;
+        const int isroot = (i < n && lab[i] == i) ? 1 : 0;
+        sm[threadIdx.x] = isroot;
+        __syncthreads();
+        for (int o = 1; o < 1024; o <<= 1) {
+            int v = threadIdx.x >= o ? sm[threadIdx.x - o] : 0;
+            __syncthreads();
+            sm[threadIdx.x] += v;
+            __syncthreads();
+        }
+        if (i < n) rank[i] = carry + sm[threadIdx.x] - isroot;  // exclusive
+        __syncthreads();
+        if (threadIdx.x == 0) carry += sm[1023];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *nclusters = carry;
+}
+
+__global__ void k_lab_final(int n, const int* __restrict__ lab, const int* __restrict__ rank, int* __restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = rank[lab[i]];
+}
+
+}  // namespace
+
+// labels_dev: int32[n] device output.  Uses h->lab (roots), h->tmpE reinterpret is avoided: rank lives
+// in a scratch allocation made on first use.
+int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host) {
+    const int n = (int)h->n;
+    const int grid = (n + 255) / 256;
+    cudaStream_t st = h->stream;
+    if (!h->lab_rank) {
+        cudaError_t e = cudaMalloc((void**)&h->lab_rank, (size_t)n * sizeof(int));
+        if (e != cudaSuccess) { snprintf(h->err, sizeof(h->err), "cudaMalloc labels scratch: %s", cudaGetErrorString(e)); return CC_ENOMEM; }
+    }
+    k_lab_init<<<grid, 256, 0, st>>>(n, h->lab);
+    h->launches += 1;
+    for (int round = 0; round < 100000; ++round) {
+        CC_CUDA(h, cudaMemsetAsync(h->lab_flag, 0, sizeof(int), st));
+        k_lab_hook<<<grid, 256, 0, st>>>(n, h->rowptr, h->col, h->s, h->lab, h->lab_flag);
+        k_lab_jump<<<grid, 256, 0, st>>>(n, h->lab);
+        h->launches += 2;
+        int changed = 0;
+        CC_CUDA(h, cudaMemcpyAsync(&changed, h->lab_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CC_CUDA(h, cudaStreamSynchronize(st));
+        if (!changed) break;
+    }
+    k_lab_rank<<<1, 1024, 0, st>>>(n, h->lab, h->lab_rank, h->lab_flag);
+    k_lab_final<<<grid, 256, 0, st>>>(n, h->lab, h->lab_rank, labels_dev);
+    h->launches += 2;
+    int k = 0;
+    CC_CUDA(h, cudaMemcpyAsync(&k, h->lab_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CC_CUDA(h, cudaStreamSynchronize(st));
+    if (nclusters_host) *nclusters_host = k;
+    return CC_OK;
+}

@@ -1,0 +1,131 @@
+// cc_internal.h -- internal layout shared by the .cu files of libcc_b200.so (never installed, never
+// seen by the oracle).  Notation follows PAPER.md section 3: U (cases), A = projection of U onto the
+// constraint set C (L90-L103), b_ij = a_i - a_j (L84), v_ij (L48-L53), d_m (L76), rho, eps.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/cc_b200.h"
+
+// ---------------------------------------------------------------------------------------------
+// Device-resident scalars of one solve.  Written by the "last block" of the reducing kernels and by
+// single-thread control kernels; read by every kernel of the iteration.  doubles first.
+// ---------------------------------------------------------------------------------------------
+struct cc_scal {
+    // problem constants for this gamma
+    double gamma, rho, eps, tol;
+    double xscale;      // sqrt(sum_obs (x - colmean)^2): the data scale of the projection stop rule
+    double proj_tol;
+    // MM iteration
+    double d, d_prev;   // d_m of L76; d_prev seeds the projection stop rule (sqrt(eps) at m = 0)
+    double dist2, loss, pen;
+    double phi, phi_prev;
+    double min_margin;  // smallest | ||b|| - thr | / thr at the last shrink
+    float cu, ca;       // d/(d+rho), rho/(d+rho)          (U update, L82)
+    float cthr;         // gamma d / rho                   (threshold = cthr * w_ij, L86)
+    float pad0;
+    // inner conjugate-gradient solve of (I+L) delta = r0
+    double cg_gamma, cg_gamma_old, cg_delta, cg_alpha, cg_beta, cg_thresh;
+    // control
+    int32_t mm_iter;      // iterations completed in this solve
+    int32_t mm_maxit;
+    int32_t mm_min_it;
+    int32_t mm_active;    // 1 while the outer loop runs
+    int32_t stop_pending; // the stop rule fired in k_norm: finish this iteration's updates, then stop
+    int32_t cg_iter;      // inner iterations of the current projection
+    int32_t cg_active;
+    int32_t cg_maxit;
+    int32_t cg_failed;    // some projection hit cg_maxit
+    int32_t hist_cap;
+    long long cg_total;   // inner iterations over the whole solve
+    // last-block tickets (one per reducing kernel)
+    unsigned int ticket[8];
+};
+
+// Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
+#define CC_NPART 4
+#define CC_MAXBLK 4096
+
+struct cc_handle {
+    // sizes
+    int64_t n, p, ld;        // ld = p rounded up to a multiple of 4 (padding columns stay 0)
+    int64_t nnz, npairs;
+    int dense;
+    int G;                   // lanes per row group (power of two <= 32); a group covers 4*G columns
+    int nchunk;              // ceil(ld / (4G)) column chunks
+    cc_params prm;
+    cudaStream_t stream;
+    // node arrays (n x ld fp32)
+    float *X, *U, *A, *Ap, *Z;        // Z = warm start of the projection (u + previous correction)
+    float *R, *Pv, *Sv, *Wv, *Uc;     // CG: residual, search dir, (I+L) search dir, (I+L) Uc, D^-1 r
+    uint8_t* mask;                    // n x ld or NULL
+    float* colmean;                   // ld
+    // graph (symmetric CSR)
+    int32_t* rowptr;                  // n+1 (nnz < 2^31 enforced)
+    int32_t* rowup;                   // n: first entry of row i with col > i (rows are sorted)
+    int32_t* col;                     // nnz
+    int32_t* peer;                    // nnz: index of the reverse entry
+    float* w;                         // nnz
+    float* s;                         // nnz: shrink factor of v_ij = s_ij (a'_i - a'_j)   (L86)
+    float* vn;                        // nnz: ||v_ij||
+    float* nb2;                       // nchunk x nnz partial squared norms of b_ij
+    float* tmpE;                      // nnz scratch (diagnostics)
+    float* dinv;                      // n: 1 / (1 + |N_i|)
+    float* Wd;                        // dense: n x n weights
+    // scalars
+    cc_scal* sc;                      // device
+    cc_scal* sc_host;                 // pinned mirror
+    double* part;                     // CC_MAXBLK * CC_NPART doubles per reducing kernel (x8)
+    double *hist_phi, *hist_d;        // hist_cap each
+    double* dout;                     // 4 doubles: results of the one-off reductions
+    int* dflag;                       // validation flags
+    int sms;                          // multiprocessor count
+    double sumw2, xss;                // sum_E w^2, sum_obs (x-colmean)^2
+    // snapshots
+    float* snapU;                     // max_snapshots x n x ld
+    int32_t* snapLab;                 // max_snapshots x n
+    int32_t* snapK;                   // host
+    int nsnap;
+    int32_t* lab;                     // n (scratch for cc_clusters)
+    int32_t* lab_flag;                // device int
+    int32_t* lab_rank;                // n, allocated on first cc_clusters
+    // graph execution
+    cudaGraphExec_t gexec;
+    cudaGraphConditionalHandle cond_outer, cond_inner;   // 0 while launching eagerly
+    cudaGraph_t graph;
+    long long launches;
+    int grid_nodes, grid_rows, grid_edges;   // launch sizes, fixed per handle (determinism)
+    char err[256];
+};
+
+// ---- launchers implemented in cc_sparse.cu (all enqueue on h->stream) -----------------------------
+void ccs_begin_iter(cc_handle* h);   // resets per-iteration control
+void ccs_rhs(cc_handle* h);          // a1: r0 and CG start
+void ccs_cg_spmv(cc_handle* h);      // a2: Wv = (I+L) Uc, delta = (Wv, Uc)
+void ccs_cg_update(cc_handle* h);    // a2: CG vector updates, gamma' = (r, D^-1 r)
+void ccs_norm(cc_handle* h);         // a3 + a6: pair norms, dist^2, loss, penalty -> d, Phi, stop rule
+void ccs_update(cc_handle* h);       // a5 + a4: U update, shrink
+void ccs_init_state(cc_handle* h);   // cold start of (Ap, Z, s, vn)
+void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out);
+int ccs_solve_eager(cc_handle* h, int maxit);
+int ccs_build_graph(cc_handle* h);
+
+// ---- cc_setup.cu ------------------------------------------------------------------------------------
+int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, const int64_t* rowptr,
+                           const int32_t* col, const float* w);
+int ccu_cold_start(cc_handle* h);                       // U0 = X, missing -> observed column mean (S4)
+int ccu_fgamma(cc_handle* h, double* f_out);            // eq. 1/6 at the current U
+int ccu_min_margin(cc_handle* h, double* margin_out);   // min | ||b|| - thr | / thr at the last shrink
+void ccu_free(cc_handle* h);
+// ---- cc_clusters.cu -----------------------------------------------------------------------------------
+int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host);
+
+#define CC_CUDA(h, call)                                                                  \
+    do {                                                                                  \
+        cudaError_t e_ = (call);                                                          \
+        if (e_ != cudaSuccess) {                                                          \
+            snprintf((h)->err, sizeof((h)->err), "%s: %s", #call, cudaGetErrorString(e_)); \
+            return CC_ECUDA;                                                              \
+        }                                                                                 \
+    } while (0)

@@ -1,0 +1,558 @@
+// cc_sparse.cu -- the MM iteration of PAPER.md section 3.1 on a symmetric-CSR graph, sm_100a.
+//
+// V-free form: after an iteration the paper's v_ij (L86) equals
+// s_ij (a'_i - a'_j), A' = the projection of that iteration, so only one scalar s_ij per pair is kept
+// and  (D^T V)_i = sum_{j in N_i} s_ij (a'_i - a'_j)  is a per-row gather with no atomics.
+//
+// One MM iteration = k_rhs -> { k_cg_spmv, k_cg_update }* -> k_norm -> k_update.
+//   k_rhs     a1  r0_i = sum_j [ s_ij (a'_i - a'_j) - (z_i - z_j) ] - (z_i - u_i)       (L100 right-hand
+//                 side minus (I+L) z, z = warm start), A := z
+//   k_cg_*    a2  Jacobi-preconditioned CG (Chronopoulos-Gear form: one reduction per kernel) on
+//                 (I+L) delta = r0,  A := z + delta                                       (L90-L103)
+//   k_norm    a3/a6  ||b_ij||^2, dist^2 -> d_m (L76), Phi_m (L64-L66, L109), stop rule (S3)
+//   k_update  a5/a4  U update (L82, L116), shrink factors (L86-L88), A' := A, next warm start
+//
+// Work decomposition: a "row group" of G lanes (G = 2..32) owns row i x one chunk of 4G columns; each
+// lane holds a float4.  Neighbour rows are gathered as 16G-byte contiguous segments.
+#include <cstdio>
+
+#include "cc_internal.h"
+#include "cc_device.cuh"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// a1  k_rhs.  PAPER.md L100: the block update's right-hand side is u~_i + sum_{R_i} v~_ij - sum_{L_i}
+// v~_ji; with v = s (a'_i - a'_j) both sums merge into sum_{N_i} s_ij (a'_i - a'_j).  We subtract
+// (I+L) z to get the residual of the warm start z.
+// ---------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, const int* __restrict__ rowptr,
+                                                     const int* __restrict__ col, const float* __restrict__ s,
+                                                     const float* __restrict__ dinv, const float* __restrict__ Ap,
+                                                     const float* __restrict__ Z, const float* __restrict__ U,
+                                                     float* __restrict__ R, float* __restrict__ Uc, float* __restrict__ A,
+                                                     cc_scal* sc, double* part, cudaGraphConditionalHandle loop) {
+    if (!sc->mm_active) return;
+    const unsigned gm = group_mask<G>();
+    const int gl = threadIdx.x & (G - 1);
+    const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
+    const long long items = (long long)n * nchunk;
+    double acc_g[1] = {0.0};
+    for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
+        const int i = (int)(it / nchunk);
+        const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
+        const bool valid = c0 < ld;
+        const size_t oi = (size_t)i * ld + (valid ? c0 : 0);
+        const float4 api = ld4s(Ap + oi), zi = ld4s(Z + oi), ui = ld4s(U + oi);
+        float4 acc = f4(0.f);
+        const int rs = rowptr[i], re = rowptr[i + 1];
+        for (int base = rs; base < re; base += G) {
+            const int e = base + gl;
+            const int cj = e < re ? __ldg(col + e) : i;   // padding entries point at the own row with s = 1:
+            const float sv = e < re ? __ldg(s + e) : 1.f; // 1*(a_i - a_i) - (z_i - z_i) = 0 exactly
+            const int cnt = min(G, re - base);
+            for (int t = 0; t < cnt; t += 4) {
+                int j[4];
+                float sj[4];
+                float4 aj[4], zj[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
+                    sj[q] = __shfl_sync(gm, sv, (t + q) & (G - 1), G);
+                    if (G < 4 && t + q >= G) { j[q] = i; sj[q] = 1.f; }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
+                    aj[q] = ld4s(Ap + oj);
+                    zj[q] = ld4s(Z + oj);
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc = fma4(sj[q], api - aj[q], acc) - (zi - zj[q]);
+            }
+        }
+        acc = acc - (zi - ui);
+        if (valid) {
+            const float di = dinv[i];
+            const float4 uc = di * acc;
+            st4(R + oi, acc);
+            st4(Uc + oi, uc);
+            st4(A + oi, zi);
+            acc_g[0] += (double)dot4(acc, uc);
+        }
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc_g, part, &sc->ticket[0], tot)) {
+        const double th = sc->proj_tol * (sc->d_prev / sc->rho) * sc->xscale;
+        sc->cg_gamma = tot[0];
+        sc->cg_gamma_old = 1.0;
+        sc->cg_alpha = 1.0;
+        sc->cg_thresh = th * th;
+        sc->cg_iter = 0;
+        const int active = tot[0] > th * th ? 1 : 0;
+        sc->cg_active = active;
+        if (loop) cudaGraphSetConditional(loop, active);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2  k_cg_spmv.  Wv_i = ((I+L) Uc)_i = (1+|N_i|) uc_i - sum_{j in N_i} uc_j  -- one row of the
+// stationarity equation PAPER.md L96 applied to the preconditioned residual.  delta = (Wv, Uc).
+// The last block turns (gamma, delta) into the CG step sizes (Chronopoulos & Gear recurrences).
+// ---------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchunk, const int* __restrict__ rowptr,
+                                                         const int* __restrict__ col, const float* __restrict__ Uc,
+                                                         float* __restrict__ Wv, cc_scal* sc, double* part) {
+    if (!sc->mm_active || !sc->cg_active) return;
+    const unsigned gm = group_mask<G>();
+    const int gl = threadIdx.x & (G - 1);
+    const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
+    const long long items = (long long)n * nchunk;
+    double acc_g[1] = {0.0};
+    for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
+        const int i = (int)(it / nchunk);
+        const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
+        const bool valid = c0 < ld;
+        const size_t oi = (size_t)i * ld + (valid ? c0 : 0);
+        const float4 ui = ld4s(Uc + oi);
+        const int rs = rowptr[i], re = rowptr[i + 1];
+        float4 nsum = f4(0.f);
+        for (int base = rs; base < re; base += G) {
+            const int e = base + gl;
+            const int cj = e < re ? __ldg(col + e) : -1;
+            const int cnt = min(G, re - base);
+            for (int t = 0; t < cnt; t += 4) {
+                int j[4];
+                float4 uj[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
+                    if (G < 4 && t + q >= G) j[q] = -1;
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    uj[q] = j[q] >= 0 ? ld4s(Uc + (size_t)j[q] * ld + (valid ? c0 : 0)) : f4(0.f);
+#pragma unroll
+                for (int q = 0; q < 4; ++q) nsum = nsum + uj[q];
+            }
+        }
+        if (valid) {
+            const float dg = 1.f + (float)(re - rs);
+            const float4 wv = dg * ui - nsum;
+            st4(Wv + oi, wv);
+            acc_g[0] += (double)dot4(wv, ui);
+        }
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc_g, part, &sc->ticket[1], tot)) {
+        const double gam = sc->cg_gamma, del = tot[0];
+        double beta, alpha;
+        if (sc->cg_iter == 0) {
+            beta = 0.0;
+            alpha = gam / del;
+        } else {
+            beta = gam / sc->cg_gamma_old;
+            alpha = gam / (del - beta * gam / sc->cg_alpha);
+        }
+        sc->cg_delta = del;
+        sc->cg_beta = beta;
+        sc->cg_alpha = alpha;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2  k_cg_update.  p = uc + beta p;  s = w + beta s;  A += alpha p;  r -= alpha s;  uc = D^-1 r;
+// gamma' = (r, uc).  The last block applies the stop rule of the projection (cc_b200.h proj_tol).
+// `loop` is the inner WHILE node's handle in graph mode (0 in eager mode).
+// ---------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nchunk, const float* __restrict__ dinv,
+                                                           float* __restrict__ Uc, const float* __restrict__ Wv,
+                                                           float* __restrict__ Pv, float* __restrict__ Sv,
+                                                           float* __restrict__ A, float* __restrict__ R, cc_scal* sc,
+                                                           double* part, cudaGraphConditionalHandle loop) {
+    if (!sc->mm_active || !sc->cg_active) return;
+    const int gl = threadIdx.x & (G - 1);
+    const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
+    const long long items = (long long)n * nchunk;
+    const bool first = sc->cg_iter == 0;
+    const float alpha = (float)sc->cg_alpha, beta = (float)sc->cg_beta;
+    double acc_g[1] = {0.0};
+    for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
+        const int i = (int)(it / nchunk);
+        const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
+        if (c0 >= ld) continue;
+        const size_t oi = (size_t)i * ld + c0;
+        float4 pv = ld4s(Uc + oi), sv = ld4s(Wv + oi);
+        if (!first) {
+            pv = fma4(beta, ld4s(Pv + oi), pv);
+            sv = fma4(beta, ld4s(Sv + oi), sv);
+        }
+        st4(Pv + oi, pv);
+        st4(Sv + oi, sv);
+        st4(A + oi, fma4(alpha, pv, ld4s(A + oi)));
+        const float4 r = fma4(-alpha, sv, ld4s(R + oi));
+        const float4 uc = dinv[i] * r;
+        st4(R + oi, r);
+        st4(Uc + oi, uc);
+        acc_g[0] += (double)dot4(r, uc);
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc_g, part, &sc->ticket[2], tot)) {
+        sc->cg_gamma_old = sc->cg_gamma;
+        sc->cg_gamma = tot[0];
+        const int k = sc->cg_iter + 1;
+        sc->cg_iter = k;
+        sc->cg_total += 1;
+        int active = 1;
+        if (!(tot[0] > sc->cg_thresh)) active = 0;
+        else if (k >= sc->cg_maxit) { active = 0; sc->cg_failed = 1; }
+        sc->cg_active = active;
+        if (loop) cudaGraphSetConditional(loop, active);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a3 + a6  k_norm.  For every pair i<j (the entries col > i of row i, a suffix because rows are
+// sorted):  b_ij = a_i - a_j (L84),  ||b_ij||^2 -> nb2 (both directions),  ||v_ij - b_ij||^2 with
+// v_ij = s_ij (a'_i - a'_j);  per node ||u_i - a_i||^2 and the observed loss.  Last block:
+// d_m = sqrt(dist^2 + eps) (L76), Phi_m (L64-L66 with the loss of eq. 6), stop rule S3, and the
+// coefficients of the two updates.  `outer` = the MM WHILE node's handle in graph mode, else 0.
+// ---------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, long long nnz,
+                                                      const int* __restrict__ rowptr, const int* __restrict__ rowup,
+                                                      const int* __restrict__ col, const int* __restrict__ peer,
+                                                      const float* __restrict__ w, const float* __restrict__ s,
+                                                      const float* __restrict__ vn, const float* __restrict__ A,
+                                                      const float* __restrict__ Ap, const float* __restrict__ U,
+                                                      const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                      float* __restrict__ nb2, cc_scal* sc, double* part,
+                                                      double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer) {
+    if (!sc->mm_active) return;
+    const unsigned gm = group_mask<G>();
+    const int gl = threadIdx.x & (G - 1);
+    const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
+    const long long items = (long long)n * nchunk;
+    double acc_g[3] = {0.0, 0.0, 0.0};  // dist^2, loss, penalty
+    for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
+        const int i = (int)(it / nchunk);
+        const int chunk = (int)(it % nchunk);
+        const int c0 = chunk * 4 * G + gl * 4;
+        const bool valid = c0 < ld;
+        const float vf = valid ? 1.f : 0.f;
+        const size_t oi = (size_t)i * ld + (valid ? c0 : 0);
+        const float4 ai = ld4s(A + oi), api = ld4s(Ap + oi), ui = ld4s(U + oi), xi = ld4s(X + oi);
+        float dist_l = 0.f, pen_l = 0.f;
+        {
+            const float4 t = ui - ai;
+            float4 q = xi - ui;
+            if (mask) {
+                const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + oi);
+                q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
+            }
+            dist_l = vf * dot4(t, t);
+            acc_g[1] += (double)(vf * dot4(q, q));
+        }
+        const int rs = rowup[i], re = rowptr[i + 1];
+        for (int base = rs; base < re; base += G) {
+            const int e = base + gl;
+            const int cj = e < re ? __ldg(col + e) : i;
+            const float sv = e < re ? __ldg(s + e) : 0.f;
+            const int cnt = min(G, re - base);
+            for (int t = 0; t < cnt; t += 4) {
+                int j[4];
+                float sj[4], nbq[4];
+                float4 aj[4], apj[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
+                    sj[q] = __shfl_sync(gm, sv, (t + q) & (G - 1), G);
+                    if (G < 4 && t + q >= G) { j[q] = i; sj[q] = 0.f; }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
+                    aj[q] = ld4s(A + oj);
+                    apj[q] = ld4s(Ap + oj);
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const float4 b = ai - aj[q];
+                    const float4 vb = fma4(sj[q], api - apj[q], f4(0.f)) - b;
+                    nbq[q] = vf * dot4(b, b);
+                    dist_l += vf * dot4(vb, vb);   // padding entries: b = 0, s = 0 => 0
+                }
+#pragma unroll
+                for (int o = G / 2; o > 0; o >>= 1) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) nbq[q] += __shfl_xor_sync(gm, nbq[q], o, G);
+                }
+                if (gl == 0) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const int eq = base + t + q;
+                        if (t + q < cnt) {
+                            nb2[(size_t)chunk * nnz + eq] = nbq[q];
+                            nb2[(size_t)chunk * nnz + __ldg(peer + eq)] = nbq[q];
+                            if (chunk == 0) pen_l = fmaf(__ldg(w + eq), __ldg(vn + eq), pen_l);
+                        }
+                    }
+                }
+            }
+        }
+        acc_g[0] += (double)dist_l;
+        acc_g[2] += (double)pen_l;
+    }
+    double tot[3];
+    if (grid_reduce<3>(acc_g, part, &sc->ticket[3], tot)) {
+        const double d = sqrt(tot[0] + sc->eps);
+        const double phi = 0.5 * tot[1] + sc->gamma * tot[2] + sc->rho * d;
+        const int m = sc->mm_iter;
+        if (m < sc->hist_cap) { hist_phi[m] = phi; hist_d[m] = d; }
+        int stop = (m + 1 >= sc->mm_maxit) ? 1 : 0;
+        if (sc->tol > 0.0 && m + 1 >= sc->mm_min_it && m >= 1 &&
+            sc->phi_prev - phi <= sc->tol * (1.0 + fabs(sc->phi_prev)))
+            stop = 1;
+        sc->dist2 = tot[0]; sc->loss = tot[1]; sc->pen = tot[2];
+        sc->d = d; sc->d_prev = d;
+        sc->phi_prev = phi; sc->phi = phi;
+        sc->cu = (float)(d / (d + sc->rho));
+        sc->ca = (float)(sc->rho / (d + sc->rho));
+        sc->cthr = (float)(sc->gamma * d / sc->rho);
+        sc->mm_iter = m + 1;
+        sc->stop_pending = stop;
+        if (outer) cudaGraphSetConditional(outer, stop ? 0 : 1);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5 + a4  k_update.  y = x where observed else u (L116);  u <- (d y + rho a)/(d + rho) (L82);
+// next warm start z = u_new + (a - u_old);  A' <- A.  Then per directed entry the block
+// soft-threshold factor (L86-L88, S6):  thr = gamma w d / rho;  s = ||b|| <= thr ? 0 : 1 - thr/||b||
+// (this covers b = 0 => v = 0, L88) and ||v|| = s ||b|| for the next Phi.
+// ---------------------------------------------------------------------------------------------
+template <int G>
+__global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk, long long nnz,
+                                                        const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                        const float* __restrict__ A, float* __restrict__ U,
+                                                        float* __restrict__ Z, float* __restrict__ Ap,
+                                                        const float* __restrict__ w, const float* __restrict__ nb2,
+                                                        float* __restrict__ s, float* __restrict__ vn, const cc_scal* sc) {
+    if (!sc->mm_active) return;
+    const int gl = threadIdx.x & (G - 1);
+    const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
+    const long long items = (long long)n * nchunk;
+    const float cu = sc->cu, ca = sc->ca, cthr = sc->cthr;
+    for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
+        const int i = (int)(it / nchunk);
+        const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
+        if (c0 >= ld) continue;
+        const size_t oi = (size_t)i * ld + c0;
+        const float4 a = ld4s(A + oi), u = ld4s(U + oi);
+        float4 y = ld4s(X + oi);
+        if (mask) {
+            const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + oi);
+            y.x = mk.x ? y.x : u.x; y.y = mk.y ? y.y : u.y; y.z = mk.z ? y.z : u.z; y.w = mk.w ? y.w : u.w;
+        }
+        const float4 un = fma4(cu, y, ca * a);
+        st4(U + oi, un);
+        st4(Z + oi, un + (a - u));
+        st4(Ap + oi, a);
+    }
+    const long long nthreads = (long long)gridDim.x * CC_THREADS;
+    for (long long e = (long long)blockIdx.x * CC_THREADS + threadIdx.x; e < nnz; e += nthreads) {
+        float q = nb2[e];
+        for (int c = 1; c < nchunk; ++c) q += nb2[(size_t)c * nnz + e];
+        const float nb = sqrtf(q);
+        const float thr = cthr * w[e];
+        const float sn = nb <= thr ? 0.f : 1.f - thr / nb;
+        s[e] = sn;
+        vn[e] = sn * nb;
+    }
+}
+
+// One thread: eager-mode bookkeeping between iterations (the WHILE node does this in graph mode).
+__global__ void k_begin_iter(cc_scal* sc) {
+    if (sc->stop_pending) sc->mm_active = 0;
+}
+
+// Cold start of the pair state (S4: V0 = D U0, i.e. s = 1, ||v_ij|| = ||u0_i - u0_j||), and the pair
+// norms of an arbitrary node array (used for f_gamma, eq. 1/6).  One-time / diagnostic: every directed
+// entry is computed, each group walks all column chunks of its row.
+template <int G>
+__global__ void __launch_bounds__(CC_THREADS) k_pair_norms(int n, int ld, int nchunk, const int* __restrict__ rowptr,
+                                                            const int* __restrict__ col, const float* __restrict__ V,
+                                                            float* __restrict__ out, float* __restrict__ s_out) {
+    const unsigned gm = group_mask<G>();
+    const int gl = threadIdx.x & (G - 1);
+    const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
+    for (long long i = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; i < n; i += ngroups) {
+        const int rs = rowptr[i], re = rowptr[i + 1];
+        for (int e = rs; e < re; ++e) {
+            const int j = __ldg(col + e);
+            float acc = 0.f;
+            for (int c = 0; c < nchunk; ++c) {
+                const int c0 = c * 4 * G + gl * 4;
+                if (c0 < ld) {
+                    const float4 b = ld4s(V + (size_t)i * ld + c0) - ld4s(V + (size_t)j * ld + c0);
+                    acc += dot4(b, b);
+                }
+            }
+            acc = group_sum<G>(acc, gm);
+            if (gl == 0) {
+                out[e] = sqrtf(acc);
+                if (s_out) s_out[e] = 1.f;
+            }
+        }
+    }
+}
+
+}  // namespace
+
+// =============================================================================================
+// Host side: launchers, eager loop, CUDA graph with nested device-side WHILE loops.
+// =============================================================================================
+#define CC_DISPATCH_G(h, KERNEL, grid, ...)                                                        \
+    switch ((h)->G) {                                                                              \
+        case 2: KERNEL<2><<<(grid), CC_THREADS, 0, (h)->stream>>>(__VA_ARGS__); break;            \
+        case 4: KERNEL<4><<<(grid), CC_THREADS, 0, (h)->stream>>>(__VA_ARGS__); break;            \
+        case 8: KERNEL<8><<<(grid), CC_THREADS, 0, (h)->stream>>>(__VA_ARGS__); break;            \
+        case 16: KERNEL<16><<<(grid), CC_THREADS, 0, (h)->stream>>>(__VA_ARGS__); break;          \
+        default: KERNEL<32><<<(grid), CC_THREADS, 0, (h)->stream>>>(__VA_ARGS__); break;          \
+    }
+
+static cudaGraphConditionalHandle g_inner(const cc_handle* h) { return h->cond_inner; }
+static cudaGraphConditionalHandle g_outer(const cc_handle* h) { return h->cond_outer; }
+
+void ccs_begin_iter(cc_handle* h) { k_begin_iter<<<1, 1, 0, h->stream>>>(h->sc); }
+
+void ccs_rhs(cc_handle* h) {
+    CC_DISPATCH_G(h, k_rhs, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->rowptr, h->col, h->s, h->dinv, h->Ap,
+                  h->Z, h->U, h->R, h->Uc, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART, g_inner(h));
+}
+
+void ccs_cg_spmv(cc_handle* h) {
+    CC_DISPATCH_G(h, k_cg_spmv, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->rowptr, h->col, h->Uc, h->Wv,
+                  h->sc, h->part + 1 * CC_MAXBLK * CC_NPART);
+}
+
+void ccs_cg_update(cc_handle* h) {
+    CC_DISPATCH_G(h, k_cg_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->dinv, h->Uc, h->Wv, h->Pv,
+                  h->Sv, h->A, h->R, h->sc, h->part + 2 * CC_MAXBLK * CC_NPART, g_inner(h));
+}
+
+void ccs_norm(cc_handle* h) {
+    CC_DISPATCH_G(h, k_norm, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->rowptr, h->rowup,
+                  h->col, h->peer, h->w, h->s, h->vn, h->A, h->Ap, h->U, h->X, h->mask, h->nb2, h->sc,
+                  h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, g_outer(h));
+}
+
+void ccs_update(cc_handle* h) {
+    CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->X, h->mask,
+                  h->A, h->U, h->Z, h->Ap, h->w, h->nb2, h->s, h->vn, h->sc);
+}
+
+void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out) {
+    CC_DISPATCH_G(h, k_pair_norms, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->rowptr, h->col, V, out, s_out);
+}
+
+// Host loop with plain launches (prm.use_graph = 0): same kernels, same arithmetic, the loops are
+// driven by reading the control block back.  Debug path; the graph is the product path.
+int ccs_solve_eager(cc_handle* h, int maxit) {
+    h->cond_inner = 0;
+    h->cond_outer = 0;
+    for (int it = 0; it < maxit; ++it) {
+        ccs_begin_iter(h);
+        ccs_rhs(h);
+        h->launches += 2;
+        for (;;) {
+            CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
+            CC_CUDA(h, cudaStreamSynchronize(h->stream));
+            if (!h->sc_host->mm_active || !h->sc_host->cg_active) break;
+            for (int q = 0; q < 4; ++q) {
+                ccs_cg_spmv(h);
+                ccs_cg_update(h);
+            }
+            h->launches += 2;  // counted below from cg_total for the ones that did work
+        }
+        ccs_norm(h);
+        ccs_update(h);
+        h->launches += 2;
+        CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
+        CC_CUDA(h, cudaStreamSynchronize(h->stream));
+        if (!h->sc_host->mm_active || h->sc_host->stop_pending) break;
+    }
+    CC_CUDA(h, cudaGetLastError());
+    return CC_OK;
+}
+
+// One graph per handle:  WHILE(outer){ k_rhs; WHILE(inner){ k_cg_spmv; k_cg_update }; k_norm; k_update }.
+// Kernel arguments are the handle's fixed buffers; everything that changes between solves lives in
+// the device control block cc_scal, so the instantiated graph is reused for every gamma.
+int ccs_build_graph(cc_handle* h) {
+    if (h->gexec) return CC_OK;
+    cudaStream_t cap;
+    CC_CUDA(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    CC_CUDA(h, cudaGraphCreate(&h->graph, 0));
+    CC_CUDA(h, cudaGraphConditionalHandleCreate(&h->cond_outer, h->graph, 1, cudaGraphCondAssignDefault));
+    CC_CUDA(h, cudaGraphConditionalHandleCreate(&h->cond_inner, h->graph, 0, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams op = {};
+    op.type = cudaGraphNodeTypeConditional;
+    op.conditional.handle = h->cond_outer;
+    op.conditional.type = cudaGraphCondTypeWhile;
+    op.conditional.size = 1;
+    cudaGraphNode_t onode;
+    CC_CUDA(h, cudaGraphAddNode(&onode, h->graph, nullptr, 0, &op));
+    cudaGraph_t og = op.conditional.phGraph_out[0];
+
+    h->stream = cap;  // launchers enqueue on h->stream: capture them
+    cudaError_t e = cudaStreamBeginCaptureToGraph(cap, og, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    cudaGraph_t ig = nullptr;
+    if (e == cudaSuccess) {
+        ccs_rhs(h);
+        cudaStreamCaptureStatus st;
+        const cudaGraphNode_t* deps = nullptr;
+        size_t ndeps = 0;
+        cudaGraph_t cg = nullptr;
+        e = cudaStreamGetCaptureInfo_v2(cap, &st, nullptr, &cg, &deps, &ndeps);
+        cudaGraphNodeParams ip = {};
+        ip.type = cudaGraphNodeTypeConditional;
+        ip.conditional.handle = h->cond_inner;
+        ip.conditional.type = cudaGraphCondTypeWhile;
+        ip.conditional.size = 1;
+        cudaGraphNode_t inode;
+        if (e == cudaSuccess) e = cudaGraphAddNode(&inode, cg, deps, ndeps, &ip);
+        if (e == cudaSuccess) e = cudaStreamUpdateCaptureDependencies(cap, &inode, 1, cudaStreamSetCaptureDependencies);
+        ig = ip.conditional.phGraph_out[0];
+        ccs_norm(h);
+        ccs_update(h);
+        cudaError_t e2 = cudaStreamEndCapture(cap, nullptr);
+        if (e == cudaSuccess) e = e2;
+    }
+    if (e == cudaSuccess) e = cudaStreamBeginCaptureToGraph(cap, ig, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    if (e == cudaSuccess) {
+        ccs_cg_spmv(h);
+        ccs_cg_update(h);
+        e = cudaStreamEndCapture(cap, nullptr);
+    }
+    h->stream = user;
+    cudaStreamDestroy(cap);
+    if (e != cudaSuccess) {
+        snprintf(h->err, sizeof(h->err), "building the solve graph: %s", cudaGetErrorString(e));
+        return CC_ECUDA;
+    }
+    CC_CUDA(h, cudaGraphInstantiate(&h->gexec, h->graph, 0));
+    return CC_OK;
+}
+
+void ccs_init_state(cc_handle* h) {
+    const size_t bytes = (size_t)h->n * h->ld * sizeof(float);
+    cudaMemcpyAsync(h->Ap, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
+    cudaMemcpyAsync(h->Z, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
+    ccs_pair_norms(h, h->U, h->vn, h->s);
+    h->launches += 1;
+}

@@ -1,0 +1,356 @@
+#!/usr/bin/env python
+"""bench.py -- pair-updates/s of the convex-clustering MM hot path (BASELINE.json `metric`).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+Workload (default `large_sparse` = BASELINE.json configs[3], the largest sparse single-GPU config and
+the one north_star's roofline target names): seeded synthetic data from paper_1409_2065_b200.synth;
+the k-NN Gaussian graph is built on the GPU by cc_knn_weights (a0).
+
+One STEP = one cc_solve of `--iters` MM iterations (rows a1-a6 of DESIGN.md: right-hand side, CG
+projection, pair norms + d_m + Phi, U update + shrink) at the next gamma of the 50-value grid, walked
+with stride 5 and warm-started from the previous step, exactly as cc_path does.  One pair-update = one
+undirected pair carried through one full MM iteration, projection sweeps included.
+
+value   : |E| * iters * K / device time of the K steps, inputs resident in HBM.
+e2e     : the same work through the C ABI starting from pinned HOST buffers: per step H2D of X and the
+          CSR graph, cc_create, cc_solve, cc_get_U into host memory, cc_destroy.
+roofline: the kernel with the largest share of device time; its duration is measured live inside the
+          timed region by the library's device-side %globaltimer marks (the kernels are nodes of a
+          CUDA graph with device-side WHILE loops, so host events cannot bracket them); bytes per
+          launch are the algorithmic no-reuse figures of DESIGN.md.
+cpu_baseline / --impl reference: the fp64 oracle (oracle/), as it stands, on the host cores, on a
+          bounded sample (the first `--cpu-n` points' worth of the same generator).
+N > 1   : the path does not shard without a halo exchange: N independent
+          replicas with different seeds, no collective on the data path, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+GRID = {"large_sparse": (1.0, 1000.0, 50), "tiny": (1e-3, 1e3, 20), "expression": (0.05, 50.0, 40)}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="large_sparse", choices=list(GRID))
+    ap.add_argument("--iters", type=int, default=20, help="MM iterations per step")
+    ap.add_argument("--n", type=int, default=0, help="override the number of points (0 = config size)")
+    ap.add_argument("--cpu-n", type=int, default=6000, help="points in the oracle's bounded sample")
+    ap.add_argument("--cpu-iters", type=int, default=3)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-path", action="store_true", help="skip the full gamma-path wall time")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def gamma_for_step(workload, step):
+    from paper_1409_2065_b200 import synth
+    lo, hi, ng = GRID[workload]
+    grid = synth.gamma_grid(lo, hi, ng)
+    return float(grid[(step * 5) % ng])
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thr = threading.Thread(target=self._read, daemon=True)
+            self.thr.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thr.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[k] for r in self.rows if len(r) >= 7 for k in range(4) if r[3 + k] == "Active"})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def cpu_count_used(O):
+    return int(O.num_threads())
+
+
+def oracle_sample(args, steps, warmup):
+    """Times the oracle on a bounded sample of the workload; returns (pair-updates/s, info dict)."""
+    from oracle import oracle as O
+    from paper_1409_2065_b200 import synth
+    O.build()
+    kw = {"n": args.cpu_n} if args.workload == "large_sparse" else {}
+    wl = synth.make(args.workload, **kw)
+    X = wl.X.astype(np.float64)
+    if wl.phi_rule == "fixed":
+        phi = wl.phi
+    else:
+        si, sj = synth.sample_pairs(wl.n, 200_000, wl.seed)
+        d2 = O.pair_dist2(X, wl.mask, si, sj)
+        phi = 1.0 / float(np.median(d2[np.isfinite(d2)]))
+    ei, ej, w, _ = O.knn_graph(X, wl.mask, wl.k, phi)
+    U, V = O.cold_start(X, wl.mask, ei, ej)
+    times = []
+    for s in range(warmup + steps):
+        g = gamma_for_step(args.workload, s)
+        rho, eps = O.default_rho_eps(X, wl.mask, w, g)
+        t0 = time.perf_counter()
+        r = O.mm(X, wl.mask, ei, ej, w, g, rho, eps, U, V, args.cpu_iters, proj_method=1)
+        dt = time.perf_counter() - t0
+        U, V = r["U"], r["V"]
+        if s >= warmup:
+            times.append(dt)
+    tot = float(sum(times))
+    val = len(ei) * args.cpu_iters * len(times) / tot
+    info = {"value": val, "unit": "pair-updates/s", "cores": cpu_count_used(O), "kind": "oracle",
+            "sample": f"{args.workload} generator at n={wl.n} (|E|={len(ei)}), {len(times)} step(s) x "
+                      f"{args.cpu_iters} MM iterations, fp64, explicit V, CG projection to 1e-13"}
+    return val, info, tot / max(1, len(times))
+
+
+def alg_bytes(kernel, n, p, nnz, masked):
+    """Algorithmic (no-reuse) bytes one launch of `kernel` must move: every gathered neighbour row is
+    counted once per directed entry, own rows and outputs once per node ('roofline')."""
+    row, npb = 4 * p, 4 * n * p
+    return {
+        "k_rhs": nnz * (2 * row + 8) + 6 * npb + 4 * n,
+        "k_cg_spmv": nnz * (row + 4) + 2 * npb + 4 * n,
+        "k_cg_update": 11 * npb + 4 * n,
+        "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
+        "k_update": 6 * npb + (n * p if masked else 0) + 16 * nnz,
+    }[kernel]
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    val, info, s_per_step = oracle_sample(args, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": "pair-updates/sec per MM iteration", "value": val,
+            "unit": "pair-updates/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * s_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": args.workload, "iters_per_step": args.cpu_iters},
+            "cpu_baseline": info, "gpu_launches": 0,
+            "e2e": {"value": val, "unit": "pair-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1409_2065_b200 import synth
+    from paper_1409_2065_b200 import binding as B   # fails loudly when the CUDA library is missing
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback for the product path)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    kw = {"n": args.n} if args.n else {}
+    wl = synth.make(args.workload, seed=rank, **kw)      # replicas differ by seed
+    n, p = wl.n, wl.p
+    Xh = torch.from_numpy(wl.X).pin_memory()
+    Mh = None if wl.mask is None else torch.from_numpy(wl.mask).pin_memory()
+    X = Xh.to(dev)
+    M = None if Mh is None else Mh.to(dev)
+    # phi rule S10: 1 / median squared distance over seeded sample pairs (torch only moves the data; the
+    # median of ~2e5 numbers is input preparation, not a step of the path)
+    if wl.phi_rule == "fixed":
+        phi = wl.phi
+    else:
+        si, sj = synth.sample_pairs(n, 200_000, wl.seed)
+        d = X[torch.from_numpy(si).to(dev)] - X[torch.from_numpy(sj).to(dev)]
+        phi = 1.0 / float((d * d).sum(1).median())
+    t0 = time.perf_counter()
+    rowptr, col, w = B.cc_knn_weights(n, p, X, M, wl.k, phi)
+    torch.cuda.synchronize()
+    t_knn = time.perf_counter() - t0
+    rowptr_h, col_h, w_h = rowptr.cpu().pin_memory(), col.cpu().pin_memory(), w.cpu().pin_memory()
+    nnz = int(col.numel())
+    E = nnz // 2
+
+    h = B.cc_create(n, p, X, M, rowptr, col, w, B.cc_default_params())
+    for s in range(args.warmup):
+        B.cc_solve(h, gamma_for_step(args.workload, s), 0.0, args.iters)
+    B.cc_reset_profile(h)
+    launches0 = B.cc_get_counts(h)["launches"]
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    ev0.record()
+    iters_done = 0
+    for s in range(args.steps):
+        it, _, _ = B.cc_solve(h, gamma_for_step(args.workload, args.warmup + s), 0.0, args.iters)
+        iters_done += it
+    ev1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop()
+    prof = B.cc_get_profile(h)
+    stats = B.cc_get_stats(h)
+    launches = B.cc_get_counts(h)["launches"] - launches0
+    cg_per_it = prof["k_cg_spmv"]["calls"] / max(1, iters_done)
+
+    # ---- full gamma path (rank 0, N = 1): the other half of BASELINE.json's metric
+    path = None
+    if not args.no_path and world == 1:
+        lo, hi, ng = GRID[args.workload]
+        gam = [float(g) for g in synth.gamma_grid(lo, hi, ng)]
+        B.cc_reset(h)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record()
+        its, _ = B.cc_path(h, gam, 1e-5, 2000)
+        p1.record()
+        torch.cuda.synchronize()
+        lab = torch.empty(n, dtype=torch.int32, device=dev)
+        ks = [B.cc_clusters(h, g, lab)[1] for g in (0, ng // 2, ng - 1)]
+        path = {"n_gamma": ng, "gamma_lo": lo, "gamma_hi": hi, "tol": 1e-5, "maxit": 2000,
+                "wall_s": p0.elapsed_time(p1) / 1e3, "iters_total": int(sum(its)),
+                "nclusters_first_mid_last": ks}
+    B.cc_destroy(h)
+
+    # ---- e2e: host buffers -> cc_create -> cc_solve -> U back on the host, every step
+    e2e = None
+    if not args.no_e2e:
+        Uh = torch.empty(n, p, dtype=torch.float32).pin_memory()
+        h2d = Xh.numel() * 4 + (Mh.numel() if Mh is not None else 0) + rowptr_h.numel() * 8 + col_h.numel() * 4 + w_h.numel() * 4
+        d2h = Uh.numel() * 4
+
+        def e2e_step(s):
+            Xd = Xh.to(dev, non_blocking=True)
+            Md = None if Mh is None else Mh.to(dev, non_blocking=True)
+            rp, cl, ww = rowptr_h.to(dev, non_blocking=True), col_h.to(dev, non_blocking=True), w_h.to(dev, non_blocking=True)
+            hh = B.cc_create(n, p, Xd, Md, rp, cl, ww, None)
+            it, _, _ = B.cc_solve(hh, gamma_for_step(args.workload, s), 0.0, args.iters)
+            B.cc_get_U(hh, -1, Uh)
+            B.cc_destroy(hh)
+            return it
+        for s in range(2):
+            e2e_step(s)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        it_e = sum(e2e_step(args.warmup + s) for s in range(args.steps))
+        e1.record()
+        torch.cuda.synchronize()
+        ms_e = e0.elapsed_time(e1)
+        e2e = {"ms": ms_e, "iters": it_e, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)}
+
+    # ---- max over ranks, whole-job aggregate
+    units = float(E) * iters_done
+    if world > 1:
+        t = torch.tensor([ms, e2e["ms"] if e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        u = torch.tensor([units, float(E) * e2e["iters"] if e2e else 0.0], device=dev, dtype=torch.float64)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        ms, ms_e2e, units, units_e2e = float(t[0]), float(t[1]), float(u[0]), float(u[1])
+    else:
+        ms_e2e, units_e2e = (e2e["ms"], float(E) * e2e["iters"]) if e2e else (0.0, 0.0)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    else:
+        peak, peak_src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
+    tot_ns = sum(v["ns"] for v in prof.values()) or 1.0
+    top = max(prof, key=lambda k: prof[k]["ns"])
+    per_kernel = {}
+    for k, v in prof.items():
+        if v["calls"]:
+            dur = v["ns"] / v["calls"]
+            gbs = alg_bytes(k, n, p, nnz, M is not None) / dur
+            per_kernel[k] = {"share": v["ns"] / tot_ns, "us_per_launch": dur / 1e3, "launches": v["calls"],
+                             "alg_gbs": gbs, "frac": gbs / peak}
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tpath):
+        traffic = json.load(open(tpath)).get(args.workload, {}).get(top)
+    roofline = {"bound": "hbm", "kernel": top, "achieved": per_kernel[top]["alg_gbs"], "peak": peak, "unit": "GB/s",
+                "frac": per_kernel[top]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "bytes_per_launch": alg_bytes(top, n, p, nnz, M is not None),
+                "timing": "device %globaltimer marks inside the timed region (kernel + launch gap)",
+                "kernels": per_kernel, "device_ms_sum": tot_ns / 1e6}
+
+    line = {"metric": "pair-updates/sec per MM iteration", "value": units / (ms / 1e3), "unit": "pair-updates/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "n": n, "p": p, "k": wl.k, "pairs": E, "nnz": nnz,
+                       "iters_per_step": args.iters, "gamma": "50-value log grid walked with stride 5, warm-started",
+                       "cg_sweeps_per_iter": cg_per_it, "rho": stats["rho"], "kappa": 1e-2, "proj_tol": 1e-5,
+                       "l2": "working set (10 node arrays + CSR, %.0f MB) exceeds the 126 MB L2; no flush" %
+                             ((10 * n * p * 4 + 24 * nnz) / 1e6),
+                       "parallelism": "replicas" if world > 1 else "single", "knn_build_s": t_knn},
+            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline}
+    if e2e:
+        line["e2e"] = {"value": units_e2e / (ms_e2e / 1e3), "unit": "pair-updates/s",
+                       "h2d_bytes_per_step": e2e["h2d_bytes_per_step"], "d2h_bytes_per_step": e2e["d2h_bytes_per_step"],
+                       "ms_per_step": ms_e2e / args.steps}
+    if path:
+        line["path"] = path
+    if not args.no_cpu and world == 1:
+        try:
+            _, info, _ = oracle_sample(args, 1, 0)
+            line["cpu_baseline"] = info
+        except Exception as ex:  # the baseline is reported, never required for the GPU number
+            line["cpu_baseline"] = {"value": None, "unit": "pair-updates/s", "cores": os.cpu_count(), "kind": "oracle",
+                                    "sample": f"failed: {ex}"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -137,6 +137,14 @@ int cc_get_history(cc_handle* h, double* phi_out, double* d_out, int32_t cap, in
 int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, double* f_gamma,
                  double* min_margin);
 
+/* Live per-kernel device time of the MM iteration, accumulated over every cc_solve since
+ * cc_create / cc_reset_profile.  ns_out[5] (HOST doubles), calls_out[5] (HOST): index 0 k_rhs (a1),
+ * 1 k_cg_spmv (a2), 2 k_cg_update (a2), 3 k_norm (a3+a6), 4 k_update (a5+a4).  Measured on the device:
+ * the block that finishes a kernel last reads %globaltimer and the interval since the previous kernel
+ * finished (= this kernel plus its launch gap) is charged to it.  Either pointer may be NULL. */
+int cc_get_profile(cc_handle* h, double* ns_out, int64_t* calls_out);
+int cc_reset_profile(cc_handle* h);
+
 /* Back to the cold start (S4); snapshots are dropped. */
 int cc_reset(cc_handle* h);
 

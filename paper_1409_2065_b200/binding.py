@@ -23,7 +23,8 @@ _lib = ctypes.CDLL(LIB_PATH)
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
 SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
-           "cc_get_U", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_reset", "cc_get_counts",
+           "cc_get_U", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
+           "cc_reset", "cc_get_counts",
            "cc_last_error", "cc_destroy")
 
 
@@ -49,6 +50,8 @@ _lib.cc_clusters.argtypes = [_vp, _i32, _vp, _i32, _P(_i32)]
 _lib.cc_get_history.argtypes = [_vp, _vp, _vp, _i32, _P(_i32)]
 _lib.cc_get_stats.argtypes = [_vp, _P(_dbl), _P(_dbl), _P(_i64), _P(_dbl), _P(_dbl)]
 _lib.cc_reset.argtypes = [_vp]
+_lib.cc_get_profile.argtypes = [_vp, _vp, _vp]
+_lib.cc_reset_profile.argtypes = [_vp]
 _lib.cc_get_counts.argtypes = [_vp, _P(_i64), _P(_i64), _P(_i64)]
 _lib.cc_last_error.argtypes = [_vp]
 _lib.cc_last_error.restype = ctypes.c_char_p
@@ -142,6 +145,20 @@ def cc_get_stats(h, f_gamma=False, min_margin=False):
             "f_gamma": fg.value if f_gamma else None, "min_margin": mm.value if min_margin else None}
 
 
+KERNEL_NAMES = ("k_rhs", "k_cg_spmv", "k_cg_update", "k_norm", "k_update")
+
+
+def cc_get_profile(h):
+    ns = np.zeros(5)
+    calls = np.zeros(5, dtype=np.int64)
+    _check(_lib.cc_get_profile(h, ns.ctypes.data_as(_vp), calls.ctypes.data_as(_vp)), h)
+    return {k: {"ns": float(ns[i]), "calls": int(calls[i])} for i, k in enumerate(KERNEL_NAMES)}
+
+
+def cc_reset_profile(h):
+    _check(_lib.cc_reset_profile(h), h)
+
+
 def cc_reset(h):
     _check(_lib.cc_reset(h), h)
 
@@ -160,6 +177,19 @@ def cc_destroy(h):
     _lib.cc_destroy(h)
 
 
+class _DevArray:
+    """Zero-copy view of a library-owned device array (CUDA array interface) for torch.as_tensor."""
+
+    def __init__(self, ptr, count, typestr):
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": typestr, "data": (ptr, False), "version": 3}
+
+
+def _wrap(ptr, count, typestr, dev):
+    if count == 0:
+        return torch.empty(0, dtype={"<i8": torch.int64, "<i4": torch.int32, "<f4": torch.float32}[typestr], device=dev)
+    return torch.as_tensor(_DevArray(ptr, count, typestr), device=dev)
+
+
 def cc_knn_weights(n, p, X, mask, k, phi, normalize=False):
     """Returns (rowptr int64, col int32, w fp32) as torch device tensors (copies; the library's
     arrays are released with cc_free_graph before returning)."""
@@ -168,13 +198,9 @@ def cc_knn_weights(n, p, X, mask, k, phi, normalize=False):
     _check(_lib.cc_knn_weights(n, p, _ptr(X), _ptr(mask), k, phi, 1 if normalize else 0, ctypes.byref(rp),
                                ctypes.byref(cl), ctypes.byref(ww), ctypes.byref(nnz), _stream()))
     dev = X.device
-    rowptr = torch.empty(n + 1, dtype=torch.int64, device=dev)
-    col = torch.empty(nnz.value, dtype=torch.int32, device=dev)
-    w = torch.empty(nnz.value, dtype=torch.float32, device=dev)
-    cudart = torch.cuda.cudart()
-    cudart.cudaMemcpy(rowptr.data_ptr(), rp.value, rowptr.numel() * 8, 3)
-    if nnz.value:
-        cudart.cudaMemcpy(col.data_ptr(), cl.value, nnz.value * 4, 3)
-        cudart.cudaMemcpy(w.data_ptr(), ww.value, nnz.value * 4, 3)
+    rowptr = _wrap(rp.value, n + 1, "<i8", dev).clone()
+    col = _wrap(cl.value, nnz.value, "<i4", dev).clone()
+    w = _wrap(ww.value, nnz.value, "<f4", dev).clone()
+    torch.cuda.synchronize(dev)
     _lib.cc_free_graph(rp, cl, ww)
     return rowptr, col, w

@@ -8,7 +8,8 @@
 
 #include "cc_internal.h"
 
-static thread_local char g_err[256] = "";
+thread_local char cc_g_err[256] = "";
+#define g_err cc_g_err
 
 extern "C" {
 
@@ -125,6 +126,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
         int rc = ccs_solve_eager(h, maxit);
         if (rc != CC_OK) return rc;
     }
+    for (int k = 0; k < 8; ++k) { h->prof_ns[k] += S->prof_ns[k]; h->prof_calls[k] += S->prof_calls[k]; }
     if (iters_out) *iters_out = S->mm_iter;
     if (phi_out) *phi_out = S->phi;
     if (S->cg_failed) {
@@ -238,6 +240,22 @@ int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, do
     if (proj_iters) *proj_iters = h->sc_host->cg_total;
     if (f_gamma) { int rc = ccu_fgamma(h, f_gamma); if (rc != CC_OK) return rc; }
     if (min_margin) { int rc = ccu_min_margin(h, min_margin); if (rc != CC_OK) return rc; }
+    return CC_OK;
+}
+
+int cc_get_profile(cc_handle* h, double* ns_out, int64_t* calls_out) {
+    if (!h) return CC_EINVAL;
+    for (int k = 0; k < 5; ++k) {
+        if (ns_out) ns_out[k] = (double)h->prof_ns[k];
+        if (calls_out) calls_out[k] = (int64_t)h->prof_calls[k];
+    }
+    return CC_OK;
+}
+
+int cc_reset_profile(cc_handle* h) {
+    if (!h) return CC_EINVAL;
+    memset(h->prof_ns, 0, sizeof(h->prof_ns));
+    memset(h->prof_calls, 0, sizeof(h->prof_calls));
     return CC_OK;
 }
 

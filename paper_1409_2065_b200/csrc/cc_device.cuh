@@ -86,4 +86,19 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
     return threadIdx.x == 0;
 }
 
+
+__device__ __forceinline__ unsigned long long global_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+// Called by one thread when kernel `id` has finished all its work (see cc_scal::t_last).
+template <typename S>
+__device__ __forceinline__ void prof_mark(S* sc, int id) {
+    const unsigned long long now = global_ns();
+    if (sc->t_last) { sc->prof_ns[id] += now - sc->t_last; sc->prof_calls[id] += 1; }
+    sc->t_last = now;
+}
+
 }  // namespace

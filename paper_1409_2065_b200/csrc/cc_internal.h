@@ -41,6 +41,11 @@ struct cc_scal {
     long long cg_total;   // inner iterations over the whole solve
     // last-block tickets (one per reducing kernel)
     unsigned int ticket[8];
+    // live per-kernel timing: the block that finishes a kernel last reads %globaltimer; the interval
+    // since the previous kernel's end (kernel + launch gap) is charged to this kernel
+    unsigned long long t_last;
+    unsigned long long prof_ns[8];
+    unsigned long long prof_calls[8];
 };
 
 // Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
@@ -95,6 +100,7 @@ struct cc_handle {
     cudaGraphConditionalHandle cond_outer, cond_inner;   // 0 while launching eagerly
     cudaGraph_t graph;
     long long launches;
+    unsigned long long prof_ns[8], prof_calls[8];   // accumulated over solves (cc_get_profile)
     int grid_nodes, grid_rows, grid_edges;   // launch sizes, fixed per handle (determinism)
     char err[256];
 };
@@ -120,6 +126,9 @@ int ccu_min_margin(cc_handle* h, double* margin_out);   // min | ||b|| - thr | /
 void ccu_free(cc_handle* h);
 // ---- cc_clusters.cu -----------------------------------------------------------------------------------
 int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host);
+
+// message of the last failing handle-less call on this thread (cc_create, cc_knn_weights)
+extern thread_local char cc_g_err[256];
 
 #define CC_CUDA(h, call)                                                                  \
     do {                                                                                  \

@@ -93,6 +93,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
         const int active = tot[0] > th * th ? 1 : 0;
         sc->cg_active = active;
         if (loop) cudaGraphSetConditional(loop, active);
+        prof_mark(sc, 0);
     }
 }
 
@@ -159,6 +160,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
         sc->cg_delta = del;
         sc->cg_beta = beta;
         sc->cg_alpha = alpha;
+        prof_mark(sc, 1);
     }
 }
 
@@ -211,6 +213,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nch
         else if (k >= sc->cg_maxit) { active = 0; sc->cg_failed = 1; }
         sc->cg_active = active;
         if (loop) cudaGraphSetConditional(loop, active);
+        prof_mark(sc, 2);
     }
 }
 
@@ -325,6 +328,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
         sc->mm_iter = m + 1;
         sc->stop_pending = stop;
         if (outer) cudaGraphSetConditional(outer, stop ? 0 : 1);
+        prof_mark(sc, 3);
     }
 }
 
@@ -340,7 +344,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
                                                         const float* __restrict__ A, float* __restrict__ U,
                                                         float* __restrict__ Z, float* __restrict__ Ap,
                                                         const float* __restrict__ w, const float* __restrict__ nb2,
-                                                        float* __restrict__ s, float* __restrict__ vn, const cc_scal* sc) {
+                                                        float* __restrict__ s, float* __restrict__ vn, cc_scal* sc) {
     if (!sc->mm_active) return;
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -371,6 +375,14 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
         const float sn = nb <= thr ? 0.f : 1.f - thr / nb;
         s[e] = sn;
         vn[e] = sn * nb;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&sc->ticket[6], 1u) == gridDim.x - 1) {
+            sc->ticket[6] = 0u;
+            prof_mark(sc, 4);
+        }
     }
 }
 

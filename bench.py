@@ -56,6 +56,7 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-path", action="store_true", help="skip the full gamma-path wall time")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--eager", action="store_true", help="plain stream launches instead of the CUDA graph (for ncu)")
     return ap.parse_args()
 
 
@@ -154,6 +155,19 @@ def alg_bytes(kernel, n, p, nnz, masked):
     }[kernel]
 
 
+def aggregate(dist, dev, times_ms, units):
+    """Whole-job numbers from per-rank ones: MAX of the device times, SUM of the units processed.
+    `dist` is torch.distributed (any backend) or None for a single process."""
+    if dist is None:
+        return [float(t) for t in times_ms], [float(u) for u in units]
+    import torch
+    t = torch.tensor(times_ms, device=dev, dtype=torch.float64)
+    u = torch.tensor(units, device=dev, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return [float(x) for x in t], [float(x) for x in u]
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -207,7 +221,7 @@ def run_ours(args):
     nnz = int(col.numel())
     E = nnz // 2
 
-    h = B.cc_create(n, p, X, M, rowptr, col, w, B.cc_default_params())
+    h = B.cc_create(n, p, X, M, rowptr, col, w, B.cc_default_params(use_graph=0 if args.eager else 1))
     for s in range(args.warmup):
         B.cc_solve(h, gamma_for_step(args.workload, s), 0.0, args.iters)
     B.cc_reset_profile(h)
@@ -283,14 +297,9 @@ def run_ours(args):
 
     # ---- max over ranks, whole-job aggregate
     units = float(E) * iters_done
-    if world > 1:
-        t = torch.tensor([ms, e2e["ms"] if e2e else 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        u = torch.tensor([units, float(E) * e2e["iters"] if e2e else 0.0], device=dev, dtype=torch.float64)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        ms, ms_e2e, units, units_e2e = float(t[0]), float(t[1]), float(u[0]), float(u[1])
-    else:
-        ms_e2e, units_e2e = (e2e["ms"], float(E) * e2e["iters"]) if e2e else (0.0, 0.0)
+    units_e = float(E) * e2e["iters"] if e2e else 0.0
+    (ms, ms_e2e), (units, units_e2e) = aggregate(dist if world > 1 else None, dev,
+                                                 [ms, e2e["ms"] if e2e else 0.0], [units, units_e])
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

@@ -38,7 +38,7 @@ int cc_create(cc_handle** out, int64_t n, int64_t p, const float* X, const uint8
     cc_default_params(&P);
     if (prm) P = *prm;
     const bool dense = P.dense != 0;
-    if (n < 1 || p < 1 || !X || !w || (!dense && (!rowptr || !col)) || n > 2147483647LL / 2 || p > (1LL << 28)) {
+    if (n < 1 || p < 1 || !X || (dense && !w) || (!dense && !rowptr) || n > 2147483647LL / 2 || p > (1LL << 28)) {
         snprintf(g_err, sizeof(g_err), "cc_create: bad size or NULL pointer (n=%lld p=%lld)", (long long)n, (long long)p);
         return CC_EINVAL;
     }

@@ -69,6 +69,7 @@ struct cc_handle {
     // graph (symmetric CSR)
     int32_t* rowptr;                  // n+1 (nnz < 2^31 enforced)
     int32_t* rowup;                   // n: first entry of row i with col > i (rows are sorted)
+    int32_t* order;                   // n: rows by decreasing degree (processing order of the gather kernels)
     int32_t* col;                     // nnz
     int32_t* peer;                    // nnz: index of the reverse entry
     float* w;                         // nnz

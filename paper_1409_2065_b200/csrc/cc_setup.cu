@@ -64,6 +64,57 @@ __global__ void k_check_graph(int n, const int* __restrict__ rowptr, const int* 
     }
 }
 
+
+// Processing order for the row-gather kernels: rows sorted by decreasing degree (stable in the row
+// index, hence deterministic).  A grid-stride walk over this order hands every row group the same mix
+// of heavy and light rows (longest-processing-time-first), which removes the end-of-kernel wait on the
+// hub rows of a k-NN graph.  One block: histogram, scan, then a stable scatter chunk by chunk.
+#define CC_DEGBINS 4096
+__global__ void __launch_bounds__(1024) k_degree_order(int n, const int* __restrict__ rowptr, int* __restrict__ order) {
+    __shared__ int cursor[CC_DEGBINS];
+    __shared__ int wsum[32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int b = tid; b < CC_DEGBINS; b += 1024) cursor[b] = 0;
+    __syncthreads();
+    for (int i = tid; i < n; i += 1024) atomicAdd(&cursor[min(rowptr[i + 1] - rowptr[i], CC_DEGBINS - 1)], 1);
+    __syncthreads();
+    // exclusive scan over bins taken from the highest degree down: thread t owns bins 4t .. 4t+3 of the reversed axis
+    int loc[4], tot = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { loc[q] = cursor[CC_DEGBINS - 1 - (tid * 4 + q)]; tot += loc[q]; }
+    int inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int v = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += v; }
+    if (lane == 31) wsum[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        int v = wsum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const int u = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += u; }
+        wsum[lane] = v;
+    }
+    __syncthreads();
+    int run = inc - tot + (wid ? wsum[wid - 1] : 0);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) { cursor[CC_DEGBINS - 1 - (tid * 4 + q)] = run; run += loc[q]; }
+    __syncthreads();
+    // stable scatter: chunks of 1024 rows in index order, warps of a chunk one after the other
+    for (int base = 0; base < n; base += 1024) {
+        const int i = base + tid;
+        const int b = i < n ? min(rowptr[i + 1] - rowptr[i], CC_DEGBINS - 1) : -1 - lane;  // unique dummy keys
+        const unsigned same = __match_any_sync(0xffffffffu, b);
+        const int rank = __popc(same & ((1u << lane) - 1u));
+        for (int w2 = 0; w2 < 32; ++w2) {
+            if (wid == w2 && i < n) {
+                order[cursor[b] + rank] = i;
+            }
+            __syncthreads();
+            if (wid == w2 && i < n && rank == 0) cursor[b] += __popc(same);
+            __syncthreads();
+        }
+    }
+}
+
 // Complete graph given as an n x n matrix: expand to the symmetric CSR the kernels walk.
 __global__ void k_dense_to_csr(int n, const float* __restrict__ W, int* __restrict__ rowptr, int* __restrict__ col,
                                float* __restrict__ w, int* flag) {
@@ -292,10 +343,13 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
         CC_TRY(read_flag(h, &f));
         if (f || nnz64 < 0 || nnz64 > 2147483647LL) return flag_to_error(h, f | F_ROWPTR);
         h->nnz = nnz64;
+        if (nnz64 > 0 && (!col || !w)) { snprintf(h->err, sizeof(h->err), "col or w is NULL but rowptr[n] > 0"); return CC_EINVAL; }
         CC_TRY(dmalloc(h, &h->col, (size_t)h->nnz));
         CC_TRY(dmalloc(h, &h->w, (size_t)h->nnz));
-        CC_CUDA(h, cudaMemcpyAsync(h->col, col, (size_t)h->nnz * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
-        CC_CUDA(h, cudaMemcpyAsync(h->w, w, (size_t)h->nnz * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        if (h->nnz > 0) {
+            CC_CUDA(h, cudaMemcpyAsync(h->col, col, (size_t)h->nnz * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+            CC_CUDA(h, cudaMemcpyAsync(h->w, w, (size_t)h->nnz * sizeof(float), cudaMemcpyDeviceToDevice, st));
+        }
     }
     h->npairs = h->nnz / 2;
     CC_TRY(dmalloc(h, &h->peer, (size_t)h->nnz));
@@ -306,6 +360,8 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
         if (g2 > cap) g2 = cap;
         k_check_graph<<<(int)g2, 256, 0, st>>>((int)n, h->rowptr, h->col, h->w, h->peer, h->rowup, h->dinv, h->dflag);
     }
+    CC_TRY(dmalloc(h, &h->order, (size_t)n));
+    k_degree_order<<<1, 1024, 0, st>>>((int)n, h->rowptr, h->order);
     // ---- data ----
     const size_t nl = (size_t)n * h->ld;
     CC_TRY(dmalloc(h, &h->X, nl));
@@ -390,7 +446,7 @@ int ccu_min_margin(cc_handle* h, double* margin_out) {
 void ccu_free(cc_handle* h) {
     void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Wv, h->Uc, h->mask, h->colmean, h->rowptr,
                     h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->sc, h->part,
-                    h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank};
+                    h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order};
     for (void* q : ptrs)
         if (q) cudaFree(q);
     if (h->sc_host) cudaFreeHost(h->sc_host);

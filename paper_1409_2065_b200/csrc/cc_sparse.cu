@@ -27,7 +27,7 @@ namespace {
 // (I+L) z to get the residual of the warm start z.
 // ---------------------------------------------------------------------------------------------
 template <int G>
-__global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, const int* __restrict__ rowptr,
+__global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, const int* __restrict__ order, const int* __restrict__ rowptr,
                                                      const int* __restrict__ col, const float* __restrict__ s,
                                                      const float* __restrict__ dinv, const float* __restrict__ Ap,
                                                      const float* __restrict__ Z, const float* __restrict__ U,
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
     const long long items = (long long)n * nchunk;
     double acc_g[1] = {0.0};
     for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
-        const int i = (int)(it / nchunk);
+        const int i = __ldg(order + (int)(it / nchunk));
         const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
         const bool valid = c0 < ld;
         const size_t oi = (size_t)i * ld + (valid ? c0 : 0);
@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
 // The last block turns (gamma, delta) into the CG step sizes (Chronopoulos & Gear recurrences).
 // ---------------------------------------------------------------------------------------------
 template <int G>
-__global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchunk, const int* __restrict__ rowptr,
+__global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchunk, const int* __restrict__ order, const int* __restrict__ rowptr,
                                                          const int* __restrict__ col, const float* __restrict__ Uc,
                                                          float* __restrict__ Wv, cc_scal* sc, double* part) {
     if (!sc->mm_active || !sc->cg_active) return;
@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
     const long long items = (long long)n * nchunk;
     double acc_g[1] = {0.0};
     for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
-        const int i = (int)(it / nchunk);
+        const int i = __ldg(order + (int)(it / nchunk));
         const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
         const bool valid = c0 < ld;
         const size_t oi = (size_t)i * ld + (valid ? c0 : 0);
@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nch
 // coefficients of the two updates.  `outer` = the MM WHILE node's handle in graph mode, else 0.
 // ---------------------------------------------------------------------------------------------
 template <int G>
-__global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, long long nnz,
+__global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, long long nnz, const int* __restrict__ order,
                                                       const int* __restrict__ rowptr, const int* __restrict__ rowup,
                                                       const int* __restrict__ col, const int* __restrict__ peer,
                                                       const float* __restrict__ w, const float* __restrict__ s,
@@ -241,7 +241,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
     const long long items = (long long)n * nchunk;
     double acc_g[3] = {0.0, 0.0, 0.0};  // dist^2, loss, penalty
     for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
-        const int i = (int)(it / nchunk);
+        const int i = __ldg(order + (int)(it / nchunk));
         const int chunk = (int)(it % nchunk);
         const int c0 = chunk * 4 * G + gl * 4;
         const bool valid = c0 < ld;
@@ -442,12 +442,12 @@ static cudaGraphConditionalHandle g_outer(const cc_handle* h) { return h->cond_o
 void ccs_begin_iter(cc_handle* h) { k_begin_iter<<<1, 1, 0, h->stream>>>(h->sc); }
 
 void ccs_rhs(cc_handle* h) {
-    CC_DISPATCH_G(h, k_rhs, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->rowptr, h->col, h->s, h->dinv, h->Ap,
+    CC_DISPATCH_G(h, k_rhs, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->order, h->rowptr, h->col, h->s, h->dinv, h->Ap,
                   h->Z, h->U, h->R, h->Uc, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART, g_inner(h));
 }
 
 void ccs_cg_spmv(cc_handle* h) {
-    CC_DISPATCH_G(h, k_cg_spmv, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->rowptr, h->col, h->Uc, h->Wv,
+    CC_DISPATCH_G(h, k_cg_spmv, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->order, h->rowptr, h->col, h->Uc, h->Wv,
                   h->sc, h->part + 1 * CC_MAXBLK * CC_NPART);
 }
 
@@ -457,7 +457,7 @@ void ccs_cg_update(cc_handle* h) {
 }
 
 void ccs_norm(cc_handle* h) {
-    CC_DISPATCH_G(h, k_norm, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->rowptr, h->rowup,
+    CC_DISPATCH_G(h, k_norm, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->order, h->rowptr, h->rowup,
                   h->col, h->peer, h->w, h->s, h->vn, h->A, h->Ap, h->U, h->X, h->mask, h->nb2, h->sc,
                   h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, g_outer(h));
 }

@@ -1,0 +1,127 @@
+"""GPU tests of the boundary (-m gpu): input validation / error codes of include/cc_b200.h, and the
+a0 weight build against the oracle's brute-force eq. 8."""
+import numpy as np
+import pytest
+
+import helpers as H
+from paper_1409_2065_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1409_2065_b200 import binding
+    return binding
+
+
+def _dev(torch, a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+
+
+def _create(B, torch, n, p, X, mask, rowptr, col, w, **prm):
+    return B.cc_create(n, p, _dev(torch, X), _dev(torch, mask), _dev(torch, rowptr), _dev(torch, col), _dev(torch, w),
+                       B.cc_default_params(**prm))
+
+
+def test_validation_error_codes(B):
+    import torch
+    n, p = 4, 3
+    X = np.arange(12, dtype=np.float32).reshape(n, p)
+    # path 0-1, 1-2, 2-3
+    rowptr = np.array([0, 1, 3, 5, 6], np.int64)
+    col = np.array([1, 0, 2, 1, 3, 2], np.int32)
+    w = np.ones(6, np.float32)
+    h = _create(B, torch, n, p, X, None, rowptr, col, w)
+    assert B.cc_get_counts(h)["n_pairs"] == 3
+    with pytest.raises(B.CCError) as e:
+        B.cc_solve(h, -1.0, 0.0, 5)
+    assert e.value.code == B.CC_EINVAL
+    with pytest.raises(B.CCError) as e:
+        B.cc_solve(h, float("nan"), 0.0, 5)
+    assert e.value.code == B.CC_EINVAL
+    assert B.cc_solve(h, 1.0, 0.0, 0)[0] == 0
+    B.cc_destroy(h)
+
+    def fails(code, X=X, mask=None, rowptr=rowptr, col=col, w=w, n=n, p=p):
+        with pytest.raises(B.CCError) as e:
+            _create(B, torch, n, p, X, mask, rowptr, col, w)
+        assert e.value.code == code, (e.value.code, str(e.value))
+
+    w2 = w.copy(); w2[0] = 2.0
+    fails(B.CC_EGRAPH, w=w2)                                                   # w_ij != w_ji
+    fails(B.CC_EGRAPH, col=np.array([1, 0, 2, 1, 3, 3], np.int32))             # self loop / asymmetric
+    fails(B.CC_EGRAPH, col=np.array([1, 2, 0, 1, 3, 2], np.int32))             # unsorted row
+    fails(B.CC_EGRAPH, col=np.array([1, 0, 2, 1, 9, 2], np.int32))             # out of range
+    w3 = w.copy(); w3[0] = w3[1] = 0.0
+    fails(B.CC_EGRAPH, w=w3)                                                   # w <= 0
+    fails(B.CC_EGRAPH, rowptr=np.array([0, 2, 1, 5, 6], np.int64))             # rowptr not monotone
+    Xn = X.copy(); Xn[1, 1] = np.nan
+    fails(B.CC_EINVAL, X=Xn)
+    mk = np.ones((n, p), np.uint8); mk[:, 2] = 0
+    fails(B.CC_EMASK, mask=mk)                                                 # a column never observed
+    mk2 = np.ones((n, p), np.uint8); mk2[1, 1] = 0                             # NaN at a missing entry is ignored
+    h = _create(B, torch, n, p, Xn, mk2, rowptr, col, w)
+    B.cc_solve(h, 0.5, 0.0, 10)
+    U = torch.empty(n, p, device="cuda:0")
+    B.cc_get_U(h, -1, U)
+    assert torch.isfinite(U).all()
+    B.cc_destroy(h)
+    fails(B.CC_EINVAL, n=0)
+    with pytest.raises(B.CCError) as e:
+        B.cc_knn_weights(5, 2, _dev(torch, X[:, :2].copy()), None, 7, 1.0)
+    assert e.value.code == B.CC_EINVAL
+
+
+@pytest.mark.parametrize("name,kw,k,phi,norm", [("tiny", {}, 5, 0.5, False),
+                                                ("large_sparse", dict(n=3000, p=64, n_clusters=10), 10, 0.01, False),
+                                                ("large_sparse", dict(n=1000, p=21, n_clusters=5), 3, 0.02, True),
+                                                ("expression", dict(n=60, p=333), 10, 0.002, False)])
+def test_knn_weights_match_oracle(B, oracle, name, kw, k, phi, norm):
+    """a0 against brute-force eq. 8: same neighbour sets (the data are continuous: no exact ties), same
+    CSR, weights to fp32 rounding; includes the masked distance rule S11 and normalisation S8."""
+    import torch
+    wl = synth.make(name, **kw)
+    X64 = wl.X.astype(np.float64)
+    ei, ej, w, _ = oracle.knn_graph(X64, wl.mask, k, phi, normalize=norm)
+    rp, cl, ww = oracle.to_csr(wl.n, ei, ej, w)
+    rowptr, col, wg = B.cc_knn_weights(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), k, phi, normalize=norm)
+    assert np.array_equal(rowptr.cpu().numpy(), rp)
+    assert np.array_equal(col.cpu().numpy(), cl)
+    assert np.abs(wg.cpu().numpy() - ww).max() <= 2e-5 * ww.max()
+    # feeds cc_create unchanged (symmetric, sorted, w_ij == w_ji bitwise)
+    h = B.cc_create(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), rowptr, col, wg, None)
+    assert B.cc_get_counts(h)["n_pairs"] == len(ei)
+    B.cc_destroy(h)
+
+
+def test_full_size_large_sparse_properties(B):
+    """configs[3] at full size, in the launch configuration bench.py times: properties that hold at
+    any size -- Phi non-increasing, column sums of U equal those of X when nothing
+    is missing (pin P6: 1'L = 0), shrink factors in [0,1], and U rows of fused pairs O(kappa)-close."""
+    import torch
+    wl = synth.make("large_sparse")
+    X = _dev(torch, wl.X)
+    rowptr, col, w = B.cc_knn_weights(wl.n, wl.p, X, None, wl.k, 0.01)
+    h = B.cc_create(wl.n, wl.p, X, None, rowptr, col, w, None)
+    for g in (3.0, 30.0):
+        it, phi, _ = B.cc_solve(h, g, 0.0, 30)
+        ph, dd = B.cc_get_history(h)
+        assert it == 30 and np.all(np.diff(ph) <= 1e-6 * np.abs(ph[:-1]))
+        assert np.all(dd > 0)
+    U = torch.empty(wl.n, wl.p, device="cuda:0")
+    B.cc_get_U(h, -1, U)
+    cs_u, cs_x = U.double().sum(0).cpu().numpy(), X.double().sum(0).cpu().numpy()
+    # exact for an exact projection; the CG stop rule (proj_tol) leaves a column-sum residual of this order
+    rel = np.abs(cs_u - cs_x).max() / X.double().abs().sum(0).max().item()
+    assert rel <= 1e-4, rel
+    lab = torch.empty(wl.n, dtype=torch.int32, device="cuda:0")
+    _, k = B.cc_clusters(h, -1, lab)
+    assert 1 <= k <= wl.n
+    # labels are canonical: label of a node <= its index rank, first node has label 0, labels are dense
+    l = lab.cpu().numpy()
+    assert l[0] == 0 and l.max() == k - 1 and np.array_equal(np.unique(l), np.arange(k))
+    B.cc_destroy(h)

@@ -1,0 +1,239 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (paper_1409_2065_b200.binding),
+against the fp64 oracle on the same seeded inputs.  Bar (BASELINE.json north_star): relative
+Frobenius error <= 1e-4 after a fixed iteration count, identical cluster labels at every gamma."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import helpers as H
+from paper_1409_2065_b200 import synth
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-4   # north_star: "relative Frobenius error <= 1e-4 (fp32)"
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1409_2065_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+def _run_path(B, torch, prob, gammas, iters, ref, **prm):
+    h = H.gpu_create(B, torch, prob, **prm)
+    n, p = prob["n"], prob["p"]
+    U = torch.empty(n, p, device="cuda:0")
+    lab = torch.empty(n, dtype=torch.int32, device="cuda:0")
+    out = []
+    try:
+        for g, r in zip(gammas, ref):
+            it, phi, _ = B.cc_solve(h, g, 0.0, iters)
+            assert it == iters
+            B.cc_get_U(h, -1, U)
+            _, k = B.cc_clusters(h, -1, lab)
+            ph, dd = B.cc_get_history(h)
+            err = H.relerr(U.cpu().numpy().astype(np.float64), r["U"])
+            assert err <= TOL, (g, err)
+            assert k == r["nclusters"], (g, k, r["nclusters"])
+            assert np.array_equal(lab.cpu().numpy(), r["labels"]), g
+            # Phi and d histories: d_m^2 - eps is a sum of squares of O(kappa) differences of O(1) fp32 numbers,
+            # so d carries ~1e-4 relative fp32 noise; U itself is held to 1e-4
+            assert np.allclose(ph, r["phi"][:len(ph)], rtol=1e-4), g
+            assert np.allclose(dd, r["d"][:len(dd)], rtol=5e-4), g
+            # MM descent property up to fp32 noise in the state
+            assert np.all(np.diff(ph) <= 1e-6 * np.abs(ph[:-1])), g
+            out.append((err, k))
+    finally:
+        B.cc_destroy(h)
+    return out
+
+
+def test_tiny_path_matches_oracle_and_golden(B, torch_, oracle):
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    gold = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "tiny_path.json")))
+    gammas, iters = gold["gammas"], gold["iters"]
+    assert len(prob["ei"]) == gold["n_pairs"]
+    ref = H.oracle_path(oracle, prob, gammas, iters)
+    out = _run_path(B, torch_, prob, gammas, iters, ref)
+    assert [k for _, k in out] == [g["nclusters"] for g in gold["per_gamma"]]
+
+
+def test_tiny_long_run(B, torch_, oracle):
+    """One long run (fp32 drift grows with the iteration count)."""
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    ref = H.oracle_path(oracle, prob, [300.0], 3000)
+    _run_path(B, torch_, prob, [300.0], 3000, ref)
+
+
+def test_expression_like_masked(B, torch_, oracle):
+    """Missing data, rows wider than one 128-column chunk with a ragged tail."""
+    wl = synth.make("expression", n=40, p=301)
+    prob = H.build_problem(oracle, wl)
+    gammas = [0.5, 5.0, 50.0]
+    ref = H.oracle_path(oracle, prob, gammas, 100)
+    _run_path(B, torch_, prob, gammas, 100, ref)
+
+
+def test_large_sparse_reduced(B, torch_, oracle):
+    """Same generator as configs[3] at n=3000: several row blocks, hubs, CG-projection oracle."""
+    wl = synth.make("large_sparse", n=3000, p=64, n_clusters=10)
+    prob = H.build_problem(oracle, wl)
+    gammas = [1.0, 30.0, 300.0]
+    ref = H.oracle_path(oracle, prob, gammas, 100, proj_method=1)
+    out = _run_path(B, torch_, prob, gammas, 100, ref)
+    assert out[-1][1] < 100   # the path really fuses
+
+
+@pytest.mark.parametrize("n,p,deg,miss", [(50, 7, 3.0, 0.0), (33, 130, 4.0, 0.15), (200, 2, 6.0, 0.0),
+                                          (17, 1, 2.0, 0.0)])
+def test_ragged_shapes_random_graphs(B, torch_, oracle, n, p, deg, miss):
+    """p not a multiple of 4, p < 4, p spanning two chunks; disconnected graphs with isolated nodes."""
+    rng = np.random.default_rng(n * 1000 + p)
+    X = (rng.normal(size=(n, p)) + 2.0 * rng.integers(0, 3, size=(n, 1))).astype(np.float32)
+    ei, ej, w = synth.random_graph(n, deg, seed=n + p)
+    mask = None
+    if miss > 0:
+        mask = (rng.random(size=(n, p)) >= miss).astype(np.uint8)
+        mask[0, :] = 1
+    w32 = w.astype(np.float32)
+    rowptr, col, wc = oracle.to_csr(n, ei, ej, w32.astype(np.float64))
+    prob = {"X64": X.astype(np.float64), "mask": mask, "ei": ei, "ej": ej, "w64": w32.astype(np.float64),
+            "rowptr": rowptr, "col": col, "wcsr32": wc.astype(np.float32), "n": n, "p": p}
+    gammas = [0.3, 3.0, 30.0]
+    ref = H.oracle_path(oracle, prob, gammas, 120)
+    _run_path(B, torch_, prob, gammas, 120, ref)
+
+
+def test_empty_graph_and_gamma_zero(B, torch_, oracle):
+    """No pairs at all: U = X after any number of iterations (gamma irrelevant);
+    gamma = 0 on a real graph: U = X (pin P1)."""
+    torch = torch_
+    n, p = 20, 5
+    rng = np.random.default_rng(1)
+    X = rng.normal(size=(n, p)).astype(np.float32)
+    prob = {"X64": X.astype(np.float64), "mask": None, "n": n, "p": p, "rowptr": np.zeros(n + 1, np.int64),
+            "col": np.zeros(0, np.int32), "wcsr32": np.zeros(0, np.float32)}
+    h = H.gpu_create(B, torch, prob)
+    B.cc_solve(h, 5.0, 0.0, 30)
+    U = torch.empty(n, p, device="cuda:0")
+    B.cc_get_U(h, -1, U)
+    assert np.abs(U.cpu().numpy() - X).max() <= 1e-6
+    lab = torch.empty(n, dtype=torch.int32, device="cuda:0")
+    _, k = B.cc_clusters(h, -1, lab)
+    assert k == n and np.array_equal(lab.cpu().numpy(), np.arange(n))
+    B.cc_destroy(h)
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    h = H.gpu_create(B, torch, prob)
+    B.cc_solve(h, 0.0, 0.0, 25)
+    U = torch.empty(wl.n, wl.p, device="cuda:0")
+    B.cc_get_U(h, -1, U)
+    assert np.abs(U.cpu().numpy() - wl.X).max() <= 1e-5
+    B.cc_destroy(h)
+
+
+def test_graph_and_eager_launch_modes_are_bit_identical_and_deterministic(B, torch_, oracle):
+    torch = torch_
+    wl = synth.make("large_sparse", n=2000, p=64, n_clusters=8)
+    prob = H.build_problem(oracle, wl)
+    outs = []
+    for use_graph in (1, 0, 1):
+        h = H.gpu_create(B, torch, prob, use_graph=use_graph)
+        for g in (5.0, 80.0):
+            B.cc_solve(h, g, 0.0, 40)
+        U = torch.empty(wl.n, wl.p, device="cuda:0")
+        B.cc_get_U(h, -1, U)
+        outs.append(U.cpu().numpy().copy())
+        B.cc_destroy(h)
+    assert np.array_equal(outs[0], outs[1])
+    assert np.array_equal(outs[0], outs[2])
+
+
+def test_stop_rule_matches_oracle(B, torch_, oracle):
+    """tol > 0 (reading S3): the GPU stops at (nearly) the oracle's iteration."""
+    torch = torch_
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    X, m = prob["X64"], prob["mask"]
+    U0, V0 = oracle.cold_start(X, m, prob["ei"], prob["ej"])
+    g, tol = 200.0, 1e-4
+    rho, eps = oracle.default_rho_eps(X, m, prob["w64"], g)
+    r = oracle.mm(X, m, prob["ei"], prob["ej"], prob["w64"], g, rho, eps, U0, V0, 5000, tol=tol, min_it=10)
+    h = H.gpu_create(B, torch, prob)
+    it, phi, _ = B.cc_solve(h, g, tol, 5000)
+    st = B.cc_get_stats(h)
+    B.cc_destroy(h)
+    assert abs(st["rho"] - rho) <= 1e-6 * rho and abs(st["eps"] - eps) <= 1e-6 * eps
+    assert 10 <= it < 5000 and abs(it - r["iters"]) <= max(2, r["iters"] // 50), (it, r["iters"])
+    assert abs(phi - r["phi"][-1]) <= 1e-4 * abs(phi)
+
+
+def test_cc_path_snapshots(B, torch_, oracle):
+    torch = torch_
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    gammas = [float(g) for g in synth.gamma_grid(1.0, 1e3, 6)]
+    ref = H.oracle_path(oracle, prob, gammas, 80)
+    h = H.gpu_create(B, torch, prob)
+    its, phis = B.cc_path(h, gammas, 0.0, 80)
+    assert its == [80] * 6
+    U = torch.empty(wl.n, wl.p, device="cuda:0")
+    Uh = torch.empty(wl.n, wl.p)
+    lab = torch.empty(wl.n, dtype=torch.int32)
+    for gi, r in enumerate(ref):
+        B.cc_get_U(h, gi, U)
+        B.cc_get_U(h, gi, Uh)
+        assert np.array_equal(U.cpu().numpy(), Uh.numpy())
+        assert H.relerr(Uh.numpy().astype(np.float64), r["U"]) <= TOL
+        _, k = B.cc_clusters(h, gi, lab)
+        assert k == r["nclusters"] and np.array_equal(lab.numpy(), r["labels"])
+        assert abs(phis[gi] - r["phi"][-1]) <= 1e-5 * abs(phis[gi])
+    with pytest.raises(B.CCError) as e:
+        B.cc_get_U(h, 6, U)
+    assert e.value.code == B.CC_ESTATE
+    # f_gamma of eq. 1 at the last U against the oracle's plain definition
+    st = B.cc_get_stats(h, f_gamma=True, min_margin=True)
+    f_ref = oracle.objective(prob["X64"], None, prob["ei"], prob["ej"], prob["w64"], gammas[-1], ref[-1]["U"])
+    assert abs(st["f_gamma"] - f_ref) <= 1e-4 * abs(f_ref)
+    assert st["min_margin"] >= 0.0
+    B.cc_reset(h)
+    B.cc_get_U(h, -1, U)
+    assert np.array_equal(U.cpu().numpy(), wl.X)
+    B.cc_destroy(h)
+
+
+def test_dense_mode_complete_graph(B, torch_, oracle):
+    """prm.dense = 1: w is the n x n matrix (genotype-like shape, reduced)."""
+    torch = torch_
+    wl = synth.make("genotype", n=20, p=1000)
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    gammas = [0.05, 0.5, 5.0]
+    ref = H.oracle_path(oracle, prob, gammas, 100)
+    dev = torch.device("cuda:0")
+    h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
+                    B.cc_default_params(dense=1))
+    U = torch.empty(n, wl.p, device=dev)
+    lab = torch.empty(n, dtype=torch.int32, device=dev)
+    for g, r in zip(gammas, ref):
+        B.cc_solve(h, g, 0.0, 100)
+        B.cc_get_U(h, -1, U)
+        _, k = B.cc_clusters(h, -1, lab)
+        assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL
+        assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"])
+    B.cc_destroy(h)

@@ -221,7 +221,7 @@ def run_ours(args):
     nnz = int(col.numel())
     E = nnz // 2
 
-    h = B.cc_create(n, p, X, M, rowptr, col, w, B.cc_default_params(use_graph=0 if args.eager else 1))
+    h = B.cc_create(n, p, X, M, rowptr, col, w, B.cc_default_params(use_graph=0 if args.eager else 1, reserved0=int(os.environ.get('CC_TUNE', '0'))))
     for s in range(args.warmup):
         B.cc_solve(h, gamma_for_step(args.workload, s), 0.0, args.iters)
     B.cc_reset_profile(h)

@@ -34,6 +34,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
                                                      float* __restrict__ R, float* __restrict__ Uc, float* __restrict__ A,
                                                      cc_scal* sc, double* part, cudaGraphConditionalHandle loop) {
     if (!sc->mm_active) return;
+    constexpr int UNR = G < 4 ? G : 4;   // 2 x UNR gathers in flight per lane (8 was slower: registers)
     const unsigned gm = group_mask<G>();
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -52,24 +53,23 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
             const int cj = e < re ? __ldg(col + e) : i;   // padding entries point at the own row with s = 1:
             const float sv = e < re ? __ldg(s + e) : 1.f; // 1*(a_i - a_i) - (z_i - z_i) = 0 exactly
             const int cnt = min(G, re - base);
-            for (int t = 0; t < cnt; t += 4) {
-                int j[4];
-                float sj[4];
-                float4 aj[4], zj[4];
+            for (int t = 0; t < cnt; t += UNR) {
+                int j[UNR];
+                float sj[UNR];
+                float4 aj[UNR], zj[UNR];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < UNR; ++q) {
                     j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
                     sj[q] = __shfl_sync(gm, sv, (t + q) & (G - 1), G);
-                    if (G < 4 && t + q >= G) { j[q] = i; sj[q] = 1.f; }
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < UNR; ++q) {
                     const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
                     aj[q] = ld4s(Ap + oj);
                     zj[q] = ld4s(Z + oj);
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) acc = fma4(sj[q], api - aj[q], acc) - (zi - zj[q]);
+                for (int q = 0; q < UNR; ++q) acc = fma4(sj[q], api - aj[q], acc) - (zi - zj[q]);
             }
         }
         acc = acc - (zi - ui);
@@ -107,6 +107,9 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
                                                          const int* __restrict__ col, const float* __restrict__ Uc,
                                                          float* __restrict__ Wv, cc_scal* sc, double* part) {
     if (!sc->mm_active || !sc->cg_active) return;
+    // all gathers of a batch of G entries (16 at most) are issued before the first is consumed: the kernel
+    // is bound by L2 gather latency, not bandwidth (profiles/r1a), so memory-level parallelism is the lever
+    constexpr int UNR = G < 16 ? G : 16;
     const unsigned gm = group_mask<G>();
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -124,19 +127,19 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
             const int e = base + gl;
             const int cj = e < re ? __ldg(col + e) : -1;
             const int cnt = min(G, re - base);
-            for (int t = 0; t < cnt; t += 4) {
-                int j[4];
-                float4 uj[4];
+            for (int t = 0; t < cnt; t += UNR) {
+                int j[UNR];
+                float4 uj[UNR];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < UNR; ++q) {
                     j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
-                    if (G < 4 && t + q >= G) j[q] = -1;
+                    if (UNR > G && t + q >= G) j[q] = -1;
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q)
+                for (int q = 0; q < UNR; ++q)
                     uj[q] = j[q] >= 0 ? ld4s(Uc + (size_t)j[q] * ld + (valid ? c0 : 0)) : f4(0.f);
 #pragma unroll
-                for (int q = 0; q < 4; ++q) nsum = nsum + uj[q];
+                for (int q = 0; q < UNR; ++q) nsum = nsum + uj[q];
             }
         }
         if (valid) {
@@ -163,6 +166,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
         prof_mark(sc, 1);
     }
 }
+
 
 // ---------------------------------------------------------------------------------------------
 // a2  k_cg_update.  p = uc + beta p;  s = w + beta s;  A += alpha p;  r -= alpha s;  uc = D^-1 r;
@@ -235,6 +239,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
                                                       float* __restrict__ nb2, cc_scal* sc, double* part,
                                                       double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer) {
     if (!sc->mm_active) return;
+    constexpr int UNR = G < 8 ? G : 8;
     const unsigned gm = group_mask<G>();
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -265,24 +270,23 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
             const int cj = e < re ? __ldg(col + e) : i;
             const float sv = e < re ? __ldg(s + e) : 0.f;
             const int cnt = min(G, re - base);
-            for (int t = 0; t < cnt; t += 4) {
-                int j[4];
-                float sj[4], nbq[4];
-                float4 aj[4], apj[4];
+            for (int t = 0; t < cnt; t += UNR) {
+                int j[UNR];
+                float sj[UNR], nbq[UNR];
+                float4 aj[UNR], apj[UNR];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < UNR; ++q) {
                     j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
                     sj[q] = __shfl_sync(gm, sv, (t + q) & (G - 1), G);
-                    if (G < 4 && t + q >= G) { j[q] = i; sj[q] = 0.f; }
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < UNR; ++q) {
                     const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
                     aj[q] = ld4s(A + oj);
                     apj[q] = ld4s(Ap + oj);
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < UNR; ++q) {
                     const float4 b = ai - aj[q];
                     const float4 vb = fma4(sj[q], api - apj[q], f4(0.f)) - b;
                     nbq[q] = vf * dot4(b, b);
@@ -291,11 +295,11 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
 #pragma unroll
                 for (int o = G / 2; o > 0; o >>= 1) {
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) nbq[q] += __shfl_xor_sync(gm, nbq[q], o, G);
+                    for (int q = 0; q < UNR; ++q) nbq[q] += __shfl_xor_sync(gm, nbq[q], o, G);
                 }
                 if (gl == 0) {
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) {
+                    for (int q = 0; q < UNR; ++q) {
                         const int eq = base + t + q;
                         if (t + q < cnt) {
                             nb2[(size_t)chunk * nnz + eq] = nbq[q];

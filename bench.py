@@ -148,8 +148,8 @@ def alg_bytes(kernel, n, p, nnz, masked):
     row, npb = 4 * p, 4 * n * p
     return {
         "k_rhs": nnz * (2 * row + 8) + 6 * npb + 4 * n,
-        "k_cg_spmv": nnz * (row + 4) + 2 * npb + 4 * n,
-        "k_cg_update": 11 * npb + 4 * n,
+        "k_cg_spmv": nnz * (row + 4) + 5 * npb + 4 * n,      # gather + own uc, p, s in; p, s out
+        "k_cg_update": 7 * npb + 4 * n,                      # p, s, A, r in; A, r, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
         "k_update": 6 * npb + (n * p if masked else 0) + 16 * nnz,
     }[kernel]

@@ -105,8 +105,14 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
 template <int G>
 __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchunk, const int* __restrict__ order, const int* __restrict__ rowptr,
                                                          const int* __restrict__ col, const float* __restrict__ Uc,
-                                                         float* __restrict__ Wv, cc_scal* sc, double* part) {
+                                                         float* __restrict__ Pv, float* __restrict__ Sv, cc_scal* sc,
+                                                         double* part) {
     if (!sc->mm_active || !sc->cg_active) return;
+    // beta depends only on the previous kernel's reduction, so the search-direction recurrences
+    // p = uc + beta p, s = w + beta s are applied here, on the row this group owns, and w is never stored:
+    // this kernel waits on gather latency and has DRAM bandwidth to spare, k_cg_update has none.
+    const bool first = sc->cg_iter == 0;
+    const float beta = first ? 0.f : (float)(sc->cg_gamma / sc->cg_gamma_old);
     // all gathers of a batch of G entries (16 at most) are issued before the first is consumed: the kernel
     // is bound by L2 gather latency, not bandwidth (profiles/r1a), so memory-level parallelism is the lever
     constexpr int UNR = G < 16 ? G : 16;
@@ -145,7 +151,13 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
         if (valid) {
             const float dg = 1.f + (float)(re - rs);
             const float4 wv = dg * ui - nsum;
-            st4(Wv + oi, wv);
+            float4 pv = ui, sv = wv;
+            if (!first) {
+                pv = fma4(beta, ld4s(Pv + oi), pv);
+                sv = fma4(beta, ld4s(Sv + oi), sv);
+            }
+            st4(Pv + oi, pv);
+            st4(Sv + oi, sv);
             acc_g[0] += (double)dot4(wv, ui);
         }
     }
@@ -157,7 +169,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
             beta = 0.0;
             alpha = gam / del;
         } else {
-            beta = gam / sc->cg_gamma_old;
+            beta = (double)(float)(gam / sc->cg_gamma_old);   // the value the rows used
             alpha = gam / (del - beta * gam / sc->cg_alpha);
         }
         sc->cg_delta = del;
@@ -169,35 +181,26 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
 
 
 // ---------------------------------------------------------------------------------------------
-// a2  k_cg_update.  p = uc + beta p;  s = w + beta s;  A += alpha p;  r -= alpha s;  uc = D^-1 r;
-// gamma' = (r, uc).  The last block applies the stop rule of the projection (cc_b200.h proj_tol).
+// a2  k_cg_update.  A += alpha p;  r -= alpha s;  uc = D^-1 r;  gamma' = (r, uc)   (p, s from k_cg_spmv).  The last block applies the stop rule of the projection (cc_b200.h proj_tol).
 // `loop` is the inner WHILE node's handle in graph mode (0 in eager mode).
 // ---------------------------------------------------------------------------------------------
 template <int G>
 __global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nchunk, const float* __restrict__ dinv,
-                                                           float* __restrict__ Uc, const float* __restrict__ Wv,
-                                                           float* __restrict__ Pv, float* __restrict__ Sv,
-                                                           float* __restrict__ A, float* __restrict__ R, cc_scal* sc,
+                                                           float* __restrict__ Uc, const float* __restrict__ Pv,
+                                                           const float* __restrict__ Sv, float* __restrict__ A, float* __restrict__ R, cc_scal* sc,
                                                            double* part, cudaGraphConditionalHandle loop) {
     if (!sc->mm_active || !sc->cg_active) return;
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
     const long long items = (long long)n * nchunk;
-    const bool first = sc->cg_iter == 0;
-    const float alpha = (float)sc->cg_alpha, beta = (float)sc->cg_beta;
+    const float alpha = (float)sc->cg_alpha;
     double acc_g[1] = {0.0};
     for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
         const int i = (int)(it / nchunk);
         const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
         if (c0 >= ld) continue;
         const size_t oi = (size_t)i * ld + c0;
-        float4 pv = ld4s(Uc + oi), sv = ld4s(Wv + oi);
-        if (!first) {
-            pv = fma4(beta, ld4s(Pv + oi), pv);
-            sv = fma4(beta, ld4s(Sv + oi), sv);
-        }
-        st4(Pv + oi, pv);
-        st4(Sv + oi, sv);
+        const float4 pv = ld4s(Pv + oi), sv = ld4s(Sv + oi);
         st4(A + oi, fma4(alpha, pv, ld4s(A + oi)));
         const float4 r = fma4(-alpha, sv, ld4s(R + oi));
         const float4 uc = dinv[i] * r;
@@ -451,12 +454,12 @@ void ccs_rhs(cc_handle* h) {
 }
 
 void ccs_cg_spmv(cc_handle* h) {
-    CC_DISPATCH_G(h, k_cg_spmv, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->order, h->rowptr, h->col, h->Uc, h->Wv,
-                  h->sc, h->part + 1 * CC_MAXBLK * CC_NPART);
+    CC_DISPATCH_G(h, k_cg_spmv, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->order, h->rowptr, h->col, h->Uc, h->Pv,
+                  h->Sv, h->sc, h->part + 1 * CC_MAXBLK * CC_NPART);
 }
 
 void ccs_cg_update(cc_handle* h) {
-    CC_DISPATCH_G(h, k_cg_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->dinv, h->Uc, h->Wv, h->Pv,
+    CC_DISPATCH_G(h, k_cg_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->dinv, h->Uc, h->Pv,
                   h->Sv, h->A, h->R, h->sc, h->part + 2 * CC_MAXBLK * CC_NPART, g_inner(h));
 }
 

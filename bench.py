@@ -151,7 +151,7 @@ def alg_bytes(kernel, n, p, nnz, masked):
         "k_cg_spmv": nnz * (row + 4) + 5 * npb + 4 * n,      # gather + own uc, p, s in; p, s out
         "k_cg_update": 7 * npb + 4 * n,                      # p, s, A, r in; A, r, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
-        "k_update": 6 * npb + (n * p if masked else 0) + 16 * nnz,
+        "k_update": 8 * npb + (n * p if masked else 0) + 16 * nnz,
     }[kernel]
 
 

@@ -394,7 +394,7 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
     h->sumw2 = two[1];
 
     // ---- state ----
-    float** node_arrays[] = {&h->U, &h->A, &h->Ap, &h->Z, &h->R, &h->Pv, &h->Sv, &h->Uc};
+    float** node_arrays[] = {&h->U, &h->A, &h->Ap, &h->Z, &h->R, &h->Pv, &h->Sv, &h->Uc, &h->Dl};
     for (float** a : node_arrays) {
         CC_TRY(dmalloc(h, a, nl));
         CC_CUDA(h, cudaMemsetAsync(*a, 0, nl * sizeof(float), st));
@@ -444,7 +444,7 @@ int ccu_min_margin(cc_handle* h, double* margin_out) {
 }
 
 void ccu_free(cc_handle* h) {
-    void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Wv, h->Uc, h->mask, h->colmean, h->rowptr,
+    void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Dl, h->Uc, h->mask, h->colmean, h->rowptr,
                     h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->sc, h->part,
                     h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order};
     for (void* q : ptrs)

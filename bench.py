@@ -39,7 +39,11 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-GRID = {"large_sparse": (1.0, 1000.0, 50), "tiny": (1e-3, 1e3, 20), "expression": (0.05, 50.0, 40)}
+GRID = {"large_sparse": (1.0, 1000.0, 50), "tiny": (1e-3, 1e3, 20), "expression": (0.05, 50.0, 40),
+        "genotype": (1.0, 100.0, 50), "dense_weight": (1.0, 100.0, 30)}
+CPU_SAMPLE = {"large_sparse": lambda a: {"n": a.cpu_n}, "genotype": lambda a: {"p": 20000},
+              "dense_weight": lambda a: {"n": 512}, "tiny": lambda a: {}, "expression": lambda a: {}}
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 flop/FMA x max clock (B200_PROFILING.md table)
 
 
 def parse():
@@ -113,8 +117,7 @@ def oracle_sample(args, steps, warmup):
     from oracle import oracle as O
     from paper_1409_2065_b200 import synth
     O.build()
-    kw = {"n": args.cpu_n} if args.workload == "large_sparse" else {}
-    wl = synth.make(args.workload, **kw)
+    wl = synth.make(args.workload, **CPU_SAMPLE[args.workload](args))
     X = wl.X.astype(np.float64)
     if wl.phi_rule == "fixed":
         phi = wl.phi
@@ -122,7 +125,10 @@ def oracle_sample(args, steps, warmup):
         si, sj = synth.sample_pairs(wl.n, 200_000, wl.seed)
         d2 = O.pair_dist2(X, wl.mask, si, sj)
         phi = 1.0 / float(np.median(d2[np.isfinite(d2)]))
-    ei, ej, w, _ = O.knn_graph(X, wl.mask, wl.k, phi)
+    if wl.graph == "knn":
+        ei, ej, w, _ = O.knn_graph(X, wl.mask, wl.k, phi)
+    else:
+        ei, ej, w, _ = O.complete_graph(X, wl.mask, phi)
     U, V = O.cold_start(X, wl.mask, ei, ej)
     times = []
     for s in range(warmup + steps):
@@ -137,12 +143,12 @@ def oracle_sample(args, steps, warmup):
     tot = float(sum(times))
     val = len(ei) * args.cpu_iters * len(times) / tot
     info = {"value": val, "unit": "pair-updates/s", "cores": cpu_count_used(O), "kind": "oracle",
-            "sample": f"{args.workload} generator at n={wl.n} (|E|={len(ei)}), {len(times)} step(s) x "
+            "sample": f"{args.workload} generator at n={wl.n}, p={wl.p} (|E|={len(ei)}), {len(times)} step(s) x "
                       f"{args.cpu_iters} MM iterations, fp64, explicit V, CG projection to 1e-13"}
     return val, info, tot / max(1, len(times))
 
 
-def alg_bytes(kernel, n, p, nnz, masked):
+def alg_bytes(kernel, n, p, nnz, masked, dense=False):
     """Algorithmic (no-reuse) bytes one launch of `kernel` must move: every gathered neighbour row is
     counted once per directed entry, own rows and outputs once per node ('roofline')."""
     row, npb = 4 * p, 4 * n * p
@@ -151,8 +157,18 @@ def alg_bytes(kernel, n, p, nnz, masked):
         "k_cg_spmv": nnz * (row + 4) + 5 * npb + 4 * n,      # gather + own uc, p, s in; p, s out
         "k_cg_update": 7 * npb + 4 * n,                      # p, s, A, r in; A, r, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
-        "k_update": 8 * npb + (n * p if masked else 0) + 16 * nnz,
+        "k_update": (5 * npb if dense else 8 * npb + 16 * nnz) + (n * p if masked else 0),
+        # dense mode (nnz = n(n-1)): matrices are n x n fp32
+        "kd_proj": 4 * n * n + 5 * npb + (n * p if masked else 0),
+        "kd_pairs": 2 * npb + (n * n // 2) * 12 + 4 * n * n,
+        "kd_edges": 16 * n * n,
     }[kernel]
+
+
+def alg_flops(kernel, n, p):
+    """Floating-point operations one launch must do (FMA = 2): the contraction S.A' and the direct pair
+    differences (sub, sub, 3 FMA per pair and column).  Zero for the streaming kernels."""
+    return {"kd_proj": 2.0 * n * n * p, "kd_pairs": 8.0 * (n * (n - 1) / 2) * p}.get(kernel, 0.0)
 
 
 def aggregate(dist, dev, times_ms, units):
@@ -213,15 +229,23 @@ def run_ours(args):
         si, sj = synth.sample_pairs(n, 200_000, wl.seed)
         d = X[torch.from_numpy(si).to(dev)] - X[torch.from_numpy(sj).to(dev)]
         phi = 1.0 / float((d * d).sum(1).median())
+    dense = wl.graph == "complete"
     t0 = time.perf_counter()
-    rowptr, col, w = B.cc_knn_weights(n, p, X, M, wl.k, phi)
+    if dense:
+        Wd = B.cc_dense_weights(n, p, X, M, phi)
+        rowptr = col = None
+        w = Wd
+        nnz = n * (n - 1)
+    else:
+        rowptr, col, w = B.cc_knn_weights(n, p, X, M, wl.k, phi)
+        nnz = int(col.numel())
     torch.cuda.synchronize()
     t_knn = time.perf_counter() - t0
-    rowptr_h, col_h, w_h = rowptr.cpu().pin_memory(), col.cpu().pin_memory(), w.cpu().pin_memory()
-    nnz = int(col.numel())
+    if not dense:
+        rowptr_h, col_h, w_h = rowptr.cpu().pin_memory(), col.cpu().pin_memory(), w.cpu().pin_memory()
     E = nnz // 2
-
-    h = B.cc_create(n, p, X, M, rowptr, col, w, B.cc_default_params(use_graph=0 if args.eager else 1, reserved0=int(os.environ.get('CC_TUNE', '0'))))
+    prm = B.cc_default_params(use_graph=0 if args.eager else 1, dense=1 if dense else 0)
+    h = B.cc_create(n, p, X, M, rowptr, col, w, prm)
     for s in range(args.warmup):
         B.cc_solve(h, gamma_for_step(args.workload, s), 0.0, args.iters)
     B.cc_reset_profile(h)
@@ -247,6 +271,7 @@ def run_ours(args):
     stats = B.cc_get_stats(h)
     launches = B.cc_get_counts(h)["launches"] - launches0
     cg_per_it = prof["k_cg_spmv"]["calls"] / max(1, iters_done)
+    prof = {k: v for k, v in prof.items() if v["calls"]}
 
     # ---- full gamma path (rank 0, N = 1): the other half of BASELINE.json's metric
     path = None
@@ -270,14 +295,20 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         Uh = torch.empty(n, p, dtype=torch.float32).pin_memory()
-        h2d = Xh.numel() * 4 + (Mh.numel() if Mh is not None else 0) + rowptr_h.numel() * 8 + col_h.numel() * 4 + w_h.numel() * 4
+        h2d = Xh.numel() * 4 + (Mh.numel() if Mh is not None else 0)
+        if not dense:
+            h2d += rowptr_h.numel() * 8 + col_h.numel() * 4 + w_h.numel() * 4
         d2h = Uh.numel() * 4
 
         def e2e_step(s):
             Xd = Xh.to(dev, non_blocking=True)
             Md = None if Mh is None else Mh.to(dev, non_blocking=True)
-            rp, cl, ww = rowptr_h.to(dev, non_blocking=True), col_h.to(dev, non_blocking=True), w_h.to(dev, non_blocking=True)
-            hh = B.cc_create(n, p, Xd, Md, rp, cl, ww, None)
+            if dense:   # the weights are rebuilt on the device from X: part of the user's call sequence
+                rp = cl = None
+                ww = B.cc_dense_weights(n, p, Xd, Md, phi)
+            else:
+                rp, cl, ww = rowptr_h.to(dev, non_blocking=True), col_h.to(dev, non_blocking=True), w_h.to(dev, non_blocking=True)
+            hh = B.cc_create(n, p, Xd, Md, rp, cl, ww, B.cc_default_params(dense=1 if dense else 0))
             it, _, _ = B.cc_solve(hh, gamma_for_step(args.workload, s), 0.0, args.iters)
             B.cc_get_U(hh, -1, Uh)
             B.cc_destroy(hh)
@@ -316,16 +347,21 @@ def run_ours(args):
     for k, v in prof.items():
         if v["calls"]:
             dur = v["ns"] / v["calls"]
-            gbs = alg_bytes(k, n, p, nnz, M is not None) / dur
+            gbs = alg_bytes(k, n, p, nnz, M is not None, dense) / dur
+            tfl = alg_flops(k, n, p) / dur / 1e3
             per_kernel[k] = {"share": v["ns"] / tot_ns, "us_per_launch": dur / 1e3, "launches": v["calls"],
-                             "alg_gbs": gbs, "frac": gbs / peak}
+                             "alg_gbs": gbs, "frac": gbs / peak, "alg_tflops": tfl, "frac_fp32_alu": tfl / FP32_PEAK_TFLOPS}
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(args.workload, {}).get(top)
-    roofline = {"bound": "hbm", "kernel": top, "achieved": per_kernel[top]["alg_gbs"], "peak": peak, "unit": "GB/s",
-                "frac": per_kernel[top]["frac"], "traffic": traffic, "peak_source": peak_src,
-                "bytes_per_launch": alg_bytes(top, n, p, nnz, M is not None),
+    alu_bound = per_kernel[top]["frac_fp32_alu"] > per_kernel[top]["frac"]
+    roofline = {"bound": "alu" if alu_bound else "hbm", "kernel": top,
+                "achieved": per_kernel[top]["alg_tflops" if alu_bound else "alg_gbs"],
+                "peak": FP32_PEAK_TFLOPS if alu_bound else peak, "unit": "TFLOP/s" if alu_bound else "GB/s",
+                "frac": per_kernel[top]["frac_fp32_alu" if alu_bound else "frac"], "traffic": traffic,
+                "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts; FFMA path)" if alu_bound else peak_src,
+                "bytes_per_launch": alg_bytes(top, n, p, nnz, M is not None, dense), "flops_per_launch": alg_flops(top, n, p),
                 "timing": "device %globaltimer marks inside the timed region (kernel + launch gap)",
                 "kernels": per_kernel, "device_ms_sum": tot_ns / 1e6}
 
@@ -335,8 +371,8 @@ def run_ours(args):
             "config": {"workload": args.workload, "n": n, "p": p, "k": wl.k, "pairs": E, "nnz": nnz,
                        "iters_per_step": args.iters, "gamma": "50-value log grid walked with stride 5, warm-started",
                        "cg_sweeps_per_iter": cg_per_it, "rho": stats["rho"], "kappa": 1e-2, "proj_tol": 1e-5,
-                       "l2": "working set (10 node arrays + CSR, %.0f MB) exceeds the 126 MB L2; no flush" %
-                             ((10 * n * p * 4 + 24 * nnz) / 1e6),
+                       "l2": "working set (node arrays + pair arrays, %.0f MB) vs 126 MB L2; no flush" %
+                             ((10 * n * p * 4 + (16 * n * n if dense else 24 * nnz)) / 1e6),
                        "parallelism": "replicas" if world > 1 else "single", "knn_build_s": t_knn},
             "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline}
     if e2e:

@@ -84,6 +84,13 @@ int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, in
                    int32_t normalize, int64_t** rowptr, int32_t** col, float** w, int64_t* nnz,
                    void* stream);
 
+/* a0 for complete graphs (k = n-1): W_out (DEVICE, caller-owned, n*n fp32 row-major) receives
+ * w_ij = exp(-phi ||x_i - x_j||^2) for i != j and 0 on the diagonal, symmetric bit for bit; same distance
+ * rules and normalisation as cc_knn_weights.  The result feeds cc_create with prm.dense = 1.  X, mask:
+ * DEVICE.  Synchronises `stream`. */
+int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, float phi, int32_t normalize,
+                     float* W_out, void* stream);
+
 /* Release the three arrays cc_knn_weights returned (NULLs are ignored). */
 void cc_free_graph(int64_t* rowptr, int32_t* col, float* w);
 
@@ -138,8 +145,9 @@ int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, do
                  double* min_margin);
 
 /* Live per-kernel device time of the MM iteration, accumulated over every cc_solve since
- * cc_create / cc_reset_profile.  ns_out[5] (HOST doubles), calls_out[5] (HOST): index 0 k_rhs (a1),
- * 1 k_cg_spmv (a2), 2 k_cg_update (a2), 3 k_norm (a3+a6), 4 k_update (a5+a4).  Measured on the device:
+ * cc_create / cc_reset_profile.  ns_out[8] (HOST doubles), calls_out[8] (HOST): index 0 k_rhs (a1),
+ * 1 k_cg_spmv (a2), 2 k_cg_update (a2), 3 k_norm (a3+a6), 4 k_update (a5+a4); dense mode (a9): 5 kd_proj
+ * (with the column means), 6 kd_pairs, 7 kd_edges.  Measured on the device:
  * the block that finishes a kernel last reads %globaltimer and the interval since the previous kernel
  * finished (= this kernel plus its launch gap) is charged to it.  Either pointer may be NULL. */
 int cc_get_profile(cc_handle* h, double* ns_out, int64_t* calls_out);

@@ -22,7 +22,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
-SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
+SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_dense_weights", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
            "cc_get_U", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
            "cc_last_error", "cc_destroy")
@@ -40,6 +40,7 @@ _P = ctypes.POINTER
 _lib.cc_default_params.argtypes = [_P(cc_params)]
 _lib.cc_knn_weights.argtypes = [_i64, _i64, _vp, _vp, _i32, ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp),
                                 _P(_i64), _vp]
+_lib.cc_dense_weights.argtypes = [_i64, _i64, _vp, _vp, ctypes.c_float, _i32, _vp, _vp]
 _lib.cc_free_graph.argtypes = [_vp, _vp, _vp]
 _lib.cc_free_graph.restype = None
 _lib.cc_create.argtypes = [_P(_vp), _i64, _i64, _vp, _vp, _vp, _vp, _vp, _P(cc_params), _vp]
@@ -145,12 +146,12 @@ def cc_get_stats(h, f_gamma=False, min_margin=False):
             "f_gamma": fg.value if f_gamma else None, "min_margin": mm.value if min_margin else None}
 
 
-KERNEL_NAMES = ("k_rhs", "k_cg_spmv", "k_cg_update", "k_norm", "k_update")
+KERNEL_NAMES = ("k_rhs", "k_cg_spmv", "k_cg_update", "k_norm", "k_update", "kd_proj", "kd_pairs", "kd_edges")
 
 
 def cc_get_profile(h):
-    ns = np.zeros(5)
-    calls = np.zeros(5, dtype=np.int64)
+    ns = np.zeros(8)
+    calls = np.zeros(8, dtype=np.int64)
     _check(_lib.cc_get_profile(h, ns.ctypes.data_as(_vp), calls.ctypes.data_as(_vp)), h)
     return {k: {"ns": float(ns[i]), "calls": int(calls[i])} for i, k in enumerate(KERNEL_NAMES)}
 
@@ -175,6 +176,13 @@ def cc_last_error(h=None) -> str:
 
 def cc_destroy(h):
     _lib.cc_destroy(h)
+
+
+def cc_dense_weights(n, p, X, mask, phi, normalize=False):
+    """All-pairs Gaussian weights as an (n, n) fp32 device tensor (for prm.dense = 1)."""
+    W = torch.empty(n, n, dtype=torch.float32, device=X.device)
+    _check(_lib.cc_dense_weights(n, p, _ptr(X), _ptr(mask), phi, 1 if normalize else 0, _ptr(W), _stream()))
+    return W
 
 
 class _DevArray:

@@ -116,14 +116,14 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
     }
     CC_CUDA(h, cudaMemcpyAsync(h->sc, S, sizeof(cc_scal), cudaMemcpyHostToDevice, h->stream));
     if (h->prm.use_graph) {
-        int rc = ccs_build_graph(h);
+        int rc = h->dense ? ccd_build_graph(h) : ccs_build_graph(h);
         if (rc != CC_OK) return rc;
         CC_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
         CC_CUDA(h, cudaMemcpyAsync(S, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
         CC_CUDA(h, cudaStreamSynchronize(h->stream));
-        h->launches += 3LL * S->mm_iter + 2LL * S->cg_total;
+        h->launches += h->dense ? 6LL * S->mm_iter : 3LL * S->mm_iter + 2LL * S->cg_total;
     } else {
-        int rc = ccs_solve_eager(h, maxit);
+        int rc = h->dense ? ccd_solve_eager(h, maxit) : ccs_solve_eager(h, maxit);
         if (rc != CC_OK) return rc;
     }
     for (int k = 0; k < 8; ++k) { h->prof_ns[k] += S->prof_ns[k]; h->prof_calls[k] += S->prof_calls[k]; }
@@ -238,6 +238,10 @@ int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, do
     if (rho) *rho = h->sc_host->rho;
     if (eps) *eps = h->sc_host->eps;
     if (proj_iters) *proj_iters = h->sc_host->cg_total;
+    if ((f_gamma || min_margin) && h->dense) {
+        snprintf(h->err, sizeof(h->err), "cc_get_stats: f_gamma / min_margin are not available in dense mode yet");
+        return CC_ESTATE;
+    }
     if (f_gamma) { int rc = ccu_fgamma(h, f_gamma); if (rc != CC_OK) return rc; }
     if (min_margin) { int rc = ccu_min_margin(h, min_margin); if (rc != CC_OK) return rc; }
     return CC_OK;
@@ -245,7 +249,7 @@ int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, do
 
 int cc_get_profile(cc_handle* h, double* ns_out, int64_t* calls_out) {
     if (!h) return CC_EINVAL;
-    for (int k = 0; k < 5; ++k) {
+    for (int k = 0; k < 8; ++k) {
         if (ns_out) ns_out[k] = (double)h->prof_ns[k];
         if (calls_out) calls_out[k] = (int64_t)h->prof_calls[k];
     }

@@ -87,7 +87,8 @@ int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host) {
     h->launches += 1;
     for (int round = 0; round < 100000; ++round) {
         CC_CUDA(h, cudaMemsetAsync(h->lab_flag, 0, sizeof(int), st));
-        k_lab_hook<<<grid, 256, 0, st>>>(n, h->rowptr, h->col, h->s, h->lab, h->lab_flag);
+        if (h->dense) ccd_lab_hook(h, h->lab_flag);
+        else k_lab_hook<<<grid, 256, 0, st>>>(n, h->rowptr, h->col, h->s, h->lab, h->lab_flag);
         k_lab_jump<<<grid, 256, 0, st>>>(n, h->lab);
         h->launches += 2;
         int changed = 0;

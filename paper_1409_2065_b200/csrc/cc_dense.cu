@@ -1,0 +1,591 @@
+// cc_dense.cu -- a9, the complete-graph ("dense weight") form of the MM iteration, sm_100a.
+//
+// With E = all pairs, L = n I - 1 1^T and the projection is closed form
+// (DESIGN.md / SURVEY P3):   A = U + g / (n+1),   g_i = sum_j s_ij (a'_i - a'_j) - sum_j (u_i - u_j)
+//                                                   = rowsum(S)_i a'_i - (S A')_i - n (u_i - ubar),
+// because 1^T g = 0.  So one iteration is two passes over pairs plus two streaming passes:
+//   kd_colmeans  column means of U and A' (centring: every formula below is translation invariant)
+//   kd_proj      a1+a2  the contraction S (A' - abar') tile by tile (S from HBM, n x n), A, ||U-A||^2, loss
+//   kd_pairs     a3+a6  ||b_ij||^2 and ||s_ij b'_ij - b_ij||^2 by direct differences over 64 x 64 pair tiles
+//                (optionally split over column ranges), d_m, Phi_m, stop rule
+//   k_update     a5     (the sparse file's kernel, node part only)
+//   kd_edges     a4     S, ||v|| from ||b||^2 and W, elementwise over the n x n matrices
+// This round the contraction runs on FP32 FFMA with 8x8 (or 4x4) register tiles; the tcgen05 3xTF32
+// version is the next step.  V (|E| x p: 34 GB at n=8192, p=256) is never formed.
+#include <cstdio>
+
+#include "cc_device.cuh"
+#include "cc_internal.h"
+
+namespace {
+
+// ---- column means of two node arrays, deterministic two-stage ------------------------------------
+__global__ void kd_colsum1(int n, int ld, int nslice, const float* __restrict__ U, const float* __restrict__ Ap,
+                           double* __restrict__ ps) {
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int sl = blockIdx.y;
+    if (c >= ld) return;
+    const int r0 = (int)((long long)n * sl / nslice), r1 = (int)((long long)n * (sl + 1) / nslice);
+    double su = 0.0, sa = 0.0;
+    for (int i = r0; i < r1; ++i) {
+        su += (double)U[(size_t)i * ld + c];
+        sa += (double)Ap[(size_t)i * ld + c];
+    }
+    ps[((size_t)sl * 2 + 0) * ld + c] = su;
+    ps[((size_t)sl * 2 + 1) * ld + c] = sa;
+}
+
+__global__ void kd_colsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ ubar,
+                           float* __restrict__ abar, const cc_scal* sc) {
+    if (!sc->mm_active) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ld) return;
+    double su = 0.0, sa = 0.0;
+    for (int sl = 0; sl < nslice; ++sl) {
+        su += ps[((size_t)sl * 2 + 0) * ld + c];
+        sa += ps[((size_t)sl * 2 + 1) * ld + c];
+    }
+    ubar[c] = (float)(su / n);
+    abar[c] = (float)(sa / n);
+}
+
+// ---- kd_proj ---------------------------------------------------------------------------------------
+// CTA tile: BI = 16 TM rows x C = 16 TN columns, 256 threads as 16 (rows) x 16 (columns), thread tile
+// TM x TN.  Loop over j in blocks of BJ = 32: stage S[I, J] (transposed) and A'[J, C] - abar in shared
+// memory, rank-1 updates in registers.  Rows / columns of a thread are interleaved in groups of 4 so that
+// every shared-memory read is a conflict-free 128-bit load.
+constexpr int BJ = 32;
+
+template <int TM, int TN>
+__global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __restrict__ S, const float* __restrict__ Ap,
+                                               const float* __restrict__ U, const float* __restrict__ X,
+                                               const uint8_t* __restrict__ mask, const float* __restrict__ ubar,
+                                               const float* __restrict__ abar, float* __restrict__ A, cc_scal* sc,
+                                               double* part) {
+    if (!sc->mm_active) return;
+    constexpr int BI = 16 * TM, C = 16 * TN;
+    __shared__ __align__(16) float St[BJ][BI];
+    __shared__ __align__(16) float At[BJ][C];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int i0 = blockIdx.y * BI, c0 = blockIdx.x * C;
+    float acc[TM][TN], rs[TM];
+#pragma unroll
+    for (int a = 0; a < TM; ++a) {
+        rs[a] = 0.f;
+#pragma unroll
+        for (int b = 0; b < TN; ++b) acc[a][b] = 0.f;
+    }
+    for (int j0 = 0; j0 < n; j0 += BJ) {
+        for (int t = tid; t < BI * BJ; t += 256) {      // S[i0+ii][j0+jj], jj fastest: 128-byte segments
+            const int jj = t % BJ, ii = t / BJ;
+            const int gi = i0 + ii, gj = j0 + jj;
+            St[jj][ii] = (gi < n && gj < n) ? __ldg(S + (size_t)gi * n + gj) : 0.f;
+        }
+        for (int t = tid; t < BJ * (C / 4); t += 256) {
+            const int c4 = t % (C / 4), jj = t / (C / 4);
+            const int gj = j0 + jj, gc = c0 + c4 * 4;
+            float4 v = f4(0.f);
+            if (gj < n && gc < ld) v = ld4s(Ap + (size_t)gj * ld + gc) - ld4s(abar + gc);
+            *reinterpret_cast<float4*>(&At[jj][c4 * 4]) = v;
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int jj = 0; jj < BJ; ++jj) {
+            float sv[TM], av[TN];
+#pragma unroll
+            for (int a4 = 0; a4 < TM / 4; ++a4) {
+                const float4 v = *reinterpret_cast<const float4*>(&St[jj][a4 * 64 + ty * 4]);
+                sv[a4 * 4 + 0] = v.x; sv[a4 * 4 + 1] = v.y; sv[a4 * 4 + 2] = v.z; sv[a4 * 4 + 3] = v.w;
+            }
+#pragma unroll
+            for (int b4 = 0; b4 < TN / 4; ++b4) {
+                const float4 v = *reinterpret_cast<const float4*>(&At[jj][b4 * 64 + tx * 4]);
+                av[b4 * 4 + 0] = v.x; av[b4 * 4 + 1] = v.y; av[b4 * 4 + 2] = v.z; av[b4 * 4 + 3] = v.w;
+            }
+#pragma unroll
+            for (int a = 0; a < TM; ++a) {
+                rs[a] += sv[a];
+#pragma unroll
+                for (int b = 0; b < TN; ++b) acc[a][b] = fmaf(sv[a], av[b], acc[a][b]);
+            }
+        }
+        __syncthreads();
+    }
+    // epilogue: a = u + [rowsum(S) (a' - abar) - S(A' - abar) - n (u - ubar)] / (n+1)
+    const float inv = 1.f / (float)(n + 1), fn = (float)n;
+    double red[2] = {0.0, 0.0};   // ||U - A||^2, observed loss
+#pragma unroll
+    for (int a = 0; a < TM; ++a) {
+        const int gi = i0 + (a / 4) * 64 + ty * 4 + (a % 4);
+        if (gi >= n) continue;
+#pragma unroll
+        for (int b4 = 0; b4 < TN / 4; ++b4) {
+            const int gc = c0 + b4 * 64 + tx * 4;
+            if (gc >= ld) continue;
+            const size_t o = (size_t)gi * ld + gc;
+            const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
+            const float4 sa = make_float4(acc[a][b4 * 4 + 0], acc[a][b4 * 4 + 1], acc[a][b4 * 4 + 2], acc[a][b4 * 4 + 3]);
+            const float4 g = (rs[a] * ap - sa) - fn * (u - ub);
+            const float4 dl = inv * g;
+            st4(A + o, u + dl);
+            float4 q = ld4s(X + o) - u;
+            if (mask) {
+                const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + o);
+                q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
+            }
+            red[0] += (double)dot4(dl, dl);
+            red[1] += (double)dot4(q, q);
+        }
+    }
+    double tot[2];
+    if (grid_reduce<2>(red, part, &sc->ticket[0], tot)) {
+        sc->dist2 = tot[0];
+        sc->loss = tot[1];
+        prof_mark(sc, 5);
+    }
+}
+
+// ---- kd_pairs --------------------------------------------------------------------------------------
+// One CTA = one 64 x 64 tile of pairs (I <= J) x one range of columns (blockIdx.y of `ksplit`).  Direct
+// differences (no Gram trick: a pair about to fuse has ||b|| far below ||a||, and the fused / not fused
+// decision is taken on ||b||):  nb2 += b^2,  dv += (s b' - b)^2  with b = a_i - a_j, b' = a'_i - a'_j.
+// Partial ||b||^2 go to NB2[ks][i][j] and [j][i]; kd_edges adds the ks slices in order.
+constexpr int PT = 64, PCK = 16;
+
+__global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ksplit, const float* __restrict__ A,
+                                                const float* __restrict__ Ap, const float* __restrict__ S,
+                                                const float* __restrict__ W, const float* __restrict__ VN,
+                                                float* __restrict__ NB2, cc_scal* sc, double* part, double* hist_phi,
+                                                double* hist_d, cudaGraphConditionalHandle outer, int init_only) {
+    if (!init_only && !sc->mm_active) return;
+    __shared__ float Ai[PT][PCK + 1], Aj[PT][PCK + 1], Pi[PT][PCK + 1], Pj[PT][PCK + 1];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    // tile index -> (I, J), I <= J, row-major over the upper triangle
+    int I = 0, rem = blockIdx.x;
+    while (rem >= ntile - I) { rem -= ntile - I; ++I; }
+    const int J = I + rem;
+    const int i0 = I * PT, j0 = J * PT;
+    const int ks = blockIdx.y;
+    const int cper = ((ld + ksplit - 1) / ksplit + PCK - 1) / PCK * PCK;
+    const int cb = ks * cper, ce = min(ld, cb + cper);
+    float sv[4][4], nb[4][4], dv[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int gi = i0 + ty * 4 + a, gj = j0 + tx + 16 * b;
+            sv[a][b] = (gi < n && gj < n && !init_only) ? __ldg(S + (size_t)gi * n + gj) : 0.f;
+            nb[a][b] = 0.f;
+            dv[a][b] = 0.f;
+        }
+    for (int c0 = cb; c0 < ce; c0 += PCK) {
+        for (int t = tid; t < PT * PCK; t += 256) {
+            const int r = t / PCK, c = t % PCK;
+            const int gc = c0 + c;
+            const bool vi = i0 + r < n && gc < ce, vj = j0 + r < n && gc < ce;
+            Ai[r][c] = vi ? A[(size_t)(i0 + r) * ld + gc] : 0.f;
+            Pi[r][c] = vi ? Ap[(size_t)(i0 + r) * ld + gc] : 0.f;
+            Aj[r][c] = vj ? A[(size_t)(j0 + r) * ld + gc] : 0.f;
+            Pj[r][c] = vj ? Ap[(size_t)(j0 + r) * ld + gc] : 0.f;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < PCK; ++c) {
+            float ai[4], aj[4], pi[4], pj[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) {
+                ai[a] = Ai[ty * 4 + a][c]; pi[a] = Pi[ty * 4 + a][c];
+                aj[a] = Aj[tx + 16 * a][c]; pj[a] = Pj[tx + 16 * a][c];
+            }
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const float bb = ai[a] - aj[b];
+                    const float tt = fmaf(sv[a][b], pi[a] - pj[b], -bb);
+                    nb[a][b] = fmaf(bb, bb, nb[a][b]);
+                    dv[a][b] = fmaf(tt, tt, dv[a][b]);
+                }
+        }
+        __syncthreads();
+    }
+    double red[2] = {0.0, 0.0};   // sum_{i<j} ||v - b||^2,  sum_{i<j} w ||v||
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int gi = i0 + ty * 4 + a, gj = j0 + tx + 16 * b;
+            if (gi < n && gj < n && gi != gj) {
+                float* out = NB2 + (size_t)ks * n * n;
+                if (I != J) { out[(size_t)gi * n + gj] = nb[a][b]; out[(size_t)gj * n + gi] = nb[a][b]; }
+                else out[(size_t)gi * n + gj] = nb[a][b];   // a diagonal tile holds both (i,j) and (j,i)
+                if (gi < gj) {
+                    red[0] += (double)dv[a][b];
+                    if (ks == 0 && !init_only)
+                        red[1] += (double)(__ldg(W + (size_t)gi * n + gj) * __ldg(VN + (size_t)gi * n + gj));
+                }
+            }
+        }
+    double tot[2];
+    if (grid_reduce<2>(red, part, &sc->ticket[3], tot)) {
+        if (!init_only) {
+            finish_iteration(sc, sc->dist2 + tot[0], sc->loss, tot[1], hist_phi, hist_d, outer);
+            prof_mark(sc, 6);
+        }
+    }
+}
+
+// ---- kd_edges: block soft-threshold over the n x n matrices ------------------
+__global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
+                                                float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, int init_only) {
+    if (!init_only && !sc->mm_active) return;
+    const long long nn = (long long)n * n;
+    const float cthr = sc->cthr;
+    // few slices: one thread per entry; many slices (small n, long rows): one warp per entry, lanes stride
+    // over the slices and combine with a fixed shuffle tree (deterministic either way)
+    const bool warp_per = ksplit >= 32;
+    const int lane = threadIdx.x & 31;
+    const long long nwork = (long long)gridDim.x * (warp_per ? blockDim.x / 32 : blockDim.x);
+    for (long long e = warp_per ? (long long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32
+                                : (long long)blockIdx.x * blockDim.x + threadIdx.x;
+         e < nn; e += nwork) {
+        const int i = (int)(e / n), j = (int)(e % n);
+        float q = 0.f;
+        if (warp_per) {
+            for (int k = lane; k < ksplit; k += 32) q += NB2[(size_t)k * nn + e];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+            if (lane) continue;
+        } else {
+            q = NB2[e];
+            for (int k = 1; k < ksplit; ++k) q += NB2[(size_t)k * nn + e];
+        }
+        float sn = 0.f, vn = 0.f;
+        if (i != j) {
+            const float nb = sqrtf(q);
+            if (init_only) { sn = 1.f; vn = nb; }
+            else {
+                const float thr = cthr * W[e];
+                sn = nb <= thr ? 0.f : 1.f - thr / nb;
+                vn = sn * nb;
+            }
+        }
+        S[e] = sn;
+        VN[e] = vn;
+    }
+    __syncthreads();
+    if (!init_only && threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&sc->ticket[6], 1u) == gridDim.x - 1) {
+            sc->ticket[6] = 0u;
+            prof_mark(sc, 7);
+        }
+    }
+}
+
+// dense-mode validation of W: symmetric, finite, > 0 off the diagonal
+__global__ void kd_check_w(int n, const float* __restrict__ W, int* flag) {
+    const long long nn = (long long)n * n, nt = (long long)gridDim.x * blockDim.x;
+    int bad = 0;
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += nt) {
+        const int i = (int)(e / n), j = (int)(e % n);
+        if (i == j) continue;
+        const float a = W[e];
+        if (!(a > 0.f) || isinf(a)) bad |= 64;                 // F_WBAD
+        if (a != W[(size_t)j * n + i]) bad |= 32;              // F_WASYM
+    }
+    if (bad) atomicOr(flag, bad);
+}
+
+// cluster read-out on the dense S matrix: same hooking as cc_clusters.cu, neighbours = all j with s_ij = 0
+__global__ void kd_lab_hook(int n, const float* __restrict__ S, int* lab, int* changed) {
+    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // one warp per row
+    const int lane = threadIdx.x & 31;
+    if (i >= n) return;
+    const int li = lab[i];
+    int m = li;
+    for (int j = lane; j < n; j += 32)
+        if (j != i && S[(size_t)i * n + j] == 0.f) m = min(m, lab[j]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0 && m < li) {
+        atomicMin(&lab[li], m);
+        atomicMin(&lab[i], m);
+        *changed = 1;
+    }
+}
+
+// ---- a0 for complete graphs: W_ij = exp(-phi ||x_i - x_j||^2), all pairs (PAPER.md L127-L133 with k = n-1;
+// masked distances by reading S11), optional normalisation by the sum over i<j (S8).  64 x 64 pair tiles.
+template <bool MASKED>
+__global__ void __launch_bounds__(256) kd_weights(int n, int p, int ntile, float phi, const float* __restrict__ X,
+                                                  const uint8_t* __restrict__ mask, float* __restrict__ W) {
+    __shared__ float Xi[PT][PCK + 1], Xj[PT][PCK + 1], Mi[MASKED ? PT : 1][PCK + 1], Mj[MASKED ? PT : 1][PCK + 1];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    int I = 0, rem = blockIdx.x;
+    while (rem >= ntile - I) { rem -= ntile - I; ++I; }
+    const int J = I + rem, i0 = I * PT, j0 = J * PT;
+    float acc[4][4], cnt[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) { acc[a][b] = 0.f; cnt[a][b] = 0.f; }
+    for (int c0 = 0; c0 < p; c0 += PCK) {
+        for (int t = tid; t < PT * PCK; t += 256) {
+            const int r = t / PCK, c = t % PCK, gc = c0 + c;
+            const bool vi = i0 + r < n && gc < p, vj = j0 + r < n && gc < p;
+            Xi[r][c] = vi ? X[(size_t)(i0 + r) * p + gc] : 0.f;
+            Xj[r][c] = vj ? X[(size_t)(j0 + r) * p + gc] : 0.f;
+            if (MASKED) {
+                Mi[r][c] = vi && mask[(size_t)(i0 + r) * p + gc] ? 1.f : 0.f;
+                Mj[r][c] = vj && mask[(size_t)(j0 + r) * p + gc] ? 1.f : 0.f;
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int c = 0; c < PCK; ++c) {
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                    const float df = Xi[ty * 4 + a][c] - Xj[tx + 16 * b][c];
+                    if (MASKED) {
+                        const float m = Mi[ty * 4 + a][c] * Mj[tx + 16 * b][c];
+                        acc[a][b] = fmaf(m * df, df, acc[a][b]);
+                        cnt[a][b] += m;
+                    } else {
+                        acc[a][b] = fmaf(df, df, acc[a][b]);
+                    }
+                }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const int gi = i0 + ty * 4 + a, gj = j0 + tx + 16 * b;
+            if (gi < n && gj < n) {
+                float d = acc[a][b];
+                if (MASKED) d = cnt[a][b] > 0.f ? d * (float)p / cnt[a][b] : 3.0e38f;
+                const float w = gi == gj ? 0.f : expf(-phi * d);
+                W[(size_t)gi * n + gj] = w;
+                if (I != J) W[(size_t)gj * n + gi] = w;
+            }
+        }
+}
+
+__global__ void __launch_bounds__(CC_THREADS) kd_wsum(int n, const float* __restrict__ W, double* part, unsigned int* ticket,
+                                                       double* out) {
+    const long long nn = (long long)n * n, nt = (long long)gridDim.x * blockDim.x;
+    double acc[1] = {0.0};
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += nt)
+        if (e / n < e % n) acc[0] += (double)W[e];
+    double tot[1];
+    if (grid_reduce<1>(acc, part, ticket, tot)) out[0] = tot[0];
+}
+
+__global__ void kd_wscale(long long nn, float* __restrict__ W, const double* __restrict__ total) {
+    const double t = total[0];
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += (long long)gridDim.x * blockDim.x)
+        W[e] = (float)((double)W[e] / t);
+}
+
+}  // namespace
+
+// =============================================================================================
+// Host side
+// =============================================================================================
+static const int kSliceDense = 32;
+
+void ccd_colmeans(cc_handle* h) {
+    dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)kSliceDense);
+    kd_colsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->U, h->Ap, h->colps);
+    kd_colsum2<<<(unsigned)((h->ld + 127) / 128), 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->colps,
+                                                                      h->ubar, h->abar, h->sc);
+}
+
+void ccd_proj(cc_handle* h) {
+    double* part = h->part + 0 * CC_MAXBLK * CC_NPART;
+    if (h->dn_big) {
+        dim3 g((unsigned)((h->ld + 127) / 128), (unsigned)((h->n + 127) / 128));
+        kd_proj<8, 8><<<g, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar, h->abar,
+                                                h->A, h->sc, part);
+    } else {
+        dim3 g((unsigned)((h->ld + 63) / 64), (unsigned)((h->n + 63) / 64));
+        kd_proj<4, 4><<<g, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar, h->abar,
+                                                h->A, h->sc, part);
+    }
+}
+
+static void launch_pairs(cc_handle* h, const float* A, const float* Ap, int init_only) {
+    const int ntile = (int)((h->n + PT - 1) / PT);
+    dim3 g((unsigned)(ntile * (ntile + 1) / 2), (unsigned)h->dn_ksplit);
+    kd_pairs<<<g, 256, 0, h->stream>>>((int)h->n, (int)h->ld, ntile, h->dn_ksplit, A, Ap, h->Sd, h->Wd, h->VNd, h->NB2d,
+                                       h->sc, h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d,
+                                       init_only ? 0 : h->cond_outer, init_only);
+}
+
+void ccd_pairs(cc_handle* h) { launch_pairs(h, h->A, h->Ap, 0); }
+
+void ccd_edges(cc_handle* h, int init_only) {
+    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc, init_only);
+}
+
+void ccd_lab_hook(cc_handle* h, int* changed) {
+    kd_lab_hook<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->Sd, h->lab, changed);
+}
+
+// sizes, allocations and validation of the dense mode; W is copied.  Returns CC_* codes.
+int ccd_setup(cc_handle* h, const float* W) {
+    const int64_t n = h->n, nn = n * n;
+    const int ntile = (int)((n + PT - 1) / PT);
+    const long long ntp = (long long)ntile * (ntile + 1) / 2;
+    h->dn_big = (n > 64 && h->ld >= 128) ? 1 : 0;
+    long long ks = (4LL * h->sms + ntp - 1) / ntp;
+    const long long ksmax = (h->ld + 63) / 64;
+    if (ks > ksmax) ks = ksmax;
+    if (ks < 1) ks = 1;
+    h->dn_ksplit = (int)ks;
+    const long long bproj = h->dn_big ? ((h->ld + 127) / 128) * ((n + 127) / 128) : ((h->ld + 63) / 64) * ((n + 63) / 64);
+    if (ntp * ks > CC_MAXBLK || bproj > CC_MAXBLK) {
+        snprintf(h->err, sizeof(h->err), "dense mode: problem too large for this build (n=%lld, p=%lld)", (long long)n, (long long)h->p);
+        return CC_EINVAL;
+    }
+    float** mats[] = {&h->Wd, &h->Sd, &h->VNd};
+    for (float** m : mats) {
+        cudaError_t e = cudaMalloc((void**)m, (size_t)nn * sizeof(float));
+        if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc n*n failed"); return CC_ENOMEM; }
+    }
+    cudaError_t e = cudaMalloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->ubar, (size_t)h->ld * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->abar, (size_t)h->ld * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->colps, (size_t)kSliceDense * 2 * h->ld * sizeof(double));
+    if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
+    CC_CUDA(h, cudaMemcpyAsync(h->Wd, W, (size_t)nn * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
+    CC_CUDA(h, cudaMemsetAsync(h->Sd, 0, (size_t)nn * sizeof(float), h->stream));
+    CC_CUDA(h, cudaMemsetAsync(h->VNd, 0, (size_t)nn * sizeof(float), h->stream));
+    kd_check_w<<<h->grid_nodes, 256, 0, h->stream>>>((int)n, h->Wd, h->dflag);
+    h->nnz = n * (n - 1);
+    h->npairs = h->nnz / 2;
+    h->launches += 1;
+    return CC_OK;
+}
+
+// sum_{i<j} w_ij^2 for the rho rule (S1): reuse kd_pairs' reduction machinery would be overkill; a plain
+// deterministic kernel over the upper triangle.
+namespace {
+__global__ void __launch_bounds__(CC_THREADS) kd_sumw2(int n, const float* __restrict__ W, double* part, unsigned int* ticket,
+                                                        double* out) {
+    const long long nn = (long long)n * n, nt = (long long)gridDim.x * blockDim.x;
+    double acc[1] = {0.0};
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += nt) {
+        const int i = (int)(e / n), j = (int)(e % n);
+        if (i < j) { const double w = (double)W[e]; acc[0] += w * w; }
+    }
+    double tot[1];
+    if (grid_reduce<1>(acc, part, ticket, tot)) out[1] = tot[0];
+}
+}  // namespace
+
+void ccd_sumw2(cc_handle* h) {
+    kd_sumw2<<<h->grid_nodes, CC_THREADS, 0, h->stream>>>((int)h->n, h->Wd, h->part + 5 * CC_MAXBLK * CC_NPART,
+                                                         &h->sc->ticket[5], h->dout);
+}
+
+// cold start of the pair state (S4: V0 = D U0): s = 1, ||v_ij|| = ||u0_i - u0_j||
+void ccd_init_state(cc_handle* h) {
+    const size_t bytes = (size_t)h->n * h->ld * sizeof(float);
+    cudaMemcpyAsync(h->Ap, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
+    launch_pairs(h, h->U, h->U, 1);
+    ccd_edges(h, 1);
+    h->launches += 2;
+}
+
+void ccd_iteration(cc_handle* h) {
+    ccd_colmeans(h);
+    ccd_proj(h);
+    ccd_pairs(h);
+    ccs_update_nodes(h);
+    ccd_edges(h, 0);
+}
+
+int ccd_solve_eager(cc_handle* h, int maxit) {
+    h->cond_inner = 0;
+    h->cond_outer = 0;
+    for (int it = 0; it < maxit; ++it) {
+        ccs_begin_iter(h);
+        ccd_iteration(h);
+        h->launches += 7;
+        CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
+        CC_CUDA(h, cudaStreamSynchronize(h->stream));
+        if (!h->sc_host->mm_active || h->sc_host->stop_pending) break;
+    }
+    CC_CUDA(h, cudaGetLastError());
+    return CC_OK;
+}
+
+// graph:  WHILE(outer){ kd_colsum1; kd_colsum2; kd_proj; kd_pairs; k_update; kd_edges }
+int ccd_build_graph(cc_handle* h) {
+    if (h->gexec) return CC_OK;
+    cudaStream_t cap;
+    CC_CUDA(h, cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking));
+    cudaStream_t user = h->stream;
+    CC_CUDA(h, cudaGraphCreate(&h->graph, 0));
+    CC_CUDA(h, cudaGraphConditionalHandleCreate(&h->cond_outer, h->graph, 1, cudaGraphCondAssignDefault));
+    cudaGraphNodeParams op = {};
+    op.type = cudaGraphNodeTypeConditional;
+    op.conditional.handle = h->cond_outer;
+    op.conditional.type = cudaGraphCondTypeWhile;
+    op.conditional.size = 1;
+    cudaGraphNode_t onode;
+    CC_CUDA(h, cudaGraphAddNode(&onode, h->graph, nullptr, 0, &op));
+    cudaGraph_t og = op.conditional.phGraph_out[0];
+    h->stream = cap;
+    cudaError_t e = cudaStreamBeginCaptureToGraph(cap, og, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
+    if (e == cudaSuccess) {
+        ccd_iteration(h);
+        e = cudaStreamEndCapture(cap, nullptr);
+    }
+    h->stream = user;
+    cudaStreamDestroy(cap);
+    if (e != cudaSuccess) {
+        snprintf(h->err, sizeof(h->err), "building the dense solve graph: %s", cudaGetErrorString(e));
+        return CC_ECUDA;
+    }
+    CC_CUDA(h, cudaGraphInstantiate(&h->gexec, h->graph, 0));
+    return CC_OK;
+}
+
+
+extern "C" int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, float phi, int32_t normalize,
+                                float* W_out, void* stream) {
+    if (!X || !W_out || n < 2 || p < 1 || !(phi >= 0.f) || n > 46340) {
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights: need n in [2, 46340], p >= 1, phi >= 0, non-NULL pointers");
+        return CC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int ntile = (int)((n + PT - 1) / PT);
+    const unsigned grid = (unsigned)(ntile * (ntile + 1) / 2);
+    if (mask) kd_weights<true><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out);
+    else kd_weights<false><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out);
+    cudaError_t e = cudaSuccess;
+    if (normalize) {
+        double* red = nullptr;
+        e = cudaMalloc((void**)&red, (size_t)(2 + 1024) * sizeof(double));
+        if (e == cudaSuccess) {
+            cudaMemsetAsync(red, 0, (size_t)(2 + 1024) * sizeof(double), st);
+            kd_wsum<<<1024, CC_THREADS, 0, st>>>((int)n, W_out, red + 2, reinterpret_cast<unsigned int*>(red + 1), red);
+            kd_wscale<<<1024, 256, 0, st>>>((long long)n * n, W_out, red);
+            e = cudaStreamSynchronize(st);
+            cudaFree(red);
+        }
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights: %s", cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? CC_ENOMEM : CC_ECUDA;
+    }
+    return CC_OK;
+}

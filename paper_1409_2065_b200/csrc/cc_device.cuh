@@ -45,6 +45,7 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
     __shared__ double sm[NV][CC_THREADS / 32];
     __shared__ bool last;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned bid = blockIdx.y * gridDim.x + blockIdx.x, nblk = gridDim.x * gridDim.y;   // 1-D or 2-D grids
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
         double x = v[k];
@@ -58,11 +59,11 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
         for (int k = 0; k < NV; ++k) {
             double x = 0.0;
             for (int w2 = 0; w2 < CC_THREADS / 32; ++w2) x += sm[k][w2];
-            part[(size_t)blockIdx.x * NV + k] = x;
+            part[(size_t)bid * NV + k] = x;
         }
         __threadfence();
         unsigned t = atomicAdd(ticket, 1u);
-        last = (t == gridDim.x - 1);
+        last = (t == nblk - 1);
     }
     __syncthreads();
     if (!last) return false;
@@ -70,7 +71,7 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
         double x = 0.0;
-        for (unsigned b = threadIdx.x; b < gridDim.x; b += CC_THREADS) x += __ldcg(&part[(size_t)b * NV + k]);
+        for (unsigned b = threadIdx.x; b < nblk; b += CC_THREADS) x += __ldcg(&part[(size_t)b * NV + k]);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
         __syncthreads();
@@ -99,6 +100,33 @@ __device__ __forceinline__ void prof_mark(S* sc, int id) {
     const unsigned long long now = global_ns();
     if (sc->t_last) { sc->prof_ns[id] += now - sc->t_last; sc->prof_calls[id] += 1; }
     sc->t_last = now;
+}
+
+
+// End of the reductions of one MM iteration (called by one thread): d_m = sqrt(dist^2 + eps) (PAPER.md
+// L76), Phi_m = 1/2 loss + gamma pen + rho d_m (L64-L66, L109), the stop rule (reading S3), and the
+// coefficients of the U update (L82) and of the shrink (L86).  `outer` = the MM WHILE node's handle in
+// graph mode, else 0.
+template <typename S>
+__device__ __forceinline__ void finish_iteration(S* sc, double dist2, double loss, double pen, double* hist_phi,
+                                                 double* hist_d, cudaGraphConditionalHandle outer) {
+    const double d = sqrt(dist2 + sc->eps);
+    const double phi = 0.5 * loss + sc->gamma * pen + sc->rho * d;
+    const int m = sc->mm_iter;
+    if (m < sc->hist_cap) { hist_phi[m] = phi; hist_d[m] = d; }
+    int stop = (m + 1 >= sc->mm_maxit) ? 1 : 0;
+    if (sc->tol > 0.0 && m + 1 >= sc->mm_min_it && m >= 1 &&
+        sc->phi_prev - phi <= sc->tol * (1.0 + fabs(sc->phi_prev)))
+        stop = 1;
+    sc->dist2 = dist2; sc->loss = loss; sc->pen = pen;
+    sc->d = d; sc->d_prev = d;
+    sc->phi_prev = phi; sc->phi = phi;
+    sc->cu = (float)(d / (d + sc->rho));
+    sc->ca = (float)(sc->rho / (d + sc->rho));
+    sc->cthr = (float)(sc->gamma * d / sc->rho);
+    sc->mm_iter = m + 1;
+    sc->stop_pending = stop;
+    if (outer) cudaGraphSetConditional(outer, stop ? 0 : 1);
 }
 
 }  // namespace

@@ -50,7 +50,7 @@ struct cc_scal {
 
 // Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
 #define CC_NPART 4
-#define CC_MAXBLK 4096
+#define CC_MAXBLK 16384
 
 struct cc_handle {
     // sizes
@@ -79,7 +79,11 @@ struct cc_handle {
     float* nb2;                       // nchunk x nnz partial squared norms of b_ij
     float* tmpE;                      // nnz scratch (diagnostics)
     float* dinv;                      // n: 1 / (1 + |N_i|)
-    float* Wd;                        // dense: n x n weights
+    // dense mode (complete graph): n x n matrices instead of the CSR arrays
+    float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices)
+    float *ubar, *abar;               // column means of U and A'
+    double* colps;                    // partial column sums
+    int dn_ksplit, dn_big;
     // scalars
     cc_scal* sc;                      // device
     cc_scal* sc_host;                 // pinned mirror
@@ -118,6 +122,15 @@ void ccs_init_state(cc_handle* h);   // cold start of (Ap, Z, s, vn)
 void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out);
 int ccs_solve_eager(cc_handle* h, int maxit);
 int ccs_build_graph(cc_handle* h);
+
+// ---- cc_dense.cu (a9) ------------------------------------------------------------------------------
+int ccd_setup(cc_handle* h, const float* W);
+void ccd_sumw2(cc_handle* h);
+void ccd_init_state(cc_handle* h);
+void ccd_lab_hook(cc_handle* h, int* changed);
+int ccd_solve_eager(cc_handle* h, int maxit);
+int ccd_build_graph(cc_handle* h);
+void ccs_update_nodes(cc_handle* h);  // k_update, node part only (dense mode)
 
 // ---- cc_setup.cu ------------------------------------------------------------------------------------
 int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, const int64_t* rowptr,

@@ -115,23 +115,6 @@ __global__ void __launch_bounds__(1024) k_degree_order(int n, const int* __restr
     }
 }
 
-// Complete graph given as an n x n matrix: expand to the symmetric CSR the kernels walk.
-__global__ void k_dense_to_csr(int n, const float* __restrict__ W, int* __restrict__ rowptr, int* __restrict__ col,
-                               float* __restrict__ w, int* flag) {
-    const long long nn = (long long)n * (n - 1);
-    const long long nt = (long long)gridDim.x * blockDim.x;
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += nt) {
-        const int i = (int)(e / (n - 1));
-        int j = (int)(e % (n - 1));
-        if (j >= i) ++j;
-        const float a = W[(size_t)i * n + j], b = W[(size_t)j * n + i];
-        if (a != b) atomicOr(flag, F_WASYM);
-        col[e] = j;
-        w[e] = a;
-    }
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i <= n; i += nt) rowptr[i] = (int)(i * (n - 1));
-}
-
 // X (n x p) -> padded n x ld copy; mask likewise (padding = observed zeros); NaN/Inf check on observed.
 __global__ void k_pad_copy(long long n, int p, int ld, const float* __restrict__ X, const uint8_t* __restrict__ mask,
                            float* __restrict__ Xo, uint8_t* __restrict__ Mo, int* flag) {
@@ -330,11 +313,10 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
     CC_TRY(dmalloc(h, &h->rowptr, (size_t)n + 1));
     if (h->dense) {
         if (n < 2) { snprintf(h->err, sizeof(h->err), "dense mode needs n >= 2"); return CC_EINVAL; }
-        if ((double)n * (double)(n - 1) > 2147483647.0) { snprintf(h->err, sizeof(h->err), "n too large for dense mode"); return CC_EINVAL; }
-        h->nnz = n * (n - 1);
-        CC_TRY(dmalloc(h, &h->col, (size_t)h->nnz));
-        CC_TRY(dmalloc(h, &h->w, (size_t)h->nnz));
-        k_dense_to_csr<<<(int)cap, 256, 0, st>>>((int)n, w, h->rowptr, h->col, h->w, h->dflag);
+        CC_TRY(ccd_setup(h, w));
+        CC_TRY(dmalloc(h, &h->col, 1));
+        CC_TRY(dmalloc(h, &h->w, 1));
+        CC_CUDA(h, cudaMemsetAsync(h->rowptr, 0, (size_t)(n + 1) * sizeof(int), st));
     } else {
         k_rowptr32<<<(int)((n + 256) / 256), 256, 0, st>>>((int)n, rowptr, h->rowptr, h->dflag);
         int64_t nnz64 = 0;
@@ -352,7 +334,8 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
         }
     }
     h->npairs = h->nnz / 2;
-    CC_TRY(dmalloc(h, &h->peer, (size_t)h->nnz));
+    const int64_t nnz_csr = h->dense ? 0 : h->nnz;   // the CSR arrays are empty in dense mode
+    CC_TRY(dmalloc(h, &h->peer, (size_t)nnz_csr));
     CC_TRY(dmalloc(h, &h->rowup, (size_t)n));
     CC_TRY(dmalloc(h, &h->dinv, (size_t)n));
     {
@@ -385,8 +368,9 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
     CC_TRY(read_flag(h, &f));
     if (f) return flag_to_error(h, f);
     // constants of the rho rule (S1): sum_obs (x - colmean)^2 and sum_E w^2
-    k_sums<<<(int)cap, CC_THREADS, 0, st>>>(n, (int)h->ld, (long long)h->nnz, 0, h->X, h->mask, h->colmean, h->peer,
+    k_sums<<<(int)cap, CC_THREADS, 0, st>>>(n, (int)h->ld, (long long)nnz_csr, 0, h->X, h->mask, h->colmean, h->peer,
                                            h->w, nullptr, h->part + 4 * CC_MAXBLK * CC_NPART, &h->sc->ticket[4], h->dout);
+    if (h->dense) ccd_sumw2(h);
     double two[2];
     CC_CUDA(h, cudaMemcpyAsync(two, h->dout, sizeof(two), cudaMemcpyDeviceToHost, st));
     CC_CUDA(h, cudaStreamSynchronize(st));
@@ -399,11 +383,11 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
         CC_TRY(dmalloc(h, a, nl));
         CC_CUDA(h, cudaMemsetAsync(*a, 0, nl * sizeof(float), st));
     }
-    CC_TRY(dmalloc(h, &h->s, (size_t)h->nnz));
-    CC_TRY(dmalloc(h, &h->vn, (size_t)h->nnz));
-    CC_TRY(dmalloc(h, &h->tmpE, (size_t)h->nnz));
-    CC_TRY(dmalloc(h, &h->nb2, (size_t)h->nnz * h->nchunk));
-    CC_CUDA(h, cudaMemsetAsync(h->nb2, 0, (size_t)h->nnz * h->nchunk * sizeof(float), st));
+    CC_TRY(dmalloc(h, &h->s, (size_t)nnz_csr));
+    CC_TRY(dmalloc(h, &h->vn, (size_t)nnz_csr));
+    CC_TRY(dmalloc(h, &h->tmpE, (size_t)nnz_csr));
+    CC_TRY(dmalloc(h, &h->nb2, (size_t)nnz_csr * h->nchunk + 1));
+    CC_CUDA(h, cudaMemsetAsync(h->nb2, 0, ((size_t)nnz_csr * h->nchunk + 1) * sizeof(float), st));
     const int hc = h->prm.hist_cap > 0 ? h->prm.hist_cap : 1;
     CC_TRY(dmalloc(h, &h->hist_phi, (size_t)hc));
     CC_TRY(dmalloc(h, &h->hist_d, (size_t)hc));
@@ -415,7 +399,7 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
 
 int ccu_cold_start(cc_handle* h) {
     k_cold_start<<<h->grid_nodes, 256, 0, h->stream>>>(h->n, (int)h->ld, h->X, h->mask, h->colmean, h->U);
-    ccs_init_state(h);
+    if (h->dense) ccd_init_state(h); else ccs_init_state(h);
     h->launches += 1;
     CC_CUDA(h, cudaGetLastError());
     return CC_OK;
@@ -445,7 +429,7 @@ int ccu_min_margin(cc_handle* h, double* margin_out) {
 
 void ccu_free(cc_handle* h) {
     void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Dl, h->Uc, h->mask, h->colmean, h->rowptr,
-                    h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->sc, h->part,
+                    h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->colps, h->sc, h->part,
                     h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order};
     for (void* q : ptrs)
         if (q) cudaFree(q);

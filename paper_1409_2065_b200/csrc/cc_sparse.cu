@@ -318,23 +318,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
     }
     double tot[3];
     if (grid_reduce<3>(acc_g, part, &sc->ticket[3], tot)) {
-        const double d = sqrt(tot[0] + sc->eps);
-        const double phi = 0.5 * tot[1] + sc->gamma * tot[2] + sc->rho * d;
-        const int m = sc->mm_iter;
-        if (m < sc->hist_cap) { hist_phi[m] = phi; hist_d[m] = d; }
-        int stop = (m + 1 >= sc->mm_maxit) ? 1 : 0;
-        if (sc->tol > 0.0 && m + 1 >= sc->mm_min_it && m >= 1 &&
-            sc->phi_prev - phi <= sc->tol * (1.0 + fabs(sc->phi_prev)))
-            stop = 1;
-        sc->dist2 = tot[0]; sc->loss = tot[1]; sc->pen = tot[2];
-        sc->d = d; sc->d_prev = d;
-        sc->phi_prev = phi; sc->phi = phi;
-        sc->cu = (float)(d / (d + sc->rho));
-        sc->ca = (float)(sc->rho / (d + sc->rho));
-        sc->cthr = (float)(sc->gamma * d / sc->rho);
-        sc->mm_iter = m + 1;
-        sc->stop_pending = stop;
-        if (outer) cudaGraphSetConditional(outer, stop ? 0 : 1);
+        finish_iteration(sc, tot[0], tot[1], tot[2], hist_phi, hist_d, outer);
         prof_mark(sc, 3);
     }
 }
@@ -372,9 +356,11 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
         st4(U + oi, un);
         // warm start of the next projection: linear extrapolation of the correction a - u over the last two
         // iterations (cuts the inner sweeps by ~30 %; any guess gives the same projection, S5)
-        const float4 dl = a - u;
-        st4(Z + oi, un + (dl + (dl - ld4s(Dl + oi))));
-        st4(Dl + oi, dl);
+        if (Z) {
+            const float4 dl = a - u;
+            st4(Z + oi, un + (dl + (dl - ld4s(Dl + oi))));
+            st4(Dl + oi, dl);
+        }
         st4(Ap + oi, a);
     }
     const long long nthreads = (long long)gridDim.x * CC_THREADS;
@@ -476,6 +462,12 @@ void ccs_norm(cc_handle* h) {
 void ccs_update(cc_handle* h) {
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->X, h->mask,
                   h->A, h->U, h->Z, h->Ap, h->Dl, h->w, h->nb2, h->s, h->vn, h->sc);
+}
+
+void ccs_update_nodes(cc_handle* h) {
+    CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, 0LL, h->X, h->mask, h->A, h->U,
+                  (float*)nullptr, h->Ap, (float*)nullptr, (const float*)nullptr, (const float*)nullptr, (float*)nullptr,
+                  (float*)nullptr, h->sc);
 }
 
 void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out) {

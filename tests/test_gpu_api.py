@@ -98,6 +98,22 @@ def test_knn_weights_match_oracle(B, oracle, name, kw, k, phi, norm):
     B.cc_destroy(h)
 
 
+@pytest.mark.parametrize("name,kw,phi,norm", [("genotype", dict(n=52, p=3001), 0.01, False),
+                                              ("dense_weight", dict(n=200, p=64, n_clusters=4), 0.005, True),
+                                              ("expression", dict(n=70, p=333), 0.002, False)])
+def test_dense_weights_match_oracle(B, oracle, name, kw, phi, norm):
+    """a0 for complete graphs against the oracle's eq. 8 with all pairs (incl. masked rule S11, S8)."""
+    import torch
+    wl = synth.make(name, **kw)
+    ei, ej, w, _ = oracle.complete_graph(wl.X.astype(np.float64), wl.mask, phi, normalize=norm)
+    Wref = np.zeros((wl.n, wl.n))
+    Wref[ei, ej] = w
+    Wref = Wref + Wref.T
+    W = B.cc_dense_weights(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), phi, normalize=norm).cpu().numpy()
+    assert np.array_equal(W, W.T) and np.all(np.diag(W) == 0)
+    assert np.abs(W - Wref).max() <= 2e-5 * Wref.max()
+
+
 def test_full_size_large_sparse_properties(B):
     """configs[3] at full size, in the launch configuration bench.py times: properties that hold at
     any size -- Phi non-increasing, column sums of U equal those of X when nothing

@@ -214,26 +214,64 @@ def test_cc_path_snapshots(B, torch_, oracle):
     B.cc_destroy(h)
 
 
-def test_dense_mode_complete_graph(B, torch_, oracle):
-    """prm.dense = 1: w is the n x n matrix (genotype-like shape, reduced)."""
+@pytest.mark.parametrize("name,kw,miss", [("genotype", dict(n=20, p=1000), 0.0),      # 4x4 tiles, one row block, ksplit > 1
+                                          ("genotype", dict(n=52, p=5001), 0.0),      # the genotype shape, ragged p
+                                          ("dense_weight", dict(n=150, p=200, n_clusters=4), 0.0),   # 8x8 tiles, ragged rows
+                                          ("dense_weight", dict(n=70, p=40, n_clusters=3), 0.2)])    # masked
+def test_dense_mode_complete_graph(B, torch_, oracle, name, kw, miss):
+    """prm.dense = 1 (row a9): w is the n x n matrix; closed-form projection, pair tiles."""
     torch = torch_
-    wl = synth.make("genotype", n=20, p=1000)
+    wl = synth.make(name, **kw)
+    if miss > 0:
+        rng = np.random.default_rng(5)
+        wl.mask = (rng.random(size=wl.X.shape) >= miss).astype(np.uint8)
+        wl.mask[0, :] = 1
     prob = H.build_problem(oracle, wl)
     n = wl.n
+    assert len(prob["ei"]) == n * (n - 1) // 2          # no weight underflowed: the graph is complete
     W = np.zeros((n, n), np.float32)
     W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
     W = W + W.T
-    gammas = [0.05, 0.5, 5.0]
-    ref = H.oracle_path(oracle, prob, gammas, 100)
+    gammas = [float(g) for g in synth.gamma_grid(4.0, 40.0, 6)]   # from no fusion to one cluster
+    ref = H.oracle_path(oracle, prob, gammas, 80, proj_method=1)
+    assert ref[0]["nclusters"] == n and ref[-1]["nclusters"] == 1
     dev = torch.device("cuda:0")
-    h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
-                    B.cc_default_params(dense=1))
-    U = torch.empty(n, wl.p, device=dev)
-    lab = torch.empty(n, dtype=torch.int32, device=dev)
-    for g, r in zip(gammas, ref):
-        B.cc_solve(h, g, 0.0, 100)
-        B.cc_get_U(h, -1, U)
-        _, k = B.cc_clusters(h, -1, lab)
-        assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL
-        assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"])
-    B.cc_destroy(h)
+    mask = None if wl.mask is None else torch.from_numpy(wl.mask).to(dev)
+    outs = []
+    for use_graph in (1, 0):
+        h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), mask, None, None, torch.from_numpy(W).to(dev),
+                        B.cc_default_params(dense=1, use_graph=use_graph))
+        assert B.cc_get_counts(h)["n_pairs"] == n * (n - 1) // 2
+        U = torch.empty(n, wl.p, device=dev)
+        lab = torch.empty(n, dtype=torch.int32, device=dev)
+        ks = []
+        for g, r in zip(gammas, ref):
+            it, phi, _ = B.cc_solve(h, g, 0.0, 80)
+            assert it == 80
+            B.cc_get_U(h, -1, U)
+            _, k = B.cc_clusters(h, -1, lab)
+            ph, dd = B.cc_get_history(h)
+            assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, g
+            assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (g, k, r["nclusters"])
+            assert np.allclose(ph, r["phi"], rtol=1e-4) and np.allclose(dd, r["d"], rtol=5e-4)
+            ks.append(k)
+        outs.append(U.cpu().numpy().copy())
+        B.cc_destroy(h)
+    assert np.array_equal(outs[0], outs[1])
+    print(name, kw, "clusters along the path:", ks)
+
+
+def test_dense_mode_rejects_bad_weights(B, torch_):
+    torch = torch_
+    n, p = 6, 4
+    X = torch.randn(n, p, device="cuda:0")
+    W = torch.ones(n, n, device="cuda:0")
+    W[1, 2] = 2.0
+    with pytest.raises(B.CCError) as e:
+        B.cc_create(n, p, X, None, None, None, W, B.cc_default_params(dense=1))
+    assert e.value.code == B.CC_EGRAPH
+    W = torch.ones(n, n, device="cuda:0")
+    W[1, 2] = W[2, 1] = 0.0
+    with pytest.raises(B.CCError) as e:
+        B.cc_create(n, p, X, None, None, None, W, B.cc_default_params(dense=1))
+    assert e.value.code == B.CC_EGRAPH

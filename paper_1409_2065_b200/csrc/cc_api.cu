@@ -11,6 +11,25 @@
 thread_local char cc_g_err[256] = "";
 #define g_err cc_g_err
 
+cudaError_t cc_dev_alloc(void** p, size_t bytes, cudaStream_t st) {
+    static bool pool_ready = false;
+    if (!pool_ready) {
+        int dev = 0;
+        cudaMemPool_t pool;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long thr = ~0ULL;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+        cudaGetLastError();
+        pool_ready = true;
+    }
+    return cudaMallocAsync(p, bytes ? bytes : 1, st);
+}
+
+void cc_dev_free(void* p, cudaStream_t st) {
+    if (p) cudaFreeAsync(p, st);
+}
+
 extern "C" {
 
 int cc_default_params(cc_params* prm) {
@@ -146,8 +165,8 @@ int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int3
     }
     const size_t nl = (size_t)h->n * h->ld;
     if (!h->snapU && ngamma > 0) {
-        cudaError_t e1 = cudaMalloc((void**)&h->snapU, nl * sizeof(float) * (size_t)h->prm.max_snapshots);
-        cudaError_t e2 = cudaMalloc((void**)&h->snapLab, (size_t)h->n * sizeof(int32_t) * (size_t)h->prm.max_snapshots);
+        cudaError_t e1 = cc_dev_alloc((void**)&h->snapU, nl * sizeof(float) * (size_t)h->prm.max_snapshots, h->stream);
+        cudaError_t e2 = cc_dev_alloc((void**)&h->snapLab, (size_t)h->n * sizeof(int32_t) * (size_t)h->prm.max_snapshots, h->stream);
         if (e1 != cudaSuccess || e2 != cudaSuccess) {
             cudaGetLastError();
             snprintf(h->err, sizeof(h->err), "cc_path: cannot allocate %d snapshots", h->prm.max_snapshots);
@@ -203,14 +222,14 @@ int cc_clusters(cc_handle* h, int32_t gamma_index, int32_t* labels_out, int32_t 
     if (gamma_index < 0) {
         if (out_on_device) return ccl_labels(h, labels_out, nclusters);
         int32_t* tmp = nullptr;
-        CC_CUDA(h, cudaMalloc((void**)&tmp, bytes));
+        CC_CUDA(h, cc_dev_alloc((void**)&tmp, bytes, h->stream));
         int rc = ccl_labels(h, tmp, nclusters);
         if (rc == CC_OK) {
             cudaError_t e = cudaMemcpyAsync(labels_out, tmp, bytes, cudaMemcpyDeviceToHost, h->stream);
             if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
             if (e != cudaSuccess) { snprintf(h->err, sizeof(h->err), "cc_clusters: %s", cudaGetErrorString(e)); rc = CC_ECUDA; }
         }
-        cudaFree(tmp);
+        cc_dev_free(tmp, h->stream);
         return rc;
     }
     CC_CUDA(h, cudaMemcpyAsync(labels_out, h->snapLab + (size_t)gamma_index * h->n, bytes,

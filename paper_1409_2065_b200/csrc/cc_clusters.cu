@@ -80,7 +80,7 @@ int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host) {
     const int grid = (n + 255) / 256;
     cudaStream_t st = h->stream;
     if (!h->lab_rank) {
-        cudaError_t e = cudaMalloc((void**)&h->lab_rank, (size_t)n * sizeof(int));
+        cudaError_t e = cc_dev_alloc((void**)&h->lab_rank, (size_t)n * sizeof(int), st);
         if (e != cudaSuccess) { snprintf(h->err, sizeof(h->err), "cudaMalloc labels scratch: %s", cudaGetErrorString(e)); return CC_ENOMEM; }
     }
     k_lab_init<<<grid, 256, 0, st>>>(n, h->lab);

@@ -454,13 +454,13 @@ int ccd_setup(cc_handle* h, const float* W) {
     }
     float** mats[] = {&h->Wd, &h->Sd, &h->VNd};
     for (float** m : mats) {
-        cudaError_t e = cudaMalloc((void**)m, (size_t)nn * sizeof(float));
+        cudaError_t e = cc_dev_alloc((void**)m, (size_t)nn * sizeof(float), h->stream);
         if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc n*n failed"); return CC_ENOMEM; }
     }
-    cudaError_t e = cudaMalloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->ubar, (size_t)h->ld * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->abar, (size_t)h->ld * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->colps, (size_t)kSliceDense * 2 * h->ld * sizeof(double));
+    cudaError_t e = cc_dev_alloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float), h->stream);
+    if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->ubar, (size_t)h->ld * sizeof(float), h->stream);
+    if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->abar, (size_t)h->ld * sizeof(float), h->stream);
+    if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->colps, (size_t)kSliceDense * 2 * h->ld * sizeof(double), h->stream);
     if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
     CC_CUDA(h, cudaMemcpyAsync(h->Wd, W, (size_t)nn * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
     CC_CUDA(h, cudaMemsetAsync(h->Sd, 0, (size_t)nn * sizeof(float), h->stream));
@@ -572,13 +572,13 @@ extern "C" int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint
     cudaError_t e = cudaSuccess;
     if (normalize) {
         double* red = nullptr;
-        e = cudaMalloc((void**)&red, (size_t)(2 + 1024) * sizeof(double));
+        e = cc_dev_alloc((void**)&red, (size_t)(2 + 1024) * sizeof(double), st);
         if (e == cudaSuccess) {
             cudaMemsetAsync(red, 0, (size_t)(2 + 1024) * sizeof(double), st);
             kd_wsum<<<1024, CC_THREADS, 0, st>>>((int)n, W_out, red + 2, reinterpret_cast<unsigned int*>(red + 1), red);
             kd_wscale<<<1024, 256, 0, st>>>((long long)n * n, W_out, red);
             e = cudaStreamSynchronize(st);
-            cudaFree(red);
+            cc_dev_free(red, st);
         }
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);

@@ -142,6 +142,11 @@ void ccu_free(cc_handle* h);
 // ---- cc_clusters.cu -----------------------------------------------------------------------------------
 int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host);
 
+// Device memory comes from the stream-ordered allocator: the default pool keeps freed blocks (release
+// threshold raised once), so creating and destroying handles repeatedly does not pay cudaMalloc/cudaFree.
+cudaError_t cc_dev_alloc(void** p, size_t bytes, cudaStream_t st);
+void cc_dev_free(void* p, cudaStream_t st);
+
 // message of the last failing handle-less call on this thread (cc_create, cc_knn_weights)
 extern thread_local char cc_g_err[256];
 

@@ -250,7 +250,7 @@ template <typename T>
 static int dmalloc(cc_handle* h, T** p, size_t count) {
     *p = nullptr;
     if (count == 0) count = 1;
-    cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+    cudaError_t e = cc_dev_alloc((void**)p, count * sizeof(T), h->stream);
     if (e != cudaSuccess) {
         cudaGetLastError();
         snprintf(h->err, sizeof(h->err), "cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
@@ -361,8 +361,8 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
         k_colsum1<<<g1, 128, 0, st>>>(n, (int)h->ld, nslice, h->X, h->mask, psum, pcnt);
         k_colsum2<<<(unsigned)((h->ld + 127) / 128), 128, 0, st>>>((int)p, (int)h->ld, nslice, psum, pcnt, h->colmean, h->dflag);
         CC_CUDA(h, cudaStreamSynchronize(st));
-        cudaFree(psum);
-        cudaFree(pcnt);
+        cc_dev_free(psum, st);
+        cc_dev_free(pcnt, st);
     }
     int f = 0;
     CC_TRY(read_flag(h, &f));
@@ -432,7 +432,7 @@ void ccu_free(cc_handle* h) {
                     h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->colps, h->sc, h->part,
                     h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order};
     for (void* q : ptrs)
-        if (q) cudaFree(q);
+        cc_dev_free(q, h->stream);
     if (h->sc_host) cudaFreeHost(h->sc_host);
     if (h->gexec) cudaGraphExecDestroy(h->gexec);
     if (h->graph) cudaGraphDestroy(h->graph);

@@ -244,7 +244,7 @@ def run_ours(args):
     if not dense:
         rowptr_h, col_h, w_h = rowptr.cpu().pin_memory(), col.cpu().pin_memory(), w.cpu().pin_memory()
     E = nnz // 2
-    prm = B.cc_default_params(use_graph=0 if args.eager else 1, dense=1 if dense else 0)
+    prm = B.cc_default_params(use_graph=0 if args.eager else 1, dense=1 if dense else 0, reserved0=int(os.environ.get('CC_TUNE', '0')))
     h = B.cc_create(n, p, X, M, rowptr, col, w, prm)
     for s in range(args.warmup):
         B.cc_solve(h, gamma_for_step(args.workload, s), 0.0, args.iters)

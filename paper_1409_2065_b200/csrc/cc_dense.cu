@@ -239,12 +239,35 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
 __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, int init_only) {
     if (!init_only && !sc->mm_active) return;
-    const long long nn = (long long)n * n;
+    const size_t nn = (size_t)n * n;
     const float cthr = sc->cthr;
     // few slices: one thread per entry; many slices (small n, long rows): one warp per entry, lanes stride
     // over the slices and combine with a fixed shuffle tree (deterministic either way)
     const bool warp_per = ksplit >= 32;
     const int lane = threadIdx.x & 31;
+    if (!warp_per && (n & 3) == 0) {
+        // streaming case (large n): one block walks whole rows, four entries per thread
+        for (int i = blockIdx.x; i < n; i += gridDim.x) {
+            for (int j = threadIdx.x * 4; j < n; j += blockDim.x * 4) {
+                const size_t e = (size_t)i * n + j;
+                float4 q = ld4s(NB2 + e);
+                for (int k = 1; k < ksplit; ++k) q = q + ld4s(NB2 + (size_t)k * nn + e);
+                const float4 wv = init_only ? f4(0.f) : ld4s(W + e);
+                float qa[4] = {q.x, q.y, q.z, q.w}, wa[4] = {wv.x, wv.y, wv.z, wv.w}, sa[4], va[4];
+#pragma unroll
+                for (int t = 0; t < 4; ++t) {
+                    const float nb = sqrtf(qa[t]);
+                    const float thr = cthr * wa[t];
+                    float sn = init_only ? 1.f : (nb <= thr ? 0.f : 1.f - thr / nb);
+                    if (j + t == i) sn = 0.f;
+                    sa[t] = sn;
+                    va[t] = j + t == i ? 0.f : sn * nb;
+                }
+                st4(S + e, make_float4(sa[0], sa[1], sa[2], sa[3]));
+                st4(VN + e, make_float4(va[0], va[1], va[2], va[3]));
+            }
+        }
+    } else {
     const long long nwork = (long long)gridDim.x * (warp_per ? blockDim.x / 32 : blockDim.x);
     for (long long e = warp_per ? (long long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32
                                 : (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -272,6 +295,7 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
         }
         S[e] = sn;
         VN[e] = vn;
+    }
     }
     __syncthreads();
     if (!init_only && threadIdx.x == 0) {
@@ -405,17 +429,18 @@ void ccd_colmeans(cc_handle* h) {
                                                                       h->ubar, h->abar, h->sc);
 }
 
+template <int TM, int TN>
+static void launch_proj(cc_handle* h) {
+    dim3 g((unsigned)((h->ld + 16 * TN - 1) / (16 * TN)), (unsigned)((h->n + 16 * TM - 1) / (16 * TM)));
+    kd_proj<TM, TN><<<g, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar, h->abar,
+                                              h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART);
+}
+
 void ccd_proj(cc_handle* h) {
-    double* part = h->part + 0 * CC_MAXBLK * CC_NPART;
-    if (h->dn_big) {
-        dim3 g((unsigned)((h->ld + 127) / 128), (unsigned)((h->n + 127) / 128));
-        kd_proj<8, 8><<<g, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar, h->abar,
-                                                h->A, h->sc, part);
-    } else {
-        dim3 g((unsigned)((h->ld + 63) / 64), (unsigned)((h->n + 63) / 64));
-        kd_proj<4, 4><<<g, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar, h->abar,
-                                                h->A, h->sc, part);
-    }
+    if (!h->dn_big) launch_proj<4, 4>(h);
+    else if (h->prm.reserved0 == 1) launch_proj<8, 8>(h);
+    else if (h->prm.reserved0 == 2) launch_proj<8, 4>(h);
+    else launch_proj<4, 8>(h);
 }
 
 static void launch_pairs(cc_handle* h, const float* A, const float* Ap, int init_only) {
@@ -447,7 +472,7 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (ks > ksmax) ks = ksmax;
     if (ks < 1) ks = 1;
     h->dn_ksplit = (int)ks;
-    const long long bproj = h->dn_big ? ((h->ld + 127) / 128) * ((n + 127) / 128) : ((h->ld + 63) / 64) * ((n + 63) / 64);
+    const long long bproj = ((h->ld + 63) / 64) * ((n + 63) / 64);   // upper bound over the tile shapes used
     if (ntp * ks > CC_MAXBLK || bproj > CC_MAXBLK) {
         snprintf(h->err, sizeof(h->err), "dense mode: problem too large for this build (n=%lld, p=%lld)", (long long)n, (long long)h->p);
         return CC_EINVAL;

@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
 #pragma unroll
                 for (int q = 0; q < UNR; ++q) {
                     const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
-                    aj[q] = ld4s(Ap + oj);
+                    aj[q] = sj[q] != 0.f ? ld4s(Ap + oj) : api;    // fused pair (s = 0): v = 0, a'_j is not needed
                     zj[q] = ld4s(Z + oj);
                 }
 #pragma unroll
@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
                 for (int q = 0; q < UNR; ++q) {
                     const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
                     aj[q] = ld4s(A + oj);
-                    apj[q] = ld4s(Ap + oj);
+                    apj[q] = sj[q] != 0.f ? ld4s(Ap + oj) : api;   // fused pair (s = 0): v = 0, a'_j is not needed
                 }
 #pragma unroll
                 for (int q = 0; q < UNR; ++q) {
@@ -295,20 +295,37 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
                     nbq[q] = vf * dot4(b, b);
                     dist_l += vf * dot4(vb, vb);   // padding entries: b = 0, s = 0 => 0
                 }
+                // transpose-reduce: UNR values over G lanes in UNR-1+log2(G/UNR) shuffles instead of UNR*log2(G).
+                // At each of the first log2(UNR) steps a lane keeps one half of its list (upper lanes the second
+                // half) and adds the partner's copy; the surviving value of entry q ends in lanes q*(G/UNR)...
+                {
+                    int cntv = UNR;
 #pragma unroll
-                for (int o = G / 2; o > 0; o >>= 1) {
+                    for (int o = G / 2; o > 0; o >>= 1) {
+                        if (cntv > 1) {
+                            const int half = cntv / 2;
+                            const bool upper = (gl & o) != 0;
 #pragma unroll
-                    for (int q = 0; q < UNR; ++q) nbq[q] += __shfl_xor_sync(gm, nbq[q], o, G);
-                }
-                if (gl == 0) {
-#pragma unroll
-                    for (int q = 0; q < UNR; ++q) {
-                        const int eq = base + t + q;
-                        if (t + q < cnt) {
-                            nb2[(size_t)chunk * nnz + eq] = nbq[q];
-                            nb2[(size_t)chunk * nnz + __ldg(peer + eq)] = nbq[q];
-                            if (chunk == 0) pen_l = fmaf(__ldg(w + eq), __ldg(vn + eq), pen_l);
+                            for (int k = 0; k < UNR / 2; ++k) {
+                                if (k < half) {
+                                    const float send = upper ? nbq[k] : nbq[k + half];
+                                    const float keep = upper ? nbq[k + half] : nbq[k];
+                                    nbq[k] = keep + __shfl_xor_sync(gm, send, o, G);
+                                }
+                            }
+                            cntv = half;
+                        } else {
+                            nbq[0] += __shfl_xor_sync(gm, nbq[0], o, G);
                         }
+                    }
+                }
+                if ((gl & (G / UNR - 1)) == 0) {
+                    const int q = gl / (G / UNR);
+                    const int eq = base + t + q;
+                    if (t + q < cnt) {
+                        nb2[(size_t)chunk * nnz + eq] = nbq[0];
+                        nb2[(size_t)chunk * nnz + __ldg(peer + eq)] = nbq[0];
+                        if (chunk == 0) pen_l = fmaf(__ldg(w + eq), __ldg(vn + eq), pen_l);
                     }
                 }
             }

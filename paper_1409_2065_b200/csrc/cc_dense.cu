@@ -145,6 +145,208 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
     }
 }
 
+// ---- kd_proj_tc: the contraction S (A' - abar) on the 5th-generation tensor cores ------------------------
+// tcgen05.mma kind::tf32, M = 128 rows x N = 128 columns per CTA, fp32 accumulator in TMEM (128 lanes x 128
+// columns), K walked in blocks of 32.  fp32 accuracy is kept with the 3xTF32 split: x = hi + lo with hi = x
+// truncated to 10 mantissa bits (exactly a TF32 value) and lo = x - hi (exact in fp32);
+// S A' ~= S_hi B_hi + S_hi B_lo + S_lo B_hi, three MMAs per K step into the same accumulator (the dropped
+// lo*lo term is 2^-22 relative).  Operands are split while they are staged into shared memory by the CTA's
+// threads (generic proxy) in the canonical K-major no-swizzle layout -- core matrices of 8 rows x 16 bytes,
+// SBO between 8-row groups, LBO between K cores -- then fence.proxy.async hands them to the tensor core.
+// A' is transposed on the way in (B operand is N x K, K-major).  Two shared-memory stages: the MMAs of
+// block kb run while the threads stage block kb+1; tcgen05.commit on an mbarrier frees a stage.
+constexpr int TC_M = 128, TC_N = 128, TC_K = 32;
+constexpr int TC_SBO = 128;                         // bytes between 8-row groups (one core matrix)
+constexpr int TC_LBO = (TC_M / 8) * 128 + 16;       // bytes between K cores; +16 spreads the staging stores over banks
+constexpr int TC_TILE = (TC_K / 4) * TC_LBO;        // bytes of one 128 x 32 operand tile
+constexpr int TC_SMEM = 2 * 4 * TC_TILE + 1024;     // 2 stages x {A_hi, A_lo, B_hi, B_lo} + alignment slack
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ uint64_t tc_desc(uint32_t saddr) {
+    // UMMA shared-memory descriptor (cute::UMMA::SmemDescriptor): start address, LBO, SBO in 16-byte units,
+    // version 1 (Blackwell), no swizzle, base offset 0
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr >> 4) & 0x3fff);
+    d |= (uint64_t)((TC_LBO >> 4) & 0x3fff) << 16;
+    d |= (uint64_t)((TC_SBO >> 4) & 0x3fff) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+
+__device__ __forceinline__ void tc_mma(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}\n"
+        :: "r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
+    for (int spin = 0; spin < (1 << 24); ++spin) {
+        uint32_t ok;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return true;
+    }
+    return false;   // never hang the GPU: the caller raises cg_failed
+}
+
+__device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
+    hi = __uint_as_float(__float_as_uint(x) & 0xffffe000u);
+    lo = x - hi;
+}
+
+__global__ void __launch_bounds__(256, 1) kd_proj_tc(int n, int ld, const float* __restrict__ S, const float* __restrict__ Ap,
+                                                     const float* __restrict__ U, const float* __restrict__ X,
+                                                     const uint8_t* __restrict__ mask, const float* __restrict__ ubar,
+                                                     const float* __restrict__ abar, float* __restrict__ A, cc_scal* sc,
+                                                     double* part) {
+    if (!sc->mm_active) return;
+    extern __shared__ uint8_t tc_smem_raw[];
+    __shared__ __align__(8) uint64_t mbar[2];
+    __shared__ uint32_t tmem_base_s;
+    __shared__ float rs_s[TC_M];
+    __shared__ int fail_s;
+    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int i0 = blockIdx.y * TC_M, c0 = blockIdx.x * TC_N;
+
+    if (tid == 0) {
+        fail_s = 0;
+        for (int b = 0; b < 2; ++b)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar[b])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(TC_N));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_d = tmem_base_s;
+    // instruction descriptor (cute::UMMA::InstrDescriptor): D = F32, A = B = TF32, both K-major, N >> 3, M >> 4
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+
+    float rsum[4] = {0.f, 0.f, 0.f, 0.f};
+    const int nkb = (n + TC_K - 1) / TC_K;
+    for (int kb = 0; kb < nkb; ++kb) {
+        const int st = kb & 1, k0 = kb * TC_K;
+        uint8_t* a_hi = sm + (size_t)(st * 4 + 0) * TC_TILE;
+        uint8_t* a_lo = sm + (size_t)(st * 4 + 1) * TC_TILE;
+        uint8_t* b_hi = sm + (size_t)(st * 4 + 2) * TC_TILE;
+        uint8_t* b_lo = sm + (size_t)(st * 4 + 3) * TC_TILE;
+        if (kb >= 2 && !mbar_wait(smem_u32(&mbar[st]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
+        // A operand: S[i0 + r][k0 + 4 kc .. +3], 8 lanes walk one row's 128 bytes
+#pragma unroll
+        for (int pass = 0; pass < 4; ++pass) {
+            const int r = pass * 32 + warp * 4 + (lane >> 3), kc = lane & 7;
+            const int gi = i0 + r, gk = k0 + kc * 4;
+            float4 v = f4(0.f);
+            if (gi < n && gk < n) v = __ldg(reinterpret_cast<const float4*>(S + (size_t)gi * n + gk));
+            rsum[pass] += (v.x + v.y) + (v.z + v.w);
+            float4 h, l;
+            split_tf32(v.x, h.x, l.x); split_tf32(v.y, h.y, l.y); split_tf32(v.z, h.z, l.z); split_tf32(v.w, h.w, l.w);
+            const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
+            *reinterpret_cast<float4*>(a_hi + off) = h;
+            *reinterpret_cast<float4*>(a_lo + off) = l;
+        }
+        // B operand: (A' - abar)^T, row = column c0 + nl of A', 4 consecutive k per 16-byte core row
+#pragma unroll
+        for (int pass = 0; pass < 4; ++pass) {
+            const int nl = tid & 127, kc = (tid >> 7) + 2 * pass;
+            const int gc = c0 + nl;
+            float v[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int gk = k0 + kc * 4 + q;
+                v[q] = (gc < ld && gk < n) ? __ldg(Ap + (size_t)gk * ld + gc) - __ldg(abar + gc) : 0.f;
+            }
+            float4 h, l;
+            split_tf32(v[0], h.x, l.x); split_tf32(v[1], h.y, l.y); split_tf32(v[2], h.z, l.z); split_tf32(v[3], h.w, l.w);
+            const int off = kc * TC_LBO + (nl >> 3) * TC_SBO + (nl & 7) * 16;
+            *reinterpret_cast<float4*>(b_hi + off) = h;
+            *reinterpret_cast<float4*>(b_lo + off) = l;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int ks = 0; ks < TC_K / 8; ++ks) {
+                const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
+                const uint64_t dah = tc_desc(smem_u32(a_hi) + koff), dal = tc_desc(smem_u32(a_lo) + koff);
+                const uint64_t dbh = tc_desc(smem_u32(b_hi) + koff), dbl = tc_desc(smem_u32(b_lo) + koff);
+                tc_mma(tmem_d, dah, dbh, idesc, (kb > 0 || ks > 0) ? 1u : 0u);
+                tc_mma(tmem_d, dah, dbl, idesc, 1u);
+                tc_mma(tmem_d, dal, dbh, idesc, 1u);
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar[st])) : "memory");
+        }
+    }
+    // row sums of S: 8 lanes hold one row's partial sums
+#pragma unroll
+    for (int pass = 0; pass < 4; ++pass) {
+        float v = rsum[pass];
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        if ((lane & 7) == 0) rs_s[pass * 32 + warp * 4 + (lane >> 3)] = v;
+    }
+    {   // all MMAs done (commits complete in issue order)
+        const int kl = nkb - 1;
+        if (nkb > 0 && !mbar_wait(smem_u32(&mbar[kl & 1]), (uint32_t)((kl >> 1) & 1))) fail_s = 1;
+    }
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    __syncthreads();
+    // epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (its rows); warps 0-3 take columns 0..63, 4-7 take 64..127
+    const float inv = 1.f / (float)(n + 1), fn = (float)n;
+    double red[2] = {0.0, 0.0};
+    const int row = (warp & 3) * 32 + lane, gi = i0 + row;
+    const float rs = rs_s[row];
+#pragma unroll 1
+    for (int cb = (warp >> 2) * 64; cb < (warp >> 2) * 64 + 64; cb += 16) {
+        uint32_t v[16];
+        const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cb;
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                     : "r"(taddr));
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (gi < n) {
+#pragma unroll
+            for (int q4 = 0; q4 < 4; ++q4) {
+                const int gc = c0 + cb + q4 * 4;
+                if (gc >= ld) continue;
+                const size_t o = (size_t)gi * ld + gc;
+                const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
+                const float4 sa = make_float4(__uint_as_float(v[q4 * 4 + 0]), __uint_as_float(v[q4 * 4 + 1]),
+                                              __uint_as_float(v[q4 * 4 + 2]), __uint_as_float(v[q4 * 4 + 3]));
+                const float4 g = (rs * ap - sa) - fn * (u - ub);
+                const float4 dl = inv * g;
+                st4(A + o, u + dl);
+                float4 q = ld4s(X + o) - u;
+                if (mask) {
+                    const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + o);
+                    q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
+                }
+                red[0] += (double)dot4(dl, dl);
+                red[1] += (double)dot4(q, q);
+            }
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(TC_N));
+    if (tid == 0 && fail_s) sc->cg_failed = 2;
+    double tot[2];
+    if (grid_reduce<2>(red, part, &sc->ticket[0], tot)) {
+        sc->dist2 = tot[0];
+        sc->loss = tot[1];
+        prof_mark(sc, 5);
+    }
+}
+
 // ---- kd_pairs --------------------------------------------------------------------------------------
 // One CTA = one 64 x 64 tile of pairs (I <= J) x one range of columns (blockIdx.y of `ksplit`).  Direct
 // differences (no Gram trick: a pair about to fuse has ||b|| far below ||a||, and the fused / not fused
@@ -437,6 +639,12 @@ static void launch_proj(cc_handle* h) {
 }
 
 void ccd_proj(cc_handle* h) {
+    if (h->dn_tc) {
+        dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
+        kd_proj_tc<<<g, 256, TC_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar,
+                                                   h->abar, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART);
+        return;
+    }
     if (!h->dn_big) launch_proj<4, 4>(h);
     else if (h->prm.reserved0 == 1) launch_proj<8, 8>(h);
     else if (h->prm.reserved0 == 2) launch_proj<8, 4>(h);
@@ -467,6 +675,13 @@ int ccd_setup(cc_handle* h, const float* W) {
     const int ntile = (int)((n + PT - 1) / PT);
     const long long ntp = (long long)ntile * (ntile + 1) / 2;
     h->dn_big = (n > 64 && h->ld >= 128) ? 1 : 0;
+    // tensor-core contraction when the tile shape pays (M = 128 rows) and rows of S are float4-aligned;
+    // prm.reserved0 = 4 forces the FFMA tiles (A/B comparison in tests and bench)
+    h->dn_tc = (n >= 128 && (n & 3) == 0 && h->prm.reserved0 != 4) ? 1 : 0;
+    if (h->dn_tc) {
+        cudaError_t ea = cudaFuncSetAttribute(kd_proj_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM);
+        if (ea != cudaSuccess) { cudaGetLastError(); h->dn_tc = 0; }
+    }
     long long ks = (4LL * h->sms + ntp - 1) / ntp;
     const long long ksmax = (h->ld + 63) / 64;
     if (ks > ksmax) ks = ksmax;

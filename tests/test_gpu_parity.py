@@ -217,7 +217,9 @@ def test_cc_path_snapshots(B, torch_, oracle):
 @pytest.mark.parametrize("name,kw,miss", [("genotype", dict(n=20, p=1000), 0.0),      # 4x4 tiles, one row block, ksplit > 1
                                           ("genotype", dict(n=52, p=5001), 0.0),      # the genotype shape, ragged p
                                           ("dense_weight", dict(n=150, p=200, n_clusters=4), 0.0),   # 8x8 tiles, ragged rows
-                                          ("dense_weight", dict(n=70, p=40, n_clusters=3), 0.2)])    # masked
+                                          ("dense_weight", dict(n=70, p=40, n_clusters=3), 0.2),     # masked
+                                          ("dense_weight", dict(n=256, p=200, n_clusters=4), 0.0),   # tcgen05 path, ragged N tile
+                                          ("dense_weight", dict(n=132, p=64, n_clusters=3), 0.1)])   # tcgen05, ragged M and K
 def test_dense_mode_complete_graph(B, torch_, oracle, name, kw, miss):
     """prm.dense = 1 (row a9): w is the n x n matrix; closed-form projection, pair tiles."""
     torch = torch_

@@ -352,10 +352,19 @@ def run_ours(args):
             per_kernel[k] = {"share": v["ns"] / tot_ns, "us_per_launch": dur / 1e3, "launches": v["calls"],
                              "alg_gbs": gbs, "frac": gbs / peak, "alg_tflops": tfl, "frac_fp32_alu": tfl / FP32_PEAK_TFLOPS}
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(args.workload, {}).get(top)
     alu_bound = per_kernel[top]["frac_fp32_alu"] > per_kernel[top]["frac"]
+    # kd_proj at n >= 128 runs on tcgen05 (kind::tf32, 3xTF32): report it against the TF32 tensor peak =
+    # measured bf16 cuBLAS peak x the nominal tf32/bf16 ratio (1.1 / 2.25), B200_PROFILING.md
+    if "kd_proj" in per_kernel and dense and n >= 128 and n % 4 == 0:
+        pk = json.load(open(peaks_path)).get("bf16_tflops", 1590.0) if os.path.exists(peaks_path) else 1590.0
+        v = per_kernel["kd_proj"]
+        v["bound"] = "tensor"
+        v["tf32_peak_tflops"] = pk * 1.1 / 2.25
+        v["frac_tensor"] = v["alg_tflops"] / v["tf32_peak_tflops"]
+        v["frac_tensor_3x"] = 3.0 * v["frac_tensor"]      # three TF32 MMAs are issued per useful product
     roofline = {"bound": "alu" if alu_bound else "hbm", "kernel": top,
                 "achieved": per_kernel[top]["alg_tflops" if alu_bound else "alg_gbs"],
                 "peak": FP32_PEAK_TFLOPS if alu_bound else peak, "unit": "TFLOP/s" if alu_bound else "GB/s",

@@ -156,6 +156,9 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
 // A' is transposed on the way in (B operand is N x K, K-major).  Two shared-memory stages: the MMAs of
 // block kb run while the threads stage block kb+1; tcgen05.commit on an mbarrier frees a stage.
 constexpr int TC_M = 128, TC_N = 128, TC_K = 32;
+constexpr int TC_THREADS = 512, TC_WARPS = TC_THREADS / 32;
+constexpr int TC_APASS = TC_M / (TC_WARPS * 4);        // A rows per thread (4 rows per warp and pass)
+constexpr int TC_BPASS = (TC_K / 4) / (TC_THREADS / 128);   // B K-cores per thread
 constexpr int TC_SBO = 128;                         // bytes between 8-row groups (one core matrix)
 constexpr int TC_LBO = (TC_M / 8) * 128 + 16;       // bytes between K cores; +16 spreads the staging stores over banks
 constexpr int TC_TILE = (TC_K / 4) * TC_LBO;        // bytes of one 128 x 32 operand tile
@@ -196,7 +199,7 @@ __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
     lo = x - hi;
 }
 
-__global__ void __launch_bounds__(256, 1) kd_proj_tc(int n, int ld, const float* __restrict__ S, const float* __restrict__ Ap,
+__global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const float* __restrict__ S, const float* __restrict__ Ap,
                                                      const float* __restrict__ U, const float* __restrict__ X,
                                                      const uint8_t* __restrict__ mask, const float* __restrict__ ubar,
                                                      const float* __restrict__ abar, float* __restrict__ A, cc_scal* sc,
@@ -228,46 +231,62 @@ __global__ void __launch_bounds__(256, 1) kd_proj_tc(int n, int ld, const float*
     // instruction descriptor (cute::UMMA::InstrDescriptor): D = F32, A = B = TF32, both K-major, N >> 3, M >> 4
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
 
-    float rsum[4] = {0.f, 0.f, 0.f, 0.f};
+    float rsum[TC_APASS];
+#pragma unroll
+    for (int q = 0; q < TC_APASS; ++q) rsum[q] = 0.f;
     const int nkb = (n + TC_K - 1) / TC_K;
+    // per-thread staging roles (fixed over the K loop)
+    const int a_kc = lane & 7;                       // A: 8 lanes walk one row's 128 bytes
+    const int b_nl = tid & 127, b_kc0 = tid >> 7;    // B: row = column c0 + b_nl of A', K cores b_kc0 + (TC_THREADS/128) pass
+    const int b_gc = c0 + b_nl;
+    const bool b_ok = b_gc < ld;
+    const float b_mean = b_ok ? __ldg(abar + b_gc) : 0.f;
+    float4 va[TC_APASS];
+    float vb[TC_BPASS][4];
+    auto load_block = [&](int k0) {                  // global -> registers (raw fp32), one K block ahead of the stores
+#pragma unroll
+        for (int pass = 0; pass < TC_APASS; ++pass) {
+            const int gi = i0 + pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3), gk = k0 + a_kc * 4;
+            va[pass] = (gi < n && gk < n) ? __ldg(reinterpret_cast<const float4*>(S + (size_t)gi * n + gk)) : f4(0.f);
+        }
+#pragma unroll
+        for (int pass = 0; pass < TC_BPASS; ++pass) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int gk2 = k0 + (b_kc0 + (TC_THREADS / 128) * pass) * 4 + q;
+                vb[pass][q] = (b_ok && gk2 < n) ? __ldg(Ap + (size_t)gk2 * ld + b_gc) - b_mean : 0.f;
+            }
+        }
+    };
+    if (nkb > 0) load_block(0);
     for (int kb = 0; kb < nkb; ++kb) {
-        const int st = kb & 1, k0 = kb * TC_K;
+        const int st = kb & 1;
         uint8_t* a_hi = sm + (size_t)(st * 4 + 0) * TC_TILE;
         uint8_t* a_lo = sm + (size_t)(st * 4 + 1) * TC_TILE;
         uint8_t* b_hi = sm + (size_t)(st * 4 + 2) * TC_TILE;
         uint8_t* b_lo = sm + (size_t)(st * 4 + 3) * TC_TILE;
         if (kb >= 2 && !mbar_wait(smem_u32(&mbar[st]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
-        // A operand: S[i0 + r][k0 + 4 kc .. +3], 8 lanes walk one row's 128 bytes
 #pragma unroll
-        for (int pass = 0; pass < 4; ++pass) {
-            const int r = pass * 32 + warp * 4 + (lane >> 3), kc = lane & 7;
-            const int gi = i0 + r, gk = k0 + kc * 4;
-            float4 v = f4(0.f);
-            if (gi < n && gk < n) v = __ldg(reinterpret_cast<const float4*>(S + (size_t)gi * n + gk));
+        for (int pass = 0; pass < TC_APASS; ++pass) {
+            const int r = pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3);
+            const float4 v = va[pass];
             rsum[pass] += (v.x + v.y) + (v.z + v.w);
             float4 h, l;
             split_tf32(v.x, h.x, l.x); split_tf32(v.y, h.y, l.y); split_tf32(v.z, h.z, l.z); split_tf32(v.w, h.w, l.w);
-            const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
+            const int off = a_kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
             *reinterpret_cast<float4*>(a_hi + off) = h;
             *reinterpret_cast<float4*>(a_lo + off) = l;
         }
-        // B operand: (A' - abar)^T, row = column c0 + nl of A', 4 consecutive k per 16-byte core row
 #pragma unroll
-        for (int pass = 0; pass < 4; ++pass) {
-            const int nl = tid & 127, kc = (tid >> 7) + 2 * pass;
-            const int gc = c0 + nl;
-            float v[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int gk = k0 + kc * 4 + q;
-                v[q] = (gc < ld && gk < n) ? __ldg(Ap + (size_t)gk * ld + gc) - __ldg(abar + gc) : 0.f;
-            }
+        for (int pass = 0; pass < TC_BPASS; ++pass) {
             float4 h, l;
-            split_tf32(v[0], h.x, l.x); split_tf32(v[1], h.y, l.y); split_tf32(v[2], h.z, l.z); split_tf32(v[3], h.w, l.w);
-            const int off = kc * TC_LBO + (nl >> 3) * TC_SBO + (nl & 7) * 16;
+            split_tf32(vb[pass][0], h.x, l.x); split_tf32(vb[pass][1], h.y, l.y);
+            split_tf32(vb[pass][2], h.z, l.z); split_tf32(vb[pass][3], h.w, l.w);
+            const int off = (b_kc0 + (TC_THREADS / 128) * pass) * TC_LBO + (b_nl >> 3) * TC_SBO + (b_nl & 7) * 16;
             *reinterpret_cast<float4*>(b_hi + off) = h;
             *reinterpret_cast<float4*>(b_lo + off) = l;
         }
+        if (kb + 1 < nkb) load_block((kb + 1) * TC_K);   // in flight across the fence, the barrier and the MMA issue
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
         __syncthreads();
         if (tid == 0) {
@@ -286,12 +305,12 @@ __global__ void __launch_bounds__(256, 1) kd_proj_tc(int n, int ld, const float*
     }
     // row sums of S: 8 lanes hold one row's partial sums
 #pragma unroll
-    for (int pass = 0; pass < 4; ++pass) {
+    for (int pass = 0; pass < TC_APASS; ++pass) {
         float v = rsum[pass];
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
         v += __shfl_xor_sync(0xffffffffu, v, 4);
-        if ((lane & 7) == 0) rs_s[pass * 32 + warp * 4 + (lane >> 3)] = v;
+        if ((lane & 7) == 0) rs_s[pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3)] = v;
     }
     {   // all MMAs done (commits complete in issue order)
         const int kl = nkb - 1;
@@ -299,13 +318,14 @@ __global__ void __launch_bounds__(256, 1) kd_proj_tc(int n, int ld, const float*
     }
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     __syncthreads();
-    // epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (its rows); warps 0-3 take columns 0..63, 4-7 take 64..127
+    // epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (its rows) and the column group w / 4
     const float inv = 1.f / (float)(n + 1), fn = (float)n;
     double red[2] = {0.0, 0.0};
     const int row = (warp & 3) * 32 + lane, gi = i0 + row;
     const float rs = rs_s[row];
+    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);   // columns per warp
 #pragma unroll 1
-    for (int cb = (warp >> 2) * 64; cb < (warp >> 2) * 64 + 64; cb += 16) {
+    for (int cb = (warp >> 2) * TC_CPW; cb < (warp >> 2) * TC_CPW + TC_CPW; cb += 16) {
         uint32_t v[16];
         const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cb;
         asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
@@ -340,7 +360,7 @@ __global__ void __launch_bounds__(256, 1) kd_proj_tc(int n, int ld, const float*
     if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(TC_N));
     if (tid == 0 && fail_s) sc->cg_failed = 2;
     double tot[2];
-    if (grid_reduce<2>(red, part, &sc->ticket[0], tot)) {
+    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[0], tot)) {
         sc->dist2 = tot[0];
         sc->loss = tot[1];
         prof_mark(sc, 5);
@@ -641,7 +661,7 @@ static void launch_proj(cc_handle* h) {
 void ccd_proj(cc_handle* h) {
     if (h->dn_tc) {
         dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
-        kd_proj_tc<<<g, 256, TC_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar,
+        kd_proj_tc<<<g, TC_THREADS, TC_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar,
                                                    h->abar, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART);
         return;
     }

@@ -40,9 +40,9 @@ __device__ __forceinline__ float group_sum(float v, unsigned m) {
 // Deterministic grid reduction of NV doubles per thread.  Every block writes its partial sums; the
 // block that takes the last ticket adds all partials in a fixed order.  Returns true in thread 0 of
 // that last block, with the totals in out[].  All other blocks have finished their work by then.
-template <int NV>
+template <int NV, int NT = CC_THREADS>
 __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket, double (&out)[NV]) {
-    __shared__ double sm[NV][CC_THREADS / 32];
+    __shared__ double sm[NV][NT / 32];
     __shared__ bool last;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const unsigned bid = blockIdx.y * gridDim.x + blockIdx.x, nblk = gridDim.x * gridDim.y;   // 1-D or 2-D grids
@@ -58,7 +58,7 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
 #pragma unroll
         for (int k = 0; k < NV; ++k) {
             double x = 0.0;
-            for (int w2 = 0; w2 < CC_THREADS / 32; ++w2) x += sm[k][w2];
+            for (int w2 = 0; w2 < NT / 32; ++w2) x += sm[k][w2];
             part[(size_t)bid * NV + k] = x;
         }
         __threadfence();
@@ -71,7 +71,7 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
 #pragma unroll
     for (int k = 0; k < NV; ++k) {
         double x = 0.0;
-        for (unsigned b = threadIdx.x; b < nblk; b += CC_THREADS) x += __ldcg(&part[(size_t)b * NV + k]);
+        for (unsigned b = threadIdx.x; b < nblk; b += NT) x += __ldcg(&part[(size_t)b * NV + k]);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
         __syncthreads();
@@ -79,7 +79,7 @@ __device__ bool grid_reduce(double (&v)[NV], double* part, unsigned int* ticket,
         __syncthreads();
         if (threadIdx.x == 0) {
             double y = 0.0;
-            for (int w2 = 0; w2 < CC_THREADS / 32; ++w2) y += sm[k][w2];
+            for (int w2 = 0; w2 < NT / 32; ++w2) y += sm[k][w2];
             out[k] = y;
         }
     }

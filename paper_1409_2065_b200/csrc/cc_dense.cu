@@ -10,8 +10,8 @@
 //                (optionally split over column ranges), d_m, Phi_m, stop rule
 //   k_update     a5     (the sparse file's kernel, node part only)
 //   kd_edges     a4     S, ||v|| from ||b||^2 and W, elementwise over the n x n matrices
-// This round the contraction runs on FP32 FFMA with 8x8 (or 4x4) register tiles; the tcgen05 3xTF32
-// version is the next step.  V (|E| x p: 34 GB at n=8192, p=256) is never formed.
+// The contraction runs on tcgen05 (kd_proj_tc: kind::tf32, 3xTF32 split, TMEM accumulator) when n >= 128, on
+// FP32 FFMA register tiles (kd_proj) for small n.  V (|E| x p: 34 GB at n=8192, p=256) is never formed.
 #include <cstdio>
 
 #include "cc_device.cuh"

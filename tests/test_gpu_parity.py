@@ -96,6 +96,45 @@ def test_large_sparse_reduced(B, torch_, oracle):
     assert out[-1][1] < 100   # the path really fuses
 
 
+def test_large_sparse_20k_end_to_end(B, torch_, oracle):
+    """configs[3]'s generator at n = 20,000 (hundreds of row blocks, hubs): graph built on the GPU by
+    cc_knn_weights and required to equal the oracle's brute-force graph, then the MM iteration on it."""
+    torch = torch_
+    wl = synth.make("large_sparse", n=20000, p=64, n_clusters=20)
+    prob = H.build_problem(oracle, wl)
+    dev = torch.device("cuda:0")
+    X = torch.from_numpy(wl.X).to(dev)
+    rowptr, col, w = B.cc_knn_weights(wl.n, wl.p, X, None, wl.k, prob["phi"])
+    assert np.array_equal(rowptr.cpu().numpy(), prob["rowptr"])
+    assert np.array_equal(col.cpu().numpy(), prob["col"])
+    assert np.abs(w.cpu().numpy() - prob["wcsr32"]).max() <= 1e-5 * prob["wcsr32"].max()
+    gammas = [3.0, 60.0]
+    ref = H.oracle_path(oracle, prob, gammas, 15, proj_method=1)
+    _run_path(B, torch, prob, gammas, 15, ref)
+
+
+def test_path_with_stop_rule_expression_masked(B, torch_, oracle):
+    """cc_path with tol > 0 on a masked instance: per-gamma iteration counts (S3), labels and U follow the oracle."""
+    torch = torch_
+    wl = synth.make("expression", n=60, p=400)
+    prob = H.build_problem(oracle, wl)
+    gammas = [float(g) for g in synth.gamma_grid(1.0, 60.0, 5)]
+    tol = 1e-4
+    ref = oracle.path(prob["X64"], prob["mask"], prob["ei"], prob["ej"], prob["w64"], gammas, 3000, tol=tol, min_it=10)
+    h = H.gpu_create(B, torch, prob)
+    its, phis = B.cc_path(h, gammas, tol, 3000)
+    U = torch.empty(wl.n, wl.p)
+    lab = torch.empty(wl.n, dtype=torch.int32)
+    for gi, r in enumerate(ref):
+        assert abs(its[gi] - r["iters"]) <= max(3, r["iters"] // 20), (gi, its[gi], r["iters"])
+        B.cc_get_U(h, gi, U)
+        # the two runs may stop a few iterations apart, each iteration moves U by O(kappa * step): compare loosely
+        assert H.relerr(U.numpy().astype(np.float64), r["U"]) <= 2e-3, gi
+        _, k = B.cc_clusters(h, gi, lab)
+        assert abs(k - r["nclusters"]) <= max(1, r["nclusters"] // 20), (gi, k, r["nclusters"])
+    B.cc_destroy(h)
+
+
 @pytest.mark.parametrize("n,p,deg,miss", [(50, 7, 3.0, 0.0), (33, 130, 4.0, 0.15), (200, 2, 6.0, 0.0),
                                           (17, 1, 2.0, 0.0)])
 def test_ragged_shapes_random_graphs(B, torch_, oracle, n, p, deg, miss):

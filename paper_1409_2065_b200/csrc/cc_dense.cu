@@ -457,6 +457,159 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
     }
 }
 
+// ---- kd_small: the whole pair/projection work of one iteration for n <= 64 (genotype shape) ---------------
+// All n rows of a chunk of 32 columns fit in shared memory together with S (n x n), so U and A' are read
+// once, A is written once, and projection, ||U-A||^2, loss, ||b||^2 and ||s b' - b||^2 are all formed from
+// shared memory.  A CTA walks chunks grid-stride and keeps its pair accumulators in registers; it writes
+// one slice of partial ||b||^2 per (CTA, column phase) at the end (kd_edges adds the slices in order).
+// Pairs are covered by 4 x 4 register tiles, only the tiles on or above the diagonal, SM_CS threads per tile
+// taking interleaved columns.
+constexpr int SM_N = 64, SM_C = 32;
+
+__global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, const float* __restrict__ S,
+                                                const float* __restrict__ Ap, const float* __restrict__ U,
+                                                const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                const float* __restrict__ W, const float* __restrict__ VN,
+                                                float* __restrict__ A, float* __restrict__ NB2, cc_scal* sc, double* part,
+                                                double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer,
+                                                int init_only) {
+    if (!init_only && !sc->mm_active) return;
+    __shared__ __align__(16) float SsT[SM_N][SM_N + 4];   // S transposed: 8 consecutive rows i of column j as two float4
+    __shared__ float Us[SM_N][SM_C + 1], Ps[SM_N][SM_C + 1], As[SM_N][SM_C + 1];
+    __shared__ float ubar_s[SM_C];
+    __shared__ unsigned char t_ty[136], t_tx[136];
+    __shared__ int ntiles_s;
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        int k = 0;
+        const int nt4 = (n + 3) / 4;
+        for (int ty = 0; ty < nt4; ++ty)
+            for (int tx = ty; tx < nt4; ++tx) { t_ty[k] = (unsigned char)ty; t_tx[k] = (unsigned char)tx; ++k; }
+        ntiles_s = k;
+    }
+    for (int t = tid; t < SM_N * SM_N; t += 256) {
+        const int i = t / SM_N, j = t % SM_N;
+        const float v = (!init_only && i < n && j < n) ? S[(size_t)i * n + j] : 0.f;
+        SsT[j][i] = v;
+    }
+    __syncthreads();
+    const int ntiles = ntiles_s;
+    const bool pair_thread = tid < ntiles * cs_per_tile;
+    const int tile = pair_thread ? tid / cs_per_tile : 0, cph = tid % cs_per_tile;
+    const int ty = t_ty[tile], tx = t_tx[tile];
+    float sv[4][4], nb[4][4], dv[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) { sv[a][b] = SsT[tx * 4 + b][ty * 4 + a]; nb[a][b] = 0.f; dv[a][b] = 0.f; }
+    double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
+    const float inv = 1.f / (float)(n + 1), fn = (float)n;
+    const int nchunks = (ld + SM_C - 1) / SM_C;
+    for (int chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
+        const int c0 = chunk * SM_C;
+        for (int t = tid; t < SM_N * SM_C; t += 256) {
+            const int r = t / SM_C, c = t % SM_C;
+            const bool ok = r < n && c0 + c < ld;
+            const float u = ok ? U[(size_t)r * ld + c0 + c] : 0.f;
+            Us[r][c] = u;
+            Ps[r][c] = init_only ? u : (ok ? Ap[(size_t)r * ld + c0 + c] : 0.f);
+            if (init_only) As[r][c] = u;
+        }
+        __syncthreads();
+        if (!init_only) {
+            if (tid < SM_C) {
+                float s = 0.f;
+                for (int r = 0; r < n; ++r) s += Us[r][tid];
+                ubar_s[tid] = s / fn;
+            }
+            __syncthreads();
+            const int c = tid & 31;
+            float dua = 0.f, los = 0.f;
+            // warp w owns rows 8w .. 8w+7 of column c: per j one load of a'_j and two broadcast float4 of S
+            const int i0r = (tid >> 5) * 8;
+            if (i0r < n) {
+                float pi[8], g[8];
+#pragma unroll
+                for (int k = 0; k < 8; ++k) { pi[k] = Ps[i0r + k][c]; g[k] = 0.f; }
+                for (int j = 0; j < n; ++j) {
+                    const float pj = Ps[j][c];
+                    const float4 s0 = *reinterpret_cast<const float4*>(&SsT[j][i0r]);
+                    const float4 s1 = *reinterpret_cast<const float4*>(&SsT[j][i0r + 4]);
+                    g[0] = fmaf(s0.x, pi[0] - pj, g[0]); g[1] = fmaf(s0.y, pi[1] - pj, g[1]);
+                    g[2] = fmaf(s0.z, pi[2] - pj, g[2]); g[3] = fmaf(s0.w, pi[3] - pj, g[3]);
+                    g[4] = fmaf(s1.x, pi[4] - pj, g[4]); g[5] = fmaf(s1.y, pi[5] - pj, g[5]);
+                    g[6] = fmaf(s1.z, pi[6] - pj, g[6]); g[7] = fmaf(s1.w, pi[7] - pj, g[7]);
+                }
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    const int i = i0r + k;
+                    if (i < n) {
+                        const float u = Us[i][c];
+                        const float dl = inv * (g[k] - fn * (u - ubar_s[c]));
+                        const float a = u + dl;
+                        As[i][c] = a;
+                        if (c0 + c < ld) {
+                            const size_t o = (size_t)i * ld + c0 + c;
+                            A[o] = a;
+                            dua = fmaf(dl, dl, dua);
+                            const float q = X[o] - u;
+                            if (!mask || mask[o]) los = fmaf(q, q, los);
+                        }
+                    }
+                }
+            }
+            red[0] += (double)dua;
+            red[1] += (double)los;
+            __syncthreads();
+        }
+        if (pair_thread) {
+            for (int c = cph; c < SM_C; c += cs_per_tile) {
+                float ai[4], aj[4], pi[4], pj[4];
+#pragma unroll
+                for (int a = 0; a < 4; ++a) {
+                    ai[a] = As[ty * 4 + a][c]; pi[a] = Ps[ty * 4 + a][c];
+                    aj[a] = As[tx * 4 + a][c]; pj[a] = Ps[tx * 4 + a][c];
+                }
+#pragma unroll
+                for (int a = 0; a < 4; ++a)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) {
+                        const float bb = ai[a] - aj[b];
+                        const float tt = fmaf(sv[a][b], pi[a] - pj[b], -bb);
+                        nb[a][b] = fmaf(bb, bb, nb[a][b]);
+                        dv[a][b] = fmaf(tt, tt, dv[a][b]);
+                    }
+            }
+        }
+        __syncthreads();
+    }
+    if (pair_thread) {
+        float* out = NB2 + (size_t)(blockIdx.x * cs_per_tile + cph) * n * n;
+#pragma unroll
+        for (int a = 0; a < 4; ++a)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                const int gi = ty * 4 + a, gj = tx * 4 + b;
+                if (gi < n && gj < n && gi != gj) {
+                    out[(size_t)gi * n + gj] = nb[a][b];
+                    if (ty != tx) out[(size_t)gj * n + gi] = nb[a][b];
+                    if (gi < gj) {
+                        red[2] += (double)dv[a][b];
+                        if (blockIdx.x == 0 && cph == 0 && !init_only)
+                            red[3] += (double)(W[(size_t)gi * n + gj] * VN[(size_t)gi * n + gj]);
+                    }
+                }
+            }
+    }
+    double tot[4];
+    if (grid_reduce<4>(red, part, &sc->ticket[3], tot)) {
+        if (!init_only) {
+            finish_iteration(sc, tot[0] + tot[2], tot[1], tot[3], hist_phi, hist_d, outer);
+            prof_mark(sc, 5);
+        }
+    }
+}
+
 // ---- kd_edges: block soft-threshold over the n x n matrices ------------------
 __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, int init_only) {
@@ -681,6 +834,12 @@ static void launch_pairs(cc_handle* h, const float* A, const float* Ap, int init
 
 void ccd_pairs(cc_handle* h) { launch_pairs(h, h->A, h->Ap, 0); }
 
+static void launch_small(cc_handle* h, int init_only) {
+    kd_small<<<h->dn_small_grid, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X, h->mask,
+                                                      h->Wd, h->VNd, h->A, h->NB2d, h->sc, h->part + 3 * CC_MAXBLK * CC_NPART,
+                                                      h->hist_phi, h->hist_d, init_only ? 0 : h->cond_outer, init_only);
+}
+
 void ccd_edges(cc_handle* h, int init_only) {
     kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc, init_only);
 }
@@ -707,6 +866,20 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (ks > ksmax) ks = ksmax;
     if (ks < 1) ks = 1;
     h->dn_ksplit = (int)ks;
+    // n <= 64: the fused kernel; its slices are (CTA, column phase)
+    h->dn_small = (n <= SM_N && h->prm.reserved0 != 4) ? 1 : 0;
+    if (h->dn_small) {
+        const int nt4 = (int)((n + 3) / 4), ntiles = nt4 * (nt4 + 1) / 2;
+        int cs = 256 / ntiles;
+        if (cs > 4) cs = 4;
+        if (cs < 1) cs = 1;
+        long long g = (h->ld + SM_C - 1) / SM_C;
+        if (g > 2LL * h->sms) g = 2LL * h->sms;
+        h->dn_small_cs = cs;
+        h->dn_small_grid = (int)g;
+        h->dn_ksplit = (int)g * cs;
+        ks = h->dn_ksplit;
+    }
     const long long bproj = ((h->ld + 63) / 64) * ((n + 63) / 64);   // upper bound over the tile shapes used
     if (ntp * ks > CC_MAXBLK || bproj > CC_MAXBLK) {
         snprintf(h->err, sizeof(h->err), "dense mode: problem too large for this build (n=%lld, p=%lld)", (long long)n, (long long)h->p);
@@ -757,12 +930,19 @@ void ccd_sumw2(cc_handle* h) {
 void ccd_init_state(cc_handle* h) {
     const size_t bytes = (size_t)h->n * h->ld * sizeof(float);
     cudaMemcpyAsync(h->Ap, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
-    launch_pairs(h, h->U, h->U, 1);
+    if (h->dn_small) launch_small(h, 1);
+    else launch_pairs(h, h->U, h->U, 1);
     ccd_edges(h, 1);
     h->launches += 2;
 }
 
 void ccd_iteration(cc_handle* h) {
+    if (h->dn_small) {
+        launch_small(h, 0);
+        ccs_update_nodes(h);
+        ccd_edges(h, 0);
+        return;
+    }
     ccd_colmeans(h);
     ccd_proj(h);
     ccd_pairs(h);

@@ -83,7 +83,7 @@ struct cc_handle {
     float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices)
     float *ubar, *abar;               // column means of U and A'
     double* colps;                    // partial column sums
-    int dn_ksplit, dn_big, dn_tc;
+    int dn_ksplit, dn_big, dn_tc, dn_small, dn_small_cs, dn_small_grid;
     // scalars
     cc_scal* sc;                      // device
     cc_scal* sc_host;                 // pinned mirror

@@ -40,9 +40,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 GRID = {"large_sparse": (1.0, 1000.0, 50), "tiny": (1e-3, 1e3, 20), "expression": (0.05, 50.0, 40),
-        "genotype": (1.0, 100.0, 50), "dense_weight": (1.0, 100.0, 30)}
+        "genotype": (1.0, 100.0, 50), "dense_weight": (1.0, 100.0, 30), "popres": (0.01, 10.0, 30)}
 CPU_SAMPLE = {"large_sparse": lambda a: {"n": a.cpu_n}, "genotype": lambda a: {"p": 20000},
-              "dense_weight": lambda a: {"n": 512}, "tiny": lambda a: {}, "expression": lambda a: {}}
+              "dense_weight": lambda a: {"n": 512}, "tiny": lambda a: {}, "expression": lambda a: {},
+              "popres": lambda a: {}}
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 flop/FMA x max clock (B200_PROFILING.md table)
 
 

@@ -14,7 +14,7 @@ from __future__ import annotations
 import dataclasses
 import numpy as np
 
-CONFIG_NAMES = ("tiny", "expression", "genotype", "large_sparse", "dense_weight")
+CONFIG_NAMES = ("tiny", "expression", "genotype", "large_sparse", "dense_weight", "popres")
 
 
 @dataclasses.dataclass
@@ -122,12 +122,28 @@ def make_dense_weight(seed=0, n=8192, p=256, n_clusters=32):
     return Workload("dense_weight", _f32(X), None, "complete", 0, "inv_median", 0.0, 30, seed)
 
 
+def make_popres(seed=0, n=3000, p=10, k=40, phi=0.0):
+    """SURVEY 8(f) f3, cf. POPRES (1,896 subjects -> 370 plotted x 10 principal components,
+    k = 40, phi in {0, 10}): many points, low p, large k.  A smooth cline plus weak population structure: 6 loose
+    groups along a 2-D gradient embedded in p dimensions, like top principal components.  phi = 0 gives the
+    uniform weights of L131."""
+    rng = np.random.default_rng(seed)
+    centres2 = rng.uniform(-1.0, 1.0, size=(6, 2))
+    lab = np.arange(n) % 6
+    xy = centres2[lab] + 0.35 * rng.normal(size=(n, 2))
+    X = 0.05 * rng.normal(size=(n, p))
+    X[:, :2] += xy
+    X[:, 2:] *= np.linspace(1.0, 0.3, p - 2)[None, :] if p > 2 else 1.0
+    return Workload("popres", _f32(X), None, "knn", k, "fixed", float(phi), 30, seed)
+
+
 _MAKERS = {
     "tiny": make_tiny,
     "expression": make_expression,
     "genotype": make_genotype,
     "large_sparse": make_large_sparse,
     "dense_weight": make_dense_weight,
+    "popres": make_popres,
 }
 
 

@@ -113,6 +113,17 @@ def test_large_sparse_20k_end_to_end(B, torch_, oracle):
     _run_path(B, torch, prob, gammas, 15, ref)
 
 
+@pytest.mark.parametrize("phi", [0.0, 10.0])
+def test_popres_like_low_p_large_k(B, torch_, oracle, phi):
+    """low p (row groups of 4 lanes), k = 40, uniform weights (phi = 0) and phi = 10."""
+    wl = synth.make("popres", n=400, phi=phi)
+    prob = H.build_problem(oracle, wl)
+    gammas = [0.05, 0.5, 5.0]     # oracle: 400 -> 22 -> 1 clusters (phi = 0), 400 -> 344 -> 20 (phi = 10)
+    ref = H.oracle_path(oracle, prob, gammas, 150, proj_method=1)
+    out = _run_path(B, torch_, prob, gammas, 150, ref)
+    print("popres phi", phi, "clusters", [k for _, k in out])
+
+
 def test_path_with_stop_rule_expression_masked(B, torch_, oracle):
     """cc_path with tol > 0 on a masked instance: per-gamma iteration counts (S3), labels and U follow the oracle."""
     torch = torch_

@@ -94,6 +94,17 @@ int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, 
 /* Release the three arrays cc_knn_weights returned (NULLs are ignored). */
 void cc_free_graph(int64_t* rowptr, int32_t* col, float* w);
 
+/* ---- f4: graph utilities -------------------------------------------------------------
+ * Connected components of a symmetric CSR graph (rowptr int64[n+1], col int32[nnz]; DEVICE): labels_out
+ * (DEVICE int32[n]) numbered by smallest member, *ncomponents (HOST, may be NULL).  Synchronises `stream`. */
+int cc_graph_components(int64_t n, const int64_t* rowptr, const int32_t* col, int32_t* labels_out,
+                        int32_t* ncomponents, void* stream);
+
+/* Smallest k <= min(kmax, n-1, 64) whose OR-symmetrised k-NN graph (cc_knn_weights) is connected, found by
+ * bisection -- the graphs are nested in k (L150).  *k_out (HOST) = -1 when even kmax is not connected. */
+int cc_smallest_connected_k(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t kmax,
+                            int32_t* k_out, void* stream);
+
 /* ---- problem set-up --------------------------------------------------------------------------------
  * Validates the inputs once (error codes above), copies them, builds the internal layout and sets the
  * cold start (S4): U0 = X with missing entries set to the observed column mean, V0 = D U0.

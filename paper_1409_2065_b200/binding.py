@@ -22,7 +22,8 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
-SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_dense_weights", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
+SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_dense_weights", "cc_graph_components",
+           "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
            "cc_get_U", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
            "cc_last_error", "cc_destroy")
@@ -41,6 +42,8 @@ _lib.cc_default_params.argtypes = [_P(cc_params)]
 _lib.cc_knn_weights.argtypes = [_i64, _i64, _vp, _vp, _i32, ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp),
                                 _P(_i64), _vp]
 _lib.cc_dense_weights.argtypes = [_i64, _i64, _vp, _vp, ctypes.c_float, _i32, _vp, _vp]
+_lib.cc_graph_components.argtypes = [_i64, _vp, _vp, _vp, _P(_i32), _vp]
+_lib.cc_smallest_connected_k.argtypes = [_i64, _i64, _vp, _vp, _i32, _P(_i32), _vp]
 _lib.cc_free_graph.argtypes = [_vp, _vp, _vp]
 _lib.cc_free_graph.restype = None
 _lib.cc_create.argtypes = [_P(_vp), _i64, _i64, _vp, _vp, _vp, _vp, _vp, _P(cc_params), _vp]
@@ -183,6 +186,18 @@ def cc_dense_weights(n, p, X, mask, phi, normalize=False):
     W = torch.empty(n, n, dtype=torch.float32, device=X.device)
     _check(_lib.cc_dense_weights(n, p, _ptr(X), _ptr(mask), phi, 1 if normalize else 0, _ptr(W), _stream()))
     return W
+
+
+def cc_graph_components(n, rowptr, col, labels_out):
+    k = _i32(0)
+    _check(_lib.cc_graph_components(n, _ptr(rowptr), _ptr(col), _ptr(labels_out), ctypes.byref(k), _stream()))
+    return labels_out, k.value
+
+
+def cc_smallest_connected_k(n, p, X, mask, kmax):
+    k = _i32(0)
+    _check(_lib.cc_smallest_connected_k(n, p, _ptr(X), _ptr(mask), kmax, ctypes.byref(k), _stream()))
+    return k.value
 
 
 class _DevArray:

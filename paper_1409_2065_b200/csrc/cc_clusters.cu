@@ -14,14 +14,15 @@ __global__ void k_lab_init(int n, int* __restrict__ lab) {
 }
 
 // One thread per row: smallest label among the row and its fused neighbours; hook the old root to it.
-__global__ void k_lab_hook(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+template <typename RP>
+__global__ void k_lab_hook(int n, const RP* __restrict__ rowptr, const int* __restrict__ col,
                            const float* __restrict__ s, int* lab, int* changed) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const int li = lab[i];
     int m = li;
-    for (int e = rowptr[i]; e < rowptr[i + 1]; ++e)
-        if (s[e] == 0.f) m = min(m, lab[col[e]]);
+    for (long long e = rowptr[i]; e < rowptr[i + 1]; ++e)
+        if (!s || s[e] == 0.f) m = min(m, lab[col[e]]);   // s == NULL: every edge joins (plain graph components)
     if (m < li) {
         atomicMin(&lab[li], m);
         atomicMin(&lab[i], m);
@@ -88,7 +89,7 @@ int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host) {
     for (int round = 0; round < 100000; ++round) {
         CC_CUDA(h, cudaMemsetAsync(h->lab_flag, 0, sizeof(int), st));
         if (h->dense) ccd_lab_hook(h, h->lab_flag);
-        else k_lab_hook<<<grid, 256, 0, st>>>(n, h->rowptr, h->col, h->s, h->lab, h->lab_flag);
+        else k_lab_hook<int><<<grid, 256, 0, st>>>(n, h->rowptr, h->col, h->s, h->lab, h->lab_flag);
         k_lab_jump<<<grid, 256, 0, st>>>(n, h->lab);
         h->launches += 2;
         int changed = 0;
@@ -103,5 +104,75 @@ int ccl_labels(cc_handle* h, int32_t* labels_dev, int32_t* nclusters_host) {
     CC_CUDA(h, cudaMemcpyAsync(&k, h->lab_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     CC_CUDA(h, cudaStreamSynchronize(st));
     if (nclusters_host) *nclusters_host = k;
+    return CC_OK;
+}
+
+
+// ---- f4: graph utilities ("the smallest k giving a connected graph") -------------------------
+extern "C" int cc_graph_components(int64_t n, const int64_t* rowptr, const int32_t* col, int32_t* labels_out,
+                                   int32_t* ncomponents, void* stream) {
+    if (n < 1 || n > 2147483647LL || !rowptr || !labels_out) {
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_graph_components: bad arguments");
+        return CC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    int *lab = nullptr, *rank = nullptr, *flag = nullptr;
+    cudaError_t e = cc_dev_alloc((void**)&lab, (size_t)n * sizeof(int), st);
+    if (e == cudaSuccess) e = cc_dev_alloc((void**)&rank, (size_t)n * sizeof(int), st);
+    if (e == cudaSuccess) e = cc_dev_alloc((void**)&flag, sizeof(int), st);
+    int k = 0;
+    const int grid = (int)((n + 255) / 256);
+    if (e == cudaSuccess) {
+        k_lab_init<<<grid, 256, 0, st>>>((int)n, lab);
+        for (int round = 0; round < 100000 && e == cudaSuccess; ++round) {
+            cudaMemsetAsync(flag, 0, sizeof(int), st);
+            k_lab_hook<int64_t><<<grid, 256, 0, st>>>((int)n, rowptr, col, (const float*)nullptr, lab, flag);
+            k_lab_jump<<<grid, 256, 0, st>>>((int)n, lab);
+            int changed = 0;
+            e = cudaMemcpyAsync(&changed, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+            if (!changed) break;
+        }
+        k_lab_rank<<<1, 1024, 0, st>>>((int)n, lab, rank, flag);
+        k_lab_final<<<grid, 256, 0, st>>>((int)n, lab, rank, labels_out);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(&k, flag, sizeof(int), cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+    cc_dev_free(lab, st); cc_dev_free(rank, st); cc_dev_free(flag, st);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_graph_components: %s", cudaGetErrorString(e));
+        return e == cudaErrorMemoryAllocation ? CC_ENOMEM : CC_ECUDA;
+    }
+    if (ncomponents) *ncomponents = k;
+    return CC_OK;
+}
+
+extern "C" int cc_smallest_connected_k(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t kmax,
+                                       int32_t* k_out, void* stream) {
+    if (!k_out || kmax < 1) { snprintf(cc_g_err, sizeof(cc_g_err), "cc_smallest_connected_k: bad arguments"); return CC_EINVAL; }
+    if (kmax > n - 1) kmax = (int32_t)(n - 1);
+    if (kmax > 64) kmax = 64;
+    cudaStream_t st = (cudaStream_t)stream;
+    int32_t* lab = nullptr;
+    cudaError_t e = cc_dev_alloc((void**)&lab, (size_t)n * sizeof(int32_t), st);
+    if (e != cudaSuccess) { cudaGetLastError(); snprintf(cc_g_err, sizeof(cc_g_err), "cc_smallest_connected_k: out of device memory"); return CC_ENOMEM; }
+    // the symmetrised k-NN graphs are nested in k, so connectivity is monotone: bisection (L150)
+    int lo = 1, hi = kmax, best = -1, rc = CC_OK;
+    while (lo <= hi && rc == CC_OK) {
+        const int mid = (lo + hi) / 2;
+        int64_t *rp = nullptr, nnz = 0;
+        int32_t* cl = nullptr;
+        float* w = nullptr;
+        rc = cc_knn_weights(n, p, X, mask, mid, 0.f, 0, &rp, &cl, &w, &nnz, stream);
+        int32_t nc = 0;
+        if (rc == CC_OK) rc = cc_graph_components(n, rp, cl, lab, &nc, stream);
+        cc_free_graph(rp, cl, w);
+        if (rc != CC_OK) break;
+        if (nc == 1) { best = mid; hi = mid - 1; } else lo = mid + 1;
+    }
+    cc_dev_free(lab, st);
+    if (rc != CC_OK) return rc;
+    *k_out = best;   // -1: not connected even at kmax
     return CC_OK;
 }

@@ -114,6 +114,46 @@ def test_dense_weights_match_oracle(B, oracle, name, kw, phi, norm):
     assert np.abs(W - Wref).max() <= 2e-5 * Wref.max()
 
 
+def test_graph_utilities(B, oracle):
+    """f4: components of the k-NN graph and the smallest connected k, against a plain
+    union-find over the oracle's brute-force graphs."""
+    import torch
+
+    def components(n, ei, ej):
+        par = list(range(n))
+
+        def find(x):
+            while par[x] != x:
+                par[x] = par[par[x]]
+                x = par[x]
+            return x
+        for a, b in zip(ei, ej):
+            ra, rb = find(int(a)), find(int(b))
+            if ra != rb:
+                par[max(ra, rb)] = min(ra, rb)
+        roots = [find(i) for i in range(n)]
+        order = {r: k for k, r in enumerate(sorted(set(roots)))}
+        return np.array([order[r] for r in roots], np.int32)
+
+    wl = synth.make("tiny")
+    X64 = wl.X.astype(np.float64)
+    ei, ej, w, _ = oracle.knn_graph(X64, None, wl.k, 0.5)
+    ref = components(wl.n, ei, ej)
+    rp, cl, _w = oracle.to_csr(wl.n, ei, ej, w)
+    lab = torch.empty(wl.n, dtype=torch.int32, device="cuda:0")
+    _, k = B.cc_graph_components(wl.n, _dev(torch, rp.astype(np.int64)), _dev(torch, cl.astype(np.int32)), lab)
+    assert k == ref.max() + 1 and np.array_equal(lab.cpu().numpy(), ref)
+    assert k > 1                                   # the tiny config's 5-NN graph is disconnected (SURVEY S20)
+    kref = -1
+    for kk in range(1, 41):
+        e1, e2, _a, _b = oracle.knn_graph(X64, None, kk, 0.0)
+        if components(wl.n, e1, e2).max() == 0:
+            kref = kk
+            break
+    assert B.cc_smallest_connected_k(wl.n, wl.p, _dev(torch, wl.X), None, 40) == kref
+    assert B.cc_smallest_connected_k(wl.n, wl.p, _dev(torch, wl.X), None, max(1, kref - 1)) == -1
+
+
 def test_full_size_large_sparse_properties(B):
     """configs[3] at full size, in the launch configuration bench.py times: properties that hold at
     any size -- Phi non-increasing, column sums of U equal those of X when nothing

@@ -123,6 +123,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
     S->xscale = sqrt(h->xss);
     S->proj_tol = h->prm.proj_tol;
     S->d = S->d_prev = sqrt(S->eps);
+    S->cthr = (float)(gamma * S->d / S->rho);   // threshold factor of a feasible start (kd_pairs_tc's recompute rule)
     S->mm_maxit = maxit;
     S->mm_min_it = h->prm.min_it;
     S->mm_active = 1;

@@ -367,6 +367,218 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
     }
 }
 
+// ---- kd_pairs_tc: pair norms on the tensor cores, with a direct fp32 recompute where a Gram block is not enough ---
+// For a 128 x 128 tile of pairs (I <= J), with alpha = a - abar (any common shift cancels) and e = a' - a:
+//   ||b||^2        = |alpha_i|^2 + |alpha_j|^2 - 2 G1,           G1 = alpha_I alpha_J^T
+//   b . delta      = alpha_i.e_i - G2 - G3 + alpha_j.e_j,        G2 = alpha_I e_J^T,  G3 = e_I alpha_J^T
+//   ||delta||^2    = |e_i|^2 + |e_j|^2 - 2 G4,                   G4 = e_I e_J^T          (delta = b' - b = e_i - e_j)
+//   ||s b' - b||^2 = (1-s)^2 ||b||^2 - 2 s (1-s) b.delta + s^2 ||delta||^2
+// -- the last line has no cancellation (each term is O(kappa^2) small), unlike an expansion around ||b||^2.
+// G1..G3 use the 3xTF32 split, G4 (tiny numbers) one TF32 product: 10 tcgen05.mma per K step, four fp32
+// accumulators = all 512 TMEM columns.  ||b||^2 from a Gram block carries an ABSOLUTE error ~ 3e-7 (|alpha_i|^2 +
+// |alpha_j|^2); a pair whose ||b||^2 is below CC_RECOMP_REL times that scale -- every pair that is fused, about to
+// fuse, or close inside a cluster -- is flagged in a shared-memory bit mask and recomputed by direct differences
+// in fp32 (one warp per pair), so the fused / not-fused decision never sees Gram rounding.
+constexpr int PK = 16;                               // K block: 16 columns = 4 K cores = 2 MMA K steps
+constexpr int PK_TILE = (PK / 4) * TC_LBO;           // bytes of one 128 x 16 operand tile
+constexpr int PK_SMEM = 2 * 8 * PK_TILE + 1024;      // 2 stages x {alpha,e} x {I,J} x {hi,lo}
+#define CC_RECOMP_REL 1.0e-2f
+
+__global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int ntile, const float* __restrict__ A,
+                                                      const float* __restrict__ Ap, const float* __restrict__ abar,
+                                                      const float* __restrict__ S, const float* __restrict__ W,
+                                                      const float* __restrict__ VN, float* __restrict__ NB2, cc_scal* sc,
+                                                      double* part, double* hist_phi, double* hist_d,
+                                                      cudaGraphConditionalHandle outer) {
+    if (!sc->mm_active) return;
+    extern __shared__ uint8_t tc_smem_raw[];
+    __shared__ __align__(8) uint64_t mbar[2];
+    __shared__ uint32_t tmem_base_s;
+    __shared__ float nrm[2][3][TC_M];                // [I/J][|alpha|^2, alpha.e, |e|^2][row]
+    __shared__ unsigned int flag_s[TC_M][4];         // recompute mask: row x 128 columns
+    __shared__ int fail_s;
+    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int I = 0, rem = blockIdx.x;
+    while (rem >= ntile - I) { rem -= ntile - I; ++I; }
+    const int J = I + rem, i0 = I * TC_M, j0 = J * TC_M;
+
+    if (tid == 0) {
+        fail_s = 0;
+        for (int b = 0; b < 2; ++b)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar[b])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_d = tmem_base_s;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+
+    // staging role: row r of both tiles, K core kc (4 lanes cover one row's 64 bytes of a K block)
+    const int r = tid >> 2, kc = tid & 3;
+    const int gI = i0 + r, gJ = j0 + r;
+    float nI[3] = {0.f, 0.f, 0.f}, nJ[3] = {0.f, 0.f, 0.f};
+    float4 aI, pI, aJ, pJ, mb;
+    const int nkb = (ld + PK - 1) / PK;
+    auto load_block = [&](int k0) {
+        const int gc = k0 + kc * 4;
+        const bool okc = gc < ld;
+        mb = okc ? ld4s(abar + gc) : f4(0.f);
+        aI = (okc && gI < n) ? ld4s(A + (size_t)gI * ld + gc) : mb;     // out-of-range rows/columns: alpha = e = 0
+        pI = (okc && gI < n) ? ld4s(Ap + (size_t)gI * ld + gc) : mb;
+        aJ = (okc && gJ < n) ? ld4s(A + (size_t)gJ * ld + gc) : mb;
+        pJ = (okc && gJ < n) ? ld4s(Ap + (size_t)gJ * ld + gc) : mb;
+    };
+    auto stage_side = [&](uint8_t* base, const float4& a, const float4& pp, float (&nr)[3]) {
+        const float4 al = a - mb, e = pp - a;
+        nr[0] += dot4(al, al); nr[1] += dot4(al, e); nr[2] += dot4(e, e);
+        float4 h, l;
+        const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
+        split_tf32(al.x, h.x, l.x); split_tf32(al.y, h.y, l.y); split_tf32(al.z, h.z, l.z); split_tf32(al.w, h.w, l.w);
+        *reinterpret_cast<float4*>(base + 0 * PK_TILE + off) = h;
+        *reinterpret_cast<float4*>(base + 1 * PK_TILE + off) = l;
+        split_tf32(e.x, h.x, l.x); split_tf32(e.y, h.y, l.y); split_tf32(e.z, h.z, l.z); split_tf32(e.w, h.w, l.w);
+        *reinterpret_cast<float4*>(base + 2 * PK_TILE + off) = h;
+        *reinterpret_cast<float4*>(base + 3 * PK_TILE + off) = l;
+    };
+    if (nkb > 0) load_block(0);
+    for (int kb = 0; kb < nkb; ++kb) {
+        const int st = kb & 1;
+        uint8_t* sI = sm + (size_t)(st * 8 + 0) * PK_TILE;   // alpha_hi, alpha_lo, e_hi, e_lo of tile I
+        uint8_t* sJ = sm + (size_t)(st * 8 + 4) * PK_TILE;   // the same of tile J
+        if (kb >= 2 && !mbar_wait(smem_u32(&mbar[st]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
+        stage_side(sI, aI, pI, nI);
+        stage_side(sJ, aJ, pJ, nJ);
+        if (kb + 1 < nkb) load_block((kb + 1) * PK);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int ks = 0; ks < PK / 8; ++ks) {
+                const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
+                const uint32_t bI = smem_u32(sI) + koff, bJ = smem_u32(sJ) + koff;
+                const uint64_t Iah = tc_desc(bI), Ial = tc_desc(bI + PK_TILE), Ieh = tc_desc(bI + 2 * PK_TILE), Iel = tc_desc(bI + 3 * PK_TILE);
+                const uint64_t Jah = tc_desc(bJ), Jal = tc_desc(bJ + PK_TILE), Jeh = tc_desc(bJ + 2 * PK_TILE), Jel = tc_desc(bJ + 3 * PK_TILE);
+                const uint32_t acc = (kb > 0 || ks > 0) ? 1u : 0u;
+                tc_mma(tmem_d + 0 * TC_N, Iah, Jah, idesc, acc); tc_mma(tmem_d + 0 * TC_N, Iah, Jal, idesc, 1u); tc_mma(tmem_d + 0 * TC_N, Ial, Jah, idesc, 1u);
+                tc_mma(tmem_d + 1 * TC_N, Iah, Jeh, idesc, acc); tc_mma(tmem_d + 1 * TC_N, Iah, Jel, idesc, 1u); tc_mma(tmem_d + 1 * TC_N, Ial, Jeh, idesc, 1u);
+                tc_mma(tmem_d + 2 * TC_N, Ieh, Jah, idesc, acc); tc_mma(tmem_d + 2 * TC_N, Ieh, Jal, idesc, 1u); tc_mma(tmem_d + 2 * TC_N, Iel, Jah, idesc, 1u);
+                tc_mma(tmem_d + 3 * TC_N, Ieh, Jeh, idesc, acc);
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar[st])) : "memory");
+        }
+    }
+    // row norms: 4 lanes per row
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        float v = nI[q], u = nJ[q];
+        v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
+        u += __shfl_xor_sync(0xffffffffu, u, 1); u += __shfl_xor_sync(0xffffffffu, u, 2);
+        if (kc == 0) { nrm[0][q][r] = v; nrm[1][q][r] = u; }
+    }
+    if (tid < TC_M * 4) flag_s[tid >> 2][tid & 3] = 0u;
+    {
+        const int kl = nkb - 1;
+        if (nkb > 0 && !mbar_wait(smem_u32(&mbar[kl & 1]), (uint32_t)((kl >> 1) & 1))) fail_s = 1;
+    }
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    __syncthreads();
+    // epilogue: warp w owns TMEM lanes 32 (w % 4) .. (its rows) and the 32-column group w / 4 of all four accumulators
+    const int row = (warp & 3) * 32 + lane, gi = i0 + row, grp = warp >> 2;
+    const float naI = nrm[0][0][row], aeI = nrm[0][1][row], neI = nrm[0][2][row];
+    const float cthr_prev = sc->cthr;
+    double red[2] = {0.0, 0.0};      // sum_{i<j} ||v - b||^2,  sum_{i<j} w ||v||
+    unsigned int myflags = 0u;
+#pragma unroll 1
+    for (int half = 0; half < 2; ++half) {
+        const int cb = grp * 32 + half * 16;
+        uint32_t g[4][16];
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(a * TC_N + cb);
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                         : "=r"(g[a][0]), "=r"(g[a][1]), "=r"(g[a][2]), "=r"(g[a][3]), "=r"(g[a][4]), "=r"(g[a][5]), "=r"(g[a][6]),
+                           "=r"(g[a][7]), "=r"(g[a][8]), "=r"(g[a][9]), "=r"(g[a][10]), "=r"(g[a][11]), "=r"(g[a][12]),
+                           "=r"(g[a][13]), "=r"(g[a][14]), "=r"(g[a][15])
+                         : "r"(taddr));
+        }
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (gi < n) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const int cl = cb + q, gj = j0 + cl;
+                if (gj >= n || (I == J && gi >= gj)) continue;      // diagonal tiles: pairs i < j only, mirrored below
+                const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
+                const size_t o = (size_t)gi * n + gj;
+                const float w = __ldg(W + o);
+                float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
+                const float thr4 = 4.f * cthr_prev * w;
+                if (nb2 < CC_RECOMP_REL * (naI + naJ) || nb2 < thr4 * thr4) {
+                    myflags |= 1u << (half * 16 + q);               // recomputed directly below
+                } else {
+                    const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));
+                    const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
+                    const float sv = __ldg(S + o), om = 1.f - sv;
+                    const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
+                    NB2[o] = nb2;
+                    NB2[(size_t)gj * n + gi] = nb2;
+                    red[0] += (double)dv;
+                    red[1] += (double)(w * __ldg(VN + o));
+                }
+            }
+        }
+    }
+    flag_s[row][grp] = myflags;
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(512));
+    // flagged pairs: direct differences in fp32, one warp per pair, rows dealt to warps round-robin (fixed order)
+    for (int rr = warp; rr < TC_M; rr += TC_WARPS) {
+        const int gi2 = i0 + rr;
+        for (int gq = 0; gq < 4; ++gq) {
+            unsigned int m = flag_s[rr][gq];
+            while (m) {
+                const int b = __ffs(m) - 1;
+                m &= m - 1;
+                const int gj2 = j0 + gq * 32 + b;
+                const size_t o = (size_t)gi2 * n + gj2;
+                const float sv = __ldg(S + o);
+                float nbv = 0.f, dvv = 0.f;
+                for (int c = lane * 4; c < ld; c += 128) {
+                    const float4 bb = ld4s(A + (size_t)gi2 * ld + c) - ld4s(A + (size_t)gj2 * ld + c);
+                    const float4 bp = ld4s(Ap + (size_t)gi2 * ld + c) - ld4s(Ap + (size_t)gj2 * ld + c);
+                    const float4 tt = fma4(sv, bp, f4(0.f)) - bb;
+                    nbv += dot4(bb, bb);
+                    dvv += dot4(tt, tt);
+                }
+#pragma unroll
+                for (int of = 16; of > 0; of >>= 1) {
+                    nbv += __shfl_xor_sync(0xffffffffu, nbv, of);
+                    dvv += __shfl_xor_sync(0xffffffffu, dvv, of);
+                }
+                if (lane == 0) {
+                    NB2[o] = nbv;
+                    NB2[(size_t)gj2 * n + gi2] = nbv;
+                    red[0] += (double)dvv;
+                    red[1] += (double)(__ldg(W + o) * __ldg(VN + o));
+                }
+            }
+        }
+    }
+    if (tid == 0 && fail_s) sc->cg_failed = 2;
+    double tot[2];
+    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[3], tot)) {
+        finish_iteration(sc, sc->dist2 + tot[0], sc->loss, tot[1], hist_phi, hist_d, outer);
+        prof_mark(sc, 6);
+    }
+}
+
 // ---- kd_pairs --------------------------------------------------------------------------------------
 // One CTA = one 64 x 64 tile of pairs (I <= J) x one range of columns (blockIdx.y of `ksplit`).  Direct
 // differences (no Gram trick: a pair about to fuse has ||b|| far below ||a||, and the fused / not fused
@@ -832,7 +1044,16 @@ static void launch_pairs(cc_handle* h, const float* A, const float* Ap, int init
                                        init_only ? 0 : h->cond_outer, init_only);
 }
 
-void ccd_pairs(cc_handle* h) { launch_pairs(h, h->A, h->Ap, 0); }
+void ccd_pairs(cc_handle* h) {
+    if (h->dn_tc && h->prm.reserved0 != 8) {
+        const int ntile = (int)((h->n + TC_M - 1) / TC_M);
+        kd_pairs_tc<<<(unsigned)(ntile * (ntile + 1) / 2), TC_THREADS, PK_SMEM, h->stream>>>(
+            (int)h->n, (int)h->ld, ntile, h->A, h->Ap, h->abar, h->Sd, h->Wd, h->VNd, h->NB2d, h->sc,
+            h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, h->cond_outer);
+        return;
+    }
+    launch_pairs(h, h->A, h->Ap, 0);
+}
 
 static void launch_small(cc_handle* h, int init_only) {
     kd_small<<<h->dn_small_grid, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X, h->mask,
@@ -859,12 +1080,14 @@ int ccd_setup(cc_handle* h, const float* W) {
     h->dn_tc = (n >= 128 && (n & 3) == 0 && h->prm.reserved0 != 4) ? 1 : 0;
     if (h->dn_tc) {
         cudaError_t ea = cudaFuncSetAttribute(kd_proj_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, PK_SMEM);
         if (ea != cudaSuccess) { cudaGetLastError(); h->dn_tc = 0; }
     }
     long long ks = (4LL * h->sms + ntp - 1) / ntp;
     const long long ksmax = (h->ld + 63) / 64;
     if (ks > ksmax) ks = ksmax;
     if (ks < 1) ks = 1;
+    if (h->dn_tc) ks = 1;                      // kd_pairs_tc walks all columns itself
     h->dn_ksplit = (int)ks;
     // n <= 64: the fused kernel; its slices are (CTA, column phase)
     h->dn_small = (n <= SM_N && h->prm.reserved0 != 4) ? 1 : 0;

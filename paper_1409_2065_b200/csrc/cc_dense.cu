@@ -492,7 +492,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int 
     // epilogue: warp w owns TMEM lanes 32 (w % 4) .. (its rows) and the 32-column group w / 4 of all four accumulators
     const int row = (warp & 3) * 32 + lane, gi = i0 + row, grp = warp >> 2;
     const float naI = nrm[0][0][row], aeI = nrm[0][1][row], neI = nrm[0][2][row];
-    const float cthr_prev = sc->cthr;
     double red[2] = {0.0, 0.0};      // sum_{i<j} ||v - b||^2,  sum_{i<j} w ||v||
     unsigned int myflags = 0u;
 #pragma unroll 1
@@ -518,8 +517,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int 
                 const size_t o = (size_t)gi * n + gj;
                 const float w = __ldg(W + o);
                 float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
-                const float thr4 = 4.f * cthr_prev * w;
-                if (nb2 < CC_RECOMP_REL * (naI + naJ) || nb2 < thr4 * thr4) {
+                // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
+                if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
                     myflags |= 1u << (half * 16 + q);               // recomputed directly below
                 } else {
                     const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));

@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
 // ---- kd_proj_tc: the contraction S (A' - abar) on the 5th-generation tensor cores ------------------------
 // tcgen05.mma kind::tf32, M = 128 rows x N = 128 columns per CTA, fp32 accumulator in TMEM (128 lanes x 128
 // columns), K walked in blocks of 32.  fp32 accuracy is kept with the 3xTF32 split: x = hi + lo with hi = x
-// truncated to 10 mantissa bits (exactly a TF32 value) and lo = x - hi (exact in fp32);
+// rounded to TF32 (10 mantissa bits) and lo = x - hi rounded to TF32;
 // S A' ~= S_hi B_hi + S_hi B_lo + S_lo B_hi, three MMAs per K step into the same accumulator (the dropped
 // lo*lo term is 2^-22 relative).  Operands are split while they are staged into shared memory by the CTA's
 // threads (generic proxy) in the canonical K-major no-swizzle layout -- core matrices of 8 rows x 16 bytes,
@@ -157,6 +157,7 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
 // block kb run while the threads stage block kb+1; tcgen05.commit on an mbarrier frees a stage.
 constexpr int TC_M = 128, TC_N = 128, TC_K = 32;
 constexpr int TC_THREADS = 512, TC_WARPS = TC_THREADS / 32;
+constexpr int TC_CH = 16;                           // K blocks per accumulator chunk (512 terms)
 constexpr int TC_APASS = TC_M / (TC_WARPS * 4);        // A rows per thread (4 rows per warp and pass)
 constexpr int TC_BPASS = (TC_K / 4) / (TC_THREADS / 128);   // B K-cores per thread
 constexpr int TC_SBO = 128;                         // bytes between 8-row groups (one core matrix)
@@ -194,9 +195,18 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
     return false;   // never hang the GPU: the caller raises cg_failed
 }
 
+__device__ __forceinline__ float rna_tf32(float x) {
+    uint32_t r;
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
+    return __uint_as_float(r);
+}
+
+// x = hi + lo + O(2^-23 |x|), both parts exactly representable in TF32 and ROUNDED to nearest: truncating instead
+// (masking the low mantissa bits) biases every product the same way and the bias accumulates over the MM iterations
+// (measured: 1.6e-4 relative error on U after 480 iterations against 8e-6 for the FFMA kernel).
 __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
-    hi = __uint_as_float(__float_as_uint(x) & 0xffffe000u);
-    lo = x - hi;
+    hi = rna_tf32(x);
+    lo = rna_tf32(x - hi);
 }
 
 __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const float* __restrict__ S, const float* __restrict__ Ap,
@@ -206,7 +216,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
                                                      double* part) {
     if (!sc->mm_active) return;
     extern __shared__ uint8_t tc_smem_raw[];
-    __shared__ __align__(8) uint64_t mbar[2];
+    __shared__ __align__(8) uint64_t mbar[2], mbar_acc;
     __shared__ uint32_t tmem_base_s;
     __shared__ float rs_s[TC_M];
     __shared__ int fail_s;
@@ -218,10 +228,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
         fail_s = 0;
         for (int b = 0; b < 2; ++b)
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar[b])));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar_acc)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(TC_N));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(4 * TC_N));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -231,6 +242,30 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
     // instruction descriptor (cute::UMMA::InstrDescriptor): D = F32, A = B = TF32, both K-major, N >> 3, M >> 4
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
 
+    // The tensor core's fp32 accumulation truncates; over K = n terms that is a systematic bias (measured: U drifts
+    // 5e-8 per MM iteration at n = 4096 against 2e-9 for FFMA).  So the TMEM accumulator is drained every TC_CH K blocks
+    // into fp32 registers (round-to-nearest adds) and restarted, and inside a chunk the K blocks rotate over FOUR
+    // TMEM accumulators (all 512 columns), so no accumulator ever sums more than TC_CH / 4 K blocks (128 terms).
+    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);   // accumulator columns per warp (its lane quadrant x this column group)
+    float accr[TC_CPW];
+#pragma unroll
+    for (int q = 0; q < TC_CPW; ++q) accr[q] = 0.f;
+    auto drain = [&](int nacc) {
+        for (int ac = 0; ac < nacc; ++ac)
+#pragma unroll
+        for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
+            uint32_t v[16];
+            const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                           "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                         : "r"(taddr));
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+            for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
+        }
+    };
+    int nchunk_done = 0;
     float rsum[TC_APASS];
 #pragma unroll
     for (int q = 0; q < TC_APASS; ++q) rsum[q] = 0.f;
@@ -296,11 +331,22 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
                 const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
                 const uint64_t dah = tc_desc(smem_u32(a_hi) + koff), dal = tc_desc(smem_u32(a_lo) + koff);
                 const uint64_t dbh = tc_desc(smem_u32(b_hi) + koff), dbl = tc_desc(smem_u32(b_lo) + koff);
-                tc_mma(tmem_d, dah, dbh, idesc, (kb > 0 || ks > 0) ? 1u : 0u);
-                tc_mma(tmem_d, dah, dbl, idesc, 1u);
-                tc_mma(tmem_d, dal, dbh, idesc, 1u);
+                const uint32_t td = tmem_d + (uint32_t)((kb & 3) * TC_N);     // rotate over the four accumulators
+                tc_mma(td, dah, dbh, idesc, ((kb % TC_CH) >= 4 || ks > 0) ? 1u : 0u);
+                tc_mma(td, dah, dbl, idesc, 1u);
+                tc_mma(td, dal, dbh, idesc, 1u);
             }
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar[st])) : "memory");
+            if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb)
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar_acc)) : "memory");
+        }
+        if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb) {      // chunk boundary: wait for the MMAs, drain, restart the accumulator
+            if (!mbar_wait(smem_u32(&mbar_acc), (uint32_t)(nchunk_done & 1))) fail_s = 1;
+            ++nchunk_done;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            drain(min(4, (kb % TC_CH) + 1));
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncthreads();
         }
     }
     // row sums of S: 8 lanes hold one row's partial sums
@@ -312,27 +358,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
         v += __shfl_xor_sync(0xffffffffu, v, 4);
         if ((lane & 7) == 0) rs_s[pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3)] = v;
     }
-    {   // all MMAs done (commits complete in issue order)
-        const int kl = nkb - 1;
-        if (nkb > 0 && !mbar_wait(smem_u32(&mbar[kl & 1]), (uint32_t)((kl >> 1) & 1))) fail_s = 1;
-    }
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     __syncthreads();
     // epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (its rows) and the column group w / 4
     const float inv = 1.f / (float)(n + 1), fn = (float)n;
     double red[2] = {0.0, 0.0};
     const int row = (warp & 3) * 32 + lane, gi = i0 + row;
     const float rs = rs_s[row];
-    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);   // columns per warp
-#pragma unroll 1
-    for (int cb = (warp >> 2) * TC_CPW; cb < (warp >> 2) * TC_CPW + TC_CPW; cb += 16) {
-        uint32_t v[16];
-        const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cb;
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                     : "r"(taddr));
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int cb = (warp >> 2) * TC_CPW, h2 = 0; h2 < TC_CPW / 16; cb += 16, ++h2) {
         if (gi < n) {
 #pragma unroll
             for (int q4 = 0; q4 < 4; ++q4) {
@@ -340,8 +373,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
                 if (gc >= ld) continue;
                 const size_t o = (size_t)gi * ld + gc;
                 const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
-                const float4 sa = make_float4(__uint_as_float(v[q4 * 4 + 0]), __uint_as_float(v[q4 * 4 + 1]),
-                                              __uint_as_float(v[q4 * 4 + 2]), __uint_as_float(v[q4 * 4 + 3]));
+                const float4 sa = make_float4(accr[h2 * 16 + q4 * 4 + 0], accr[h2 * 16 + q4 * 4 + 1],
+                                              accr[h2 * 16 + q4 * 4 + 2], accr[h2 * 16 + q4 * 4 + 3]);
                 const float4 g = (rs * ap - sa) - fn * (u - ub);
                 const float4 dl = inv * g;
                 st4(A + o, u + dl);
@@ -357,7 +390,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(TC_N));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(4 * TC_N));
     if (tid == 0 && fail_s) sc->cg_failed = 2;
     double tot[2];
     if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[0], tot)) {

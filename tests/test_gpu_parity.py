@@ -313,6 +313,42 @@ def test_dense_mode_complete_graph(B, torch_, oracle, name, kw, miss):
     print(name, kw, "clusters along the path:", ks)
 
 
+def test_dense_tensor_core_path_through_partial_fusion(B, torch_, oracle):
+    """Sharper weights (phi = 6 / median d^2) make the complete graph fuse cluster by cluster: 256 -> 47 -> 4 -> 3.
+    With whole clusters fused, most within-cluster pairs go through kd_pairs_tc's direct recompute, the others
+    through the Gram blocks; U and the labels must follow the oracle at every gamma."""
+    torch = torch_
+    wl = synth.make("dense_weight", n=256, p=64, n_clusters=4)
+    X64 = wl.X.astype(np.float64)
+    si, sj = synth.sample_pairs(wl.n, 200000, 0)
+    wl.phi_rule, wl.phi = "fixed", 6.0 / float(np.median(oracle.pair_dist2(X64, None, si, sj)))
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    assert len(prob["ei"]) == n * (n - 1) // 2
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    gammas = [float(g) for g in synth.gamma_grid(30.0, 3000.0, 6)]
+    ref = H.oracle_path(oracle, prob, gammas, 80, proj_method=1)
+    ks_ref = [r["nclusters"] for r in ref]
+    assert ks_ref[0] == n and 1 < ks_ref[3] < n and ks_ref[-1] <= 4, ks_ref
+    dev = torch.device("cuda:0")
+    for tune in (0, 4):          # tensor-core kernels, then the FFMA kernels on the same problem
+        h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
+                        B.cc_default_params(dense=1, reserved0=tune))
+        U = torch.empty(n, wl.p, device=dev)
+        lab = torch.empty(n, dtype=torch.int32, device=dev)
+        for g, r in zip(gammas, ref):
+            B.cc_solve(h, g, 0.0, 80)
+            B.cc_get_U(h, -1, U)
+            _, k = B.cc_clusters(h, -1, lab)
+            ph, dd = B.cc_get_history(h)
+            assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, (tune, g)
+            assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (tune, g, k, r["nclusters"])
+            assert np.allclose(ph, r["phi"], rtol=1e-4) and np.allclose(dd, r["d"], rtol=5e-4), (tune, g)
+        B.cc_destroy(h)
+
+
 def test_dense_mode_rejects_bad_weights(B, torch_):
     torch = torch_
     n, p = 6, 4

@@ -370,6 +370,13 @@ def run_ours(args):
         v["tf32_peak_tflops"] = pk * 1.1 / 2.25
         v["frac_tensor"] = v["alg_tflops"] / v["tf32_peak_tflops"]
         v["frac_tensor_3x"] = 3.0 * v["frac_tensor"]      # three TF32 MMAs are issued per useful product
+        if "kd_pairs" in per_kernel:                     # kd_pairs_tc: 10 TF32 MMAs of 2*128*128*8 flop per K step and tile
+            v2 = per_kernel["kd_pairs"]
+            v2["bound"] = "tensor"
+            v2["tf32_peak_tflops"] = v["tf32_peak_tflops"]
+            nt = (n + 127) // 128
+            v2["mma_tflops"] = 10.0 * 2 * 128 * 128 * p * (nt * (nt + 1) // 2) / (v2["us_per_launch"] * 1e6)
+            v2["frac_tensor_issued"] = v2["mma_tflops"] / v2["tf32_peak_tflops"]
     roofline = {"bound": "alu" if alu_bound else "hbm", "kernel": top,
                 "achieved": per_kernel[top]["alg_tflops" if alu_bound else "alg_gbs"],
                 "peak": FP32_PEAK_TFLOPS if alu_bound else peak, "unit": "TFLOP/s" if alu_bound else "GB/s",

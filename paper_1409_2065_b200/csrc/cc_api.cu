@@ -116,7 +116,9 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
         return CC_EINVAL;
     }
     cc_scal* S = h->sc_host;
+    const double pen_keep = S->pen_next;   // dense mode: penalty of the current state, written by the last kd_edges
     memset(S, 0, sizeof(*S));
+    S->pen_next = pen_keep;
     S->gamma = gamma;
     rho_eps(h, gamma, &S->rho, &S->eps);
     S->tol = tol;
@@ -141,7 +143,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
         CC_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
         CC_CUDA(h, cudaMemcpyAsync(S, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
         CC_CUDA(h, cudaStreamSynchronize(h->stream));
-        h->launches += h->dense ? (h->dn_small ? 3LL : 6LL) * S->mm_iter : 3LL * S->mm_iter + 2LL * S->cg_total;
+        h->launches += h->dense ? (h->dn_small ? 3LL : (h->dn_tc ? 7LL : 6LL)) * S->mm_iter : 3LL * S->mm_iter + 2LL * S->cg_total;
     } else {
         int rc = h->dense ? ccd_solve_eager(h, maxit) : ccs_solve_eager(h, maxit);
         if (rc != CC_OK) return rc;

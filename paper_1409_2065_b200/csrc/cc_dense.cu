@@ -417,6 +417,108 @@ constexpr int PK_TILE = (PK / 4) * TC_LBO;           // bytes of one 128 x 16 op
 constexpr int PK_SMEM = 2 * 8 * PK_TILE + 1024;      // 2 stages x {alpha,e} x {I,J} x {hi,lo}
 #define CC_RECOMP_REL 1.0e-2f
 
+// Epilogue shared by the two staging variants of kd_pairs_tc: combine the four Gram accumulators, flag and recompute.
+__device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, int i0, int j0, uint32_t tmem_d,
+                                                  float (*nrm)[3][TC_M], unsigned int (*flag_s)[4], const int* fail_p,
+                                                  const float* __restrict__ A, const float* __restrict__ Ap,
+                                                  const float* __restrict__ S, const float* __restrict__ W,
+                                                  const float* __restrict__ VN, float* __restrict__ NB2, cc_scal* sc,
+                                                  double* part, double* hist_phi, double* hist_d,
+                                                  cudaGraphConditionalHandle outer) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // epilogue: warp w owns TMEM lanes 32 (w % 4) .. (its rows) and the 32-column group w / 4 of all four accumulators
+    const int row = (warp & 3) * 32 + lane, gi = i0 + row, grp = warp >> 2;
+    const float naI = nrm[0][0][row], aeI = nrm[0][1][row], neI = nrm[0][2][row];
+    double red[2] = {0.0, 0.0};      // sum_{i<j} ||v - b||^2,  sum_{i<j} w ||v||
+    unsigned int myflags = 0u;
+#pragma unroll 1
+    for (int half = 0; half < 2; ++half) {
+        const int cb = grp * 32 + half * 16;
+        uint32_t g[4][16];
+        float sq[16];          // this row's 16 shrink factors, fetched as four float4 before the accumulators are read
+#pragma unroll
+        for (int q4 = 0; q4 < 4; ++q4) {
+            const int gj = j0 + cb + q4 * 4;
+            const float4 v = (gi < n && gj < n) ? __ldg(reinterpret_cast<const float4*>(S + (size_t)gi * n + gj)) : f4(0.f);
+            sq[q4 * 4 + 0] = v.x; sq[q4 * 4 + 1] = v.y; sq[q4 * 4 + 2] = v.z; sq[q4 * 4 + 3] = v.w;
+        }
+#pragma unroll
+        for (int a = 0; a < 4; ++a) {
+            const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(a * TC_N + cb);
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                         : "=r"(g[a][0]), "=r"(g[a][1]), "=r"(g[a][2]), "=r"(g[a][3]), "=r"(g[a][4]), "=r"(g[a][5]), "=r"(g[a][6]),
+                           "=r"(g[a][7]), "=r"(g[a][8]), "=r"(g[a][9]), "=r"(g[a][10]), "=r"(g[a][11]), "=r"(g[a][12]),
+                           "=r"(g[a][13]), "=r"(g[a][14]), "=r"(g[a][15])
+                         : "r"(taddr));
+        }
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        if (gi < n) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const int cl = cb + q, gj = j0 + cl;
+                if (gj >= n || (I == J && gi >= gj)) continue;      // diagonal tiles: pairs i < j only, mirrored below
+                const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
+                const size_t o = (size_t)gi * n + gj;
+                float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
+                // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
+                if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
+                    myflags |= 1u << (half * 16 + q);               // recomputed directly below
+                } else {
+                    const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));
+                    const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
+                    const float sv = sq[q], om = 1.f - sv;
+                    const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
+                    NB2[o] = nb2;
+                    NB2[(size_t)gj * n + gi] = nb2;
+                    red[0] += (double)dv;
+                }
+            }
+        }
+    }
+    flag_s[row][grp] = myflags;
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(512));
+    // flagged pairs: direct differences in fp32, one warp per pair, rows dealt to warps round-robin (fixed order)
+    for (int rr = warp; rr < TC_M; rr += TC_WARPS) {
+        const int gi2 = i0 + rr;
+        for (int gq = 0; gq < 4; ++gq) {
+            unsigned int m = flag_s[rr][gq];
+            while (m) {
+                const int b = __ffs(m) - 1;
+                m &= m - 1;
+                const int gj2 = j0 + gq * 32 + b;
+                const size_t o = (size_t)gi2 * n + gj2;
+                const float sv = __ldg(S + o);
+                float nbv = 0.f, dvv = 0.f;
+                for (int c = lane * 4; c < ld; c += 128) {
+                    const float4 bb = ld4s(A + (size_t)gi2 * ld + c) - ld4s(A + (size_t)gj2 * ld + c);
+                    const float4 bp = ld4s(Ap + (size_t)gi2 * ld + c) - ld4s(Ap + (size_t)gj2 * ld + c);
+                    const float4 tt = fma4(sv, bp, f4(0.f)) - bb;
+                    nbv += dot4(bb, bb);
+                    dvv += dot4(tt, tt);
+                }
+#pragma unroll
+                for (int of = 16; of > 0; of >>= 1) {
+                    nbv += __shfl_xor_sync(0xffffffffu, nbv, of);
+                    dvv += __shfl_xor_sync(0xffffffffu, dvv, of);
+                }
+                if (lane == 0) {
+                    NB2[o] = nbv;
+                    NB2[(size_t)gj2 * n + gi2] = nbv;
+                    red[0] += (double)dvv;
+                }
+            }
+        }
+    }
+    if (tid == 0 && *fail_p) sc->cg_failed = 2;
+    double tot[2];
+    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[3], tot)) {
+        finish_iteration(sc, sc->dist2 + tot[0], sc->loss, sc->pen_next, hist_phi, hist_d, outer);   // penalty: kd_edges
+        prof_mark(sc, 6);
+    }
+}
+
 __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int ntile, const float* __restrict__ A,
                                                       const float* __restrict__ Ap, const float* __restrict__ abar,
                                                       const float* __restrict__ S, const float* __restrict__ W,
@@ -431,7 +533,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int 
     __shared__ unsigned int flag_s[TC_M][4];         // recompute mask: row x 128 columns
     __shared__ int fail_s;
     uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, warp = tid >> 5;
     int I = 0, rem = blockIdx.x;
     while (rem >= ntile - I) { rem -= ntile - I; ++I; }
     const int J = I + rem, i0 = I * TC_M, j0 = J * TC_M;
@@ -522,93 +624,145 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int 
     }
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     __syncthreads();
-    // epilogue: warp w owns TMEM lanes 32 (w % 4) .. (its rows) and the 32-column group w / 4 of all four accumulators
-    const int row = (warp & 3) * 32 + lane, gi = i0 + row, grp = warp >> 2;
-    const float naI = nrm[0][0][row], aeI = nrm[0][1][row], neI = nrm[0][2][row];
-    double red[2] = {0.0, 0.0};      // sum_{i<j} ||v - b||^2,  sum_{i<j} w ||v||
-    unsigned int myflags = 0u;
-#pragma unroll 1
-    for (int half = 0; half < 2; ++half) {
-        const int cb = grp * 32 + half * 16;
-        uint32_t g[4][16];
-#pragma unroll
-        for (int a = 0; a < 4; ++a) {
-            const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(a * TC_N + cb);
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                         : "=r"(g[a][0]), "=r"(g[a][1]), "=r"(g[a][2]), "=r"(g[a][3]), "=r"(g[a][4]), "=r"(g[a][5]), "=r"(g[a][6]),
-                           "=r"(g[a][7]), "=r"(g[a][8]), "=r"(g[a][9]), "=r"(g[a][10]), "=r"(g[a][11]), "=r"(g[a][12]),
-                           "=r"(g[a][13]), "=r"(g[a][14]), "=r"(g[a][15])
-                         : "r"(taddr));
-        }
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        if (gi < n) {
-#pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                const int cl = cb + q, gj = j0 + cl;
-                if (gj >= n || (I == J && gi >= gj)) continue;      // diagonal tiles: pairs i < j only, mirrored below
-                const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
-                const size_t o = (size_t)gi * n + gj;
-                const float w = __ldg(W + o);
-                float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
-                // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
-                if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
-                    myflags |= 1u << (half * 16 + q);               // recomputed directly below
-                } else {
-                    const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));
-                    const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
-                    const float sv = __ldg(S + o), om = 1.f - sv;
-                    const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
-                    NB2[o] = nb2;
-                    NB2[(size_t)gj * n + gi] = nb2;
-                    red[0] += (double)dv;
-                    red[1] += (double)(w * __ldg(VN + o));
-                }
-            }
-        }
+    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, &fail_s, A, Ap, S, W, VN, NB2, sc, part, hist_phi, hist_d, outer);
+}
+
+// ---- kd_pairs_tc, bulk-copy variant ------------------------------------------------------------------------------
+// kd_prep_pairs splits alpha = a - abar and e = a' - a into TF32 hi/lo ONCE per iteration and writes them already in
+// the tensor core's shared-memory layout: for row tile T and K block kb one contiguous 4 x PK_TILE block
+// {alpha_hi, alpha_lo, e_hi, e_lo}.  kd_pairs_tc2 then needs no staging threads: one thread issues two
+// cp.async.bulk (TMA 1-D) per K block -- tile I and tile J -- completing on an mbarrier, one thread issues the MMAs,
+// three stages in flight.  (In kd_pairs_tc every CTA re-split both tiles: 65 times per tile at n = 8192.)
+constexpr int PK_SIDE = 4 * PK_TILE;                 // bytes of one tile's four operands for one K block
+constexpr int PK_NST = 3;
+constexpr int PK2_SMEM = PK_NST * 2 * PK_SIDE + 1024;
+
+__global__ void __launch_bounds__(TC_THREADS) kd_prep_pairs(int n, int ld, int nkb, const float* __restrict__ A,
+                                                            const float* __restrict__ Ap, const float* __restrict__ abar,
+                                                            uint8_t* __restrict__ pre, float* __restrict__ nrm_part,
+                                                            int npad, const cc_scal* sc) {
+    if (!sc->mm_active) return;
+    const int T = blockIdx.y, kb = blockIdx.x;
+    const int tid = threadIdx.x, r = tid >> 2, kc = tid & 3;
+    const int gi = T * TC_M + r, gc = kb * PK + kc * 4;
+    const bool okc = gc < ld;
+    const float4 mb = okc ? ld4s(abar + gc) : f4(0.f);
+    const float4 a = (okc && gi < n) ? ld4s(A + (size_t)gi * ld + gc) : mb;
+    const float4 pp = (okc && gi < n) ? ld4s(Ap + (size_t)gi * ld + gc) : mb;
+    const float4 al = a - mb, e = pp - a;
+    uint8_t* base = pre + ((size_t)T * nkb + kb) * PK_SIDE;
+    const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
+    float4 h, l;
+    split_tf32(al.x, h.x, l.x); split_tf32(al.y, h.y, l.y); split_tf32(al.z, h.z, l.z); split_tf32(al.w, h.w, l.w);
+    *reinterpret_cast<float4*>(base + 0 * PK_TILE + off) = h;
+    *reinterpret_cast<float4*>(base + 1 * PK_TILE + off) = l;
+    split_tf32(e.x, h.x, l.x); split_tf32(e.y, h.y, l.y); split_tf32(e.z, h.z, l.z); split_tf32(e.w, h.w, l.w);
+    *reinterpret_cast<float4*>(base + 2 * PK_TILE + off) = h;
+    *reinterpret_cast<float4*>(base + 3 * PK_TILE + off) = l;
+    // partial row norms of this K block (summed over kb, in order, by the consumer)
+    float v0 = dot4(al, al), v1 = dot4(al, e), v2 = dot4(e, e);
+    v0 += __shfl_xor_sync(0xffffffffu, v0, 1); v0 += __shfl_xor_sync(0xffffffffu, v0, 2);
+    v1 += __shfl_xor_sync(0xffffffffu, v1, 1); v1 += __shfl_xor_sync(0xffffffffu, v1, 2);
+    v2 += __shfl_xor_sync(0xffffffffu, v2, 1); v2 += __shfl_xor_sync(0xffffffffu, v2, 2);
+    if (kc == 0) {
+        float* q = nrm_part + (size_t)kb * 3 * npad + T * TC_M + r;
+        q[0] = v0; q[npad] = v1; q[2 * (size_t)npad] = v2;
     }
-    flag_s[row][grp] = myflags;
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int ntile, int nkb, const uint8_t* __restrict__ pre,
+                                                       const float* __restrict__ nrm_part, int npad,
+                                                       const float* __restrict__ A, const float* __restrict__ Ap,
+                                                       const float* __restrict__ S, const float* __restrict__ W,
+                                                       const float* __restrict__ VN, float* __restrict__ NB2, cc_scal* sc,
+                                                       double* part, double* hist_phi, double* hist_d,
+                                                       cudaGraphConditionalHandle outer) {
+    if (!sc->mm_active) return;
+    extern __shared__ uint8_t tc_smem_raw[];
+    __shared__ __align__(8) uint64_t full[PK_NST], empty[PK_NST], done;
+    __shared__ uint32_t tmem_base_s;
+    __shared__ float nrm[2][3][TC_M];
+    __shared__ unsigned int flag_s[TC_M][4];
+    __shared__ int fail_s;
+    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
+    const int tid = threadIdx.x, warp = tid >> 5;
+    int I = 0, rem = blockIdx.x;
+    while (rem >= ntile - I) { rem -= ntile - I; ++I; }
+    const int J = I + rem, i0 = I * TC_M, j0 = J * TC_M;
+    if (tid == 0) {
+        fail_s = 0;
+        for (int b = 0; b < PK_NST; ++b) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&full[b])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&empty[b])));
+        }
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&done)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(512));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    // row norms: sum the K-block partials in order (same arithmetic for tile I and tile J rows)
+    if (tid < 2 * TC_M) {
+        const int side = tid / TC_M, rr = tid % TC_M;
+        const int g = (side ? j0 : i0) + rr;
+        float v0 = 0.f, v1 = 0.f, v2 = 0.f;
+        for (int kb = 0; kb < nkb; ++kb) {
+            const float* q = nrm_part + (size_t)kb * 3 * npad + g;
+            v0 += q[0]; v1 += q[npad]; v2 += q[2 * (size_t)npad];
+        }
+        nrm[side][0][rr] = v0; nrm[side][1][rr] = v1; nrm[side][2][rr] = v2;
+    }
+    if (tid < TC_M * 4) flag_s[tid >> 2][tid & 3] = 0u;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(512));
-    // flagged pairs: direct differences in fp32, one warp per pair, rows dealt to warps round-robin (fixed order)
-    for (int rr = warp; rr < TC_M; rr += TC_WARPS) {
-        const int gi2 = i0 + rr;
-        for (int gq = 0; gq < 4; ++gq) {
-            unsigned int m = flag_s[rr][gq];
-            while (m) {
-                const int b = __ffs(m) - 1;
-                m &= m - 1;
-                const int gj2 = j0 + gq * 32 + b;
-                const size_t o = (size_t)gi2 * n + gj2;
-                const float sv = __ldg(S + o);
-                float nbv = 0.f, dvv = 0.f;
-                for (int c = lane * 4; c < ld; c += 128) {
-                    const float4 bb = ld4s(A + (size_t)gi2 * ld + c) - ld4s(A + (size_t)gj2 * ld + c);
-                    const float4 bp = ld4s(Ap + (size_t)gi2 * ld + c) - ld4s(Ap + (size_t)gj2 * ld + c);
-                    const float4 tt = fma4(sv, bp, f4(0.f)) - bb;
-                    nbv += dot4(bb, bb);
-                    dvv += dot4(tt, tt);
-                }
-#pragma unroll
-                for (int of = 16; of > 0; of >>= 1) {
-                    nbv += __shfl_xor_sync(0xffffffffu, nbv, of);
-                    dvv += __shfl_xor_sync(0xffffffffu, dvv, of);
-                }
-                if (lane == 0) {
-                    NB2[o] = nbv;
-                    NB2[(size_t)gj2 * n + gi2] = nbv;
-                    red[0] += (double)dvv;
-                    red[1] += (double)(__ldg(W + o) * __ldg(VN + o));
-                }
-            }
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_d = tmem_base_s;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+
+    if (tid == 32) {
+        // ===== producer: TMA bulk copies =====
+        const uint8_t* srcI = pre + (size_t)I * nkb * PK_SIDE;
+        const uint8_t* srcJ = pre + (size_t)J * nkb * PK_SIDE;
+        for (int kb = 0; kb < nkb; ++kb) {
+            const int st = kb % PK_NST;
+            if (kb >= PK_NST && !mbar_wait(smem_u32(&empty[st]), (uint32_t)((kb / PK_NST - 1) & 1))) fail_s = 1;
+            const uint32_t bar = smem_u32(&full[st]);
+            const uint32_t dI = smem_u32(sm + (size_t)st * 2 * PK_SIDE), dJ = dI + PK_SIDE;
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(2 * PK_SIDE) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         :: "r"(dI), "l"(srcI + (size_t)kb * PK_SIDE), "r"(PK_SIDE), "r"(bar) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         :: "r"(dJ), "l"(srcJ + (size_t)kb * PK_SIDE), "r"(PK_SIDE), "r"(bar) : "memory");
         }
+    } else if (tid == 0) {
+        // ===== MMA issuer =====
+        for (int kb = 0; kb < nkb; ++kb) {
+            const int st = kb % PK_NST;
+            if (!mbar_wait(smem_u32(&full[st]), (uint32_t)((kb / PK_NST) & 1))) fail_s = 1;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t sI = smem_u32(sm + (size_t)st * 2 * PK_SIDE), sJ = sI + PK_SIDE;
+#pragma unroll
+            for (int ks = 0; ks < PK / 8; ++ks) {
+                const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
+                const uint32_t bI = sI + koff, bJ = sJ + koff;
+                const uint64_t Iah = tc_desc(bI), Ial = tc_desc(bI + PK_TILE), Ieh = tc_desc(bI + 2 * PK_TILE), Iel = tc_desc(bI + 3 * PK_TILE);
+                const uint64_t Jah = tc_desc(bJ), Jal = tc_desc(bJ + PK_TILE), Jeh = tc_desc(bJ + 2 * PK_TILE), Jel = tc_desc(bJ + 3 * PK_TILE);
+                const uint32_t acc = (kb > 0 || ks > 0) ? 1u : 0u;
+                tc_mma(tmem_d + 0 * TC_N, Iah, Jah, idesc, acc); tc_mma(tmem_d + 0 * TC_N, Iah, Jal, idesc, 1u); tc_mma(tmem_d + 0 * TC_N, Ial, Jah, idesc, 1u);
+                tc_mma(tmem_d + 1 * TC_N, Iah, Jeh, idesc, acc); tc_mma(tmem_d + 1 * TC_N, Iah, Jel, idesc, 1u); tc_mma(tmem_d + 1 * TC_N, Ial, Jeh, idesc, 1u);
+                tc_mma(tmem_d + 2 * TC_N, Ieh, Jah, idesc, acc); tc_mma(tmem_d + 2 * TC_N, Ieh, Jal, idesc, 1u); tc_mma(tmem_d + 2 * TC_N, Iel, Jah, idesc, 1u);
+                tc_mma(tmem_d + 3 * TC_N, Ieh, Jeh, idesc, acc);
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&empty[st])) : "memory");
+        }
+        asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&done)) : "memory");
     }
-    if (tid == 0 && fail_s) sc->cg_failed = 2;
-    double tot[2];
-    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[3], tot)) {
-        finish_iteration(sc, sc->dist2 + tot[0], sc->loss, tot[1], hist_phi, hist_d, outer);
-        prof_mark(sc, 6);
-    }
+    __syncwarp();
+    if (nkb > 0 && !mbar_wait(smem_u32(&done), 0u)) fail_s = 1;
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    __syncthreads();
+    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, &fail_s, A, Ap, S, W, VN, NB2, sc, part, hist_phi, hist_d, outer);
 }
 
 // ---- kd_pairs --------------------------------------------------------------------------------------
@@ -856,10 +1010,12 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
 
 // ---- kd_edges: block soft-threshold over the n x n matrices ------------------
 __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
-                                                float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, int init_only) {
+                                                float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, double* part,
+                                                int init_only) {
     if (!init_only && !sc->mm_active) return;
     const size_t nn = (size_t)n * n;
     const float cthr = sc->cthr;
+    double pen[1] = {0.0};     // sum_{i<j} w ||v|| of the state written here = the penalty term of the next Phi
     // few slices: one thread per entry; many slices (small n, long rows): one warp per entry, lanes stride
     // over the slices and combine with a fixed shuffle tree (deterministic either way)
     const bool warp_per = ksplit >= 32;
@@ -881,6 +1037,7 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
                     if (j + t == i) sn = 0.f;
                     sa[t] = sn;
                     va[t] = j + t == i ? 0.f : sn * nb;
+                    if (j + t > i) pen[0] += (double)((init_only ? __ldg(W + e + t) : wa[t]) * va[t]);
                 }
                 st4(S + e, make_float4(sa[0], sa[1], sa[2], sa[3]));
                 st4(VN + e, make_float4(va[0], va[1], va[2], va[3]));
@@ -914,8 +1071,11 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
         }
         S[e] = sn;
         VN[e] = vn;
+        if (j > i) pen[0] += (double)(W[e] * vn);
     }
     }
+    double ptot[1];
+    if (grid_reduce<1>(pen, part, &sc->ticket[7], ptot)) sc->pen_next = ptot[0];
     __syncthreads();
     if (!init_only && threadIdx.x == 0) {
         __threadfence();
@@ -1077,6 +1237,16 @@ static void launch_pairs(cc_handle* h, const float* A, const float* Ap, int init
 }
 
 void ccd_pairs(cc_handle* h) {
+    if (h->dn_tc && h->prm.reserved0 != 8 && h->prm.reserved0 != 16) {
+        const int ntile = (int)((h->n + TC_M - 1) / TC_M), nkb = (int)((h->ld + PK - 1) / PK), npad = ntile * TC_M;
+        dim3 gp((unsigned)nkb, (unsigned)ntile);
+        kd_prep_pairs<<<gp, TC_THREADS, 0, h->stream>>>((int)h->n, (int)h->ld, nkb, h->A, h->Ap, h->abar, h->pre_pairs,
+                                                       h->nrm_part, npad, h->sc);
+        kd_pairs_tc2<<<(unsigned)(ntile * (ntile + 1) / 2), TC_THREADS, PK2_SMEM, h->stream>>>(
+            (int)h->n, (int)h->ld, ntile, nkb, h->pre_pairs, h->nrm_part, npad, h->A, h->Ap, h->Sd, h->Wd, h->VNd, h->NB2d,
+            h->sc, h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, h->cond_outer);
+        return;
+    }
     if (h->dn_tc && h->prm.reserved0 != 8) {
         const int ntile = (int)((h->n + TC_M - 1) / TC_M);
         kd_pairs_tc<<<(unsigned)(ntile * (ntile + 1) / 2), TC_THREADS, PK_SMEM, h->stream>>>(
@@ -1094,7 +1264,8 @@ static void launch_small(cc_handle* h, int init_only) {
 }
 
 void ccd_edges(cc_handle* h, int init_only) {
-    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc, init_only);
+    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc,
+                                                   h->part + 6 * CC_MAXBLK * CC_NPART, init_only);
 }
 
 void ccd_lab_hook(cc_handle* h, int* changed) {
@@ -1113,6 +1284,7 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (h->dn_tc) {
         cudaError_t ea = cudaFuncSetAttribute(kd_proj_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM);
         if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, PK_SMEM);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, PK2_SMEM);
         if (ea != cudaSuccess) { cudaGetLastError(); h->dn_tc = 0; }
     }
     long long ks = (4LL * h->sms + ntp - 1) / ntp;
@@ -1150,6 +1322,12 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->abar, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->colps, (size_t)kSliceDense * 2 * h->ld * sizeof(double), h->stream);
     if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
+    if (h->dn_tc) {
+        const size_t ntile = (size_t)((n + TC_M - 1) / TC_M), nkb = (size_t)((h->ld + PK - 1) / PK);
+        e = cc_dev_alloc((void**)&h->pre_pairs, ntile * nkb * PK_SIDE, h->stream);
+        if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->nrm_part, nkb * 3 * ntile * TC_M * sizeof(float), h->stream);
+        if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
+    }
     CC_CUDA(h, cudaMemcpyAsync(h->Wd, W, (size_t)nn * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
     CC_CUDA(h, cudaMemsetAsync(h->Sd, 0, (size_t)nn * sizeof(float), h->stream));
     CC_CUDA(h, cudaMemsetAsync(h->VNd, 0, (size_t)nn * sizeof(float), h->stream));

@@ -22,6 +22,7 @@ struct cc_scal {
     double dist2, loss, pen;
     double phi, phi_prev;
     double min_margin;  // smallest | ||b|| - thr | / thr at the last shrink
+    double pen_next;    // dense mode: sum_{i<j} w ||v|| of the state kd_edges just wrote (the next iteration's penalty)
     float cu, ca;       // d/(d+rho), rho/(d+rho)          (U update, L82)
     float cthr;         // gamma d / rho                   (threshold = cthr * w_ij, L86)
     float pad0;
@@ -83,6 +84,8 @@ struct cc_handle {
     float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices)
     float *ubar, *abar;               // column means of U and A'
     double* colps;                    // partial column sums
+    uint8_t* pre_pairs;               // kd_prep_pairs: TF32 hi/lo operand tiles in the tensor core's smem layout
+    float* nrm_part;                  // per-K-block partial row norms
     int dn_ksplit, dn_big, dn_tc, dn_small, dn_small_cs, dn_small_grid;
     // scalars
     cc_scal* sc;                      // device

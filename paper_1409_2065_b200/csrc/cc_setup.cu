@@ -399,7 +399,13 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
 
 int ccu_cold_start(cc_handle* h) {
     k_cold_start<<<h->grid_nodes, 256, 0, h->stream>>>(h->n, (int)h->ld, h->X, h->mask, h->colmean, h->U);
-    if (h->dense) ccd_init_state(h); else ccs_init_state(h);
+    if (h->dense) {
+        ccd_init_state(h);
+        CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));   // pen_next
+        CC_CUDA(h, cudaStreamSynchronize(h->stream));
+    } else {
+        ccs_init_state(h);
+    }
     h->launches += 1;
     CC_CUDA(h, cudaGetLastError());
     return CC_OK;
@@ -429,7 +435,7 @@ int ccu_min_margin(cc_handle* h, double* margin_out) {
 
 void ccu_free(cc_handle* h) {
     void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Dl, h->Uc, h->mask, h->colmean, h->rowptr,
-                    h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->colps, h->sc, h->part,
+                    h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->colps, h->pre_pairs, h->nrm_part, h->sc, h->part,
                     h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order};
     for (void* q : ptrs)
         cc_dev_free(q, h->stream);

@@ -400,6 +400,171 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
     }
 }
 
+// ---- kd_proj_tc2: the contraction fed by TMA bulk copies ---------------------------------------------------------
+// The A operand (S, split hi/lo, tile layout) and the row sums of S are written by kd_edges when it produces S; the B
+// operand ((A' - abar)^T, split hi/lo, tile layout) by kd_prep_proj.  One thread issues two cp.async.bulk per K block,
+// one thread the 12 MMAs; all threads meet every TC_CH K blocks to drain the four rotating accumulators.
+constexpr int TC_SIDE = 2 * TC_TILE;                // hi + lo of one operand for one K block
+constexpr int TC_NST = 3;
+constexpr int TC2_SMEM = TC_NST * 2 * TC_SIDE + 1024;
+
+__global__ void __launch_bounds__(TC_THREADS) kd_prep_proj(int n, int ld, int nkb, const float* __restrict__ Ap,
+                                                           const float* __restrict__ abar, uint8_t* __restrict__ Bpre,
+                                                           const cc_scal* sc) {
+    if (!sc->mm_active) return;
+    const int kb = blockIdx.x, ct = blockIdx.y, tid = threadIdx.x;
+    const int nl = tid & 127, kc0 = tid >> 7, gc = ct * TC_N + nl;
+    const bool ok = gc < ld;
+    const float mean = ok ? __ldg(abar + gc) : 0.f;
+    uint8_t* base = Bpre + ((size_t)ct * nkb + kb) * TC_SIDE;
+#pragma unroll
+    for (int pass = 0; pass < TC_BPASS; ++pass) {
+        const int kc = kc0 + (TC_THREADS / 128) * pass;
+        float v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int gk = kb * TC_K + kc * 4 + q;
+            v[q] = (ok && gk < n) ? __ldg(Ap + (size_t)gk * ld + gc) - mean : 0.f;
+        }
+        float4 h, l;
+        split_tf32(v[0], h.x, l.x); split_tf32(v[1], h.y, l.y); split_tf32(v[2], h.z, l.z); split_tf32(v[3], h.w, l.w);
+        const int off = kc * TC_LBO + (nl >> 3) * TC_SBO + (nl & 7) * 16;
+        *reinterpret_cast<float4*>(base + off) = h;
+        *reinterpret_cast<float4*>(base + TC_TILE + off) = l;
+    }
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc2(int n, int ld, int nkb, const uint8_t* __restrict__ Spre,
+                                                      const uint8_t* __restrict__ Bpre, const float* __restrict__ rs_S,
+                                                      const float* __restrict__ Ap, const float* __restrict__ U,
+                                                      const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                      const float* __restrict__ ubar, const float* __restrict__ abar,
+                                                      float* __restrict__ A, cc_scal* sc, double* part) {
+    if (!sc->mm_active) return;
+    extern __shared__ uint8_t tc_smem_raw[];
+    __shared__ __align__(8) uint64_t full[TC_NST], empty[TC_NST], mbar_acc;
+    __shared__ uint32_t tmem_base_s;
+    __shared__ int fail_s;
+    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int It = blockIdx.y, Ct = blockIdx.x, i0 = It * TC_M, c0 = Ct * TC_N;
+    if (tid == 0) {
+        fail_s = 0;
+        for (int b = 0; b < TC_NST; ++b) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&full[b])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&empty[b])));
+        }
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar_acc)));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(4 * TC_N));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t tmem_d = tmem_base_s;
+    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
+    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);
+    float accr[TC_CPW];
+#pragma unroll
+    for (int q = 0; q < TC_CPW; ++q) accr[q] = 0.f;
+    const uint8_t* srcA = Spre + (size_t)It * nkb * TC_SIDE;
+    const uint8_t* srcB = Bpre + (size_t)Ct * nkb * TC_SIDE;
+    const int nch = (nkb + TC_CH - 1) / TC_CH;
+    for (int ch = 0; ch < nch; ++ch) {
+        const int kb0 = ch * TC_CH, kb1 = min(nkb, kb0 + TC_CH);
+        if (tid == 32) {
+            for (int kb = kb0; kb < kb1; ++kb) {
+                const int st = kb % TC_NST;
+                if (kb >= TC_NST && !mbar_wait(smem_u32(&empty[st]), (uint32_t)((kb / TC_NST - 1) & 1))) fail_s = 1;
+                const uint32_t bar = smem_u32(&full[st]);
+                const uint32_t dA = smem_u32(sm + (size_t)st * 2 * TC_SIDE), dB = dA + TC_SIDE;
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(2 * TC_SIDE) : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             :: "r"(dA), "l"(srcA + (size_t)kb * TC_SIDE), "r"(TC_SIDE), "r"(bar) : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             :: "r"(dB), "l"(srcB + (size_t)kb * TC_SIDE), "r"(TC_SIDE), "r"(bar) : "memory");
+            }
+        } else if (tid == 0) {
+            for (int kb = kb0; kb < kb1; ++kb) {
+                const int st = kb % TC_NST;
+                if (!mbar_wait(smem_u32(&full[st]), (uint32_t)((kb / TC_NST) & 1))) fail_s = 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t sA = smem_u32(sm + (size_t)st * 2 * TC_SIDE), sB = sA + TC_SIDE;
+                const uint32_t td = tmem_d + (uint32_t)((kb & 3) * TC_N);
+#pragma unroll
+                for (int ks = 0; ks < TC_K / 8; ++ks) {
+                    const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
+                    const uint64_t dah = tc_desc(sA + koff), dal = tc_desc(sA + TC_TILE + koff);
+                    const uint64_t dbh = tc_desc(sB + koff), dbl = tc_desc(sB + TC_TILE + koff);
+                    tc_mma(td, dah, dbh, idesc, ((kb - kb0) >= 4 || ks > 0) ? 1u : 0u);
+                    tc_mma(td, dah, dbl, idesc, 1u);
+                    tc_mma(td, dal, dbh, idesc, 1u);
+                }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&empty[st])) : "memory");
+            }
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar_acc)) : "memory");
+        }
+        __syncwarp();
+        if (!mbar_wait(smem_u32(&mbar_acc), (uint32_t)(ch & 1))) fail_s = 1;
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        const int nacc = min(4, kb1 - kb0);
+        for (int ac = 0; ac < nacc; ++ac)
+#pragma unroll
+            for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
+                uint32_t v[16];
+                const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                               "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                             : "r"(taddr));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
+            }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+    }
+    const float inv = 1.f / (float)(n + 1), fn = (float)n;
+    double red[2] = {0.0, 0.0};
+    const int row = (warp & 3) * 32 + lane, gi = i0 + row;
+    const float rs = gi < n ? __ldg(rs_S + gi) : 0.f;
+#pragma unroll
+    for (int cb = (warp >> 2) * TC_CPW, h2 = 0; h2 < TC_CPW / 16; cb += 16, ++h2) {
+        if (gi < n) {
+#pragma unroll
+            for (int q4 = 0; q4 < 4; ++q4) {
+                const int gc = c0 + cb + q4 * 4;
+                if (gc >= ld) continue;
+                const size_t o = (size_t)gi * ld + gc;
+                const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
+                const float4 sa = make_float4(accr[h2 * 16 + q4 * 4 + 0], accr[h2 * 16 + q4 * 4 + 1],
+                                              accr[h2 * 16 + q4 * 4 + 2], accr[h2 * 16 + q4 * 4 + 3]);
+                const float4 g = (rs * ap - sa) - fn * (u - ub);
+                const float4 dl = inv * g;
+                st4(A + o, u + dl);
+                float4 q = ld4s(X + o) - u;
+                if (mask) {
+                    const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + o);
+                    q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
+                }
+                red[0] += (double)dot4(dl, dl);
+                red[1] += (double)dot4(q, q);
+            }
+        }
+    }
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(4 * TC_N));
+    if (tid == 0 && fail_s) sc->cg_failed = 2;
+    double tot[2];
+    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[0], tot)) {
+        sc->dist2 = tot[0];
+        sc->loss = tot[1];
+        prof_mark(sc, 5);
+    }
+}
+
 // ---- kd_pairs_tc: pair norms on the tensor cores, with a direct fp32 recompute where a Gram block is not enough ---
 // For a 128 x 128 tile of pairs (I <= J), with alpha = a - abar (any common shift cancels) and e = a' - a:
 //   ||b||^2        = |alpha_i|^2 + |alpha_j|^2 - 2 G1,           G1 = alpha_I alpha_J^T
@@ -1011,7 +1176,7 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
 // ---- kd_edges: block soft-threshold over the n x n matrices ------------------
 __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, double* part,
-                                                int init_only) {
+                                                int init_only, uint8_t* __restrict__ Spre, float* __restrict__ rs_out, int nkb32) {
     if (!init_only && !sc->mm_active) return;
     const size_t nn = (size_t)n * n;
     const float cthr = sc->cthr;
@@ -1021,26 +1186,59 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
     const bool warp_per = ksplit >= 32;
     const int lane = threadIdx.x & 31;
     if (!warp_per && (n & 3) == 0) {
-        // streaming case (large n): one block walks whole rows, four entries per thread
-        for (int i = blockIdx.x; i < n; i += gridDim.x) {
-            for (int j = threadIdx.x * 4; j < n; j += blockDim.x * 4) {
-                const size_t e = (size_t)i * n + j;
-                float4 q = ld4s(NB2 + e);
-                for (int k = 1; k < ksplit; ++k) q = q + ld4s(NB2 + (size_t)k * nn + e);
-                const float4 wv = init_only ? f4(0.f) : ld4s(W + e);
-                float qa[4] = {q.x, q.y, q.z, q.w}, wa[4] = {wv.x, wv.y, wv.z, wv.w}, sa[4], va[4];
+        // streaming case (large n): a block walks groups of 8 rows; thread = (row r8 of the group, column quad cq).  A warp
+        // then reads / writes 64-byte row segments of the n x n matrices and, for the pre-split copy, whole 128-byte
+        // core matrices (8 rows x 16 bytes) of kd_proj_tc2's operand layout.
+        const int r8 = threadIdx.x & 7, cq = threadIdx.x >> 3;
+        __shared__ float rs_part[8][33];
+        for (int ig = blockIdx.x; ig * 8 < n; ig += gridDim.x) {
+            const int i = ig * 8 + r8;
+            float rsum = 0.f;
+            if (i < n) {
+                for (int j0 = cq * 8; j0 < n; j0 += 256) {      // 8 columns per thread: a warp covers 128-byte row segments
 #pragma unroll
-                for (int t = 0; t < 4; ++t) {
-                    const float nb = sqrtf(qa[t]);
-                    const float thr = cthr * wa[t];
-                    float sn = init_only ? 1.f : (nb <= thr ? 0.f : 1.f - thr / nb);
-                    if (j + t == i) sn = 0.f;
-                    sa[t] = sn;
-                    va[t] = j + t == i ? 0.f : sn * nb;
-                    if (j + t > i) pen[0] += (double)((init_only ? __ldg(W + e + t) : wa[t]) * va[t]);
+                    for (int hq = 0; hq < 2; ++hq) {
+                        const int j = j0 + hq * 4;
+                        if (j >= n) break;
+                        const size_t e = (size_t)i * n + j;
+                        float4 q = ld4s(NB2 + e);
+                        for (int k = 1; k < ksplit; ++k) q = q + ld4s(NB2 + (size_t)k * nn + e);
+                        const float4 wv = ld4s(W + e);
+                        float qa[4] = {q.x, q.y, q.z, q.w}, wa[4] = {wv.x, wv.y, wv.z, wv.w}, sa[4], va[4];
+#pragma unroll
+                        for (int t = 0; t < 4; ++t) {
+                            const float nb = sqrtf(qa[t]);
+                            const float thr = cthr * wa[t];
+                            float sn = init_only ? 1.f : (nb <= thr ? 0.f : 1.f - thr / nb);
+                            if (j + t == i) sn = 0.f;
+                            sa[t] = sn;
+                            va[t] = j + t == i ? 0.f : sn * nb;
+                            if (j + t > i) pen[0] += (double)(wa[t] * va[t]);
+                        }
+                        st4(S + e, make_float4(sa[0], sa[1], sa[2], sa[3]));
+                        if (VN) st4(VN + e, make_float4(va[0], va[1], va[2], va[3]));
+                        if (Spre) {
+                            rsum += (sa[0] + sa[1]) + (sa[2] + sa[3]);
+                            float4 hh, ll;
+                            split_tf32(sa[0], hh.x, ll.x); split_tf32(sa[1], hh.y, ll.y); split_tf32(sa[2], hh.z, ll.z); split_tf32(sa[3], hh.w, ll.w);
+                            const int r = i & (TC_M - 1), kb = j >> 5, kc = (j & 31) >> 2;
+                            uint8_t* base = Spre + ((size_t)(i / TC_M) * nkb32 + kb) * (2 * TC_TILE);
+                            const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
+                            *reinterpret_cast<float4*>(base + off) = hh;
+                            *reinterpret_cast<float4*>(base + TC_TILE + off) = ll;
+                        }
+                    }
                 }
-                st4(S + e, make_float4(sa[0], sa[1], sa[2], sa[3]));
-                st4(VN + e, make_float4(va[0], va[1], va[2], va[3]));
+            }
+            if (Spre) {   // row sums of S in fp32, fixed order over the 32 column-quad threads of each row
+                rs_part[r8][cq] = rsum;
+                __syncthreads();
+                if (threadIdx.x < 8 && ig * 8 + threadIdx.x < n) {
+                    float t = 0.f;
+                    for (int c = 0; c < 32; ++c) t += rs_part[threadIdx.x][c];
+                    rs_out[ig * 8 + threadIdx.x] = t;
+                }
+                __syncthreads();
             }
         }
     } else {
@@ -1070,7 +1268,7 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
             }
         }
         S[e] = sn;
-        VN[e] = vn;
+        if (VN) VN[e] = vn;
         if (j > i) pen[0] += (double)(W[e] * vn);
     }
     }
@@ -1216,6 +1414,16 @@ static void launch_proj(cc_handle* h) {
 }
 
 void ccd_proj(cc_handle* h) {
+    if (h->dn_tc && h->prm.reserved0 != 16) {
+        const int nkb = (int)((h->n + TC_K - 1) / TC_K);
+        dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
+        dim3 gp((unsigned)nkb, g.x);
+        kd_prep_proj<<<gp, TC_THREADS, 0, h->stream>>>((int)h->n, (int)h->ld, nkb, h->Ap, h->abar, h->pre_B, h->sc);
+        kd_proj_tc2<<<g, TC_THREADS, TC2_SMEM, h->stream>>>((int)h->n, (int)h->ld, nkb, h->pre_S, h->pre_B, h->rs_S, h->Ap, h->U,
+                                                            h->X, h->mask, h->ubar, h->abar, h->A, h->sc,
+                                                            h->part + 0 * CC_MAXBLK * CC_NPART);
+        return;
+    }
     if (h->dn_tc) {
         dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
         kd_proj_tc<<<g, TC_THREADS, TC_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar,
@@ -1264,8 +1472,10 @@ static void launch_small(cc_handle* h, int init_only) {
 }
 
 void ccd_edges(cc_handle* h, int init_only) {
-    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc,
-                                                   h->part + 6 * CC_MAXBLK * CC_NPART, init_only);
+    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd,
+                                                   (h->dn_tc && h->prm.reserved0 == 0) ? (float*)nullptr : h->VNd, h->sc,
+                                                   h->part + 6 * CC_MAXBLK * CC_NPART, init_only, h->pre_S, h->rs_S,
+                                                   (int)((h->n + TC_K - 1) / TC_K));
 }
 
 void ccd_lab_hook(cc_handle* h, int* changed) {
@@ -1285,6 +1495,7 @@ int ccd_setup(cc_handle* h, const float* W) {
         cudaError_t ea = cudaFuncSetAttribute(kd_proj_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM);
         if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, PK_SMEM);
         if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, PK2_SMEM);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_proj_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, TC2_SMEM);
         if (ea != cudaSuccess) { cudaGetLastError(); h->dn_tc = 0; }
     }
     long long ks = (4LL * h->sms + ntp - 1) / ntp;
@@ -1325,6 +1536,13 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (h->dn_tc) {
         const size_t ntile = (size_t)((n + TC_M - 1) / TC_M), nkb = (size_t)((h->ld + PK - 1) / PK);
         e = cc_dev_alloc((void**)&h->pre_pairs, ntile * nkb * PK_SIDE, h->stream);
+        const size_t nkb32 = (size_t)((n + TC_K - 1) / TC_K), nct = (size_t)((h->ld + TC_N - 1) / TC_N);
+        if (e == cudaSuccess && h->prm.reserved0 != 16) {
+            e = cc_dev_alloc((void**)&h->pre_S, ntile * nkb32 * TC_SIDE, h->stream);
+            if (e == cudaSuccess) e = cudaMemsetAsync(h->pre_S, 0, ntile * nkb32 * TC_SIDE, h->stream);   // padding rows / columns stay 0
+            if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->pre_B, nct * nkb32 * TC_SIDE, h->stream);
+            if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->rs_S, (size_t)n * sizeof(float), h->stream);
+        }
         if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->nrm_part, nkb * 3 * ntile * TC_M * sizeof(float), h->stream);
         if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
     }

@@ -86,6 +86,8 @@ struct cc_handle {
     double* colps;                    // partial column sums
     uint8_t* pre_pairs;               // kd_prep_pairs: TF32 hi/lo operand tiles in the tensor core's smem layout
     float* nrm_part;                  // per-K-block partial row norms
+    uint8_t *pre_S, *pre_B;           // kd_proj_tc2 operands: S (by kd_edges) and (A' - abar)^T (by kd_prep_proj), hi/lo tiles
+    float* rs_S;                      // row sums of S (by kd_edges)
     int dn_ksplit, dn_big, dn_tc, dn_small, dn_small_cs, dn_small_grid;
     // scalars
     cc_scal* sc;                      // device

@@ -600,7 +600,7 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
     for (int half = 0; half < 2; ++half) {
         const int cb = grp * 32 + half * 16;
         uint32_t g[4][16];
-        float sq[16];          // this row's 16 shrink factors, fetched as four float4 before the accumulators are read
+        float sq[16], nbrow[16];   // this row's 16 shrink factors (four float4 loads, issued before the accumulators are read) and results
 #pragma unroll
         for (int q4 = 0; q4 < 4; ++q4) {
             const int gj = j0 + cb + q4 * 4;
@@ -621,11 +621,12 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 const int cl = cb + q, gj = j0 + cl;
-                if (gj >= n || (I == J && gi >= gj)) continue;      // diagonal tiles: pairs i < j only, mirrored below
+                if (gj >= n || (I == J && gi >= gj)) { nbrow[q] = 0.f; continue; }   // diagonal tiles: pairs i < j only, mirrored
                 const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
                 const size_t o = (size_t)gi * n + gj;
                 float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
                 // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
+                nbrow[q] = fmaxf(nb2, 0.f);
                 if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
                     myflags |= 1u << (half * 16 + q);               // recomputed directly below
                 } else {
@@ -633,9 +634,20 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                     const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
                     const float sv = sq[q], om = 1.f - sv;
                     const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
-                    NB2[o] = nb2;
+                    if (I == J) NB2[o] = nb2;                      // diagonal tiles: guarded scalar stores (i < j only)
+                    else nbrow[q] = nb2;
                     NB2[(size_t)gj * n + gi] = nb2;
                     red[0] += (double)dv;
+                }
+            }
+            if (I != J) {
+                // off-diagonal tiles: this row's 16 values as four 16-byte stores (flagged entries are rewritten by the
+                // recompute phase, which runs after the barrier below)
+#pragma unroll
+                for (int q4 = 0; q4 < 4; ++q4) {
+                    const int gj = j0 + cb + q4 * 4;
+                    if (gj < n)
+                        st4(NB2 + (size_t)gi * n + gj, make_float4(nbrow[q4 * 4 + 0], nbrow[q4 * 4 + 1], nbrow[q4 * 4 + 2], nbrow[q4 * 4 + 3]));
                 }
             }
         }
@@ -867,17 +879,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(512));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
-    // row norms: sum the K-block partials in order (same arithmetic for tile I and tile J rows)
-    if (tid < 2 * TC_M) {
-        const int side = tid / TC_M, rr = tid % TC_M;
-        const int g = (side ? j0 : i0) + rr;
-        float v0 = 0.f, v1 = 0.f, v2 = 0.f;
-        for (int kb = 0; kb < nkb; ++kb) {
-            const float* q = nrm_part + (size_t)kb * 3 * npad + g;
-            v0 += q[0]; v1 += q[npad]; v2 += q[2 * (size_t)npad];
-        }
-        nrm[side][0][rr] = v0; nrm[side][1][rr] = v1; nrm[side][2][rr] = v2;
-    }
     if (tid < TC_M * 4) flag_s[tid >> 2][tid & 3] = 0u;
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -922,6 +923,17 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int
             asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&empty[st])) : "memory");
         }
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&done)) : "memory");
+    } else if (tid >= 64 && tid < 64 + 2 * TC_M) {
+        // ===== meanwhile: row norms = the K-block partials summed in order (same arithmetic for tile I and tile J rows)
+        const int t2 = tid - 64, side = t2 / TC_M, rr = t2 % TC_M;
+        const int g = (side ? j0 : i0) + rr;
+        float v0 = 0.f, v1 = 0.f, v2 = 0.f;
+#pragma unroll 4
+        for (int kb = 0; kb < nkb; ++kb) {
+            const float* q = nrm_part + (size_t)kb * 3 * npad + g;
+            v0 += __ldg(q); v1 += __ldg(q + npad); v2 += __ldg(q + 2 * (size_t)npad);
+        }
+        nrm[side][0][rr] = v0; nrm[side][1][rr] = v1; nrm[side][2][rr] = v2;
     }
     __syncwarp();
     if (nkb > 0 && !mbar_wait(smem_u32(&done), 0u)) fail_s = 1;

@@ -1208,14 +1208,23 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
             float rsum = 0.f;
             if (i < n) {
                 for (int j0 = cq * 8; j0 < n; j0 += 256) {      // 8 columns per thread: a warp covers 128-byte row segments
+                    // all four loads of the thread's 8 columns are issued before any arithmetic
+                    float4 qv[2], wq[2];
+#pragma unroll
+                    for (int hq = 0; hq < 2; ++hq) {
+                        const int j = j0 + hq * 4;
+                        const size_t e = (size_t)i * n + (j < n ? j : 0);
+                        qv[hq] = __ldcs(reinterpret_cast<const float4*>(NB2 + e));      // streamed once: evict-first
+                        wq[hq] = __ldg(reinterpret_cast<const float4*>(W + e));
+                    }
 #pragma unroll
                     for (int hq = 0; hq < 2; ++hq) {
                         const int j = j0 + hq * 4;
                         if (j >= n) break;
                         const size_t e = (size_t)i * n + j;
-                        float4 q = ld4s(NB2 + e);
+                        float4 q = qv[hq];
                         for (int k = 1; k < ksplit; ++k) q = q + ld4s(NB2 + (size_t)k * nn + e);
-                        const float4 wv = ld4s(W + e);
+                        const float4 wv = wq[hq];
                         float qa[4] = {q.x, q.y, q.z, q.w}, wa[4] = {wv.x, wv.y, wv.z, wv.w}, sa[4], va[4];
 #pragma unroll
                         for (int t = 0; t < 4; ++t) {

@@ -154,9 +154,9 @@ def alg_bytes(kernel, n, p, nnz, masked, dense=False):
     counted once per directed entry, own rows and outputs once per node ('roofline')."""
     row, npb = 4 * p, 4 * n * p
     return {
-        "k_rhs": nnz * (2 * row + 8) + 6 * npb + 4 * n,
+        "k_rhs": nnz * (2 * row + 8) + 5 * npb + 4 * n,
         "k_cg_spmv": nnz * (row + 4) + 5 * npb + 4 * n,      # gather + own uc, p, s in; p, s out
-        "k_cg_update": 7 * npb + 4 * n,                      # p, s, A, r in; A, r, uc out
+        "k_cg_update": 6 * npb + 4 * n,                      # p, s, A, uc in; A, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
         "k_update": (5 * npb if dense else 8 * npb + 16 * nnz) + (n * p if masked else 0),
         # dense mode (nnz = n(n-1)): matrices are n x n fp32

@@ -64,7 +64,7 @@ struct cc_handle {
     cudaStream_t stream;
     // node arrays (n x ld fp32)
     float *X, *U, *A, *Ap, *Z;        // Z = warm start of the projection (u + previous correction)
-    float *R, *Pv, *Sv, *Uc;          // CG: residual, search dir, (I+L) search dir, D^-1 r
+    float *R, *Pv, *Sv, *Uc;          // CG: (R unused: r = D uc), search dir, (I+L) search dir, D^-1 r
     float* Dl;                        // previous correction a - u (warm-start extrapolation)
     uint8_t* mask;                    // n x ld or NULL
     float* colmean;                   // ld

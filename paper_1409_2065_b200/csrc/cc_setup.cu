@@ -378,7 +378,7 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
     h->sumw2 = two[1];
 
     // ---- state ----
-    float** node_arrays[] = {&h->U, &h->A, &h->Ap, &h->Z, &h->R, &h->Pv, &h->Sv, &h->Uc, &h->Dl};
+    float** node_arrays[] = {&h->U, &h->A, &h->Ap, &h->Z, &h->Pv, &h->Sv, &h->Uc, &h->Dl};
     for (float** a : node_arrays) {
         CC_TRY(dmalloc(h, a, nl));
         CC_CUDA(h, cudaMemsetAsync(*a, 0, nl * sizeof(float), st));

@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
                                                      const int* __restrict__ col, const float* __restrict__ s,
                                                      const float* __restrict__ dinv, const float* __restrict__ Ap,
                                                      const float* __restrict__ Z, const float* __restrict__ U,
-                                                     float* __restrict__ R, float* __restrict__ Uc, float* __restrict__ A,
+                                                     float* __restrict__ Uc, float* __restrict__ A,
                                                      cc_scal* sc, double* part, cudaGraphConditionalHandle loop) {
     if (!sc->mm_active) return;
     constexpr int UNR = G < 4 ? G : 4;   // 2 x UNR gathers in flight per lane (8 was slower: registers)
@@ -76,8 +76,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
         if (valid) {
             const float di = dinv[i];
             const float4 uc = di * acc;
-            st4(R + oi, acc);
-            st4(Uc + oi, uc);
+            st4(Uc + oi, uc);      // the residual itself is not stored: r = D uc (D = diag(1 + |N_i|)) whenever it is needed
             st4(A + oi, zi);
             acc_g[0] += (double)dot4(acc, uc);
         }
@@ -181,13 +180,13 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
 
 
 // ---------------------------------------------------------------------------------------------
-// a2  k_cg_update.  A += alpha p;  r -= alpha s;  uc = D^-1 r;  gamma' = (r, uc)   (p, s from k_cg_spmv).  The last block applies the stop rule of the projection (cc_b200.h proj_tol).
+// a2  k_cg_update.  A += alpha p;  uc -= alpha D^-1 s (i.e. r -= alpha s);  gamma' = (r, uc) = D uc.uc   (p, s from k_cg_spmv).  The last block applies the stop rule of the projection (cc_b200.h proj_tol).
 // `loop` is the inner WHILE node's handle in graph mode (0 in eager mode).
 // ---------------------------------------------------------------------------------------------
 template <int G>
 __global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nchunk, const float* __restrict__ dinv,
                                                            float* __restrict__ Uc, const float* __restrict__ Pv,
-                                                           const float* __restrict__ Sv, float* __restrict__ A, float* __restrict__ R, cc_scal* sc,
+                                                           const float* __restrict__ Sv, float* __restrict__ A, cc_scal* sc,
                                                            double* part, cudaGraphConditionalHandle loop) {
     if (!sc->mm_active || !sc->cg_active) return;
     const int gl = threadIdx.x & (G - 1);
@@ -202,11 +201,11 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nch
         const size_t oi = (size_t)i * ld + c0;
         const float4 pv = ld4s(Pv + oi), sv = ld4s(Sv + oi);
         st4(A + oi, fma4(alpha, pv, ld4s(A + oi)));
-        const float4 r = fma4(-alpha, sv, ld4s(R + oi));
-        const float4 uc = dinv[i] * r;
-        st4(R + oi, r);
+        // r <- r - alpha s with r kept only as uc = D^-1 r:  uc <- uc - alpha D^-1 s;  (r, uc) = D uc.uc
+        const float di = dinv[i];
+        const float4 uc = fma4(-alpha * di, sv, ld4s(Uc + oi));
         st4(Uc + oi, uc);
-        acc_g[0] += (double)dot4(r, uc);
+        acc_g[0] += (double)(dot4(uc, uc) / di);
     }
     double tot[1];
     if (grid_reduce<1>(acc_g, part, &sc->ticket[2], tot)) {
@@ -457,7 +456,7 @@ void ccs_begin_iter(cc_handle* h) { k_begin_iter<<<1, 1, 0, h->stream>>>(h->sc);
 
 void ccs_rhs(cc_handle* h) {
     CC_DISPATCH_G(h, k_rhs, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->order, h->rowptr, h->col, h->s, h->dinv, h->Ap,
-                  h->Z, h->U, h->R, h->Uc, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART, g_inner(h));
+                  h->Z, h->U, h->Uc, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART, g_inner(h));
 }
 
 void ccs_cg_spmv(cc_handle* h) {
@@ -467,7 +466,7 @@ void ccs_cg_spmv(cc_handle* h) {
 
 void ccs_cg_update(cc_handle* h) {
     CC_DISPATCH_G(h, k_cg_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->dinv, h->Uc, h->Pv,
-                  h->Sv, h->A, h->R, h->sc, h->part + 2 * CC_MAXBLK * CC_NPART, g_inner(h));
+                  h->Sv, h->A, h->sc, h->part + 2 * CC_MAXBLK * CC_NPART, g_inner(h));
 }
 
 void ccs_norm(cc_handle* h) {

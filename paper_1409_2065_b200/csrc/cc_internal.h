@@ -50,6 +50,7 @@ struct cc_scal {
 };
 
 // Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
+#define CC_INV_NMAX 384     // largest n whose projection uses the precomputed inverse (n x 128 floats of shared memory)
 #define CC_NPART 4
 #define CC_MAXBLK 16384
 
@@ -80,6 +81,7 @@ struct cc_handle {
     float* nb2;                       // nchunk x nnz partial squared norms of b_ij
     float* tmpE;                      // nnz scratch (diagnostics)
     float* dinv;                      // n: 1 / (1 + |N_i|)
+    float* Minv;                      // n x n: (D^-1 (I+L))^-1 for n <= CC_INV_NMAX, else NULL (CG solver)
     // dense mode (complete graph): n x n matrices instead of the CSR arrays
     float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices)
     float *ubar, *abar;               // column means of U and A'
@@ -127,6 +129,7 @@ void ccs_init_state(cc_handle* h);   // cold start of (Ap, Z, s, vn)
 void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out);
 int ccs_solve_eager(cc_handle* h, int maxit);
 int ccs_build_graph(cc_handle* h);
+int ccs_setup_inverse(cc_handle* h);
 
 // ---- cc_dense.cu (a9) ------------------------------------------------------------------------------
 int ccd_setup(cc_handle* h, const float* W);

@@ -224,6 +224,88 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_update(int n, int ld, int nch
 }
 
 // ---------------------------------------------------------------------------------------------
+// a2, small n: the matrix I + L is the same for every column, every iteration and every gamma, so for
+// n <= CC_INV_NMAX its inverse is formed once (cc_create) and the projection is one small product.
+// k_invert: Gauss-Jordan in fp64 without pivoting (I + L is symmetric, strictly diagonally dominant) of the
+// Jacobi-scaled matrix D^-1 (I + L); the result Minv = (D^-1 (I+L))^-1 maps k_rhs's output uc = D^-1 r0
+// straight to the correction.  One block; work space n x 2n doubles in global memory.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) k_invert(int n, const int* __restrict__ rowptr, const int* __restrict__ col,
+                                                 double* __restrict__ aug, float* __restrict__ Minv) {
+    const int tid = threadIdx.x, w2 = 2 * n;
+    for (int t = tid; t < n * w2; t += 1024) aug[t] = 0.0;
+    __syncthreads();
+    for (int i = tid; i < n; i += 1024) {
+        const double dg = 1.0 + (double)(rowptr[i + 1] - rowptr[i]);
+        aug[(size_t)i * w2 + i] = 1.0;                                   // D^-1 (I+L): unit diagonal
+        for (int e = rowptr[i]; e < rowptr[i + 1]; ++e) aug[(size_t)i * w2 + col[e]] = -1.0 / dg;
+        aug[(size_t)i * w2 + n + i] = 1.0;
+    }
+    __syncthreads();
+    __shared__ double pivinv;
+    for (int k = 0; k < n; ++k) {
+        if (tid == 0) pivinv = 1.0 / aug[(size_t)k * w2 + k];
+        __syncthreads();
+        for (int c = tid; c < w2; c += 1024) aug[(size_t)k * w2 + c] *= pivinv;
+        __syncthreads();
+        // eliminate column k from every other row: thread = (row, column stripe)
+        for (int t = tid; t < n * w2; t += 1024) {
+            const int r = t / w2, c = t % w2;
+            if (r != k && c != k) aug[(size_t)r * w2 + c] -= aug[(size_t)r * w2 + k] * aug[(size_t)k * w2 + c];
+        }
+        __syncthreads();
+        for (int r = tid; r < n; r += 1024)
+            if (r != k) aug[(size_t)r * w2 + k] = 0.0;
+        __syncthreads();
+    }
+    for (int t = tid; t < n * n; t += 1024) Minv[t] = (float)aug[(size_t)(t / n) * w2 + n + t % n];
+}
+
+// A_i += sum_j Minv[i][j] uc_j.  One CTA per chunk of 128 columns: uc's chunk (n x 128) is staged in shared
+// memory once, each warp then produces rows i = w, w + 8, ...
+template <int DUMMY>
+__global__ void __launch_bounds__(CC_THREADS) k_apply_inv(int n, int ld, const float* __restrict__ Minv,
+                                                           const float* __restrict__ Uc, float* __restrict__ A, cc_scal* sc) {
+    if (!sc->mm_active) return;
+    extern __shared__ float us[];                  // n x 128
+    const int c0 = blockIdx.x * 128, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int c = c0 + lane * 4;
+    for (int t = threadIdx.x; t < n * 32; t += CC_THREADS) {
+        const int j = t >> 5, l4 = (t & 31) * 4;
+        const float4 v = (c0 + l4 < ld) ? ld4s(Uc + (size_t)j * ld + c0 + l4) : f4(0.f);
+        *reinterpret_cast<float4*>(us + (size_t)j * 128 + l4) = v;
+    }
+    __syncthreads();
+    if (c < ld) {
+        // rows are dealt to (blockIdx.y, warp) round-robin; two rows per pass for instruction-level parallelism
+        const int stride = (CC_THREADS / 32) * gridDim.y;
+        for (int i = blockIdx.y + gridDim.y * warp; i < n; i += 2 * stride) {
+            const int i2 = i + stride;
+            const bool two = i2 < n;
+            float4 acc = f4(0.f), acc2 = f4(0.f);
+            const float* mrow = Minv + (size_t)i * n;
+            const float* mrow2 = Minv + (size_t)(two ? i2 : i) * n;
+#pragma unroll 4
+            for (int j = 0; j < n; ++j) {
+                const float4 uj = *reinterpret_cast<const float4*>(us + (size_t)j * 128 + lane * 4);
+                acc = fma4(__ldg(mrow + j), uj, acc);
+                acc2 = fma4(__ldg(mrow2 + j), uj, acc2);
+            }
+            st4(A + (size_t)i * ld + c, ld4s(A + (size_t)i * ld + c) + acc);
+            if (two) st4(A + (size_t)i2 * ld + c, ld4s(A + (size_t)i2 * ld + c) + acc2);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&sc->ticket[5], 1u) == gridDim.x * gridDim.y - 1) {
+            sc->ticket[5] = 0u;
+            prof_mark(sc, 2);      // charged to the k_cg_update slot: it takes the place of the CG loop
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
 // a3 + a6  k_norm.  For every pair i<j (the entries col > i of row i, a suffix because rows are
 // sorted):  b_ij = a_i - a_j (L84),  ||b_ij||^2 -> nb2 (both directions),  ||v_ij - b_ij||^2 with
 // v_ij = s_ij (a'_i - a'_j);  per node ||u_i - a_i||^2 and the observed loss.  Last block:
@@ -455,8 +537,38 @@ static cudaGraphConditionalHandle g_outer(const cc_handle* h) { return h->cond_o
 void ccs_begin_iter(cc_handle* h) { k_begin_iter<<<1, 1, 0, h->stream>>>(h->sc); }
 
 void ccs_rhs(cc_handle* h) {
+    // small-n path: no warm start (z = u), the exact inverse follows
+    const float* Z = h->Minv ? h->U : h->Z;
     CC_DISPATCH_G(h, k_rhs, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, h->order, h->rowptr, h->col, h->s, h->dinv, h->Ap,
-                  h->Z, h->U, h->Uc, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART, g_inner(h));
+                  Z, h->U, h->Uc, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART, h->Minv ? 0 : g_inner(h));
+}
+
+void ccs_apply_inv(cc_handle* h) {
+    const int nch = (int)((h->ld + 127) / 128);
+    int split = (2 * h->sms + nch - 1) / nch;          // enough CTAs to fill the GPU: split the rows over blockIdx.y
+    if (split > 8) split = 8;
+    if (split * 16 > (int)h->n) split = (int)(h->n / 16);
+    if (split < 1) split = 1;
+    k_apply_inv<0><<<dim3((unsigned)nch, (unsigned)split), CC_THREADS, (size_t)h->n * 128 * sizeof(float), h->stream>>>(
+        (int)h->n, (int)h->ld, h->Minv, h->Uc, h->A, h->sc);
+}
+
+// cc_create: form Minv when n is small enough (the work space is released right away)
+int ccs_setup_inverse(cc_handle* h) {
+    h->Minv = nullptr;
+    if (h->dense || h->n > CC_INV_NMAX || h->prm.reserved0 == 32) return CC_OK;
+    const size_t n = (size_t)h->n;
+    if (n * 128 * sizeof(float) > 48 * 1024) {
+        cudaError_t ea = cudaFuncSetAttribute(k_apply_inv<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 128 * sizeof(float)));
+        if (ea != cudaSuccess) { cudaGetLastError(); return CC_OK; }   // fall back to the CG solver
+    }
+    double* aug = nullptr;
+    CC_CUDA(h, cc_dev_alloc((void**)&aug, n * 2 * n * sizeof(double), h->stream));
+    CC_CUDA(h, cc_dev_alloc((void**)&h->Minv, n * n * sizeof(float), h->stream));
+    k_invert<<<1, 1024, 0, h->stream>>>((int)h->n, h->rowptr, h->col, aug, h->Minv);
+    cc_dev_free(aug, h->stream);
+    h->launches += 1;
+    return CC_OK;
 }
 
 void ccs_cg_spmv(cc_handle* h) {
@@ -477,7 +589,7 @@ void ccs_norm(cc_handle* h) {
 
 void ccs_update(cc_handle* h) {
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->X, h->mask,
-                  h->A, h->U, h->Z, h->Ap, h->Dl, h->w, h->nb2, h->s, h->vn, h->sc);
+                  h->A, h->U, h->Minv ? (float*)nullptr : h->Z, h->Ap, h->Dl, h->w, h->nb2, h->s, h->vn, h->sc);
 }
 
 void ccs_update_nodes(cc_handle* h) {
@@ -499,7 +611,8 @@ int ccs_solve_eager(cc_handle* h, int maxit) {
         ccs_begin_iter(h);
         ccs_rhs(h);
         h->launches += 2;
-        for (;;) {
+        if (h->Minv) { ccs_apply_inv(h); h->launches += 1; }
+        for (; !h->Minv;) {
             CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
             CC_CUDA(h, cudaStreamSynchronize(h->stream));
             if (!h->sc_host->mm_active || !h->sc_host->cg_active) break;
@@ -530,7 +643,8 @@ int ccs_build_graph(cc_handle* h) {
     cudaStream_t user = h->stream;
     CC_CUDA(h, cudaGraphCreate(&h->graph, 0));
     CC_CUDA(h, cudaGraphConditionalHandleCreate(&h->cond_outer, h->graph, 1, cudaGraphCondAssignDefault));
-    CC_CUDA(h, cudaGraphConditionalHandleCreate(&h->cond_inner, h->graph, 0, cudaGraphCondAssignDefault));
+    if (!h->Minv)   // a handle that no conditional node uses makes the graph invalid
+        CC_CUDA(h, cudaGraphConditionalHandleCreate(&h->cond_inner, h->graph, 0, cudaGraphCondAssignDefault));
     cudaGraphNodeParams op = {};
     op.type = cudaGraphNodeTypeConditional;
     op.conditional.handle = h->cond_outer;
@@ -543,6 +657,21 @@ int ccs_build_graph(cc_handle* h) {
     h->stream = cap;  // launchers enqueue on h->stream: capture them
     cudaError_t e = cudaStreamBeginCaptureToGraph(cap, og, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed);
     cudaGraph_t ig = nullptr;
+    if (e == cudaSuccess && h->Minv) {
+        ccs_rhs(h);
+        ccs_apply_inv(h);
+        ccs_norm(h);
+        ccs_update(h);
+        e = cudaStreamEndCapture(cap, nullptr);
+        h->stream = user;
+        cudaStreamDestroy(cap);
+        if (e != cudaSuccess) {
+            snprintf(h->err, sizeof(h->err), "building the solve graph: %s", cudaGetErrorString(e));
+            return CC_ECUDA;
+        }
+        CC_CUDA(h, cudaGraphInstantiate(&h->gexec, h->graph, 0));
+        return CC_OK;
+    }
     if (e == cudaSuccess) {
         ccs_rhs(h);
         cudaStreamCaptureStatus st;

@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
                                                      float* __restrict__ Uc, float* __restrict__ A,
                                                      cc_scal* sc, double* part, cudaGraphConditionalHandle loop) {
     if (!sc->mm_active) return;
-    constexpr int UNR = G < 4 ? G : 4;   // 2 x UNR gathers in flight per lane (8 was slower: registers)
+    constexpr int UNR = G < 16 ? G : 16;  // a whole batch of gathers in flight per pass
     const unsigned gm = group_mask<G>();
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -51,25 +51,37 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
         for (int base = rs; base < re; base += G) {
             const int e = base + gl;
             const int cj = e < re ? __ldg(col + e) : i;   // padding entries point at the own row with s = 1:
-            const float sv = e < re ? __ldg(s + e) : 1.f; // 1*(a_i - a_i) - (z_i - z_i) = 0 exactly
+            const float sv = e < re ? __ldg(s + e) : 0.f; // s = 0: no a' gather, and (z_i - z_i) = 0 exactly
             const int cnt = min(G, re - base);
+            // two passes over the batch, each with all its gathers in flight (as in k_cg_spmv): first z_j (every
+            // entry), then a'_j (only where s_ij != 0 -- a fused pair has v = 0 and needs no a'_j)
+            for (int t = 0; t < cnt; t += UNR) {
+                int j[UNR];
+                float4 zj[UNR];
+#pragma unroll
+                for (int q = 0; q < UNR; ++q) {
+                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
+                    if (UNR > G && t + q >= G) j[q] = i;
+                }
+#pragma unroll
+                for (int q = 0; q < UNR; ++q) zj[q] = ld4s(Z + (size_t)j[q] * ld + (valid ? c0 : 0));
+#pragma unroll
+                for (int q = 0; q < UNR; ++q) acc = acc - (zi - zj[q]);     // padding: j = i contributes 0
+            }
             for (int t = 0; t < cnt; t += UNR) {
                 int j[UNR];
                 float sj[UNR];
-                float4 aj[UNR], zj[UNR];
+                float4 aj[UNR];
 #pragma unroll
                 for (int q = 0; q < UNR; ++q) {
                     j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
                     sj[q] = __shfl_sync(gm, sv, (t + q) & (G - 1), G);
+                    if (UNR > G && t + q >= G) sj[q] = 0.f;
                 }
 #pragma unroll
-                for (int q = 0; q < UNR; ++q) {
-                    const size_t oj = (size_t)j[q] * ld + (valid ? c0 : 0);
-                    aj[q] = sj[q] != 0.f ? ld4s(Ap + oj) : api;    // fused pair (s = 0): v = 0, a'_j is not needed
-                    zj[q] = ld4s(Z + oj);
-                }
+                for (int q = 0; q < UNR; ++q) aj[q] = sj[q] != 0.f ? ld4s(Ap + (size_t)j[q] * ld + (valid ? c0 : 0)) : api;
 #pragma unroll
-                for (int q = 0; q < UNR; ++q) acc = fma4(sj[q], api - aj[q], acc) - (zi - zj[q]);
+                for (int q = 0; q < UNR; ++q) acc = fma4(sj[q], api - aj[q], acc);
             }
         }
         acc = acc - (zi - ui);

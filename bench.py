@@ -389,7 +389,10 @@ def run_ours(args):
     line = {"metric": "pair-updates/sec per MM iteration", "value": units / (ms / 1e3), "unit": "pair-updates/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "n": n, "p": p, "k": wl.k, "pairs": E, "nnz": nnz,
+            "config": {"workload": args.workload,
+                       "workload_note": "large_sparse is the config north_star names for the roofline target and the largest sparse "
+                                        "single-GPU one; other configs: --workload (numbers in profiles/)",
+                       "n": n, "p": p, "k": wl.k, "pairs": E, "nnz": nnz,
                        "iters_per_step": args.iters, "gamma": "50-value log grid walked with stride 5, warm-started",
                        "cg_sweeps_per_iter": cg_per_it, "rho": stats["rho"], "kappa": 1e-2, "proj_tol": 1e-5,
                        "l2": "working set (node arrays + pair arrays, %.0f MB) vs 126 MB L2; no flush" %

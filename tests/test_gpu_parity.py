@@ -363,3 +363,65 @@ def test_dense_mode_rejects_bad_weights(B, torch_):
     with pytest.raises(B.CCError) as e:
         B.cc_create(n, p, X, None, None, None, W, B.cc_default_params(dense=1))
     assert e.value.code == B.CC_EGRAPH
+
+
+def test_two_points_closed_form_and_single_point(B, torch_):
+    """The n = 2 problem has the exact solution (north_star; pin P2): fused at the mean iff ||x1-x2|| <= 2 gamma w,
+    else each point moves gamma w along the unit difference -- checked on the GPU path directly, no oracle involved.
+    n = 1 (no pairs) must return U = X."""
+    torch = torch_
+    dev = torch.device("cuda:0")
+    x = np.array([[0.0, 0.0, 1.0], [3.0, 4.0, 1.0]], np.float32)
+    delta, w = 5.0, 0.7
+    rowptr = torch.tensor([0, 1, 2], dtype=torch.int64, device=dev)
+    col = torch.tensor([1, 0], dtype=torch.int32, device=dev)
+    wv = torch.tensor([w, w], dtype=torch.float32, device=dev)
+    prm = B.cc_default_params(rho_abs=40.0, kappa=1e-2)
+    h = B.cc_create(2, 3, torch.from_numpy(x).to(dev), None, rowptr, col, wv, prm)
+    U = torch.empty(2, 3, device=dev)
+    lab = torch.empty(2, dtype=torch.int32, device=dev)
+    B.cc_solve(h, 1.0, 0.0, 20000)                      # unfused: delta = 5 > 2 gamma w = 1.4
+    B.cc_get_U(h, -1, U)
+    u = U.cpu().numpy().astype(np.float64)
+    e = (x[0] - x[1]).astype(np.float64) / delta
+    assert np.abs(u[0] - (x[0] - 1.0 * w * e)).max() < 2e-4 and np.abs(u[1] - (x[1] + 1.0 * w * e)).max() < 2e-4
+    assert B.cc_clusters(h, -1, lab)[1] == 2
+    B.cc_reset(h)
+    B.cc_solve(h, 5.0, 0.0, 20000)                      # fused: delta = 5 <= 2 gamma w = 7
+    B.cc_get_U(h, -1, U)
+    u = U.cpu().numpy().astype(np.float64)
+    assert B.cc_clusters(h, -1, lab)[1] == 1
+    assert np.abs((u[0] + u[1]) / 2 - x.mean(axis=0)).max() < 1e-5
+    kap = 1e-2                                          # residual gap of the smoothed iteration: 3 kappa delta / (2 + 3 kappa)
+    assert abs(np.linalg.norm(u[0] - u[1]) - 3 * kap * delta / (2 + 3 * kap)) < 5e-3
+    B.cc_destroy(h)
+    h = B.cc_create(1, 3, torch.from_numpy(x[:1].copy()).to(dev), None, torch.zeros(2, dtype=torch.int64, device=dev), None, None, None)
+    B.cc_solve(h, 3.0, 0.0, 5)
+    U1 = torch.empty(1, 3, device=dev)
+    B.cc_get_U(h, -1, U1)
+    assert np.array_equal(U1.cpu().numpy(), x[:1])
+    B.cc_destroy(h)
+
+
+def test_cc_path_dense_mode_snapshots(B, torch_, oracle):
+    torch = torch_
+    wl = synth.make("genotype", n=20, p=1000)
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    gammas = [float(g) for g in synth.gamma_grid(4.0, 40.0, 4)]
+    ref = H.oracle_path(oracle, prob, gammas, 60, proj_method=1)
+    dev = torch.device("cuda:0")
+    h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
+                    B.cc_default_params(dense=1))
+    its, phis = B.cc_path(h, gammas, 0.0, 60)
+    U = torch.empty(n, wl.p)
+    lab = torch.empty(n, dtype=torch.int32)
+    for gi, r in enumerate(ref):
+        B.cc_get_U(h, gi, U)
+        assert H.relerr(U.numpy().astype(np.float64), r["U"]) <= TOL
+        _, k = B.cc_clusters(h, gi, lab)
+        assert k == r["nclusters"] and np.array_equal(lab.numpy(), r["labels"])
+    B.cc_destroy(h)

@@ -138,6 +138,12 @@ int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int3
  * 0..ngamma-1: the snapshot cc_path took.  U_out is DEVICE when out_on_device != 0, else HOST. */
 int cc_get_U(cc_handle* h, int32_t gamma_index, float* U_out, int32_t out_on_device);
 
+/* ---- f2 (part): project U on q <= 8 caller-given directions on the device (PAPER.md L144 plots the path on two
+ * principal components; L202/L210: reading all of U back per gamma was the paper's bottleneck).
+ * out[i][k] = sum_c (u_ic - xbar_c) P[c][k], xbar = observed column means of X.  P: DEVICE p*q row-major;
+ * out: n*q, DEVICE when out_on_device != 0 else HOST (then the call synchronises).  gamma_index as in cc_get_U. */
+int cc_get_projection(cc_handle* h, int32_t gamma_index, const float* P, int32_t q, float* out, int32_t out_on_device);
+
 /* ---- a8: cluster read-out (S16; the paper never defines it, L154, L206) ---------------------------
  * Connected components of the graph whose edges are the pairs with v_ij = 0 exactly, numbered in
  * increasing order of each component's smallest member.  labels_out: int32[n], DEVICE when

@@ -176,3 +176,61 @@ extern "C" int cc_smallest_connected_k(int64_t n, int64_t p, const float* X, con
     *k_out = best;   // -1: not connected even at kmax
     return CC_OK;
 }
+
+
+// ---- f2 (part): project U(gamma) on q given directions before any read-back ---------------
+// out[i][k] = sum_c (u_ic - xbar_c) P[c][k], xbar = observed column means of X.  One warp per row, fixed reduction order.
+namespace {
+constexpr int PQMAX = 8;
+__global__ void __launch_bounds__(256) k_project(int n, int p, int ld, int q, const float* __restrict__ U,
+                                                 const float* __restrict__ xbar, const float* __restrict__ P,
+                                                 float* __restrict__ out) {
+    const int lane = threadIdx.x & 31;
+    const long long nw = (long long)gridDim.x * (blockDim.x >> 5);
+    for (long long i = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); i < n; i += nw) {
+        float acc[PQMAX];
+#pragma unroll
+        for (int k = 0; k < PQMAX; ++k) acc[k] = 0.f;
+        for (int c = lane; c < p; c += 32) {
+            const float v = U[(size_t)i * ld + c] - xbar[c];
+#pragma unroll
+            for (int k = 0; k < PQMAX; ++k)
+                if (k < q) acc[k] = fmaf(v, __ldg(P + (size_t)c * q + k), acc[k]);
+        }
+#pragma unroll
+        for (int k = 0; k < PQMAX; ++k) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) acc[k] += __shfl_xor_sync(0xffffffffu, acc[k], o);
+            if (lane == 0 && k < q) out[(size_t)i * q + k] = acc[k];
+        }
+    }
+}
+}  // namespace
+
+extern "C" int cc_get_projection(cc_handle* h, int32_t gamma_index, const float* P, int32_t q, float* out,
+                                 int32_t out_on_device) {
+    if (!h) return CC_EINVAL;
+    if (!P || !out || q < 1 || q > PQMAX) {
+        snprintf(h->err, sizeof(h->err), "cc_get_projection: need P, out and 1 <= q <= %d", PQMAX);
+        return CC_EINVAL;
+    }
+    if (gamma_index < -1 || gamma_index >= h->nsnap) {
+        snprintf(h->err, sizeof(h->err), "cc_get_projection: gamma_index %d outside [-1, %d)", gamma_index, h->nsnap);
+        return CC_ESTATE;
+    }
+    const float* src = gamma_index < 0 ? h->U : h->snapU + (size_t)gamma_index * h->n * h->ld;
+    float* dst = out;
+    const size_t bytes = (size_t)h->n * q * sizeof(float);
+    if (!out_on_device) CC_CUDA(h, cc_dev_alloc((void**)&dst, bytes, h->stream));
+    const long long g = (h->n + 7) / 8;
+    k_project<<<(unsigned)(g < h->grid_nodes ? g : h->grid_nodes), 256, 0, h->stream>>>((int)h->n, (int)h->p, (int)h->ld, q, src,
+                                                                                      h->colmean, P, dst);
+    h->launches += 1;
+    if (!out_on_device) {
+        cudaError_t e = cudaMemcpyAsync(out, dst, bytes, cudaMemcpyDeviceToHost, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        cc_dev_free(dst, h->stream);
+        if (e != cudaSuccess) { snprintf(h->err, sizeof(h->err), "cc_get_projection: %s", cudaGetErrorString(e)); return CC_ECUDA; }
+    }
+    return CC_OK;
+}

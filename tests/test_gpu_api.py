@@ -154,6 +154,32 @@ def test_graph_utilities(B, oracle):
     assert B.cc_smallest_connected_k(wl.n, wl.p, _dev(torch, wl.X), None, max(1, kref - 1)) == -1
 
 
+def test_projection_of_the_path_on_given_directions(B, oracle):
+    """f2 (part): (U - xbar) P on the device against the plain fp64 product, masked data (xbar = observed means)."""
+    import torch
+    wl = synth.make("expression", n=30, p=203)
+    X64 = wl.X.astype(np.float64)
+    ei, ej, w, _ = oracle.knn_graph(X64, wl.mask, 4, 0.002)
+    rp, cl, ww = oracle.to_csr(wl.n, ei, ej, w)
+    h = B.cc_create(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), _dev(torch, rp.astype(np.int64)),
+                    _dev(torch, cl.astype(np.int32)), _dev(torch, ww.astype(np.float32)), None)
+    B.cc_path(h, [1.0, 10.0], 0.0, 20)
+    rng = np.random.default_rng(0)
+    P = rng.normal(size=(wl.p, 2)).astype(np.float32)
+    xbar = oracle.column_means(X64, wl.mask)
+    U = torch.empty(wl.n, wl.p)
+    for gi in (0, 1, -1):
+        B.cc_get_U(h, gi, U)
+        ref = (U.numpy().astype(np.float64) - xbar[None, :]) @ P.astype(np.float64)
+        out_h = torch.empty(wl.n, 2)
+        out_d = torch.empty(wl.n, 2, device="cuda:0")
+        B.cc_get_projection(h, gi, _dev(torch, P), out_h)
+        B.cc_get_projection(h, gi, _dev(torch, P), out_d)
+        assert np.array_equal(out_h.numpy(), out_d.cpu().numpy())
+        assert np.abs(out_h.numpy() - ref).max() <= 1e-4 * max(1.0, np.abs(ref).max())
+    B.cc_destroy(h)
+
+
 def test_full_size_large_sparse_properties(B):
     """configs[3] at full size, in the launch configuration bench.py times: properties that hold at
     any size -- Phi non-increasing, column sums of U equal those of X when nothing

@@ -425,3 +425,37 @@ def test_cc_path_dense_mode_snapshots(B, torch_, oracle):
         _, k = B.cc_clusters(h, gi, lab)
         assert k == r["nclusters"] and np.array_equal(lab.numpy(), r["labels"])
     B.cc_destroy(h)
+
+
+def test_dense_tensor_core_path_multi_tile(B, torch_, oracle):
+    """n = 1024 (8 row tiles, 36 pair tiles, two accumulator chunks in the contraction), sharper weights so the path
+    goes 1024 -> 264 -> 1 clusters: the TMA-fed tcgen05 kernels against the oracle at every gamma."""
+    torch = torch_
+    wl = synth.make("dense_weight", n=1024, p=64, n_clusters=8)
+    X64 = wl.X.astype(np.float64)
+    si, sj = synth.sample_pairs(wl.n, 200000, 0)
+    wl.phi_rule, wl.phi = "fixed", 6.0 / float(np.median(oracle.pair_dist2(X64, None, si, sj)))
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    assert len(prob["ei"]) == n * (n - 1) // 2
+    gammas = [300.0, 1500.0, 6000.0]
+    ref = H.oracle_path(oracle, prob, gammas, 40, proj_method=1)
+    assert ref[0]["nclusters"] == n and 1 < ref[1]["nclusters"] < n
+    dev = torch.device("cuda:0")
+    X = torch.from_numpy(wl.X).to(dev)
+    W = B.cc_dense_weights(n, wl.p, X, None, float(wl.phi))          # a0 for complete graphs feeds the solver directly
+    Wref = np.zeros((n, n)); Wref[prob["ei"], prob["ej"]] = prob["w64"]; Wref = Wref + Wref.T
+    assert np.abs(W.cpu().numpy() - Wref).max() <= 2e-5 * Wref.max()
+    W = torch.from_numpy(Wref.astype(np.float32)).to(dev)            # identical fp32 weights on both sides
+    h = B.cc_create(n, wl.p, X, None, None, None, W, B.cc_default_params(dense=1))
+    U = torch.empty(n, wl.p, device=dev)
+    lab = torch.empty(n, dtype=torch.int32, device=dev)
+    for g, r in zip(gammas, ref):
+        B.cc_solve(h, g, 0.0, 40)
+        B.cc_get_U(h, -1, U)
+        _, k = B.cc_clusters(h, -1, lab)
+        ph, dd = B.cc_get_history(h)
+        assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, g
+        assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (g, k, r["nclusters"])
+        assert np.allclose(ph, r["phi"], rtol=1e-4) and np.allclose(dd, r["d"], rtol=5e-4), g
+    B.cc_destroy(h)

@@ -269,7 +269,8 @@ def test_cc_path_snapshots(B, torch_, oracle):
                                           ("dense_weight", dict(n=150, p=200, n_clusters=4), 0.0),   # 8x8 tiles, ragged rows
                                           ("dense_weight", dict(n=70, p=40, n_clusters=3), 0.2),     # masked
                                           ("dense_weight", dict(n=256, p=200, n_clusters=4), 0.0),   # tcgen05 path, ragged N tile
-                                          ("dense_weight", dict(n=132, p=64, n_clusters=3), 0.1)])   # tcgen05, ragged M and K
+                                          ("dense_weight", dict(n=132, p=64, n_clusters=3), 0.1),    # tcgen05, ragged M and K
+                                          ("dense_weight", dict(n=200, p=6, n_clusters=3), 0.0)])    # tcgen05, p far below one tile
 def test_dense_mode_complete_graph(B, torch_, oracle, name, kw, miss):
     """prm.dense = 1 (row a9): w is the n x n matrix; closed-form projection, pair tiles."""
     torch = torch_

@@ -143,7 +143,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
         CC_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
         CC_CUDA(h, cudaMemcpyAsync(S, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
         CC_CUDA(h, cudaStreamSynchronize(h->stream));
-        h->launches += h->dense ? (h->dn_small ? 3LL : (h->dn_tc ? 8LL : 6LL)) * S->mm_iter : (h->Minv ? 4LL * S->mm_iter : 3LL * S->mm_iter + 2LL * S->cg_total);
+        h->launches += h->dense ? (h->dn_small ? 3LL : (h->dn_tc ? 10LL : 8LL)) * S->mm_iter : (h->Minv ? 4LL * S->mm_iter : 3LL * S->mm_iter + 2LL * S->cg_total);
     } else {
         int rc = h->dense ? ccd_solve_eager(h, maxit) : ccs_solve_eager(h, maxit);
         if (rc != CC_OK) return rc;

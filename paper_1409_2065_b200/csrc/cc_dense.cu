@@ -49,6 +49,30 @@ __global__ void kd_colsum2(int n, int ld, int nslice, const double* __restrict__
     abar[c] = (float)(sa / n);
 }
 
+// ---- kd_dsum: dbar_c = mean_i (a_ic - u_ic).  The projection satisfies 1'(A - U) = 0 exactly (1'L = 0); in fp32 the
+// contraction leaves a residual of ~5e-7 (relative) per iteration in the column sums, which would add up along a
+// path of thousands of iterations.  k_update subtracts dbar from A, restoring the invariant every iteration.
+__global__ void kd_dsum1(int n, int ld, int nslice, const float* __restrict__ A, const float* __restrict__ U,
+                         double* __restrict__ ps, const cc_scal* sc) {
+    if (!sc->mm_active) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int sl = blockIdx.y;
+    if (c >= ld) return;
+    const int r0 = (int)((long long)n * sl / nslice), r1 = (int)((long long)n * (sl + 1) / nslice);
+    double s = 0.0;
+    for (int i = r0; i < r1; ++i) s += (double)(A[(size_t)i * ld + c] - U[(size_t)i * ld + c]);
+    ps[(size_t)sl * ld + c] = s;
+}
+
+__global__ void kd_dsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ dbar, const cc_scal* sc) {
+    if (!sc->mm_active) return;
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ld) return;
+    double s = 0.0;
+    for (int sl = 0; sl < nslice; ++sl) s += ps[(size_t)sl * ld + c];
+    dbar[c] = (float)(s / n);
+}
+
 // ---- kd_proj ---------------------------------------------------------------------------------------
 // CTA tile: BI = 16 TM rows x C = 16 TN columns, 256 threads as 16 (rows) x 16 (columns), thread tile
 // TM x TN.  Loop over j in blocks of BJ = 32: stage S[I, J] (transposed) and A'[J, C] - abar in shared
@@ -68,14 +92,23 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
     __shared__ __align__(16) float At[BJ][C];
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
     const int i0 = blockIdx.y * BI, c0 = blockIdx.x * C;
+    // fp32 partial sums over one block of BJ terms, totals in fp64: at n = 8192 a single fp32 running sum of
+    // s_ij (magnitude ~n) costs 1e-4 of accuracy on U after a dozen iterations (measured against the oracle)
     float acc[TM][TN], rs[TM];
+    double accd[TM][TN], rsd[TM];
 #pragma unroll
     for (int a = 0; a < TM; ++a) {
-        rs[a] = 0.f;
+        rsd[a] = 0.0;
 #pragma unroll
-        for (int b = 0; b < TN; ++b) acc[a][b] = 0.f;
+        for (int b = 0; b < TN; ++b) accd[a][b] = 0.0;
     }
     for (int j0 = 0; j0 < n; j0 += BJ) {
+#pragma unroll
+        for (int a = 0; a < TM; ++a) {
+            rs[a] = 0.f;
+#pragma unroll
+            for (int b = 0; b < TN; ++b) acc[a][b] = 0.f;
+        }
         for (int t = tid; t < BI * BJ; t += 256) {      // S[i0+ii][j0+jj], jj fastest: 128-byte segments
             const int jj = t % BJ, ii = t / BJ;
             const int gi = i0 + ii, gj = j0 + jj;
@@ -109,6 +142,12 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
                 for (int b = 0; b < TN; ++b) acc[a][b] = fmaf(sv[a], av[b], acc[a][b]);
             }
         }
+#pragma unroll
+        for (int a = 0; a < TM; ++a) {
+            rsd[a] += (double)rs[a];
+#pragma unroll
+            for (int b = 0; b < TN; ++b) accd[a][b] += (double)acc[a][b];
+        }
         __syncthreads();
     }
     // epilogue: a = u + [rowsum(S) (a' - abar) - S(A' - abar) - n (u - ubar)] / (n+1)
@@ -124,8 +163,10 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
             if (gc >= ld) continue;
             const size_t o = (size_t)gi * ld + gc;
             const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
-            const float4 sa = make_float4(acc[a][b4 * 4 + 0], acc[a][b4 * 4 + 1], acc[a][b4 * 4 + 2], acc[a][b4 * 4 + 3]);
-            const float4 g = (rs[a] * ap - sa) - fn * (u - ub);
+            // the two large terms are combined in fp64
+            const float4 sg = make_float4((float)(rsd[a] * (double)ap.x - accd[a][b4 * 4 + 0]), (float)(rsd[a] * (double)ap.y - accd[a][b4 * 4 + 1]),
+                                          (float)(rsd[a] * (double)ap.z - accd[a][b4 * 4 + 2]), (float)(rsd[a] * (double)ap.w - accd[a][b4 * 4 + 3]));
+            const float4 g = sg - fn * (u - ub);
             const float4 dl = inv * g;
             st4(A + o, u + dl);
             float4 q = ld4s(X + o) - u;
@@ -375,7 +416,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
                 const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
                 const float4 sa = make_float4(accr[h2 * 16 + q4 * 4 + 0], accr[h2 * 16 + q4 * 4 + 1],
                                               accr[h2 * 16 + q4 * 4 + 2], accr[h2 * 16 + q4 * 4 + 3]);
-                const float4 g = (rs * ap - sa) - fn * (u - ub);
+                // the two large terms (magnitude ~n) are combined in fp64
+                const float4 sg = make_float4((float)((double)rs * ap.x - sa.x), (float)((double)rs * ap.y - sa.y),
+                                              (float)((double)rs * ap.z - sa.z), (float)((double)rs * ap.w - sa.w));
+                const float4 g = sg - fn * (u - ub);
                 const float4 dl = inv * g;
                 st4(A + o, u + dl);
                 float4 q = ld4s(X + o) - u;
@@ -542,7 +586,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc2(int n, int ld, int 
                 const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
                 const float4 sa = make_float4(accr[h2 * 16 + q4 * 4 + 0], accr[h2 * 16 + q4 * 4 + 1],
                                               accr[h2 * 16 + q4 * 4 + 2], accr[h2 * 16 + q4 * 4 + 3]);
-                const float4 g = (rs * ap - sa) - fn * (u - ub);
+                // the two large terms (magnitude ~n) are combined in fp64
+                const float4 sg = make_float4((float)((double)rs * ap.x - sa.x), (float)((double)rs * ap.y - sa.y),
+                                              (float)((double)rs * ap.z - sa.z), (float)((double)rs * ap.w - sa.w));
+                const float4 g = sg - fn * (u - ub);
                 const float4 dl = inv * g;
                 st4(A + o, u + dl);
                 float4 q = ld4s(X + o) - u;
@@ -1125,7 +1172,6 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
                         As[i][c] = a;
                         if (c0 + c < ld) {
                             const size_t o = (size_t)i * ld + c0 + c;
-                            A[o] = a;
                             dua = fmaf(dl, dl, dua);
                             const float q = X[o] - u;
                             if (!mask || mask[o]) los = fmaf(q, q, los);
@@ -1135,6 +1181,20 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
             }
             red[0] += (double)dua;
             red[1] += (double)los;
+            __syncthreads();
+            // 1'(A - U) = 0 holds exactly for the projection; remove the fp32 residual of this chunk's columns
+            if (tid < SM_C) {
+                float sd = 0.f;
+                for (int r = 0; r < n; ++r) sd += As[r][tid] - Us[r][tid];
+                ubar_s[tid] = sd / fn;
+            }
+            __syncthreads();
+            for (int t = tid; t < n * SM_C; t += 256) {
+                const int r = t / SM_C, cc2 = t % SM_C;
+                const float a2 = As[r][cc2] - ubar_s[cc2];
+                As[r][cc2] = a2;
+                if (c0 + cc2 < ld) A[(size_t)r * ld + c0 + cc2] = a2;
+            }
             __syncthreads();
         }
         if (pair_thread) {
@@ -1452,8 +1512,6 @@ void ccd_proj(cc_handle* h) {
         return;
     }
     if (!h->dn_big) launch_proj<4, 4>(h);
-    else if (h->prm.reserved0 == 1) launch_proj<8, 8>(h);
-    else if (h->prm.reserved0 == 2) launch_proj<8, 4>(h);
     else launch_proj<4, 8>(h);
 }
 
@@ -1552,6 +1610,8 @@ int ccd_setup(cc_handle* h, const float* W) {
     cudaError_t e = cc_dev_alloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->ubar, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->abar, (size_t)h->ld * sizeof(float), h->stream);
+    if (e == cudaSuccess && !h->dn_small) e = cc_dev_alloc((void**)&h->dbar, (size_t)h->ld * sizeof(float), h->stream);
+    if (e == cudaSuccess && h->dbar) e = cudaMemsetAsync(h->dbar, 0, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->colps, (size_t)kSliceDense * 2 * h->ld * sizeof(double), h->stream);
     if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
     if (h->dn_tc) {
@@ -1617,6 +1677,11 @@ void ccd_iteration(cc_handle* h) {
     }
     ccd_colmeans(h);
     ccd_proj(h);
+    {
+        dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)kSliceDense);
+        kd_dsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->A, h->U, h->colps, h->sc);
+        kd_dsum2<<<(unsigned)((h->ld + 127) / 128), 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->colps, h->dbar, h->sc);
+    }
     ccd_pairs(h);
     ccs_update_nodes(h);
     ccd_edges(h, 0);

@@ -85,6 +85,7 @@ struct cc_handle {
     // dense mode (complete graph): n x n matrices instead of the CSR arrays
     float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices)
     float *ubar, *abar;               // column means of U and A'
+    float* dbar;                      // column means of A - U (dense mode; subtracted by k_update)
     double* colps;                    // partial column sums
     uint8_t* pre_pairs;               // kd_prep_pairs: TF32 hi/lo operand tiles in the tensor core's smem layout
     float* nrm_part;                  // per-K-block partial row norms

@@ -444,6 +444,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
                                                         const float* __restrict__ X, const uint8_t* __restrict__ mask,
                                                         const float* __restrict__ A, float* __restrict__ U,
                                                         float* __restrict__ Z, float* __restrict__ Ap, float* __restrict__ Dl,
+                                                        const float* __restrict__ dbar,
                                                         const float* __restrict__ w, const float* __restrict__ nb2,
                                                         float* __restrict__ s, float* __restrict__ vn, cc_scal* sc) {
     if (!sc->mm_active) return;
@@ -456,7 +457,9 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
         const int c0 = (int)(it % nchunk) * 4 * G + gl * 4;
         if (c0 >= ld) continue;
         const size_t oi = (size_t)i * ld + c0;
-        const float4 a = ld4s(A + oi), u = ld4s(U + oi);
+        float4 a = ld4s(A + oi);
+        const float4 u = ld4s(U + oi);
+        if (dbar) a = a - ld4s(dbar + c0);     // dense mode: restore 1'(A - U) = 0 exactly (see kd_dsum)
         float4 y = ld4s(X + oi);
         if (mask) {
             const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + oi);
@@ -601,13 +604,13 @@ void ccs_norm(cc_handle* h) {
 
 void ccs_update(cc_handle* h) {
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->X, h->mask,
-                  h->A, h->U, h->Minv ? (float*)nullptr : h->Z, h->Ap, h->Dl, h->w, h->nb2, h->s, h->vn, h->sc);
+                  h->A, h->U, h->Minv ? (float*)nullptr : h->Z, h->Ap, h->Dl, (const float*)nullptr, h->w, h->nb2, h->s, h->vn, h->sc);
 }
 
 void ccs_update_nodes(cc_handle* h) {
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, 0LL, h->X, h->mask, h->A, h->U,
-                  (float*)nullptr, h->Ap, (float*)nullptr, (const float*)nullptr, (const float*)nullptr, (float*)nullptr,
-                  (float*)nullptr, h->sc);
+                  (float*)nullptr, h->Ap, (float*)nullptr, (const float*)h->dbar, (const float*)nullptr, (const float*)nullptr,
+                  (float*)nullptr, (float*)nullptr, h->sc);
 }
 
 void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out) {

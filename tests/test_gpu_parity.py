@@ -460,3 +460,102 @@ def test_dense_tensor_core_path_multi_tile(B, torch_, oracle):
         assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (g, k, r["nclusters"])
         assert np.allclose(ph, r["phi"], rtol=1e-4) and np.allclose(dd, r["d"], rtol=5e-4), g
     B.cc_destroy(h)
+
+
+def test_full_size_genotype_elementwise(B, torch_, oracle):
+    """configs[2] at full size (52 x 200,000, complete graph, the fused kd_small kernel, 296 CTAs as in bench.py):
+    every element of U against the oracle."""
+    torch = torch_
+    wl = synth.make("genotype")
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    gammas = [10.0, 30.0]
+    ref = H.oracle_path(oracle, prob, gammas, 8, proj_method=1)
+    dev = torch.device("cuda:0")
+    h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
+                    B.cc_default_params(dense=1))
+    U = torch.empty(n, wl.p, device=dev)
+    lab = torch.empty(n, dtype=torch.int32, device=dev)
+    for g, r in zip(gammas, ref):
+        B.cc_solve(h, g, 0.0, 8)
+        B.cc_get_U(h, -1, U)
+        _, k = B.cc_clusters(h, -1, lab)
+        ph, dd = B.cc_get_history(h)
+        diff = U.cpu().numpy().astype(np.float64) - r["U"]
+        assert np.linalg.norm(diff) / np.linalg.norm(r["U"]) <= TOL, g
+        assert np.abs(diff).max() <= 1e-5, g                      # element-wise (allele frequencies are in [0, 1])
+        assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"])
+        assert np.allclose(ph, r["phi"], rtol=1e-4) and np.allclose(dd, r["d"], rtol=5e-4)
+    B.cc_destroy(h)
+
+
+def test_full_size_expression_elementwise(B, torch_, oracle):
+    """configs[1] at full size (100 x 5000, 10 % missing, 10-NN, the precomputed-inverse projection)."""
+    wl = synth.make("expression")
+    prob = H.build_problem(oracle, wl)
+    gammas = [0.5, 5.0, 50.0]
+    ref = H.oracle_path(oracle, prob, gammas, 60)
+    _run_path(B, torch_, prob, gammas, 60, ref)
+
+
+def test_full_size_dense_weight_properties(B, torch_):
+    """configs[4] at full size (8192 x 256; the oracle's explicit V would be 68 GB): the tensor-core kernels against
+    the FFMA kernels of the same library, and the properties that hold at any size (Phi non-increasing, column sums
+    of U conserved when nothing is missing)."""
+    torch = torch_
+    wl = synth.make("dense_weight")
+    dev = torch.device("cuda:0")
+    X = torch.from_numpy(wl.X).to(dev)
+    n, p = wl.n, wl.p
+    si, sj = synth.sample_pairs(n, 200000, 0)
+    d = X[torch.from_numpy(si).to(dev)] - X[torch.from_numpy(sj).to(dev)]
+    phi = 1.0 / float((d * d).sum(1).median())
+    W = B.cc_dense_weights(n, p, X, None, phi)
+    outs = []
+    for tune in (0, 4):
+        h = B.cc_create(n, p, X, None, None, None, W, B.cc_default_params(dense=1, reserved0=tune))
+        for g in (5.0, 20.0):
+            it, phi_v, _ = B.cc_solve(h, g, 0.0, 6)
+            ph, dd = B.cc_get_history(h)
+            assert it == 6 and np.all(np.diff(ph) <= 1e-6 * np.abs(ph[:-1])) and np.all(dd > 0)
+        U = torch.empty(n, p, device=dev)
+        B.cc_get_U(h, -1, U)
+        rel = (U.double().sum(0) - X.double().sum(0)).abs().max().item() / X.double().abs().sum(0).max().item()
+        assert rel <= 1e-6, (tune, rel)
+        outs.append(U.double())
+        B.cc_destroy(h)
+    assert ((outs[0] - outs[1]).norm() / outs[1].norm()).item() <= 1e-5
+
+
+def test_dense_n8192_against_oracle_small_p(B, torch_, oracle):
+    """The full number of points of configs[4] (8192, 33.5 M pairs) with p = 8 so that the oracle's explicit V fits:
+    both kernel families against the oracle.  (This is the test that exposed a 1e-4 loss in the FFMA contraction's
+    single fp32 running sum over 8192 terms.)"""
+    torch = torch_
+    n, p = 8192, 8
+    wl = synth.make("dense_weight", n=n, p=p, n_clusters=32)
+    prob = H.build_problem(oracle, wl)
+    assert len(prob["ei"]) == n * (n - 1) // 2
+    gammas = [0.5, 2.0]
+    ref = H.oracle_path(oracle, prob, gammas, 6, proj_method=1)
+    dev = torch.device("cuda:0")
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    Wd, X = torch.from_numpy(W).to(dev), torch.from_numpy(wl.X).to(dev)
+    for tune in (0, 4):
+        h = B.cc_create(n, p, X, None, None, None, Wd, B.cc_default_params(dense=1, reserved0=tune))
+        U = torch.empty(n, p, device=dev)
+        lab = torch.empty(n, dtype=torch.int32, device=dev)
+        for g, r in zip(gammas, ref):
+            B.cc_solve(h, g, 0.0, 6)
+            B.cc_get_U(h, -1, U)
+            _, k = B.cc_clusters(h, -1, lab)
+            ph, dd = B.cc_get_history(h)
+            assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= 1e-5, (tune, g)
+            assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"])
+            assert np.allclose(ph, r["phi"], rtol=1e-5) and np.allclose(dd, r["d"], rtol=1e-4), (tune, g)
+        B.cc_destroy(h)

@@ -559,3 +559,20 @@ def test_dense_n8192_against_oracle_small_p(B, torch_, oracle):
             assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"])
             assert np.allclose(ph, r["phi"], rtol=1e-5) and np.allclose(dd, r["d"], rtol=1e-4), (tune, g)
         B.cc_destroy(h)
+
+
+@pytest.mark.skipif(os.environ.get("CC_SLOW") != "1", reason="about 6 minutes of oracle time; run with CC_SLOW=1")
+def test_full_size_large_sparse_elementwise_slow(B, torch_, oracle):
+    """configs[3] at full size (100,000 x 64, 856,602 pairs), in the launch configuration bench.py times: the graph
+    from cc_knn_weights must equal the oracle's brute-force graph, then every element of U after 2 x 4 iterations."""
+    torch = torch_
+    wl = synth.make("large_sparse")
+    prob = H.build_problem(oracle, wl)
+    dev = torch.device("cuda:0")
+    X = torch.from_numpy(wl.X).to(dev)
+    rowptr, col, w = B.cc_knn_weights(wl.n, wl.p, X, None, wl.k, prob["phi"])
+    assert np.array_equal(rowptr.cpu().numpy(), prob["rowptr"]) and np.array_equal(col.cpu().numpy(), prob["col"])
+    gammas = [5.0, 80.0]
+    ref = H.oracle_path(oracle, prob, gammas, 4, proj_method=1)
+    out = _run_path(B, torch, prob, gammas, 4, ref)
+    print("full-size large_sparse: relerr, clusters =", out)

@@ -561,17 +561,38 @@ def test_dense_n8192_against_oracle_small_p(B, torch_, oracle):
         B.cc_destroy(h)
 
 
-@pytest.mark.skipif(os.environ.get("CC_SLOW") != "1", reason="about 6 minutes of oracle time; run with CC_SLOW=1")
-def test_full_size_large_sparse_elementwise_slow(B, torch_, oracle):
+def test_full_size_large_sparse_elementwise(B, torch_, oracle):
     """configs[3] at full size (100,000 x 64, 856,602 pairs), in the launch configuration bench.py times: the graph
-    from cc_knn_weights must equal the oracle's brute-force graph, then every element of U after 2 x 4 iterations."""
+    from cc_knn_weights against the oracle's brute-force graph, then every element of U after 2 x 4 iterations
+    (about 80 s, most of it the oracle's 10^10-pair neighbour search)."""
     torch = torch_
     wl = synth.make("large_sparse")
     prob = H.build_problem(oracle, wl)
     dev = torch.device("cuda:0")
     X = torch.from_numpy(wl.X).to(dev)
     rowptr, col, w = B.cc_knn_weights(wl.n, wl.p, X, None, wl.k, prob["phi"])
-    assert np.array_equal(rowptr.cpu().numpy(), prob["rowptr"]) and np.array_equal(col.cpu().numpy(), prob["col"])
+    # 10^10 candidate pairs: a few k-th / (k+1)-th neighbours are closer than fp32 can tell apart, and the kernel decides in
+    # fp32 where the oracle decides in fp64.  What is unique must agree; every other entry must be such a near-tie.
+    n = wl.n
+    rows_g = np.repeat(np.arange(n, dtype=np.int64), np.diff(rowptr.cpu().numpy()))
+    key_g = rows_g * n + col.cpu().numpy().astype(np.int64)
+    rows_o = np.repeat(np.arange(n, dtype=np.int64), np.diff(prob["rowptr"]))
+    key_o = rows_o * n + prob["col"].astype(np.int64)
+    extra = np.concatenate([np.setdiff1d(key_g, key_o), np.setdiff1d(key_o, key_g)])
+    assert extra.size <= 200, extra.size
+    if extra.size:
+        X64 = wl.X.astype(np.float64)
+        ii, jj = extra // n, extra % n
+        touched = np.unique(np.concatenate([ii, jj]))
+        _, d2k = oracle.knn(X64, None, wl.k + 1, rows=touched)
+        kth = dict(zip(touched.tolist(), d2k[:, wl.k - 1].tolist()))
+        kth1 = dict(zip(touched.tolist(), d2k[:, wl.k].tolist()))
+        dij = ((X64[ii] - X64[jj]) ** 2).sum(1)
+        for a, b2, dd2 in zip(ii.tolist(), jj.tolist(), dij.tolist()):
+            near = min(abs(dd2 - kth[a]) / kth[a], abs(dd2 - kth1[a]) / kth1[a],
+                       abs(dd2 - kth[b2]) / kth[b2], abs(dd2 - kth1[b2]) / kth1[b2])
+            assert near <= 1e-5, (a, b2, near)
+    print("full-size k-NN graph: directed entries that differ from the fp64 brute force (all near-ties):", extra.size)
     gammas = [5.0, 80.0]
     ref = H.oracle_path(oracle, prob, gammas, 4, proj_method=1)
     out = _run_path(B, torch, prob, gammas, 4, ref)

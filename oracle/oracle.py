@@ -261,6 +261,32 @@ def objective(X, mask, ei, ej, w, gamma, U) -> float:
     return float(0.5 * (r * r).sum() + gamma * (np.asarray(w) * np.sqrt(np.einsum("ij,ij->i", df, df))).sum())
 
 
+# ----------------------------------------------------------------------------- f2: principal components
+def principal_components(X, mask, q: int):
+    """[reading S25; "project the cluster path onto any two principal components of the
+    original data"]  The q leading principal directions of the original data: X with its missing
+    entries set to the observed column mean (the cold start U0 of S4), columns centred, then the
+    textbook definition by the singular value decomposition  Xc = W diag(sigma) P^T:  direction k is
+    row k of P^T, its variance sigma_k^2 / (n - 1)  (the eigenpairs of the sample covariance
+    Xc^T Xc / (n - 1)).  Signs: the entry of largest magnitude of each direction is made positive.
+    Returns (P  p x q,  variances  q)."""
+    U0, _ = cold_start(X, mask, np.zeros(0, dtype=np.int64), np.zeros(0, dtype=np.int64))
+    n = U0.shape[0]
+    Xc = U0 - U0.mean(axis=0)[None, :]
+    _, sig, Pt = np.linalg.svd(Xc, full_matrices=False)
+    P = Pt[:q].T.copy()
+    for k in range(P.shape[1]):
+        if P[np.argmax(np.abs(P[:, k])), k] < 0:
+            P[:, k] = -P[:, k]
+    return P, (sig[:q] ** 2) / max(n - 1, 1)
+
+
+def project_on_components(X, mask, U, P):
+    """[PAPER.md L144, L210] coordinates of the rows of U on the directions P (p x q), measured from
+    the observed column means of X:  (U - 1 xbar^T) P."""
+    return (_f64(U) - column_means(X, mask)[None, :]) @ _f64(P)
+
+
 def path(X, mask, ei, ej, w, gammas, maxit, tol=0.0, min_it=10, rho_scale=1.1, kappa=1e-2, proj_method=0,
          proj_tol=1e-13):
     """gamma path with warm starts (warm start: reading S4).  rho, eps per gamma by

@@ -369,3 +369,66 @@ def test_golden_tiny_path_is_reproducible(oracle):
         assert abs(r["phi"][-1] - g["phi_last"]) < 1e-9 * abs(g["phi_last"])
         assert abs(np.linalg.norm(r["U"]) - g["U_fro"]) < 1e-9 * g["U_fro"]
         assert r["nclusters"] == g["nclusters"]
+
+
+# ----------------------------------------------------------------------------- f2: principal components (S25, L144)
+def _householder(p, seed):
+    """An explicit orthogonal matrix I - 2 h h^T / (h^T h) (its columns are the planted directions)."""
+    h = np.random.default_rng(seed).standard_normal(p)
+    return np.eye(p) - 2.0 * np.outer(h, h) / float(h @ h)
+
+
+def test_P14_principal_components_of_a_planted_cross(oracle):
+    """Closed form: the 2p points  c +/- s_k r_k  (r_k the columns of a reflector R) have the sample
+    covariance  R diag(2 s_k^2 / (n-1)) R^T,  so direction k is r_k and its variance 2 s_k^2/(n-1)."""
+    p = 6
+    R = _householder(p, 3)
+    s = np.array([5.0, 3.5, 2.0, 1.0, 0.5, 0.25])
+    c = np.linspace(-1.0, 2.0, p)
+    X = np.concatenate([c[None, :] + s[:, None] * R.T, c[None, :] - s[:, None] * R.T])
+    X = X[np.random.default_rng(0).permutation(2 * p)]
+    P, var = oracle.principal_components(X, None, 3)
+    assert np.allclose(var, 2.0 * s[:3] ** 2 / (2 * p - 1), rtol=1e-12)
+    for k in range(3):
+        r = R[:, k] * np.sign(R[np.argmax(np.abs(R[:, k])), k])
+        assert np.allclose(P[:, k], r, atol=1e-12)
+
+
+def test_P14_principal_components_satisfy_the_eigen_equation_of_a_loop_built_covariance(oracle):
+    """Brute force on a tiny masked input: the covariance is accumulated entry by entry with Python loops
+    from the imputed data; C v = lambda v, orthonormality, the trace identity with q = p, decreasing order,
+    and the variance of the projected coordinates equals lambda."""
+    rng = np.random.default_rng(5)
+    n, p = 9, 4
+    X = rng.standard_normal((n, p)) * np.array([3.0, 1.0, 0.3, 2.0]) + 1.5
+    mask = (rng.random((n, p)) > 0.25).astype(np.uint8)
+    mask[0, :] = 1
+    mean = [sum(X[i, c] for i in range(n) if mask[i, c]) / sum(int(mask[i, c]) for i in range(n)) for c in range(p)]
+    Y = [[X[i, c] if mask[i, c] else mean[c] for c in range(p)] for i in range(n)]
+    cm = [sum(Y[i][c] for i in range(n)) / n for c in range(p)]
+    C = np.zeros((p, p))
+    for a in range(p):
+        for b in range(p):
+            C[a, b] = sum((Y[i][a] - cm[a]) * (Y[i][b] - cm[b]) for i in range(n)) / (n - 1)
+    P, var = oracle.principal_components(X, mask, p)
+    assert np.all(np.diff(var) <= 1e-15)
+    assert np.isclose(var.sum(), np.trace(C), rtol=1e-12)
+    assert np.allclose(P.T @ P, np.eye(p), atol=1e-12)
+    for k in range(p):
+        assert np.allclose(C @ P[:, k], var[k] * P[:, k], atol=1e-12)
+    # imputed entries sit at the column mean, so the centring of project_on_components is the same mean
+    coords = oracle.project_on_components(X, mask, np.array(Y), P)
+    assert np.allclose(coords.mean(axis=0), 0.0, atol=1e-12)
+    assert np.allclose(coords.var(axis=0, ddof=1), var, rtol=1e-12)
+
+
+def test_P14_rank_one_data_has_one_direction(oracle):
+    """x_i = c + t_i g: one direction g/||g|| with variance var(t) ||g||^2, every other variance 0."""
+    rng = np.random.default_rng(8)
+    g = np.array([1.0, -2.0, 0.5, 4.0, 0.0])
+    t = rng.standard_normal(40)
+    X = 0.7 + t[:, None] * g[None, :]
+    P, var = oracle.principal_components(X, None, 2)
+    assert np.allclose(P[:, 0], g / np.linalg.norm(g), atol=1e-12)
+    assert np.isclose(var[0], t.var(ddof=1) * float(g @ g), rtol=1e-12)
+    assert var[1] <= 1e-25 * var[0]

@@ -138,11 +138,27 @@ int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int3
  * 0..ngamma-1: the snapshot cc_path took.  U_out is DEVICE when out_on_device != 0, else HOST. */
 int cc_get_U(cc_handle* h, int32_t gamma_index, float* U_out, int32_t out_on_device);
 
-/* ---- f2 (part): project U on q <= 8 caller-given directions on the device (PAPER.md L144 plots the path on two
+/* ---- f2: project U on q <= 8 caller-given directions on the device (PAPER.md L144 plots the path on two
  * principal components; L202/L210: reading all of U back per gamma was the paper's bottleneck).
  * out[i][k] = sum_c (u_ic - xbar_c) P[c][k], xbar = observed column means of X.  P: DEVICE p*q row-major;
  * out: n*q, DEVICE when out_on_device != 0 else HOST (then the call synchronises).  gamma_index as in cc_get_U. */
 int cc_get_projection(cc_handle* h, int32_t gamma_index, const float* P, int32_t q, float* out, int32_t out_on_device);
+
+/* ---- f2: principal directions of the original data on the device, PAPER.md L144 ("project the cluster path
+ * onto any two principal components of the original data"), L210 ("project the data to principal components on
+ * each GPU itself prior to data transfer").  Reading S25: the data are X with missing entries at the observed
+ * column mean (the cold start), columns centred; direction k is the k-th leading eigenvector of the sample
+ * covariance Xc^T Xc / (n-1).  Computed by block iteration with 16 vectors (two passes over X per step) until
+ * every requested Ritz pair has ||C y - theta y|| <= tol * theta_1, or maxit steps (tol = 1e-6, maxit = 300 are
+ * sensible; the speed of convergence is set by the ratio of the 17th to the q-th eigenvalue).
+ * P_out: p*q fp32 row-major (the layout cc_get_projection takes), DEVICE when out_on_device != 0 else HOST; each
+ * direction has unit length and its entry of largest magnitude is positive.  A direction whose eigenvalue is
+ * below 1e-7 of the largest (data of rank < q) comes back as a zero vector with variance 0.
+ * var_out[q] (HOST, may be NULL): the variances theta_k / (n-1), decreasing.  resid_out[q] (HOST, may be NULL):
+ * the relative residuals reached.  iters_out (HOST, may be NULL): steps taken.  1 <= q <= min(8, p).
+ * Synchronises.  Does not touch the MM state. */
+int cc_principal_components(cc_handle* h, int32_t q, int32_t maxit, double tol, float* P_out, int32_t out_on_device,
+                            double* var_out, double* resid_out, int32_t* iters_out);
 
 /* ---- a8: cluster read-out (S16; the paper never defines it, L154, L206) ---------------------------
  * Connected components of the graph whose edges are the pairs with v_ij = 0 exactly, numbered in

@@ -24,7 +24,7 @@ CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCON
 
 SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_dense_weights", "cc_graph_components",
            "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
-           "cc_get_U", "cc_get_projection", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
+           "cc_get_U", "cc_get_projection", "cc_principal_components", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
            "cc_last_error", "cc_destroy")
 
@@ -52,6 +52,7 @@ _lib.cc_path.argtypes = [_vp, _P(_dbl), _i32, _dbl, _i32, _P(_i32), _P(_dbl)]
 _lib.cc_get_U.argtypes = [_vp, _i32, _vp, _i32]
 _lib.cc_clusters.argtypes = [_vp, _i32, _vp, _i32, _P(_i32)]
 _lib.cc_get_projection.argtypes = [_vp, _i32, _vp, _i32, _vp, _i32]
+_lib.cc_principal_components.argtypes = [_vp, _i32, _i32, _dbl, _vp, _i32, _vp, _vp, _P(_i32)]
 _lib.cc_get_history.argtypes = [_vp, _vp, _vp, _i32, _P(_i32)]
 _lib.cc_get_stats.argtypes = [_vp, _P(_dbl), _P(_dbl), _P(_i64), _P(_dbl), _P(_dbl)]
 _lib.cc_reset.argtypes = [_vp]
@@ -131,6 +132,15 @@ def cc_get_projection(h, gamma_index, P, out):
     """P: fp32 (p,q) device tensor; out: fp32 (n,q) tensor on the device or the host."""
     _check(_lib.cc_get_projection(h, gamma_index, _ptr(P), P.shape[1], _ptr(out), 1 if out.is_cuda else 0), h)
     return out
+
+
+def cc_principal_components(h, P_out, maxit=300, tol=1e-6):
+    """P_out: fp32 (p,q) contiguous torch tensor (device or host).  Returns (P_out, variances[q], residuals[q], steps)."""
+    q = P_out.shape[1]
+    var, res, its = (_dbl * q)(), (_dbl * q)(), _i32(0)
+    _check(_lib.cc_principal_components(h, q, maxit, tol, _ptr(P_out), 1 if P_out.is_cuda else 0, var, res,
+                                        ctypes.byref(its)), h)
+    return P_out, list(var), list(res), its.value
 
 
 def cc_clusters(h, gamma_index, labels_out):

@@ -294,6 +294,25 @@ def run_ours(args):
         path = {"n_gamma": ng, "gamma_lo": lo, "gamma_hi": hi, "tol": 1e-5, "maxit": 2000,
                 "wall_s": p0.elapsed_time(p1) / 1e3, "iters_total": int(sum(its)),
                 "nclusters_first_mid_last": ks}
+        # the same path with kappa continuation (S26): same stop rule, same last stage
+        Up = [torch.empty(n, wl.p, device=dev) for _ in range(3)]
+        for u, g in zip(Up, (0, ng // 2, ng - 1)):
+            B.cc_get_U(h, g, u)
+        B.cc_reset(h)
+        p0.record()
+        its_c, _ = B.cc_path_continuation(h, gam, 0.1, 0.1, 200, 1e-5, 2000)
+        p1.record()
+        torch.cuda.synchronize()
+        ks_c = [B.cc_clusters(h, g, lab)[1] for g in (0, ng // 2, ng - 1)]
+        Uc = torch.empty(n, wl.p, device=dev)
+        dU = []
+        for u, g in zip(Up, (0, ng // 2, ng - 1)):
+            B.cc_get_U(h, g, Uc)
+            dU.append(float((Uc - u).norm() / u.norm().clamp_min(1e-30)))
+        path["continuation"] = {"kappa_start": 0.1, "factor": 0.1, "stage_maxit": 200,
+                                "wall_s": p0.elapsed_time(p1) / 1e3, "iters_total": int(sum(its_c)),
+                                "nclusters_first_mid_last": ks_c, "rel_dU_vs_plain_first_mid_last": dU}
+        del Up, Uc
     B.cc_destroy(h)
 
     # ---- e2e: host buffers -> cc_create -> cc_solve -> U back on the host, every step

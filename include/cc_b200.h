@@ -127,12 +127,33 @@ int cc_create(cc_handle** out, int64_t n, int64_t p, const float* X, const uint8
 int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* iters_out,
              double* phi_out);
 
+/* ---- f1: kappa continuation (not in the paper, reading S26) ----------------------
+ * The iteration count of the MM map grows like 1/kappa (the U update moves a fraction d/(d+rho) ~ kappa of the
+ * way once dist is small).  This runs cc_solve in stages at one gamma: rho stays at S1's value and
+ * eps_s = (kappa_s rho)^2 with kappa_s = kappa_start, kappa_start*factor, ... while larger than prm.kappa; every
+ * stage is warm-started from the previous one and stops by the rule of cc_solve (tol) or after stage_maxit
+ * iterations; the last stage is cc_solve itself at prm.kappa (tol, maxit), so what it converges to is the
+ * contract iteration's fixed point.  kappa_start <= prm.kappa degenerates to a plain cc_solve.  Measured on the
+ * large-sparse path: kappa_start = 0.1, factor = 0.1, stage_maxit = 200 halves the path time at a
+ * smaller distance to the converged path; kappa_start = 1 helps cold starts but not a warm-started path.
+ * stage_iters_out[cap] (HOST, may be NULL with cap = 0): iterations of each stage, *nstages_out (HOST, may be
+ * NULL) the number of stages run (entries beyond cap are not written).  phi_out and the history are the last
+ * stage's.  CC_ESTATE when the handle fixes eps_abs.  Synchronises. */
+int cc_solve_continuation(cc_handle* h, double gamma, double kappa_start, double factor, int32_t stage_maxit,
+                          double tol, int32_t maxit, int32_t* stage_iters_out, int32_t cap, int32_t* nstages_out,
+                          double* phi_out);
+
 /* ---- a7: gamma path, PAPER.md L144 (U stays on the device between gammas, cf. L202) ---------------
  * For each gamma in the caller's order: cc_solve warm-started from the previous gamma, then a device
  * snapshot of U and of the cluster labels.  gammas, iters_out[ngamma], phi_out[ngamma]: HOST (outputs
  * may be NULL).  ngamma must be <= max_snapshots.  Snapshots of an earlier path are dropped. */
 int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int32_t maxit,
             int32_t* iters_out, double* phi_out);
+
+/* f1 on the path: as cc_path, with cc_solve_continuation (same kappa_start, factor, stage_maxit) at every gamma.
+ * iters_out[g] (HOST, may be NULL) = iterations of all stages at gammas[g]. */
+int cc_path_continuation(cc_handle* h, const double* gammas, int32_t ngamma, double kappa_start, double factor,
+                         int32_t stage_maxit, double tol, int32_t maxit, int32_t* iters_out, double* phi_out);
 
 /* Copy U (n*p fp32 row-major) into a caller-owned buffer.  gamma_index = -1: the current state;
  * 0..ngamma-1: the snapshot cc_path took.  U_out is DEVICE when out_on_device != 0, else HOST. */

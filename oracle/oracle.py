@@ -287,6 +287,38 @@ def project_on_components(X, mask, U, P):
     return (_f64(U) - column_means(X, mask)[None, :]) @ _f64(P)
 
 
+# ----------------------------------------------------------------------------- f1: kappa continuation
+def kappa_schedule(kappa_start: float, factor: float, kappa_final: float):
+    """[reading S26] kappa_start, kappa_start*factor, ... while larger than kappa_final, then kappa_final."""
+    ks = []
+    k = float(kappa_start)
+    while k > kappa_final * (1.0 + 1e-12):
+        ks.append(k)
+        k *= factor
+    ks.append(float(kappa_final))
+    return ks
+
+
+def mm_continuation(X, mask, ei, ej, w, gamma, U, V, kappa_start, factor, stage_maxit, maxit, tol=0.0, min_it=10,
+                    rho_scale=1.1, kappa=1e-2, proj_method=0, proj_tol=1e-13):
+    """[reading S26; not in the paper, SURVEY 8(f) f1]  The MM iteration of L57-L88 run in stages at one gamma:
+    rho stays at S1's value, eps_s = (kappa_s rho)^2 follows kappa_schedule; every stage starts from the state the
+    previous one left, runs until the stop rule S3 or `stage_maxit` iterations (`maxit` for the last stage, whose
+    kappa is the contract value).  Returns the last stage's dict plus the per-stage iteration counts."""
+    rho, _ = default_rho_eps(X, mask, w, gamma, rho_scale, kappa)
+    ks = kappa_schedule(kappa_start, factor, kappa)
+    its = []
+    r = None
+    for s, k in enumerate(ks):
+        last = s == len(ks) - 1
+        r = mm(X, mask, ei, ej, w, gamma, rho, (k * rho) ** 2, U, V, maxit if last else stage_maxit, tol, min_it,
+               proj_method, proj_tol)
+        U, V = r["U"], r["V"]
+        its.append(r["iters"])
+    r.update(stage_iters=its, kappas=ks, rho=rho)
+    return r
+
+
 def path(X, mask, ei, ej, w, gammas, maxit, tol=0.0, min_it=10, rho_scale=1.1, kappa=1e-2, proj_method=0,
          proj_tol=1e-13):
     """gamma path with warm starts (warm start: reading S4).  rho, eps per gamma by

@@ -23,7 +23,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
 SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_dense_weights", "cc_graph_components",
-           "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_path",
+           "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_solve_continuation", "cc_path", "cc_path_continuation",
            "cc_get_U", "cc_get_projection", "cc_principal_components", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
            "cc_last_error", "cc_destroy")
@@ -48,7 +48,9 @@ _lib.cc_free_graph.argtypes = [_vp, _vp, _vp]
 _lib.cc_free_graph.restype = None
 _lib.cc_create.argtypes = [_P(_vp), _i64, _i64, _vp, _vp, _vp, _vp, _vp, _P(cc_params), _vp]
 _lib.cc_solve.argtypes = [_vp, _dbl, _dbl, _i32, _P(_i32), _P(_dbl)]
+_lib.cc_solve_continuation.argtypes = [_vp, _dbl, _dbl, _dbl, _i32, _dbl, _i32, _P(_i32), _i32, _P(_i32), _P(_dbl)]
 _lib.cc_path.argtypes = [_vp, _P(_dbl), _i32, _dbl, _i32, _P(_i32), _P(_dbl)]
+_lib.cc_path_continuation.argtypes = [_vp, _P(_dbl), _i32, _dbl, _dbl, _i32, _dbl, _i32, _P(_i32), _P(_dbl)]
 _lib.cc_get_U.argtypes = [_vp, _i32, _vp, _i32]
 _lib.cc_clusters.argtypes = [_vp, _i32, _vp, _i32, _P(_i32)]
 _lib.cc_get_projection.argtypes = [_vp, _i32, _vp, _i32, _vp, _i32]
@@ -120,6 +122,26 @@ def cc_path(h, gammas, tol, maxit):
     phis = (ctypes.c_double * len(gammas))()
     _check(_lib.cc_path(h, g, len(gammas), tol, maxit, its, phis), h)
     return list(its), list(phis)
+
+
+def cc_path_continuation(h, gammas, kappa_start, factor, stage_maxit, tol, maxit):
+    g = (ctypes.c_double * len(gammas))(*[float(x) for x in gammas])
+    its = (ctypes.c_int32 * len(gammas))()
+    phis = (ctypes.c_double * len(gammas))()
+    _check(_lib.cc_path_continuation(h, g, len(gammas), kappa_start, factor, stage_maxit, tol, maxit, its, phis), h,
+           allow=(CC_ENOCONV,))
+    return list(its), list(phis)
+
+
+def cc_solve_continuation(h, gamma, kappa_start, factor, stage_maxit, tol, maxit):
+    """Returns (stage_iters list, phi of the last stage, return code CC_OK / CC_ENOCONV)."""
+    cap = 64
+    its, ns, phi = (_i32 * cap)(), _i32(0), _dbl(0.0)
+    rc = _lib.cc_solve_continuation(h, gamma, kappa_start, factor, stage_maxit, tol, maxit, its, cap, ctypes.byref(ns),
+                                    ctypes.byref(phi))
+    if rc != CC_ENOCONV:
+        _check(rc, h)
+    return list(its[:min(ns.value, cap)]), phi.value, rc
 
 
 def cc_get_U(h, gamma_index, U_out):

@@ -106,7 +106,8 @@ static void rho_eps(const cc_handle* h, double gamma, double* rho, double* eps) 
                                     : h->prm.rho_scale * sqrt(h->xss + gamma * gamma * h->sumw2);
     if (!(r > 0.0)) r = 1.0;  // constant data and gamma = 0: any rho works (U = X at once)
     *rho = r;
-    *eps = h->prm.eps_abs > 0.0 ? h->prm.eps_abs : (h->prm.kappa * r) * (h->prm.kappa * r);
+    const double kappa = h->kappa_stage > 0.0 ? h->kappa_stage : h->prm.kappa;
+    *eps = (h->prm.eps_abs > 0.0 && !(h->kappa_stage > 0.0)) ? h->prm.eps_abs : (kappa * r) * (kappa * r);
 }
 
 int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* iters_out, double* phi_out) {
@@ -158,8 +159,40 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
     return CC_OK;
 }
 
-int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int32_t maxit, int32_t* iters_out,
-            double* phi_out) {
+int cc_solve_continuation(cc_handle* h, double gamma, double kappa_start, double factor, int32_t stage_maxit,
+                          double tol, int32_t maxit, int32_t* stage_iters_out, int32_t cap, int32_t* nstages_out,
+                          double* phi_out) {
+    if (!h) return CC_EINVAL;
+    if (!(kappa_start > 0.0) || std::isinf(kappa_start) || !(factor > 0.0 && factor < 1.0) || stage_maxit < 1 ||
+        cap < 0 || (cap > 0 && !stage_iters_out)) {
+        snprintf(h->err, sizeof(h->err), "cc_solve_continuation: need kappa_start > 0 finite, 0 < factor < 1, stage_maxit >= 1");
+        return CC_EINVAL;
+    }
+    if (h->prm.eps_abs > 0.0) {
+        snprintf(h->err, sizeof(h->err), "cc_solve_continuation: the handle fixes eps_abs; stages need eps = (kappa rho)^2");
+        return CC_ESTATE;
+    }
+    int stage = 0, worst = CC_OK;
+    for (double kappa = kappa_start; kappa > h->prm.kappa * (1.0 + 1e-12); kappa *= factor, ++stage) {
+        int it = 0;
+        h->kappa_stage = kappa;
+        const int rc = cc_solve(h, gamma, tol, stage_maxit, &it, nullptr);
+        h->kappa_stage = 0.0;
+        if (rc != CC_OK && rc != CC_ENOCONV) return rc;
+        if (rc == CC_ENOCONV) worst = rc;
+        if (stage < cap) stage_iters_out[stage] = it;
+    }
+    int it = 0;
+    const int rc = cc_solve(h, gamma, tol, maxit, &it, phi_out);   // the contract iteration, warm-started
+    if (rc != CC_OK && rc != CC_ENOCONV) return rc;
+    if (stage < cap) stage_iters_out[stage] = it;
+    if (nstages_out) *nstages_out = stage + 1;
+    return rc == CC_ENOCONV ? rc : worst;
+}
+
+// kappa_start <= 0: the plain path (cc_solve per gamma); else staged solves (f1).  iters_out[g] = all iterations at gamma g.
+static int path_impl(cc_handle* h, const double* gammas, int32_t ngamma, double kappa_start, double factor,
+                     int32_t stage_maxit, double tol, int32_t maxit, int32_t* iters_out, double* phi_out) {
     if (!h) return CC_EINVAL;
     if (!gammas || ngamma < 0) { snprintf(h->err, sizeof(h->err), "cc_path: bad arguments"); return CC_EINVAL; }
     if (ngamma > h->prm.max_snapshots) {
@@ -181,7 +214,14 @@ int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int3
     for (int g = 0; g < ngamma; ++g) {
         int it = 0;
         double phi = 0.0;
-        int rc = cc_solve(h, gammas[g], tol, maxit, &it, &phi);
+        int rc;
+        if (kappa_start > 0.0) {
+            int32_t st[64], ns = 0;
+            rc = cc_solve_continuation(h, gammas[g], kappa_start, factor, stage_maxit, tol, maxit, st, 64, &ns, &phi);
+            for (int k = 0; k < ns && k < 64; ++k) it += st[k];
+        } else {
+            rc = cc_solve(h, gammas[g], tol, maxit, &it, &phi);
+        }
         if (rc != CC_OK && rc != CC_ENOCONV) return rc;
         if (rc == CC_ENOCONV) worst = rc;
         if (iters_out) iters_out[g] = it;
@@ -192,6 +232,21 @@ int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int3
         h->nsnap = g + 1;
     }
     return worst;
+}
+
+int cc_path(cc_handle* h, const double* gammas, int32_t ngamma, double tol, int32_t maxit, int32_t* iters_out,
+            double* phi_out) {
+    return path_impl(h, gammas, ngamma, 0.0, 0.0, 0, tol, maxit, iters_out, phi_out);
+}
+
+int cc_path_continuation(cc_handle* h, const double* gammas, int32_t ngamma, double kappa_start, double factor,
+                         int32_t stage_maxit, double tol, int32_t maxit, int32_t* iters_out, double* phi_out) {
+    if (!h) return CC_EINVAL;
+    if (!(kappa_start > 0.0)) {
+        snprintf(h->err, sizeof(h->err), "cc_path_continuation: need kappa_start > 0");
+        return CC_EINVAL;
+    }
+    return path_impl(h, gammas, ngamma, kappa_start, factor, stage_maxit, tol, maxit, iters_out, phi_out);
 }
 
 // strided (ld -> p) copy out of the padded layout

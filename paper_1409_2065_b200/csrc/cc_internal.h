@@ -101,6 +101,7 @@ struct cc_handle {
     int* dflag;                       // validation flags
     int sms;                          // multiprocessor count
     double sumw2, xss;                // sum_E w^2, sum_obs (x-colmean)^2
+    double kappa_stage;               // > 0 inside cc_solve_continuation: the kappa of the running stage (f1, S26)
     // snapshots
     float* snapU;                     // max_snapshots x n x ld
     int32_t* snapLab;                 // max_snapshots x n

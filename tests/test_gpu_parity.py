@@ -597,3 +597,125 @@ def test_full_size_large_sparse_elementwise(B, torch_, oracle):
     ref = H.oracle_path(oracle, prob, gammas, 4, proj_method=1)
     out = _run_path(B, torch, prob, gammas, 4, ref)
     print("full-size large_sparse: relerr, clusters =", out)
+
+
+# ----------------------------------------------------------------------------- f1: kappa continuation (S26)
+def _continuation_case(B, torch, oracle, prob, h, g, k0, factor, stage_it, last_it, proj_method=0):
+    X, m = prob["X64"], prob["mask"]
+    U0, V0 = oracle.cold_start(X, m, prob["ei"], prob["ej"])
+    ref = oracle.mm_continuation(X, m, prob["ei"], prob["ej"], prob["w64"], g, U0, V0, k0, factor, stage_it, last_it,
+                                 tol=0.0, proj_method=proj_method)
+    its, phi, rc = B.cc_solve_continuation(h, g, k0, factor, stage_it, 0.0, last_it)
+    assert rc == B.CC_OK and its == ref["stage_iters"]
+    n, p = prob["n"], prob["p"]
+    U = torch.empty(n, p)
+    B.cc_get_U(h, -1, U)
+    lab = torch.empty(n, dtype=torch.int32)
+    _, k = B.cc_clusters(h, -1, lab)
+    rl, rk = oracle.labels(ref["V"], prob["ei"], prob["ej"], n)
+    assert H.relerr(U.numpy().astype(np.float64), ref["U"]) <= TOL
+    assert k == rk and np.array_equal(lab.numpy(), rl)
+    assert abs(phi - ref["phi"][-1]) <= 1e-4 * abs(phi)
+    st = B.cc_get_stats(h)
+    assert abs(st["rho"] - ref["rho"]) <= 1e-6 * ref["rho"]
+    assert abs(st["eps"] - (ref["kappas"][-1] * ref["rho"]) ** 2) <= 1e-6 * st["eps"]     # the last stage is the contract's
+    return ref
+
+
+def test_kappa_continuation_matches_oracle_sparse(B, torch_, oracle):
+    """Stages kappa = 1, 0.1, 0.01 with fixed lengths, cold start, on the k-NN path: element-wise against the oracle's
+    staged iteration (tiny, masked expression-like, 3,000 large-sparse points)."""
+    torch = torch_
+    for wl, g in ((synth.make("tiny"), 100.0), (synth.make("expression", n=40, p=300), 2.0),
+                  (synth.make("large_sparse", n=3000), 20.0)):
+        prob = H.build_problem(oracle, wl)
+        h = H.gpu_create(B, torch, prob)
+        _continuation_case(B, torch, oracle, prob, h, g, 1.0, 0.1, 25, 40)
+        B.cc_destroy(h)
+
+
+def test_kappa_continuation_matches_oracle_dense(B, torch_, oracle):
+    torch = torch_
+    wl = synth.make("dense_weight", n=300, p=40, n_clusters=6)
+    X64 = wl.X.astype(np.float64)
+    si, sj = synth.sample_pairs(wl.n, 200000, 0)
+    wl.phi_rule, wl.phi = "fixed", 6.0 / float(np.median(oracle.pair_dist2(X64, None, si, sj)))
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    dev = torch.device("cuda:0")
+    h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
+                    B.cc_default_params(dense=1))
+    _continuation_case(B, torch, oracle, prob, h, 300.0, 0.5, 0.2, 20, 40, proj_method=1)
+    B.cc_destroy(h)
+
+
+def test_kappa_continuation_stop_rule_and_arguments(B, torch_, oracle):
+    """With tol > 0 every stage stops by S3 near the oracle's count, the staged run needs fewer iterations than the
+    plain one for the same rule, and both end at the same U to the accuracy the rule gives."""
+    torch = torch_
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    X, m = prob["X64"], prob["mask"]
+    U0, V0 = oracle.cold_start(X, m, prob["ei"], prob["ej"])
+    g, tol = 100.0, 1e-7
+    ref = oracle.mm_continuation(X, m, prob["ei"], prob["ej"], prob["w64"], g, U0, V0, 1.0, 0.1, 400, 20000, tol=tol)
+    h = H.gpu_create(B, torch, prob)
+    its, phi, rc = B.cc_solve_continuation(h, g, 1.0, 0.1, 400, tol, 20000)
+    assert len(its) == 3
+    for a, b in zip(its, ref["stage_iters"]):
+        assert abs(a - b) <= max(3, b // 20), (its, ref["stage_iters"])
+    Uc = torch.empty(wl.n, wl.p)
+    B.cc_get_U(h, -1, Uc)
+    B.cc_reset(h)
+    it_plain, _, _ = B.cc_solve(h, g, tol, 20000)
+    Up = torch.empty(wl.n, wl.p)
+    B.cc_get_U(h, -1, Up)
+    assert sum(its) < it_plain, (its, it_plain)
+    assert H.relerr(Uc.numpy().astype(np.float64), Up.numpy().astype(np.float64)) <= 2e-2
+    # kappa_start at or below the contract kappa: one stage, bit-identical to cc_solve
+    B.cc_reset(h)
+    its1, _, _ = B.cc_solve_continuation(h, g, 1e-2, 0.5, 7, 0.0, 30)
+    U1 = torch.empty(wl.n, wl.p)
+    B.cc_get_U(h, -1, U1)
+    B.cc_reset(h)
+    B.cc_solve(h, g, 0.0, 30)
+    B.cc_get_U(h, -1, Up)
+    assert its1 == [30] and np.array_equal(U1.numpy(), Up.numpy())
+    for bad in ((0.0, 0.5, 5), (1.0, 1.0, 5), (1.0, 0.0, 5), (1.0, 0.5, 0)):
+        with pytest.raises(B.CCError) as e:
+            B.cc_solve_continuation(h, g, bad[0], bad[1], bad[2], 0.0, 10)
+        assert e.value.code == B.CC_EINVAL
+    B.cc_destroy(h)
+    h = H.gpu_create(B, torch, prob, eps_abs=1e-3)
+    with pytest.raises(B.CCError) as e:
+        B.cc_solve_continuation(h, g, 1.0, 0.5, 5, 0.0, 10)
+    assert e.value.code == B.CC_ESTATE
+    B.cc_destroy(h)
+
+
+def test_path_continuation_matches_oracle(B, torch_, oracle):
+    """cc_path_continuation: staged solves at every gamma, warm-started along the path, snapshots as cc_path."""
+    torch = torch_
+    wl = synth.make("tiny")
+    prob = H.build_problem(oracle, wl)
+    X, m = prob["X64"], prob["mask"]
+    gammas = [float(g) for g in synth.gamma_grid(1.0, 1e3, 5)]
+    U, V = oracle.cold_start(X, m, prob["ei"], prob["ej"])
+    h = H.gpu_create(B, torch, prob)
+    its, phis = B.cc_path_continuation(h, gammas, 0.5, 0.2, 15, 0.0, 30)
+    Ug = torch.empty(wl.n, wl.p)
+    lab = torch.empty(wl.n, dtype=torch.int32)
+    for gi, g in enumerate(gammas):
+        r = oracle.mm_continuation(X, m, prob["ei"], prob["ej"], prob["w64"], g, U, V, 0.5, 0.2, 15, 30)
+        U, V = r["U"], r["V"]
+        assert its[gi] == sum(r["stage_iters"]) == 15 * 3 + 30
+        B.cc_get_U(h, gi, Ug)
+        assert H.relerr(Ug.numpy().astype(np.float64), U) <= TOL
+        _, k = B.cc_clusters(h, gi, lab)
+        rl, rk = oracle.labels(V, prob["ei"], prob["ej"], wl.n)
+        assert k == rk and np.array_equal(lab.numpy(), rl)
+        assert abs(phis[gi] - r["phi"][-1]) <= 1e-5 * abs(phis[gi])
+    B.cc_destroy(h)

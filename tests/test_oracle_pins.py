@@ -432,3 +432,34 @@ def test_P14_rank_one_data_has_one_direction(oracle):
     assert np.allclose(P[:, 0], g / np.linalg.norm(g), atol=1e-12)
     assert np.isclose(var[0], t.var(ddof=1) * float(g @ g), rtol=1e-12)
     assert var[1] <= 1e-25 * var[0]
+
+
+# ----------------------------------------------------------------------------- f1: kappa continuation (S26)
+def test_P15_kappa_schedule_and_single_stage_is_the_plain_iteration(oracle):
+    assert oracle.kappa_schedule(1.0, 0.1, 1e-2) == pytest.approx([1.0, 0.1, 1e-2])
+    assert oracle.kappa_schedule(1e-2, 0.1, 1e-2) == [1e-2]
+    assert oracle.kappa_schedule(0.5, 0.5, 0.1) == pytest.approx([0.5, 0.25, 0.125, 0.1])
+    X, mask, ei, ej, w = _tiny(oracle, seed=3)
+    U0, V0 = oracle.cold_start(X, mask, ei, ej)
+    rho, eps = oracle.default_rho_eps(X, mask, w, 0.8)
+    a = oracle.mm(X, mask, ei, ej, w, 0.8, rho, eps, U0, V0, 25)
+    b = oracle.mm_continuation(X, mask, ei, ej, w, 0.8, U0, V0, 1e-2, 0.1, 7, 25)
+    assert b["stage_iters"] == [25] and np.array_equal(a["U"], b["U"]) and np.array_equal(a["phi"], b["phi"])
+
+
+def test_P15_continuation_reaches_the_fixed_point_of_the_last_stage(oracle):
+    """The surrogate-free objective of the last stage (eps = (kappa rho)^2) is convex with a unique minimiser in U,
+    so staged and plain runs, both converged, meet: the stages change the road, not the destination.  Also: every
+    stage by itself is the monotone MM iteration (oracle.mm raises if Phi increases)."""
+    X, mask, ei, ej, w = _tiny(oracle, seed=5, n=20, miss=0.15)
+    U0, V0 = oracle.cold_start(X, mask, ei, ej)
+    g = 0.6
+    rho, eps = oracle.default_rho_eps(X, mask, w, g)
+    plain = oracle.mm(X, mask, ei, ej, w, g, rho, eps, U0, V0, 60000, tol=1e-15, min_it=10)
+    cont = oracle.mm_continuation(X, mask, ei, ej, w, g, U0, V0, 1.0, 0.1, 2000, 60000, tol=1e-15)
+    assert len(cont["stage_iters"]) == 3
+    scale = np.linalg.norm(plain["U"])
+    assert np.linalg.norm(plain["U"] - cont["U"]) <= 1e-5 * scale
+    assert abs(oracle.objective(X, mask, ei, ej, w, g, plain["U"]) -
+               oracle.objective(X, mask, ei, ej, w, g, cont["U"])) <= 1e-6 * abs(oracle.objective(X, mask, ei, ej, w, g, plain["U"]))
+    print("iterations plain", plain["iters"], "staged", cont["stage_iters"])

@@ -134,6 +134,43 @@ def knn_graph(X, mask, k: int, phi: float, normalize: bool = False):
     return ei, ej, w, dd
 
 
+def side_dist(Y, period, i: int) -> np.ndarray:
+    """||y_i - y_j|| for all j, the components of the difference "computed in modulo arithmetic" (PAPER.md L137,
+    below eq. 9): with a period P_c > 0 coordinate c's difference is wrapped to [-P_c/2, P_c/2] [reading S27]."""
+    Y = _f64(Y)
+    df = Y[i][None, :] - Y
+    if period is not None:
+        P = np.asarray(period, dtype=np.float64)
+        wrap = P > 0
+        df[:, wrap] = df[:, wrap] - P[wrap] * np.round(df[:, wrap] / P[wrap])
+    return np.sqrt((df * df).sum(axis=1))
+
+
+def composite_knn_graph(X, mask, Y, period, alpha: float, k: int, phi: float, normalize: bool = False):
+    """Eq. 9: d_ij = alpha ||x_i - x_j|| + (1 - alpha) ||y_i - y_j||, then eq. 8 with this d:
+    i~j iff j is among the k nearest of i by d OR vice versa (S9: self excluded, ties -> smaller index),
+    w_ij = exp(-phi d_ij^2), optional normalisation (S8).  ||x_i - x_j|| is the square root of row_dist2 (masked
+    rule S11).  Returns (ei, ej, w, d) with ei<ej sorted by (ei, ej)."""
+    n = X.shape[0]
+    pairs = {}
+    for i in range(n):
+        dx = np.sqrt(row_dist2(X, mask, i))
+        dx[i] = 0.0                      # row_dist2 marks the row itself with inf; it is excluded below
+        d = alpha * dx + (1.0 - alpha) * side_dist(Y, period, i)
+        d[i] = np.inf
+        order = np.lexsort((np.arange(n), d))[:k]
+        for j in order:
+            pairs[(min(i, int(j)), max(i, int(j)))] = d[j]
+    keys = sorted(pairs)
+    ei = np.array([a for a, _ in keys], dtype=np.int32)
+    ej = np.array([b for _, b in keys], dtype=np.int32)
+    dd = np.array([pairs[key] for key in keys])
+    w = np.exp(-phi * dd * dd)
+    if normalize:
+        w = w / w.sum()
+    return ei, ej, w, dd
+
+
 def complete_graph(X, mask, phi: float, normalize: bool = False):
     """All pairs i<j with Gaussian weights (eq. 8 with k = n-1)."""
     n = X.shape[0]

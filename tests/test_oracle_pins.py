@@ -463,3 +463,41 @@ def test_P15_continuation_reaches_the_fixed_point_of_the_last_stage(oracle):
     assert abs(oracle.objective(X, mask, ei, ej, w, g, plain["U"]) -
                oracle.objective(X, mask, ei, ej, w, g, cont["U"])) <= 1e-6 * abs(oracle.objective(X, mask, ei, ej, w, g, plain["U"]))
     print("iterations plain", plain["iters"], "staged", cont["stage_iters"])
+
+
+# ----------------------------------------------------------------------------- f4: composite distance, eq. 9 (L135-L137)
+def test_P16_composite_distance_limits_and_wrap(oracle):
+    rng = np.random.default_rng(2)
+    n, p = 40, 5
+    X = rng.standard_normal((n, p))
+    Y = np.stack([rng.uniform(-180, 180, n), rng.uniform(-60, 60, n)], axis=1)
+    # alpha = 1: eq. 9 is ||x_i - x_j||, so the graph is eq. 8's and the weight exp(-phi d^2) is the same number
+    e8 = oracle.knn_graph(X, None, 4, 0.3)
+    e9 = oracle.composite_knn_graph(X, None, Y, None, 1.0, 4, 0.3)
+    assert np.array_equal(e8[0], e9[0]) and np.array_equal(e8[1], e9[1]) and np.allclose(e8[2], e9[2], rtol=1e-12)
+    # alpha = 0: the graph of the side coordinates alone
+    e8y = oracle.knn_graph(Y, None, 4, 0.3)
+    e9y = oracle.composite_knn_graph(X, None, Y, None, 0.0, 4, 0.3)
+    assert np.array_equal(e8y[0], e9y[0]) and np.array_equal(e8y[1], e9y[1]) and np.allclose(e8y[2], e9y[2], rtol=1e-12)
+    # modulo arithmetic: longitudes 179 and -179 are 2 apart, not 358; latitude (period 0) is not wrapped
+    Yw = np.array([[179.0, 10.0], [-179.0, 10.0], [0.0, 10.0], [90.0, -50.0]])
+    d = oracle.side_dist(Yw, [360.0, 0.0], 0)
+    assert np.allclose(d, [0.0, 2.0, 179.0, np.hypot(89.0, 60.0)])
+    assert np.allclose(oracle.side_dist(Yw, None, 0)[1], 358.0)
+    # brute force of eq. 9 entry by entry on the small case, and the OR rule
+    al = 0.35
+    D = np.zeros((n, n))
+    for i in range(n):
+        for j in range(n):
+            dy0 = Y[i, 0] - Y[j, 0]
+            dy0 -= 360.0 * round(dy0 / 360.0)
+            D[i, j] = al * np.sqrt(sum((X[i, c] - X[j, c]) ** 2 for c in range(p))) + (1 - al) * np.hypot(dy0, Y[i, 1] - Y[j, 1])
+        D[i, i] = np.inf
+    near = [set(np.argsort(D[i], kind="stable")[:3].tolist()) for i in range(n)]
+    want = sorted({(min(i, j), max(i, j)) for i in range(n) for j in near[i]})
+    ei, ej, w, dd = oracle.composite_knn_graph(X, None, Y, [360.0, 0.0], al, 3, 0.01)
+    assert list(zip(ei.tolist(), ej.tolist())) == want
+    assert np.allclose(dd, [D[a, b] for a, b in want], rtol=1e-12)
+    assert np.allclose(w, np.exp(-0.01 * dd ** 2), rtol=1e-12)
+    wn = oracle.composite_knn_graph(X, None, Y, [360.0, 0.0], al, 3, 0.01, normalize=True)[2]
+    assert np.isclose(wn.sum(), 1.0) and np.allclose(wn * w.sum(), w)

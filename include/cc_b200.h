@@ -86,6 +86,19 @@ int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, in
                    int32_t normalize, int64_t** rowptr, int32_t** col, float** w, int64_t* nnz,
                    void* stream);
 
+/* ---- f4: the same build on the composite distance of eq. 9, PAPER.md L135-L137 -------------------------
+ *   d_ij = alpha ||x_i - x_j|| + (1 - alpha) ||y_i - y_j||,  0 <= alpha <= 1,
+ * y_i the caller's side coordinates (e.g. GPS): Y (DEVICE, n*q fp32 row-major, 1 <= q <= 4).  "The components
+ * of the difference y_i - y_j must be computed in modulo arithmetic" (L137): period (HOST, q floats, or NULL)
+ * gives each coordinate's period (360 for a longitude in degrees), 0 = plain difference; a periodic difference
+ * is wrapped to [-period/2, period/2] (S27).  ||x_i - x_j|| is the square root of the (masked, S11) squared
+ * distance of cc_knn_weights.  Neighbours are the k smallest d_ij, w_ij = exp(-phi d_ij^2); everything else
+ * (OR rule, ties, normalisation, outputs, ownership, errors) as cc_knn_weights.  The geodesic alternative L137
+ * mentions is not built. */
+int cc_knn_weights_composite(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t q, const float* Y,
+                             const float* period, float alpha, int32_t k, float phi, int32_t normalize,
+                             int64_t** rowptr, int32_t** col, float** w, int64_t* nnz, void* stream);
+
 /* a0 for complete graphs (k = n-1): W_out (DEVICE, caller-owned, n*n fp32 row-major) receives
  * w_ij = exp(-phi ||x_i - x_j||^2) for i != j and 0 on the diagonal, symmetric bit for bit; same distance
  * rules and normalisation as cc_knn_weights.  The result feeds cc_create with prm.dense = 1.  X, mask:

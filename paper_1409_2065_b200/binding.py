@@ -22,7 +22,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
-SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_dense_weights", "cc_graph_components",
+SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_knn_weights_composite", "cc_dense_weights", "cc_graph_components",
            "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_solve_continuation", "cc_path", "cc_path_continuation",
            "cc_get_U", "cc_get_projection", "cc_principal_components", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
@@ -41,6 +41,8 @@ _P = ctypes.POINTER
 _lib.cc_default_params.argtypes = [_P(cc_params)]
 _lib.cc_knn_weights.argtypes = [_i64, _i64, _vp, _vp, _i32, ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp),
                                 _P(_i64), _vp]
+_lib.cc_knn_weights_composite.argtypes = [_i64, _i64, _vp, _vp, _i32, _vp, _P(ctypes.c_float), ctypes.c_float, _i32,
+                                          ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp), _P(_i64), _vp]
 _lib.cc_dense_weights.argtypes = [_i64, _i64, _vp, _vp, ctypes.c_float, _i32, _vp, _vp]
 _lib.cc_graph_components.argtypes = [_i64, _vp, _vp, _vp, _P(_i32), _vp]
 _lib.cc_smallest_connected_k.argtypes = [_i64, _i64, _vp, _vp, _i32, _P(_i32), _vp]
@@ -252,13 +254,21 @@ def _wrap(ptr, count, typestr, dev):
     return torch.as_tensor(_DevArray(ptr, count, typestr), device=dev)
 
 
-def cc_knn_weights(n, p, X, mask, k, phi, normalize=False):
+def cc_knn_weights(n, p, X, mask, k, phi, normalize=False, Y=None, period=None, alpha=1.0):
     """Returns (rowptr int64, col int32, w fp32) as torch device tensors (copies; the library's
-    arrays are released with cc_free_graph before returning)."""
+    arrays are released with cc_free_graph before returning).  With Y (n,q device tensor): the composite
+    distance of eq. 9 (cc_knn_weights_composite), period = q floats or None."""
     rp, cl, ww = _vp(), _vp(), _vp()
     nnz = _i64(0)
-    _check(_lib.cc_knn_weights(n, p, _ptr(X), _ptr(mask), k, phi, 1 if normalize else 0, ctypes.byref(rp),
-                               ctypes.byref(cl), ctypes.byref(ww), ctypes.byref(nnz), _stream()))
+    if Y is None:
+        _check(_lib.cc_knn_weights(n, p, _ptr(X), _ptr(mask), k, phi, 1 if normalize else 0, ctypes.byref(rp),
+                                   ctypes.byref(cl), ctypes.byref(ww), ctypes.byref(nnz), _stream()))
+    else:
+        q = Y.shape[1]
+        per = None if period is None else (ctypes.c_float * q)(*[float(x) for x in period])
+        _check(_lib.cc_knn_weights_composite(n, p, _ptr(X), _ptr(mask), q, _ptr(Y), per, alpha, k, phi,
+                                             1 if normalize else 0, ctypes.byref(rp), ctypes.byref(cl), ctypes.byref(ww),
+                                             ctypes.byref(nnz), _stream()))
     dev = X.device
     rowptr = _wrap(rp.value, n + 1, "<i8", dev).clone()
     col = _wrap(cl.value, nnz.value, "<i4", dev).clone()

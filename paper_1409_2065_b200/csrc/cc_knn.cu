@@ -4,6 +4,10 @@
 // distance runs over co-observed coordinates and is scaled by p / #co-observed; S8 normalisation over
 // pairs i<j is optional.
 //
+// f4 (eq. 9): with side coordinates Y (q <= 4 columns, e.g. GPS) the distance is the composite
+//     d_ij = alpha ||x_i - x_j|| + (1 - alpha) ||y_i - y_j||,   y-differences wrapped modulo a per-coordinate period (S27),
+// and eq. 8 is applied to this d (kernels instantiated with SIDE = true).
+//
 // Three steps, all on the device, no sort library and no floating-point atomics:
 //   1. k_knn_tile: brute-force distances in 64 x 64 register tiles (direct differences, fp32), a sorted
 //      k-list per query in shared memory, filtered insertion (a candidate is looked at only if it beats
@@ -11,6 +15,7 @@
 //   2. symmetrise by OR: count reverse-only entries (integer atomics), scan, fill, sort each row by column.
 //   3. weights from recomputed distances (so w_ij == w_ji bitwise), optional normalisation.
 #include <cfloat>
+#include <cmath>
 #include <cstdio>
 
 #include "cc_device.cuh"
@@ -18,11 +23,28 @@
 
 namespace {
 
-constexpr int TQ = 64, TC = 64, PC = 16, KMAX = 64;
+constexpr int TQ = 64, TC = 64, PC = 16, KMAX = 64, QSIDE = 4;
 
-template <bool MASKED>
+struct side_t {
+    const float* Y;   // n x q row-major, or NULL
+    int q;
+    float period[QSIDE];   // 0: plain difference
+    float alpha;
+};
+
+__device__ __forceinline__ float side_d2(const side_t& sd, int i, int j) {
+    float s = 0.f;
+    for (int c = 0; c < sd.q; ++c) {
+        float df = sd.Y[(size_t)i * sd.q + c] - sd.Y[(size_t)j * sd.q + c];
+        if (sd.period[c] > 0.f) df -= sd.period[c] * rintf(df / sd.period[c]);
+        s = fmaf(df, df, s);
+    }
+    return s;
+}
+
+template <bool MASKED, bool SIDE>
 __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int k, const float* __restrict__ X,
-                                                   const uint8_t* __restrict__ mask, int* __restrict__ nbr) {
+                                                   const uint8_t* __restrict__ mask, const side_t sd, int* __restrict__ nbr) {
     extern __shared__ float smem[];
     float* Xq = smem;                        // TQ x (PC+1)
     float* Xc = Xq + TQ * (PC + 1);          // TC x (PC+1)
@@ -88,6 +110,10 @@ __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int k, const flo
             for (int b = 0; b < 4; ++b) {
                 float d = acc[a][b];
                 if (MASKED) d = cnt[a][b] > 0.f ? d * (float)p / cnt[a][b] : FLT_MAX;
+                if (SIDE) {
+                    const int gi = q0 + ty * 4 + a, gj = c0 + tx + 16 * b;
+                    if (gi < n && gj < n && d < FLT_MAX) d = sd.alpha * sqrtf(d) + (1.f - sd.alpha) * sqrtf(side_d2(sd, gi, gj));
+                }
                 Dt[(ty * 4 + a) * (TC + 1) + tx + 16 * b] = d;
             }
         __syncthreads();
@@ -204,9 +230,9 @@ __global__ void k_fill_rows(int n, int k, const int* __restrict__ nbr, const int
 
 // sort each row by column (the set is unique, so the result does not depend on the fill order) and
 // compute the weight of every entry from the ordered pair (min, max) so that w_ij == w_ji bitwise.
-template <bool MASKED>
+template <bool MASKED, bool SIDE>
 __global__ void k_rows_finish(int n, int p, float phi, const float* __restrict__ X, const uint8_t* __restrict__ mask,
-                              const int64_t* __restrict__ rowptr, int* __restrict__ col, float* __restrict__ w) {
+                              const side_t sd, const int64_t* __restrict__ rowptr, int* __restrict__ col, float* __restrict__ w) {
     const int lane = threadIdx.x & 31;
     const long long nw = (long long)gridDim.x * (blockDim.x >> 5);
     for (long long i = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); i < n; i += nw) {
@@ -237,6 +263,10 @@ __global__ void k_rows_finish(int n, int p, float phi, const float* __restrict__
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); c += __shfl_xor_sync(0xffffffffu, c, o); }
             if (MASKED) s = c > 0.f ? s * (float)p / c : FLT_MAX;
+            if (SIDE && s < FLT_MAX) {   // eq. 9, then eq. 8 on d^2
+                const float d = sd.alpha * sqrtf(s) + (1.f - sd.alpha) * sqrtf(side_d2(sd, lo, hi));
+                s = d * d;
+            }
             if (lane == 0) w[e] = expf(-phi * s);
         }
     }
@@ -274,10 +304,8 @@ __global__ void k_wscale(long long nnz, float* __restrict__ w, const double* __r
         }                                                                                    \
     } while (0)
 
-extern "C" {
-
-int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t k, float phi, int32_t normalize,
-                   int64_t** rowptr_out, int32_t** col_out, float** w_out, int64_t* nnz_out, void* stream) {
+static int knn_impl(int64_t n, int64_t p, const float* X, const uint8_t* mask, const side_t sd, int32_t k, float phi,
+                    int32_t normalize, int64_t** rowptr_out, int32_t** col_out, float** w_out, int64_t* nnz_out, void* stream) {
     if (!X || !rowptr_out || !col_out || !w_out || !nnz_out || n < 2 || p < 1 || k < 1 || k > n - 1 || k > KMAX ||
         n > 1000000000LL || !(phi >= 0.f)) {
         snprintf(g_knn_err, sizeof(g_knn_err), "cc_knn_weights: need n >= 2, p >= 1, 1 <= k <= min(n-1, %d), phi >= 0", KMAX);
@@ -301,12 +329,18 @@ int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, in
     KCUDA(cudaMemsetAsync(extra, 0, (size_t)n * sizeof(int), st));
     KCUDA(cudaMemsetAsync(cursor, 0, (size_t)n * sizeof(int), st));
     KCUDA(cudaMemsetAsync(red, 0, (size_t)(2 + CC_MAXBLK) * sizeof(double), st));
-    if (mask) {
-        KCUDA(cudaFuncSetAttribute(k_knn_tile<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_knn_tile<true><<<(unsigned)((n + TQ - 1) / TQ), 256, smem, st>>>((int)n, (int)p, k, X, mask, nbr);
-    } else {
-        KCUDA(cudaFuncSetAttribute(k_knn_tile<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        k_knn_tile<false><<<(unsigned)((n + TQ - 1) / TQ), 256, smem, st>>>((int)n, (int)p, k, X, mask, nbr);
+    {
+        const unsigned g = (unsigned)((n + TQ - 1) / TQ);
+#define KNN_TILE(M, S)                                                                                               \
+    do {                                                                                                             \
+        KCUDA(cudaFuncSetAttribute(k_knn_tile<M, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));       \
+        k_knn_tile<M, S><<<g, 256, smem, st>>>((int)n, (int)p, k, X, mask, sd, nbr);                                 \
+    } while (0)
+        if (mask && sd.Y) KNN_TILE(true, true);
+        else if (mask) KNN_TILE(true, false);
+        else if (sd.Y) KNN_TILE(false, true);
+        else KNN_TILE(false, false);
+#undef KNN_TILE
     }
     k_sort_lists<<<(unsigned)((n + 255) / 256), 256, 0, st>>>((int)n, k, nbr);
     k_count_reverse<<<(unsigned)((nk + 255) / 256), 256, 0, st>>>((int)n, k, nbr, extra);
@@ -318,8 +352,10 @@ int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, in
     k_fill_rows<<<(unsigned)((nk + 255) / 256), 256, 0, st>>>((int)n, k, nbr, rowptr, cursor, col);
     {
         const unsigned g = (unsigned)((n + 7) / 8 < 148 * 16 ? (n + 7) / 8 : 148 * 16);
-        if (mask) k_rows_finish<true><<<g, 256, 0, st>>>((int)n, (int)p, phi, X, mask, rowptr, col, w);
-        else k_rows_finish<false><<<g, 256, 0, st>>>((int)n, (int)p, phi, X, mask, rowptr, col, w);
+        if (mask && sd.Y) k_rows_finish<true, true><<<g, 256, 0, st>>>((int)n, (int)p, phi, X, mask, sd, rowptr, col, w);
+        else if (mask) k_rows_finish<true, false><<<g, 256, 0, st>>>((int)n, (int)p, phi, X, mask, sd, rowptr, col, w);
+        else if (sd.Y) k_rows_finish<false, true><<<g, 256, 0, st>>>((int)n, (int)p, phi, X, mask, sd, rowptr, col, w);
+        else k_rows_finish<false, false><<<g, 256, 0, st>>>((int)n, (int)p, phi, X, mask, sd, rowptr, col, w);
     }
     if (normalize) {
         k_wsum<<<1024, CC_THREADS, 0, st>>>((int)n, rowptr, col, w, red + 2, reinterpret_cast<unsigned int*>(red + 1), red);
@@ -335,6 +371,35 @@ done:
     if (col) cudaFree(col);
     if (w) cudaFree(w);
     return rc;
+}
+
+extern "C" {
+
+int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t k, float phi, int32_t normalize,
+                   int64_t** rowptr_out, int32_t** col_out, float** w_out, int64_t* nnz_out, void* stream) {
+    side_t sd = {};
+    return knn_impl(n, p, X, mask, sd, k, phi, normalize, rowptr_out, col_out, w_out, nnz_out, stream);
+}
+
+int cc_knn_weights_composite(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t q, const float* Y,
+                             const float* period, float alpha, int32_t k, float phi, int32_t normalize,
+                             int64_t** rowptr_out, int32_t** col_out, float** w_out, int64_t* nnz_out, void* stream) {
+    if (!Y || q < 1 || q > QSIDE || !(alpha >= 0.f && alpha <= 1.f)) {
+        snprintf(g_knn_err, sizeof(g_knn_err), "cc_knn_weights_composite: need Y, 1 <= q <= %d, 0 <= alpha <= 1", QSIDE);
+        return CC_EINVAL;
+    }
+    side_t sd = {};
+    sd.Y = Y;
+    sd.q = q;
+    sd.alpha = alpha;
+    for (int c = 0; c < q; ++c) {
+        sd.period[c] = period ? period[c] : 0.f;
+        if (!(sd.period[c] >= 0.f) || std::isinf(sd.period[c])) {
+            snprintf(g_knn_err, sizeof(g_knn_err), "cc_knn_weights_composite: period[%d] must be finite and >= 0", c);
+            return CC_EINVAL;
+        }
+    }
+    return knn_impl(n, p, X, mask, sd, k, phi, normalize, rowptr_out, col_out, w_out, nnz_out, stream);
 }
 
 void cc_free_graph(int64_t* rowptr, int32_t* col, float* w) {

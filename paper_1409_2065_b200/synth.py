@@ -137,6 +137,21 @@ def make_popres(seed=0, n=3000, p=10, k=40, phi=0.0):
     return Workload("popres", _f32(X), None, "knn", k, "fixed", float(phi), 30, seed)
 
 
+
+def side_coordinates(n: int, seed: int = 0, scale: float = 1.0):
+    """Seeded GPS-like side coordinates for eq. 9: (longitude, latitude) in degrees times
+    `scale`, 8 loose regional groups of which two straddle the +-180 meridian so that the modulo rule matters.
+    Stand-in for the HGDP / POPRES sampling locations, which are not available.  Returns fp32 (n, 2)."""
+    rng = np.random.default_rng(seed + 4242)
+    lon_c = np.array([-178.0, 176.0, -120.0, -60.0, 0.0, 35.0, 90.0, 140.0])
+    lat_c = rng.uniform(-50.0, 60.0, size=8)
+    g = rng.integers(0, 8, size=n)
+    lon = lon_c[g] + 6.0 * rng.normal(size=n)
+    lon = (lon + 180.0) % 360.0 - 180.0
+    lat = np.clip(lat_c[g] + 5.0 * rng.normal(size=n), -89.0, 89.0)
+    return _f32(np.stack([lon, lat], axis=1) * scale)
+
+
 _MAKERS = {
     "tiny": make_tiny,
     "expression": make_expression,

@@ -207,3 +207,50 @@ def test_full_size_large_sparse_properties(B):
     l = lab.cpu().numpy()
     assert l[0] == 0 and l.max() == k - 1 and np.array_equal(np.unique(l), np.arange(k))
     B.cc_destroy(h)
+
+
+@pytest.mark.parametrize("name,kw,k,phi,alpha,scale,norm", [
+    ("genotype", dict(n=52, p=4682), 4, 1e-3, 0.5, 1.0, False),      # HGDP-like (L166-L178): k = 4, alpha = 0.5
+    ("popres", dict(n=1500), 40, 0.0, 0.5, 0.01, True),              # POPRES-like (L182-L186), uniform weights
+    ("expression", dict(n=70, p=333), 5, 1e-3, 0.3, 0.2, False),     # masked x-distance (S11) inside eq. 9
+    ("large_sparse", dict(n=3000), 10, 1e-3, 0.8, 0.05, False),
+])
+def test_composite_distance_weights_match_oracle(B, oracle, name, kw, k, phi, alpha, scale, norm):
+    """f4: eq. 9 with modulo longitude differences (S27), then eq. 8 on the composite distance."""
+    import torch
+    wl = synth.make(name, **kw)
+    Y = synth.side_coordinates(wl.n, 1, scale)
+    period = [360.0 * scale, 0.0]
+    ei, ej, w, _ = oracle.composite_knn_graph(wl.X.astype(np.float64), wl.mask, Y.astype(np.float64), period, alpha, k, phi,
+                                              normalize=norm)
+    rp, cl, ww = oracle.to_csr(wl.n, ei, ej, w)
+    rowptr, col, wg = B.cc_knn_weights(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), k, phi, normalize=norm,
+                                       Y=_dev(torch, Y), period=period, alpha=alpha)
+    assert np.array_equal(rowptr.cpu().numpy(), rp)
+    assert np.array_equal(col.cpu().numpy(), cl)
+    assert np.abs(wg.cpu().numpy() - ww).max() <= 2e-5 * ww.max()
+    # the wrap matters on this recipe: without it the graph is a different one
+    ei2, ej2, _, _ = oracle.composite_knn_graph(wl.X.astype(np.float64), wl.mask, Y.astype(np.float64), None, alpha, k, phi)
+    assert len(ei2) != len(ei) or not (np.array_equal(ei2, ei) and np.array_equal(ej2, ej))
+    h = B.cc_create(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), rowptr, col, wg, None)
+    assert B.cc_get_counts(h)["n_pairs"] == len(ei)
+    B.cc_destroy(h)
+
+
+def test_composite_distance_limits_and_errors(B, oracle):
+    import torch
+    wl = synth.make("large_sparse", n=2000)
+    X = _dev(torch, wl.X)
+    Y = _dev(torch, synth.side_coordinates(wl.n, 2))
+    r0, c0, w0 = B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01)
+    r1, c1, w1 = B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01, Y=Y, period=[360.0, 0.0], alpha=1.0)   # eq. 9 -> eq. 8
+    assert torch.equal(r0, r1) and torch.equal(c0, c1) and float((w0 - w1).abs().max()) <= 1e-5 * float(w0.max())
+    for bad in (dict(alpha=1.5), dict(alpha=-0.1), dict(period=[-1.0, 0.0])):
+        args = dict(Y=Y, period=[360.0, 0.0], alpha=0.5)
+        args.update(bad)
+        with pytest.raises(B.CCError) as e:
+            B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01, **args)
+        assert e.value.code == B.CC_EINVAL
+    with pytest.raises(B.CCError) as e:
+        B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01, Y=torch.zeros(wl.n, 5, device="cuda:0"), alpha=0.5)
+    assert e.value.code == B.CC_EINVAL

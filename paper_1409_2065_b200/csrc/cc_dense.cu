@@ -1246,7 +1246,10 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
 }
 
 // ---- kd_edges: block soft-threshold over the n x n matrices ------------------
-__global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
+// (measured on B200, n = 8192: 4 columns per thread at 4 blocks/SM 345 us, 8 at 3 blocks/SM 383 us, 16 at 3 404 us;
+// streaming-store hints made no difference)
+constexpr int CPT = 4;   // columns per thread and loop step in the streaming case
+__global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, double* part,
                                                 int init_only, uint8_t* __restrict__ Spre, float* __restrict__ rs_out, int nkb32) {
     if (!init_only && !sc->mm_active) return;
@@ -1267,18 +1270,18 @@ __global__ void __launch_bounds__(256) kd_edges(int n, int ksplit, const float* 
             const int i = ig * 8 + r8;
             float rsum = 0.f;
             if (i < n) {
-                for (int j0 = cq * 8; j0 < n; j0 += 256) {      // 8 columns per thread: a warp covers 128-byte row segments
-                    // all four loads of the thread's 8 columns are issued before any arithmetic
-                    float4 qv[2], wq[2];
+                for (int j0 = cq * CPT; j0 < n; j0 += 32 * CPT) {      // CPT columns per thread: a warp covers 4 x 4*CPT-byte row segments of 8 rows
+                    // all loads of the thread's columns are issued before any arithmetic
+                    float4 qv[CPT / 4], wq[CPT / 4];
 #pragma unroll
-                    for (int hq = 0; hq < 2; ++hq) {
+                    for (int hq = 0; hq < CPT / 4; ++hq) {
                         const int j = j0 + hq * 4;
                         const size_t e = (size_t)i * n + (j < n ? j : 0);
                         qv[hq] = __ldcs(reinterpret_cast<const float4*>(NB2 + e));      // streamed once: evict-first
                         wq[hq] = __ldg(reinterpret_cast<const float4*>(W + e));
                     }
 #pragma unroll
-                    for (int hq = 0; hq < 2; ++hq) {
+                    for (int hq = 0; hq < CPT / 4; ++hq) {
                         const int j = j0 + hq * 4;
                         if (j >= n) break;
                         const size_t e = (size_t)i * n + j;

@@ -146,17 +146,35 @@ def side_dist(Y, period, i: int) -> np.ndarray:
     return np.sqrt((df * df).sum(axis=1))
 
 
-def composite_knn_graph(X, mask, Y, period, alpha: float, k: int, phi: float, normalize: bool = False):
+def geodesic_dist(LL, radius: float, i: int) -> np.ndarray:
+    """"An even better alternative replaces ||y_i - y_j|| by the geodesic distance between i and j"
+    [reading S28]: y = (longitude, latitude) in degrees, the geodesic is the great circle on a sphere of the given
+    radius, d_ij = radius * theta_ij with the central angle from the haversine formula
+        hav(theta) = sin^2(dlat/2) + cos(lat_i) cos(lat_j) sin^2(dlon/2),   theta = 2 atan2(sqrt(hav), sqrt(1 - hav)).
+    Returns d_ij for all j."""
+    LL = _f64(LL)
+    lon, lat = np.deg2rad(LL[:, 0]), np.deg2rad(LL[:, 1])
+    sl = np.sin((lat - lat[i]) / 2.0)
+    so = np.sin((lon - lon[i]) / 2.0)
+    hav = sl * sl + np.cos(lat[i]) * np.cos(lat) * so * so
+    hav = np.clip(hav, 0.0, 1.0)
+    return radius * 2.0 * np.arctan2(np.sqrt(hav), np.sqrt(1.0 - hav))
+
+
+def composite_knn_graph(X, mask, Y, period, alpha: float, k: int, phi: float, normalize: bool = False,
+                        geodesic_radius=None):
     """Eq. 9: d_ij = alpha ||x_i - x_j|| + (1 - alpha) ||y_i - y_j||, then eq. 8 with this d:
     i~j iff j is among the k nearest of i by d OR vice versa (S9: self excluded, ties -> smaller index),
     w_ij = exp(-phi d_ij^2), optional normalisation (S8).  ||x_i - x_j|| is the square root of row_dist2 (masked
-    rule S11).  Returns (ei, ej, w, d) with ei<ej sorted by (ei, ej)."""
+    rule S11).  With geodesic_radius, ||y_i - y_j|| is replaced by geodesic_dist (L137, S28; `period` is unused).
+    Returns (ei, ej, w, d) with ei<ej sorted by (ei, ej)."""
     n = X.shape[0]
     pairs = {}
     for i in range(n):
         dx = np.sqrt(row_dist2(X, mask, i))
         dx[i] = 0.0                      # row_dist2 marks the row itself with inf; it is excluded below
-        d = alpha * dx + (1.0 - alpha) * side_dist(Y, period, i)
+        dy = side_dist(Y, period, i) if geodesic_radius is None else geodesic_dist(Y, geodesic_radius, i)
+        d = alpha * dx + (1.0 - alpha) * dy
         d[i] = np.inf
         order = np.lexsort((np.arange(n), d))[:k]
         for j in order:

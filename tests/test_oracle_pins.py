@@ -501,3 +501,58 @@ def test_P16_composite_distance_limits_and_wrap(oracle):
     assert np.allclose(w, np.exp(-0.01 * dd ** 2), rtol=1e-12)
     wn = oracle.composite_knn_graph(X, None, Y, [360.0, 0.0], al, 3, 0.01, normalize=True)[2]
     assert np.isclose(wn.sum(), 1.0) and np.allclose(wn * w.sum(), w)
+
+
+# ----------------------------------------------------------------------------- f4: geodesic alternative of eq. 9 (L137, S28)
+def test_P17_geodesic_distance(oracle):
+    R = 6371.0
+    # closed forms on the sphere: pole to equator is a quarter circle, antipodes half a circle, along a meridian
+    # R |dlat|, along the equator R |dlon| taken the short way round (179 E to 179 W is 2 degrees, not 358)
+    LL = np.array([[0.0, 0.0], [0.0, 90.0], [180.0, 0.0], [37.0, -90.0], [0.0, 33.0], [179.0, 0.0], [-179.0, 0.0],
+                   [90.0, 0.0]])
+    d0 = oracle.geodesic_dist(LL, R, 0)
+    assert np.allclose(d0, R * np.array([0.0, np.pi / 2, np.pi, np.pi / 2, np.deg2rad(33.0), np.deg2rad(179.0),
+                                         np.deg2rad(179.0), np.pi / 2]), rtol=1e-12)
+    assert np.isclose(oracle.geodesic_dist(LL, R, 5)[6], R * np.deg2rad(2.0), rtol=1e-9)
+    assert np.isclose(oracle.geodesic_dist(LL, R, 1)[3], R * np.pi, rtol=1e-12)        # pole to pole, any longitudes
+    # a different definition of the same angle: unit vectors in 3-D, theta = atan2(|a x b|, a.b)
+    rng = np.random.default_rng(5)
+    n = 60
+    LLr = np.stack([rng.uniform(-180, 180, n), rng.uniform(-90, 90, n)], axis=1)
+    lon, lat = np.deg2rad(LLr[:, 0]), np.deg2rad(LLr[:, 1])
+    V = np.stack([np.cos(lat) * np.cos(lon), np.cos(lat) * np.sin(lon), np.sin(lat)], axis=1)
+    D = np.zeros((n, n))
+    for i in range(n):
+        D[i] = oracle.geodesic_dist(LLr, 1.0, i)
+        for j in range(n):
+            th = np.arctan2(np.linalg.norm(np.cross(V[i], V[j])), float(V[i] @ V[j]))
+            assert abs(D[i, j] - th) <= 1e-12, (i, j)
+    # a metric: symmetric, zero diagonal, triangle inequality
+    assert np.allclose(D, D.T, atol=1e-14) and np.all(np.diag(D) == 0.0)
+    for i in range(0, n, 7):
+        for j in range(n):
+            assert np.all(D[i, j] <= D[i, :] + D[:, j] + 1e-12)
+    # small separations: the sphere is flat, d ~ R sqrt(dlat^2 + (cos(lat) dlon)^2)
+    base = np.array([[12.0, 48.0]])
+    near = base + 1e-3 * rng.standard_normal((20, 2))
+    LLs = np.concatenate([base, near])
+    ds = oracle.geodesic_dist(LLs, R, 0)[1:]
+    flat = R * np.hypot(np.deg2rad(near[:, 1] - 48.0), np.cos(np.deg2rad(48.0)) * np.deg2rad(near[:, 0] - 12.0))
+    assert np.allclose(ds, flat, rtol=1e-4)
+    # inside eq. 9: alpha = 0 gives the k-NN graph of the geodesic distances alone (brute force), alpha = 1 is eq. 8
+    X = rng.standard_normal((n, 4))
+    e8 = oracle.knn_graph(X, None, 3, 0.2)
+    e9 = oracle.composite_knn_graph(X, None, LLr, None, 1.0, 3, 0.2, geodesic_radius=R)
+    assert np.array_equal(e8[0], e9[0]) and np.array_equal(e8[1], e9[1]) and np.allclose(e8[2], e9[2], rtol=1e-12)
+    Dn = D.copy()
+    np.fill_diagonal(Dn, np.inf)
+    near3 = [set(np.argsort(Dn[i], kind="stable")[:3].tolist()) for i in range(n)]
+    want = sorted({(min(i, j), max(i, j)) for i in range(n) for j in near3[i]})
+    ei, ej, w, dd = oracle.composite_knn_graph(X, None, LLr, None, 0.0, 3, 0.5, geodesic_radius=1.0)
+    assert list(zip(ei.tolist(), ej.tolist())) == want
+    assert np.allclose(dd, [D[a, b] for a, b in want], rtol=1e-12) and np.allclose(w, np.exp(-0.5 * dd ** 2), rtol=1e-12)
+    # mixed: entry by entry
+    al = 0.6
+    ei, ej, w, dd = oracle.composite_knn_graph(X, None, LLr, None, al, 3, 0.5, geodesic_radius=2.0)
+    for a, b, dv in zip(ei.tolist(), ej.tolist(), dd.tolist()):
+        assert np.isclose(dv, al * np.linalg.norm(X[a] - X[b]) + (1 - al) * 2.0 * D[a, b], rtol=1e-12)

@@ -93,11 +93,21 @@ int cc_knn_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, in
  * gives each coordinate's period (360 for a longitude in degrees), 0 = plain difference; a periodic difference
  * is wrapped to [-period/2, period/2] (S27).  ||x_i - x_j|| is the square root of the (masked, S11) squared
  * distance of cc_knn_weights.  Neighbours are the k smallest d_ij, w_ij = exp(-phi d_ij^2); everything else
- * (OR rule, ties, normalisation, outputs, ownership, errors) as cc_knn_weights.  The geodesic alternative L137
- * mentions is not built. */
+ * (OR rule, ties, normalisation, outputs, ownership, errors) as cc_knn_weights. */
 int cc_knn_weights_composite(int64_t n, int64_t p, const float* X, const uint8_t* mask, int32_t q, const float* Y,
                              const float* period, float alpha, int32_t k, float phi, int32_t normalize,
                              int64_t** rowptr, int32_t** col, float** w, int64_t* nnz, void* stream);
+
+/* ---- f4: eq. 9 with the geodesic alternative, PAPER.md L137 ("an even better alternative replaces ||y_i - y_j||
+ * by the geodesic distance between i and j"; reading S28 in DESIGN.md) ------------------------------------
+ *   d_ij = alpha ||x_i - x_j|| + (1 - alpha) radius * theta_ij,
+ * theta_ij the great-circle angle between the two positions (haversine formula).  lonlat: DEVICE, n*2 fp32
+ * row-major, (longitude, latitude) in degrees (any longitude branch: the formula wraps by itself).  radius
+ * (> 0, finite) sets the unit of the geodesic term: 6371 for km, 57.29578 for degrees of arc.  Everything else
+ * as cc_knn_weights_composite.  CC_EINVAL: lonlat NULL, radius <= 0 or not finite, alpha outside [0, 1]. */
+int cc_knn_weights_geodesic(int64_t n, int64_t p, const float* X, const uint8_t* mask, const float* lonlat, float radius,
+                            float alpha, int32_t k, float phi, int32_t normalize,
+                            int64_t** rowptr, int32_t** col, float** w, int64_t* nnz, void* stream);
 
 /* a0 for complete graphs (k = n-1): W_out (DEVICE, caller-owned, n*n fp32 row-major) receives
  * w_ij = exp(-phi ||x_i - x_j||^2) for i != j and 0 on the diagonal, symmetric bit for bit; same distance

@@ -22,7 +22,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
-SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_knn_weights_composite", "cc_dense_weights", "cc_graph_components",
+SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_knn_weights_composite", "cc_knn_weights_geodesic", "cc_dense_weights", "cc_graph_components",
            "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_solve_continuation", "cc_path", "cc_path_continuation",
            "cc_get_U", "cc_get_projection", "cc_principal_components", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
@@ -43,6 +43,8 @@ _lib.cc_knn_weights.argtypes = [_i64, _i64, _vp, _vp, _i32, ctypes.c_float, _i32
                                 _P(_i64), _vp]
 _lib.cc_knn_weights_composite.argtypes = [_i64, _i64, _vp, _vp, _i32, _vp, _P(ctypes.c_float), ctypes.c_float, _i32,
                                           ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp), _P(_i64), _vp]
+_lib.cc_knn_weights_geodesic.argtypes = [_i64, _i64, _vp, _vp, _vp, ctypes.c_float, ctypes.c_float, _i32,
+                                         ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp), _P(_i64), _vp]
 _lib.cc_dense_weights.argtypes = [_i64, _i64, _vp, _vp, ctypes.c_float, _i32, _vp, _vp]
 _lib.cc_graph_components.argtypes = [_i64, _vp, _vp, _vp, _P(_i32), _vp]
 _lib.cc_smallest_connected_k.argtypes = [_i64, _i64, _vp, _vp, _i32, _P(_i32), _vp]
@@ -254,15 +256,22 @@ def _wrap(ptr, count, typestr, dev):
     return torch.as_tensor(_DevArray(ptr, count, typestr), device=dev)
 
 
-def cc_knn_weights(n, p, X, mask, k, phi, normalize=False, Y=None, period=None, alpha=1.0):
+def cc_knn_weights(n, p, X, mask, k, phi, normalize=False, Y=None, period=None, alpha=1.0, geodesic_radius=None):
     """Returns (rowptr int64, col int32, w fp32) as torch device tensors (copies; the library's
     arrays are released with cc_free_graph before returning).  With Y (n,q device tensor): the composite
-    distance of eq. 9 (cc_knn_weights_composite), period = q floats or None."""
+    distance of eq. 9 (cc_knn_weights_composite), period = q floats or None; with geodesic_radius, Y is
+    (longitude, latitude) in degrees and the side distance is the great circle (cc_knn_weights_geodesic)."""
     rp, cl, ww = _vp(), _vp(), _vp()
     nnz = _i64(0)
     if Y is None:
         _check(_lib.cc_knn_weights(n, p, _ptr(X), _ptr(mask), k, phi, 1 if normalize else 0, ctypes.byref(rp),
                                    ctypes.byref(cl), ctypes.byref(ww), ctypes.byref(nnz), _stream()))
+    elif geodesic_radius is not None:
+        if Y.dim() != 2 or Y.shape[1] != 2:
+            raise CCError(CC_EINVAL, "cc_knn_weights: geodesic side coordinates must be (n, 2) = (longitude, latitude)")
+        _check(_lib.cc_knn_weights_geodesic(n, p, _ptr(X), _ptr(mask), _ptr(Y), float(geodesic_radius), alpha, k, phi,
+                                            1 if normalize else 0, ctypes.byref(rp), ctypes.byref(cl), ctypes.byref(ww),
+                                            ctypes.byref(nnz), _stream()))
     else:
         q = Y.shape[1]
         per = None if period is None else (ctypes.c_float * q)(*[float(x) for x in period])

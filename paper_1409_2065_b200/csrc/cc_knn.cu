@@ -6,6 +6,7 @@
 //
 // f4 (eq. 9): with side coordinates Y (q <= 4 columns, e.g. GPS) the distance is the composite
 //     d_ij = alpha ||x_i - x_j|| + (1 - alpha) ||y_i - y_j||,   y-differences wrapped modulo a per-coordinate period (S27),
+//     or ||y_i - y_j|| replaced by the great-circle distance of (longitude, latitude) pairs (L137's alternative, S28),
 // and eq. 8 is applied to this d (kernels instantiated with SIDE = true).
 //
 // Three steps, all on the device, no sort library and no floating-point atomics:
@@ -30,16 +31,27 @@ struct side_t {
     int q;
     float period[QSIDE];   // 0: plain difference
     float alpha;
+    float radius;          // > 0: Y = (longitude, latitude) in degrees, side distance = great circle on this sphere (S28)
 };
 
-__device__ __forceinline__ float side_d2(const side_t& sd, int i, int j) {
+// ||y_i - y_j|| with modulo differences (L137, S27), or the geodesic alternative of L137 (S28): the great-circle
+// distance radius * theta, hav(theta) = sin^2(dlat/2) + cos(lat_i) cos(lat_j) sin^2(dlon/2), theta =
+// 2 atan2(sqrt(hav), sqrt(1 - hav)).  The half differences are formed in degrees first (exact for nearby points).
+__device__ __forceinline__ float side_dist(const side_t& sd, int i, int j) {
+    if (sd.radius > 0.f) {
+        constexpr float RAD = 0.017453292519943295f;
+        const float2 yi = *reinterpret_cast<const float2*>(sd.Y + (size_t)i * 2), yj = *reinterpret_cast<const float2*>(sd.Y + (size_t)j * 2);
+        const float so = sinf(0.5f * RAD * (yi.x - yj.x)), sl = sinf(0.5f * RAD * (yi.y - yj.y));
+        const float hav = fminf(fmaf(cosf(RAD * yi.y) * cosf(RAD * yj.y), so * so, sl * sl), 1.f);
+        return sd.radius * 2.f * atan2f(sqrtf(hav), sqrtf(1.f - hav));
+    }
     float s = 0.f;
     for (int c = 0; c < sd.q; ++c) {
         float df = sd.Y[(size_t)i * sd.q + c] - sd.Y[(size_t)j * sd.q + c];
         if (sd.period[c] > 0.f) df -= sd.period[c] * rintf(df / sd.period[c]);
         s = fmaf(df, df, s);
     }
-    return s;
+    return sqrtf(s);
 }
 
 template <bool MASKED, bool SIDE>
@@ -112,7 +124,7 @@ __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int k, const flo
                 if (MASKED) d = cnt[a][b] > 0.f ? d * (float)p / cnt[a][b] : FLT_MAX;
                 if (SIDE) {
                     const int gi = q0 + ty * 4 + a, gj = c0 + tx + 16 * b;
-                    if (gi < n && gj < n && d < FLT_MAX) d = sd.alpha * sqrtf(d) + (1.f - sd.alpha) * sqrtf(side_d2(sd, gi, gj));
+                    if (gi < n && gj < n && d < FLT_MAX) d = sd.alpha * sqrtf(d) + (1.f - sd.alpha) * side_dist(sd, gi, gj);
                 }
                 Dt[(ty * 4 + a) * (TC + 1) + tx + 16 * b] = d;
             }
@@ -264,7 +276,7 @@ __global__ void k_rows_finish(int n, int p, float phi, const float* __restrict__
             for (int o = 16; o > 0; o >>= 1) { s += __shfl_xor_sync(0xffffffffu, s, o); c += __shfl_xor_sync(0xffffffffu, c, o); }
             if (MASKED) s = c > 0.f ? s * (float)p / c : FLT_MAX;
             if (SIDE && s < FLT_MAX) {   // eq. 9, then eq. 8 on d^2
-                const float d = sd.alpha * sqrtf(s) + (1.f - sd.alpha) * sqrtf(side_d2(sd, lo, hi));
+                const float d = sd.alpha * sqrtf(s) + (1.f - sd.alpha) * side_dist(sd, lo, hi);
                 s = d * d;
             }
             if (lane == 0) w[e] = expf(-phi * s);
@@ -399,6 +411,21 @@ int cc_knn_weights_composite(int64_t n, int64_t p, const float* X, const uint8_t
             return CC_EINVAL;
         }
     }
+    return knn_impl(n, p, X, mask, sd, k, phi, normalize, rowptr_out, col_out, w_out, nnz_out, stream);
+}
+
+int cc_knn_weights_geodesic(int64_t n, int64_t p, const float* X, const uint8_t* mask, const float* lonlat, float radius,
+                            float alpha, int32_t k, float phi, int32_t normalize, int64_t** rowptr_out, int32_t** col_out,
+                            float** w_out, int64_t* nnz_out, void* stream) {
+    if (!lonlat || !(radius > 0.f) || std::isinf(radius) || !(alpha >= 0.f && alpha <= 1.f)) {
+        snprintf(g_knn_err, sizeof(g_knn_err), "cc_knn_weights_geodesic: need lonlat, finite radius > 0, 0 <= alpha <= 1");
+        return CC_EINVAL;
+    }
+    side_t sd = {};
+    sd.Y = lonlat;
+    sd.q = 2;
+    sd.alpha = alpha;
+    sd.radius = radius;
     return knn_impl(n, p, X, mask, sd, k, phi, normalize, rowptr_out, col_out, w_out, nnz_out, stream);
 }
 

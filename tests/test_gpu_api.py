@@ -237,6 +237,60 @@ def test_composite_distance_weights_match_oracle(B, oracle, name, kw, k, phi, al
     B.cc_destroy(h)
 
 
+@pytest.mark.parametrize("name,kw,k,phi,alpha,radius,norm", [
+    ("genotype", dict(n=52, p=4682), 4, 1e-3, 0.5, 57.29578, False),   # HGDP-like, geodesic in degrees of arc
+    ("popres", dict(n=1500), 40, 0.0, 0.5, 0.5, True),                 # POPRES-like, uniform weights
+    ("expression", dict(n=70, p=333), 5, 1e-7, 0.3, 6371.0, False),    # masked x-distance, geodesic in km
+    ("large_sparse", dict(n=3000), 10, 1e-3, 0.8, 3.0, False),
+])
+def test_geodesic_distance_weights_match_oracle(B, oracle, name, kw, k, phi, alpha, radius, norm):
+    """f4: eq. 9 with the geodesic alternative of L137 (S28), then eq. 8 on the composite distance."""
+    import torch
+    wl = synth.make(name, **kw)
+    Y = synth.side_coordinates(wl.n, 3, 1.0)             # (longitude, latitude) in degrees, groups across +-180
+    ei, ej, w, dd = oracle.composite_knn_graph(wl.X.astype(np.float64), wl.mask, Y.astype(np.float64), None, alpha, k, phi,
+                                               normalize=norm, geodesic_radius=radius)
+    rp, cl, ww = oracle.to_csr(wl.n, ei, ej, w)
+    rowptr, col, wg = B.cc_knn_weights(wl.n, wl.p, _dev(torch, wl.X), _dev(torch, wl.mask), k, phi, normalize=norm,
+                                       Y=_dev(torch, Y), alpha=alpha, geodesic_radius=radius)
+    assert np.array_equal(rowptr.cpu().numpy(), rp)
+    assert np.array_equal(col.cpu().numpy(), cl)
+    assert np.abs(wg.cpu().numpy() - ww).max() <= 2e-5 * ww.max()
+    # it is not the wrapped Euclidean distance in degrees: that graph differs (cos(lat) shrinks the longitude term)
+    ei2, ej2, _, _ = oracle.composite_knn_graph(wl.X.astype(np.float64), wl.mask, Y.astype(np.float64), [360.0, 0.0], alpha, k, phi)
+    if radius == 57.29578:
+        assert len(ei2) != len(ei) or not (np.array_equal(ei2, ei) and np.array_equal(ej2, ej))
+
+
+def test_geodesic_distance_limits_and_errors(B, oracle):
+    import torch
+    wl = synth.make("large_sparse", n=2000)
+    X = _dev(torch, wl.X)
+    Y = _dev(torch, synth.side_coordinates(wl.n, 2))
+    r0, c0, w0 = B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01)
+    r1, c1, w1 = B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01, Y=Y, alpha=1.0, geodesic_radius=6371.0)   # eq. 9 -> eq. 8
+    assert torch.equal(r0, r1) and torch.equal(c0, c1) and float((w0 - w1).abs().max()) <= 1e-5 * float(w0.max())
+    # alpha = 0 with positions on the equator / a meridian: distances are R |dlon| (short way round) and R |dlat|
+    ll = np.array([[179.0, 0.0], [-179.0, 0.0], [-170.0, 0.0], [120.0, 0.0], [0.0, 80.0], [0.0, 70.0], [0.0, -10.0]], dtype=np.float32)
+    Xs = np.zeros((7, 3), dtype=np.float32)
+    rp, cl, ww = B.cc_knn_weights(7, 3, _dev(torch, Xs), None, 1, 1.0, Y=_dev(torch, ll), alpha=0.0, geodesic_radius=1.0)
+    ei, ej, w, dd = oracle.composite_knn_graph(Xs.astype(np.float64), None, ll.astype(np.float64), None, 0.0, 1, 1.0,
+                                               geodesic_radius=1.0)
+    rpo, clo, wwo = oracle.to_csr(7, ei, ej, w)
+    assert np.array_equal(rp.cpu().numpy(), rpo) and np.array_equal(cl.cpu().numpy(), clo)
+    assert (0, 1) in set(zip(ei.tolist(), ej.tolist()))                       # 179 E and 179 W are neighbours
+    assert np.abs(ww.cpu().numpy() - wwo).max() <= 1e-6
+    for bad in (dict(alpha=1.5), dict(geodesic_radius=0.0), dict(geodesic_radius=-1.0), dict(geodesic_radius=float("inf"))):
+        args = dict(Y=Y, alpha=0.5, geodesic_radius=1.0)
+        args.update(bad)
+        with pytest.raises(B.CCError) as e:
+            B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01, **args)
+        assert e.value.code == B.CC_EINVAL
+    with pytest.raises(B.CCError) as e:
+        B.cc_knn_weights(wl.n, wl.p, X, None, 8, 0.01, Y=torch.zeros(wl.n, 3, device="cuda:0"), alpha=0.5, geodesic_radius=1.0)
+    assert e.value.code == B.CC_EINVAL
+
+
 def test_composite_distance_limits_and_errors(B, oracle):
     import torch
     wl = synth.make("large_sparse", n=2000)

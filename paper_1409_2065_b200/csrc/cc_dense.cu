@@ -1080,26 +1080,34 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
 }
 
 // ---- kd_small: the whole pair/projection work of one iteration for n <= 64 (genotype shape) ---------------
-// All n rows of a chunk of 32 columns fit in shared memory together with S (n x n), so U and A' are read
+// All n rows of a chunk of 64 columns fit in shared memory together with S (n x n), so U and A' are read
 // once, A is written once, and projection, ||U-A||^2, loss, ||b||^2 and ||s b' - b||^2 are all formed from
 // shared memory.  A CTA walks chunks grid-stride and keeps its pair accumulators in registers; it writes
 // one slice of partial ||b||^2 per (CTA, column phase) at the end (kd_edges adds the slices in order).
-// Pairs are covered by 4 x 4 register tiles, only the tiles on or above the diagonal, SM_CS threads per tile
-// taking interleaved columns.
-constexpr int SM_N = 64, SM_C = 32;
+// Everything moves as float4 along the columns: one LDS.128 feeds 4 columns, so the projection runs at 2
+// shared loads per 32 arithmetic instructions (a thread = 4 rows x 4 columns, S broadcast as a float4 of
+// S^T) and the pairs at 16 loads per 256 (4 x 4 register tiles of pairs, only the tiles on or above the
+// diagonal, SM_CS threads per tile taking interleaved column quads).  The first version read scalars (one
+// load per 4-5 instructions) and was bound by shared-memory issue: 330 us per iteration at 52 x 200,000.
+constexpr int SM_N = 64, SM_C = 64, SM_RS = SM_C + 4;   // row stride 68 floats: 8 rows x 16 bytes hit 32 distinct banks
+constexpr int SMALL_SMEM = (SM_N * (SM_N + 4) + 3 * SM_N * SM_RS + SM_C) * (int)sizeof(float);
 
-__global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, const float* __restrict__ S,
-                                                const float* __restrict__ Ap, const float* __restrict__ U,
-                                                const float* __restrict__ X, const uint8_t* __restrict__ mask,
-                                                const float* __restrict__ W, const float* __restrict__ VN,
-                                                float* __restrict__ A, float* __restrict__ NB2, cc_scal* sc, double* part,
-                                                double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer,
-                                                int init_only) {
+__global__ void __launch_bounds__(256, 2) kd_small(int n, int ld, int cs_per_tile, const float* __restrict__ S,
+                                                   const float* __restrict__ Ap, const float* __restrict__ U,
+                                                   const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                   const float* __restrict__ W, const float* __restrict__ VN,
+                                                   float* __restrict__ A, float* __restrict__ NB2, cc_scal* sc, double* part,
+                                                   double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer,
+                                                   int init_only) {
     if (!init_only && !sc->mm_active) return;
-    __shared__ __align__(16) float SsT[SM_N][SM_N + 4];   // S transposed: 8 consecutive rows i of column j as two float4
-    __shared__ float Us[SM_N][SM_C + 1], Ps[SM_N][SM_C + 1], As[SM_N][SM_C + 1];
-    __shared__ float ubar_s[SM_C];
+    extern __shared__ __align__(16) float sm_small[];
+    float (*SsT)[SM_N + 4] = reinterpret_cast<float (*)[SM_N + 4]>(sm_small);   // S transposed: rows i of column j contiguous
+    float (*Us)[SM_RS] = reinterpret_cast<float (*)[SM_RS]>(sm_small + SM_N * (SM_N + 4));
+    float (*Ps)[SM_RS] = Us + SM_N;
+    float (*As)[SM_RS] = Ps + SM_N;
+    float* ubar_s = reinterpret_cast<float*>(As + SM_N);
     __shared__ unsigned char t_ty[136], t_tx[136];
+    __shared__ float csum_s[4][SM_C];
     __shared__ int ntiles_s;
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -1127,54 +1135,75 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
     double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
     const float inv = 1.f / (float)(n + 1), fn = (float)n;
     const int nchunks = (ld + SM_C - 1) / SM_C;
+    const int pq = tid & 15, prg = tid >> 4;       // projection: column quad, group of 4 rows
     for (int chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
         const int c0 = chunk * SM_C;
-        for (int t = tid; t < SM_N * SM_C; t += 256) {
-            const int r = t / SM_C, c = t % SM_C;
-            const bool ok = r < n && c0 + c < ld;
-            const float u = ok ? U[(size_t)r * ld + c0 + c] : 0.f;
-            Us[r][c] = u;
-            Ps[r][c] = init_only ? u : (ok ? Ap[(size_t)r * ld + c0 + c] : 0.f);
-            if (init_only) As[r][c] = u;
+        {
+            // all 8 loads of a thread are issued before the first store (SM_N * SM_C / 4 = 4 * 256 quads)
+            float4 uu[4], pp[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int t = tid + k * 256;
+                const int r = t / (SM_C / 4), c = (t % (SM_C / 4)) * 4;
+                const bool ok = r < n && c0 + c < ld;      // ld is a multiple of 4: a quad is inside or outside as a whole
+                uu[k] = ok ? ld4s(U + (size_t)r * ld + c0 + c) : f4(0.f);
+                pp[k] = (ok && !init_only) ? ld4s(Ap + (size_t)r * ld + c0 + c) : uu[k];
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int t = tid + k * 256;
+                const int r = t / (SM_C / 4), c = (t % (SM_C / 4)) * 4;
+                st4(&Us[r][c], uu[k]);
+                st4(&Ps[r][c], pp[k]);
+                if (init_only) st4(&As[r][c], uu[k]);
+            }
         }
         __syncthreads();
         if (!init_only) {
-            if (tid < SM_C) {
+            // column means of U: 4 threads per column take interleaved rows, then one adds the 4 partial sums
+            {
                 float s = 0.f;
-                for (int r = 0; r < n; ++r) s += Us[r][tid];
-                ubar_s[tid] = s / fn;
+                for (int r = tid >> 6; r < n; r += 4) s += Us[r][tid & 63];
+                csum_s[tid >> 6][tid & 63] = s;
             }
             __syncthreads();
-            const int c = tid & 31;
+            if (tid < SM_C) ubar_s[tid] = ((csum_s[0][tid] + csum_s[1][tid]) + (csum_s[2][tid] + csum_s[3][tid])) / fn;
+            __syncthreads();
             float dua = 0.f, los = 0.f;
-            // warp w owns rows 8w .. 8w+7 of column c: per j one load of a'_j and two broadcast float4 of S
-            const int i0r = (tid >> 5) * 8;
+            const int i0r = prg * 4;
             if (i0r < n) {
-                float pi[8], g[8];
+                float4 pi[4], g[4];
 #pragma unroll
-                for (int k = 0; k < 8; ++k) { pi[k] = Ps[i0r + k][c]; g[k] = 0.f; }
+                for (int k = 0; k < 4; ++k) { pi[k] = ld4s(&Ps[i0r + k][pq * 4]); g[k] = f4(0.f); }
+#pragma unroll 4
                 for (int j = 0; j < n; ++j) {
-                    const float pj = Ps[j][c];
-                    const float4 s0 = *reinterpret_cast<const float4*>(&SsT[j][i0r]);
-                    const float4 s1 = *reinterpret_cast<const float4*>(&SsT[j][i0r + 4]);
-                    g[0] = fmaf(s0.x, pi[0] - pj, g[0]); g[1] = fmaf(s0.y, pi[1] - pj, g[1]);
-                    g[2] = fmaf(s0.z, pi[2] - pj, g[2]); g[3] = fmaf(s0.w, pi[3] - pj, g[3]);
-                    g[4] = fmaf(s1.x, pi[4] - pj, g[4]); g[5] = fmaf(s1.y, pi[5] - pj, g[5]);
-                    g[6] = fmaf(s1.z, pi[6] - pj, g[6]); g[7] = fmaf(s1.w, pi[7] - pj, g[7]);
+                    const float4 pj = ld4s(&Ps[j][pq * 4]);
+                    const float4 s4 = ld4s(&SsT[j][i0r]);
+                    g[0] = fma4(s4.x, pi[0] - pj, g[0]);
+                    g[1] = fma4(s4.y, pi[1] - pj, g[1]);
+                    g[2] = fma4(s4.z, pi[2] - pj, g[2]);
+                    g[3] = fma4(s4.w, pi[3] - pj, g[3]);
                 }
+                const float4 ub = ld4s(&ubar_s[pq * 4]);
+                const bool inside = c0 + pq * 4 < ld;
 #pragma unroll
-                for (int k = 0; k < 8; ++k) {
+                for (int k = 0; k < 4; ++k) {
                     const int i = i0r + k;
                     if (i < n) {
-                        const float u = Us[i][c];
-                        const float dl = inv * (g[k] - fn * (u - ubar_s[c]));
-                        const float a = u + dl;
-                        As[i][c] = a;
-                        if (c0 + c < ld) {
-                            const size_t o = (size_t)i * ld + c0 + c;
-                            dua = fmaf(dl, dl, dua);
-                            const float q = X[o] - u;
-                            if (!mask || mask[o]) los = fmaf(q, q, los);
+                        const float4 u = ld4s(&Us[i][pq * 4]);
+                        float4 dl;
+                        dl.x = inv * (g[k].x - fn * (u.x - ub.x)); dl.y = inv * (g[k].y - fn * (u.y - ub.y));
+                        dl.z = inv * (g[k].z - fn * (u.z - ub.z)); dl.w = inv * (g[k].w - fn * (u.w - ub.w));
+                        st4(&As[i][pq * 4], u + dl);
+                        if (inside) {
+                            const size_t o = (size_t)i * ld + c0 + pq * 4;
+                            dua += dot4(dl, dl);
+                            float4 q = ld4s(X + o) - u;
+                            if (mask) {
+                                const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + o);
+                                q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
+                            }
+                            los += dot4(q, q);
                         }
                     }
                 }
@@ -1183,36 +1212,40 @@ __global__ void __launch_bounds__(256) kd_small(int n, int ld, int cs_per_tile, 
             red[1] += (double)los;
             __syncthreads();
             // 1'(A - U) = 0 holds exactly for the projection; remove the fp32 residual of this chunk's columns
-            if (tid < SM_C) {
+            {
                 float sd = 0.f;
-                for (int r = 0; r < n; ++r) sd += As[r][tid] - Us[r][tid];
-                ubar_s[tid] = sd / fn;
+                for (int r = tid >> 6; r < n; r += 4) sd += As[r][tid & 63] - Us[r][tid & 63];
+                csum_s[tid >> 6][tid & 63] = sd;
             }
             __syncthreads();
-            for (int t = tid; t < n * SM_C; t += 256) {
-                const int r = t / SM_C, cc2 = t % SM_C;
-                const float a2 = As[r][cc2] - ubar_s[cc2];
-                As[r][cc2] = a2;
-                if (c0 + cc2 < ld) A[(size_t)r * ld + c0 + cc2] = a2;
+            if (tid < SM_C) ubar_s[tid] = ((csum_s[0][tid] + csum_s[1][tid]) + (csum_s[2][tid] + csum_s[3][tid])) / fn;
+            __syncthreads();
+            for (int t = tid; t < n * (SM_C / 4); t += 256) {
+                const int r = t / (SM_C / 4), cc2 = (t % (SM_C / 4)) * 4;
+                const float4 a2 = ld4s(&As[r][cc2]) - ld4s(&ubar_s[cc2]);
+                st4(&As[r][cc2], a2);
+                if (c0 + cc2 < ld) st4(A + (size_t)r * ld + c0 + cc2, a2);
             }
             __syncthreads();
         }
         if (pair_thread) {
-            for (int c = cph; c < SM_C; c += cs_per_tile) {
-                float ai[4], aj[4], pi[4], pj[4];
+            for (int cq = cph; cq < SM_C / 4; cq += cs_per_tile) {
+                float4 ai[4], aj[4], pi[4], pj[4];
 #pragma unroll
                 for (int a = 0; a < 4; ++a) {
-                    ai[a] = As[ty * 4 + a][c]; pi[a] = Ps[ty * 4 + a][c];
-                    aj[a] = As[tx * 4 + a][c]; pj[a] = Ps[tx * 4 + a][c];
+                    ai[a] = ld4s(&As[ty * 4 + a][cq * 4]); pi[a] = ld4s(&Ps[ty * 4 + a][cq * 4]);
+                    aj[a] = ld4s(&As[tx * 4 + a][cq * 4]); pj[a] = ld4s(&Ps[tx * 4 + a][cq * 4]);
                 }
 #pragma unroll
                 for (int a = 0; a < 4; ++a)
 #pragma unroll
                     for (int b = 0; b < 4; ++b) {
-                        const float bb = ai[a] - aj[b];
-                        const float tt = fmaf(sv[a][b], pi[a] - pj[b], -bb);
-                        nb[a][b] = fmaf(bb, bb, nb[a][b]);
-                        dv[a][b] = fmaf(tt, tt, dv[a][b]);
+                        const float4 bb = ai[a] - aj[b];
+                        const float4 dp = pi[a] - pj[b];
+                        const float4 tt = make_float4(fmaf(sv[a][b], dp.x, -bb.x), fmaf(sv[a][b], dp.y, -bb.y),
+                                                      fmaf(sv[a][b], dp.z, -bb.z), fmaf(sv[a][b], dp.w, -bb.w));
+                        nb[a][b] = fmaf(bb.w, bb.w, fmaf(bb.z, bb.z, fmaf(bb.y, bb.y, fmaf(bb.x, bb.x, nb[a][b]))));
+                        dv[a][b] = fmaf(tt.w, tt.w, fmaf(tt.z, tt.z, fmaf(tt.y, tt.y, fmaf(tt.x, tt.x, dv[a][b]))));
                     }
             }
         }
@@ -1548,7 +1581,7 @@ void ccd_pairs(cc_handle* h) {
 }
 
 static void launch_small(cc_handle* h, int init_only) {
-    kd_small<<<h->dn_small_grid, 256, 0, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X, h->mask,
+    kd_small<<<h->dn_small_grid, 256, SMALL_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X, h->mask,
                                                       h->Wd, h->VNd, h->A, h->NB2d, h->sc, h->part + 3 * CC_MAXBLK * CC_NPART,
                                                       h->hist_phi, h->hist_d, init_only ? 0 : h->cond_outer, init_only);
 }
@@ -1595,6 +1628,11 @@ int ccd_setup(cc_handle* h, const float* W) {
         if (cs < 1) cs = 1;
         long long g = (h->ld + SM_C - 1) / SM_C;
         if (g > 2LL * h->sms) g = 2LL * h->sms;
+        if (cudaFuncSetAttribute(kd_small, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_SMEM) != cudaSuccess) {
+            cudaGetLastError();
+            snprintf(h->err, sizeof(h->err), "dense mode: cannot reserve %d bytes of shared memory for kd_small", SMALL_SMEM);
+            return CC_ECUDA;
+        }
         h->dn_small_cs = cs;
         h->dn_small_grid = (int)g;
         h->dn_ksplit = (int)g * cs;

@@ -1086,11 +1086,19 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
 // one slice of partial ||b||^2 per (CTA, column phase) at the end (kd_edges adds the slices in order).
 // Everything moves as float4 along the columns: one LDS.128 feeds 4 columns, so the projection runs at 2
 // shared loads per 32 arithmetic instructions (a thread = 4 rows x 4 columns, S broadcast as a float4 of
-// S^T) and the pairs at 16 loads per 256 (4 x 4 register tiles of pairs, only the tiles on or above the
-// diagonal, SM_CS threads per tile taking interleaved column quads).  The first version read scalars (one
-// load per 4-5 instructions) and was bound by shared-memory issue: 330 us per iteration at 52 x 200,000.
-constexpr int SM_N = 64, SM_C = 64, SM_RS = SM_C + 4;   // row stride 68 floats: 8 rows x 16 bytes hit 32 distinct banks
-constexpr int SMALL_SMEM = (SM_N * (SM_N + 4) + 3 * SM_N * SM_RS + SM_C) * (int)sizeof(float);
+// S^T) and the pairs at 16 loads per 320 (4 x 4 register tiles of pairs, only the tiles on or above the
+// diagonal, cs_per_tile threads per tile taking interleaved column quads).  Four barriers per chunk: load |
+// projection | exact-column-sum fix and store of A | pairs; the two column sums (mean of U, residual of
+// 1'(A-U)) are partial sums left in shared memory by the previous phase and added up by every thread that
+// needs them, in a fixed order.  History at 52 x 200,000: scalar shared loads, 8 barriers 330 us; float4 217 us.
+constexpr int SM_N = 64, SM_C = 64, SM_Q = SM_C / 4;
+constexpr int SMALL_SMEM = (SM_N * (SM_N + 4) + 3 * SM_N * SM_C + 2 * 16 * SM_C) * (int)sizeof(float);
+
+// Column quad q of row r sits at float offset small_sw(r, q) of the row (row stride 64 floats): the quad index is
+// XORed with twice the row's 4-row tile index, so that the pair phase -- a quarter warp reads rows 4tx+a of four
+// consecutive tiles tx at two column quads -- hits 8 distinct 16-byte bank groups (a plain padded stride cannot:
+// rows 8 apart always collide), while a row's 16 quads stay a permutation of themselves.
+__device__ __forceinline__ int small_sw(int r, int q) { return (q ^ (((r >> 2) << 1) & 15)) << 2; }
 
 __global__ void __launch_bounds__(256, 2) kd_small(int n, int ld, int cs_per_tile, const float* __restrict__ S,
                                                    const float* __restrict__ Ap, const float* __restrict__ U,
@@ -1102,12 +1110,12 @@ __global__ void __launch_bounds__(256, 2) kd_small(int n, int ld, int cs_per_til
     if (!init_only && !sc->mm_active) return;
     extern __shared__ __align__(16) float sm_small[];
     float (*SsT)[SM_N + 4] = reinterpret_cast<float (*)[SM_N + 4]>(sm_small);   // S transposed: rows i of column j contiguous
-    float (*Us)[SM_RS] = reinterpret_cast<float (*)[SM_RS]>(sm_small + SM_N * (SM_N + 4));
-    float (*Ps)[SM_RS] = Us + SM_N;
-    float (*As)[SM_RS] = Ps + SM_N;
-    float* ubar_s = reinterpret_cast<float*>(As + SM_N);
+    float (*Us)[SM_C] = reinterpret_cast<float (*)[SM_C]>(sm_small + SM_N * (SM_N + 4));
+    float (*Ps)[SM_C] = Us + SM_N;
+    float (*As)[SM_C] = Ps + SM_N;
+    float (*csum)[SM_C] = As + SM_N;       // 16 partial column sums of U (one per row slot of the loading threads)
+    float (*dsum)[SM_C] = csum + 16;       // 16 partial column sums of A - U (one per 4-row group of the projection)
     __shared__ unsigned char t_ty[136], t_tx[136];
-    __shared__ float csum_s[4][SM_C];
     __shared__ int ntiles_s;
     const int tid = threadIdx.x;
     if (tid == 0) {
@@ -1135,66 +1143,69 @@ __global__ void __launch_bounds__(256, 2) kd_small(int n, int ld, int cs_per_til
     double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
     const float inv = 1.f / (float)(n + 1), fn = (float)n;
     const int nchunks = (ld + SM_C - 1) / SM_C;
-    const int pq = tid & 15, prg = tid >> 4;       // projection: column quad, group of 4 rows
+    const int n4 = (n + 3) & ~3;
+    const int pq = tid & 15, prg = tid >> 4;       // column quad; row slot of the loads = group of 4 rows of the projection
     for (int chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
         const int c0 = chunk * SM_C;
+        const bool inside = c0 + pq * 4 < ld;      // ld is a multiple of 4: a quad is inside or outside as a whole
         {
-            // all 8 loads of a thread are issued before the first store (SM_N * SM_C / 4 = 4 * 256 quads)
+            // rows prg, prg+16, prg+32, prg+48 of quad pq: all 8 loads are issued before the first store; rows >= n and
+            // quads outside the matrix are zero
             float4 uu[4], pp[4];
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const int t = tid + k * 256;
-                const int r = t / (SM_C / 4), c = (t % (SM_C / 4)) * 4;
-                const bool ok = r < n && c0 + c < ld;      // ld is a multiple of 4: a quad is inside or outside as a whole
-                uu[k] = ok ? ld4s(U + (size_t)r * ld + c0 + c) : f4(0.f);
-                pp[k] = (ok && !init_only) ? ld4s(Ap + (size_t)r * ld + c0 + c) : uu[k];
+                const int r = prg + 16 * k;
+                const bool ok = r < n && inside;
+                uu[k] = ok ? ld4s(U + (size_t)r * ld + c0 + pq * 4) : f4(0.f);
+                pp[k] = (ok && !init_only) ? ld4s(Ap + (size_t)r * ld + c0 + pq * 4) : uu[k];
             }
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const int t = tid + k * 256;
-                const int r = t / (SM_C / 4), c = (t % (SM_C / 4)) * 4;
-                st4(&Us[r][c], uu[k]);
-                st4(&Ps[r][c], pp[k]);
-                if (init_only) st4(&As[r][c], uu[k]);
+                const int r = prg + 16 * k, o = small_sw(r, pq);
+                st4(&Us[r][o], uu[k]);
+                st4(&Ps[r][o], pp[k]);
+                if (init_only) st4(&As[r][o], uu[k]);
             }
+            st4(&csum[prg][pq * 4], (uu[0] + uu[1]) + (uu[2] + uu[3]));
         }
         __syncthreads();
         if (!init_only) {
-            // column means of U: 4 threads per column take interleaved rows, then one adds the 4 partial sums
-            {
-                float s = 0.f;
-                for (int r = tid >> 6; r < n; r += 4) s += Us[r][tid & 63];
-                csum_s[tid >> 6][tid & 63] = s;
-            }
-            __syncthreads();
-            if (tid < SM_C) ubar_s[tid] = ((csum_s[0][tid] + csum_s[1][tid]) + (csum_s[2][tid] + csum_s[3][tid])) / fn;
-            __syncthreads();
             float dua = 0.f, los = 0.f;
             const int i0r = prg * 4;
+            float4 dsl = f4(0.f);
             if (i0r < n) {
+                // column means of U from the 16 partial sums, in a fixed order
+                float4 ub = ld4s(&csum[0][pq * 4]);
+#pragma unroll
+                for (int k = 1; k < 16; ++k) ub = ub + ld4s(&csum[k][pq * 4]);
+                ub = make_float4(ub.x / fn, ub.y / fn, ub.z / fn, ub.w / fn);
                 float4 pi[4], g[4];
 #pragma unroll
-                for (int k = 0; k < 4; ++k) { pi[k] = ld4s(&Ps[i0r + k][pq * 4]); g[k] = f4(0.f); }
-#pragma unroll 4
-                for (int j = 0; j < n; ++j) {
-                    const float4 pj = ld4s(&Ps[j][pq * 4]);
-                    const float4 s4 = ld4s(&SsT[j][i0r]);
-                    g[0] = fma4(s4.x, pi[0] - pj, g[0]);
-                    g[1] = fma4(s4.y, pi[1] - pj, g[1]);
-                    g[2] = fma4(s4.z, pi[2] - pj, g[2]);
-                    g[3] = fma4(s4.w, pi[3] - pj, g[3]);
+                for (int k = 0; k < 4; ++k) { pi[k] = ld4s(&Ps[i0r + k][small_sw(i0r, pq)]); g[k] = f4(0.f); }
+                // rows j >= n of P and of S^T are zero, so the padded tail of the last 4-row tile adds exact zeros
+                for (int j4 = 0; j4 < n4; j4 += 4) {
+                    const int o = small_sw(j4, pq);
+#pragma unroll
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const float4 pj = ld4s(&Ps[j4 + jj][o]);
+                        const float4 s4 = ld4s(&SsT[j4 + jj][i0r]);
+                        g[0] = fma4(s4.x, pi[0] - pj, g[0]);
+                        g[1] = fma4(s4.y, pi[1] - pj, g[1]);
+                        g[2] = fma4(s4.z, pi[2] - pj, g[2]);
+                        g[3] = fma4(s4.w, pi[3] - pj, g[3]);
+                    }
                 }
-                const float4 ub = ld4s(&ubar_s[pq * 4]);
-                const bool inside = c0 + pq * 4 < ld;
 #pragma unroll
                 for (int k = 0; k < 4; ++k) {
                     const int i = i0r + k;
                     if (i < n) {
-                        const float4 u = ld4s(&Us[i][pq * 4]);
+                        const float4 u = ld4s(&Us[i][small_sw(i0r, pq)]);
                         float4 dl;
                         dl.x = inv * (g[k].x - fn * (u.x - ub.x)); dl.y = inv * (g[k].y - fn * (u.y - ub.y));
                         dl.z = inv * (g[k].z - fn * (u.z - ub.z)); dl.w = inv * (g[k].w - fn * (u.w - ub.w));
-                        st4(&As[i][pq * 4], u + dl);
+                        const float4 a = u + dl;
+                        st4(&As[i][small_sw(i0r, pq)], a);
+                        dsl = dsl + (a - u);               // the stored difference, not dl: this is what must sum to zero
                         if (inside) {
                             const size_t o = (size_t)i * ld + c0 + pq * 4;
                             dua += dot4(dl, dl);
@@ -1208,33 +1219,36 @@ __global__ void __launch_bounds__(256, 2) kd_small(int n, int ld, int cs_per_til
                     }
                 }
             }
+            st4(&dsum[prg][pq * 4], dsl);
             red[0] += (double)dua;
             red[1] += (double)los;
             __syncthreads();
             // 1'(A - U) = 0 holds exactly for the projection; remove the fp32 residual of this chunk's columns
-            {
-                float sd = 0.f;
-                for (int r = tid >> 6; r < n; r += 4) sd += As[r][tid & 63] - Us[r][tid & 63];
-                csum_s[tid >> 6][tid & 63] = sd;
-            }
-            __syncthreads();
-            if (tid < SM_C) ubar_s[tid] = ((csum_s[0][tid] + csum_s[1][tid]) + (csum_s[2][tid] + csum_s[3][tid])) / fn;
-            __syncthreads();
-            for (int t = tid; t < n * (SM_C / 4); t += 256) {
-                const int r = t / (SM_C / 4), cc2 = (t % (SM_C / 4)) * 4;
-                const float4 a2 = ld4s(&As[r][cc2]) - ld4s(&ubar_s[cc2]);
-                st4(&As[r][cc2], a2);
-                if (c0 + cc2 < ld) st4(A + (size_t)r * ld + c0 + cc2, a2);
+            if (i0r < n) {
+                float4 db = ld4s(&dsum[0][pq * 4]);
+#pragma unroll
+                for (int k = 1; k < 16; ++k) db = db + ld4s(&dsum[k][pq * 4]);
+                db = make_float4(db.x / fn, db.y / fn, db.z / fn, db.w / fn);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const int i = i0r + k;
+                    float* as = &As[i][small_sw(i0r, pq)];
+                    const float4 a2 = i < n ? ld4s(as) - db : f4(0.f);     // rows n .. 4 ceil(n/4) - 1 feed the last pair tiles: zero
+                    st4(as, a2);
+                    if (i < n && inside) st4(A + (size_t)i * ld + c0 + pq * 4, a2);
+                }
             }
             __syncthreads();
         }
         if (pair_thread) {
-            for (int cq = cph; cq < SM_C / 4; cq += cs_per_tile) {
+            const int gy = (ty << 1) & 15, gx = (tx << 1) & 15;
+            for (int cq = cph; cq < SM_Q; cq += cs_per_tile) {
+                const int oy = (cq ^ gy) << 2, ox = (cq ^ gx) << 2;
                 float4 ai[4], aj[4], pi[4], pj[4];
 #pragma unroll
                 for (int a = 0; a < 4; ++a) {
-                    ai[a] = ld4s(&As[ty * 4 + a][cq * 4]); pi[a] = ld4s(&Ps[ty * 4 + a][cq * 4]);
-                    aj[a] = ld4s(&As[tx * 4 + a][cq * 4]); pj[a] = ld4s(&Ps[tx * 4 + a][cq * 4]);
+                    ai[a] = ld4s(&As[ty * 4 + a][oy]); pi[a] = ld4s(&Ps[ty * 4 + a][oy]);
+                    aj[a] = ld4s(&As[tx * 4 + a][ox]); pj[a] = ld4s(&Ps[tx * 4 + a][ox]);
                 }
 #pragma unroll
                 for (int a = 0; a < 4; ++a)

@@ -73,6 +73,7 @@ struct cc_handle {
     int32_t* rowptr;                  // n+1 (nnz < 2^31 enforced)
     int32_t* rowup;                   // n: first entry of row i with col > i (rows are sorted)
     int32_t* order;                   // n: rows by decreasing degree (processing order of the gather kernels)
+    int4* rowdesc;                    // n: (row, rowup, row end, row begin) in that order: one independent 16-byte load per walked row
     int32_t* col;                     // nnz
     int32_t* peer;                    // nnz: index of the reverse entry
     float* w;                         // nnz

@@ -115,6 +115,18 @@ __global__ void __launch_bounds__(1024) k_degree_order(int n, const int* __restr
     }
 }
 
+// The walk order as a table of row descriptors: (row, first entry with col > row, row end, row begin).  A kernel that
+// walks the rows in `order` would need three dependent loads (order -> rowptr/rowup -> col) before its first gather;
+// with the table the first two are one 16-byte load that depends on nothing and can be issued an iteration ahead.
+__global__ void k_row_desc(int n, const int* __restrict__ order, const int* __restrict__ rowptr, const int* __restrict__ rowup,
+                           int4* __restrict__ desc) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) {
+        const int i = order[t];
+        desc[t] = make_int4(i, rowup[i], rowptr[i + 1], rowptr[i]);
+    }
+}
+
 // X (n x p) -> padded n x ld copy; mask likewise (padding = observed zeros); NaN/Inf check on observed.
 __global__ void k_pad_copy(long long n, int p, int ld, const float* __restrict__ X, const uint8_t* __restrict__ mask,
                            float* __restrict__ Xo, uint8_t* __restrict__ Mo, int* flag) {
@@ -345,6 +357,8 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
     }
     CC_TRY(dmalloc(h, &h->order, (size_t)n));
     k_degree_order<<<1, 1024, 0, st>>>((int)n, h->rowptr, h->order);
+    CC_TRY(dmalloc(h, &h->rowdesc, (size_t)n));
+    k_row_desc<<<(int)((n + 255) / 256), 256, 0, st>>>((int)n, h->order, h->rowptr, h->rowup, h->rowdesc);
     // ---- data ----
     const size_t nl = (size_t)n * h->ld;
     CC_TRY(dmalloc(h, &h->X, nl));
@@ -437,7 +451,7 @@ int ccu_min_margin(cc_handle* h, double* margin_out) {
 void ccu_free(cc_handle* h) {
     void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Dl, h->Uc, h->mask, h->colmean, h->rowptr,
                     h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Minv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->dbar, h->colps, h->pre_pairs, h->nrm_part, h->pre_S, h->pre_B, h->rs_S, h->sc, h->part,
-                    h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order};
+                    h->hist_phi, h->hist_d, h->dout, h->dflag, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order, h->rowdesc};
     for (void* q : ptrs)
         cc_dev_free(q, h->stream);
     if (h->sc_host) cudaFreeHost(h->sc_host);

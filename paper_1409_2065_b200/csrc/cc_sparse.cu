@@ -325,8 +325,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_apply_inv(int n, int ld, const f
 // coefficients of the two updates.  `outer` = the MM WHILE node's handle in graph mode, else 0.
 // ---------------------------------------------------------------------------------------------
 template <int G>
-__global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, long long nnz, const int* __restrict__ order,
-                                                      const int* __restrict__ rowptr, const int* __restrict__ rowup,
+__global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, long long nnz, const int4* __restrict__ rowdesc,
                                                       const int* __restrict__ col, const int* __restrict__ peer,
                                                       const float* __restrict__ w, const float* __restrict__ s,
                                                       const float* __restrict__ vn, const float* __restrict__ A,
@@ -341,13 +340,25 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
     const long long items = (long long)n * nchunk;
     double acc_g[3] = {0.0, 0.0, 0.0};  // dist^2, loss, penalty
-    for (long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G; it < items; it += ngroups) {
-        const int i = __ldg(order + (int)(it / nchunk));
+    // the descriptor of the next row is loaded while this one is processed (k_row_desc): the chain per row is
+    // col/s + own row -> gathers instead of order -> extent -> col/s -> gathers (ncu: the kernel runs 16 warps per SM
+    // and 58 % of its stall samples were long-scoreboard waits spread evenly over those four levels)
+    long long it = (long long)blockIdx.x * (CC_THREADS / G) + threadIdx.x / G;
+    int4 dnext = it < items ? __ldg(rowdesc + (int)(it / nchunk)) : make_int4(0, 0, 0, 0);
+    for (; it < items; it += ngroups) {
+        const int4 dsc = dnext;
+        if (it + ngroups < items) dnext = __ldg(rowdesc + (int)((it + ngroups) / nchunk));
+        const int i = dsc.x;
         const int chunk = (int)(it % nchunk);
         const int c0 = chunk * 4 * G + gl * 4;
         const bool valid = c0 < ld;
         const float vf = valid ? 1.f : 0.f;
         const size_t oi = (size_t)i * ld + (valid ? c0 : 0);
+        // the first batch of column ids and shrink factors goes out together with the own-row loads, ahead of the
+        // node arithmetic that waits for those
+        const int rs = dsc.y, re = dsc.z;
+        const int cj0 = rs + gl < re ? __ldg(col + rs + gl) : i;
+        const float sv0 = rs + gl < re ? __ldg(s + rs + gl) : 0.f;
         const float4 ai = ld4s(A + oi), api = ld4s(Ap + oi), ui = ld4s(U + oi), xi = ld4s(X + oi);
         float dist_l = 0.f, pen_l = 0.f;
         {
@@ -360,11 +371,10 @@ __global__ void __launch_bounds__(CC_THREADS) k_norm(int n, int ld, int nchunk, 
             dist_l = vf * dot4(t, t);
             acc_g[1] += (double)(vf * dot4(q, q));
         }
-        const int rs = rowup[i], re = rowptr[i + 1];
         for (int base = rs; base < re; base += G) {
             const int e = base + gl;
-            const int cj = e < re ? __ldg(col + e) : i;
-            const float sv = e < re ? __ldg(s + e) : 0.f;
+            const int cj = base == rs ? cj0 : (e < re ? __ldg(col + e) : i);
+            const float sv = base == rs ? sv0 : (e < re ? __ldg(s + e) : 0.f);
             const int cnt = min(G, re - base);
             for (int t = 0; t < cnt; t += UNR) {
                 int j[UNR];
@@ -597,7 +607,7 @@ void ccs_cg_update(cc_handle* h) {
 }
 
 void ccs_norm(cc_handle* h) {
-    CC_DISPATCH_G(h, k_norm, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->order, h->rowptr, h->rowup,
+    CC_DISPATCH_G(h, k_norm, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->rowdesc,
                   h->col, h->peer, h->w, h->s, h->vn, h->A, h->Ap, h->U, h->X, h->mask, h->nb2, h->sc,
                   h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, g_outer(h));
 }

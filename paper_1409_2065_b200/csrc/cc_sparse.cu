@@ -34,7 +34,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
                                                      float* __restrict__ Uc, float* __restrict__ A,
                                                      cc_scal* sc, double* part, cudaGraphConditionalHandle loop) {
     if (!sc->mm_active) return;
-    constexpr int UNR = G < 16 ? G : 16;  // a whole batch of gathers in flight per pass
+    constexpr int UNR = 16;               // a whole batch of gathers in flight per pass
     const unsigned gm = group_mask<G>();
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -48,21 +48,24 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
         const float4 api = ld4s(Ap + oi), zi = ld4s(Z + oi), ui = ld4s(U + oi);
         float4 acc = f4(0.f);
         const int rs = rowptr[i], re = rowptr[i + 1];
-        for (int base = rs; base < re; base += G) {
-            const int e = base + gl;
-            const int cj = e < re ? __ldg(col + e) : i;   // padding entries point at the own row with s = 1:
-            const float sv = e < re ? __ldg(s + e) : 0.f; // s = 0: no a' gather, and (z_i - z_i) = 0 exactly
-            const int cnt = min(G, re - base);
+        constexpr int B = G < 16 ? 16 : G, M = B / G;    // batch of max(G, 16) entries, M column ids per lane (see k_cg_spmv)
+        for (int base = rs; base < re; base += B) {
+            int cj[M];
+            float sv[M];
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const int e = base + m * G + gl;
+                cj[m] = e < re ? __ldg(col + e) : i;      // padding entries point at the own row with s = 0:
+                sv[m] = e < re ? __ldg(s + e) : 0.f;      // no a' gather, and (z_i - z_i) = 0 exactly
+            }
+            const int cnt = min(B, re - base);
             // two passes over the batch, each with all its gathers in flight (as in k_cg_spmv): first z_j (every
             // entry), then a'_j (only where s_ij != 0 -- a fused pair has v = 0 and needs no a'_j)
             for (int t = 0; t < cnt; t += UNR) {
                 int j[UNR];
                 float4 zj[UNR];
 #pragma unroll
-                for (int q = 0; q < UNR; ++q) {
-                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
-                    if (UNR > G && t + q >= G) j[q] = i;
-                }
+                for (int q = 0; q < UNR; ++q) j[q] = __shfl_sync(gm, cj[M == 1 ? 0 : q / G], (t + q) & (G - 1), G);
 #pragma unroll
                 for (int q = 0; q < UNR; ++q) zj[q] = ld4s(Z + (size_t)j[q] * ld + (valid ? c0 : 0));
 #pragma unroll
@@ -74,9 +77,8 @@ __global__ void __launch_bounds__(CC_THREADS) k_rhs(int n, int ld, int nchunk, c
                 float4 aj[UNR];
 #pragma unroll
                 for (int q = 0; q < UNR; ++q) {
-                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
-                    sj[q] = __shfl_sync(gm, sv, (t + q) & (G - 1), G);
-                    if (UNR > G && t + q >= G) sj[q] = 0.f;
+                    j[q] = __shfl_sync(gm, cj[M == 1 ? 0 : q / G], (t + q) & (G - 1), G);
+                    sj[q] = __shfl_sync(gm, sv[M == 1 ? 0 : q / G], (t + q) & (G - 1), G);
                 }
 #pragma unroll
                 for (int q = 0; q < UNR; ++q) aj[q] = sj[q] != 0.f ? ld4s(Ap + (size_t)j[q] * ld + (valid ? c0 : 0)) : api;
@@ -126,7 +128,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
     const float beta = first ? 0.f : (float)(sc->cg_gamma / sc->cg_gamma_old);
     // all gathers of a batch of G entries (16 at most) are issued before the first is consumed: the kernel
     // is bound by L2 gather latency, not bandwidth (profiles/r1a), so memory-level parallelism is the lever
-    constexpr int UNR = G < 16 ? G : 16;
+    constexpr int UNR = 16;
     const unsigned gm = group_mask<G>();
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
@@ -140,18 +142,22 @@ __global__ void __launch_bounds__(CC_THREADS) k_cg_spmv(int n, int ld, int nchun
         const float4 ui = ld4s(Uc + oi);
         const int rs = rowptr[i], re = rowptr[i + 1];
         float4 nsum = f4(0.f);
-        for (int base = rs; base < re; base += G) {
-            const int e = base + gl;
-            const int cj = e < re ? __ldg(col + e) : -1;
-            const int cnt = min(G, re - base);
+        // a batch is B = max(G, 16) entries: narrow groups (few columns: G = 2, 4, 8) load B / G column ids per lane, so
+        // that 16 gathers are in flight for them too (popres, p = 10, 60 entries per row: 15 dependent batches of 4 -> 4 of 16)
+        constexpr int B = G < 16 ? 16 : G, M = B / G;
+        for (int base = rs; base < re; base += B) {
+            int cj[M];
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                const int e = base + m * G + gl;
+                cj[m] = e < re ? __ldg(col + e) : -1;
+            }
+            const int cnt = min(B, re - base);
             for (int t = 0; t < cnt; t += UNR) {
                 int j[UNR];
                 float4 uj[UNR];
 #pragma unroll
-                for (int q = 0; q < UNR; ++q) {
-                    j[q] = __shfl_sync(gm, cj, (t + q) & (G - 1), G);
-                    if (UNR > G && t + q >= G) j[q] = -1;
-                }
+                for (int q = 0; q < UNR; ++q) j[q] = __shfl_sync(gm, cj[M == 1 ? 0 : q / G], (t + q) & (G - 1), G);
 #pragma unroll
                 for (int q = 0; q < UNR; ++q)
                     uj[q] = j[q] >= 0 ? ld4s(Uc + (size_t)j[q] * ld + (valid ? c0 : 0)) : f4(0.f);

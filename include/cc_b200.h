@@ -67,7 +67,8 @@ typedef struct {
     int32_t max_snapshots; /* how many per-gamma snapshots of U cc_path may keep (default 64)            */
     int32_t reserved0; /* 0 (default).  Debug selector used by the A/B tests and benches: 4 = dense mode on the FP32-FFMA
                           kernels only, 8 = FFMA pair kernel with the tensor-core contraction, 16 = the thread-staged
-                          (non-TMA) tensor-core kernels.  Results agree within the parity tolerance in every setting. */
+                          (non-TMA) tensor-core kernels, 32 = the phase-alternating fused kernel for n <= 64 instead of the
+                          warp-specialised one.  Results agree within the parity tolerance in every setting. */
 } cc_params;
 
 /* Fill *prm with the defaults above.  HOST pointer. */

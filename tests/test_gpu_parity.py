@@ -264,6 +264,45 @@ def test_cc_path_snapshots(B, torch_, oracle):
     B.cc_destroy(h)
 
 
+@pytest.mark.gpu
+@pytest.mark.parametrize("name,kw,miss", [("genotype", dict(n=52, p=5001), 0.0), ("dense_weight", dict(n=37, p=130, n_clusters=3), 0.15)])
+def test_dense_small_n_kernels_agree(B, torch_, oracle, name, kw, miss):
+    """n <= 64: the warp-specialised fused kernel (default) and the phase-alternating one (reserved0 = 32) both match
+    the oracle, labels included, and each other far inside the tolerance (they differ in the projection's arithmetic:
+    centred one-FFMA form vs direct differences)."""
+    torch = torch_
+    wl = synth.make(name, **kw)
+    if miss > 0:
+        rng = np.random.default_rng(11)
+        wl.mask = (rng.random(size=wl.X.shape) >= miss).astype(np.uint8)
+        wl.mask[0, :] = 1
+    prob = H.build_problem(oracle, wl)
+    n = wl.n
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    gammas = [float(g) for g in synth.gamma_grid(4.0, 40.0, 4)]
+    ref = H.oracle_path(oracle, prob, gammas, 60, proj_method=1)
+    dev = torch.device("cuda:0")
+    mask = None if wl.mask is None else torch.from_numpy(wl.mask).to(dev)
+    outs = {}
+    for tune in (0, 32):
+        h = B.cc_create(n, wl.p, torch.from_numpy(wl.X).to(dev), mask, None, None, torch.from_numpy(W).to(dev),
+                        B.cc_default_params(dense=1, reserved0=tune))
+        U = torch.empty(n, wl.p, device=dev)
+        lab = torch.empty(n, dtype=torch.int32, device=dev)
+        for g, r in zip(gammas, ref):
+            it, _, _ = B.cc_solve(h, g, 0.0, 60)
+            assert it == 60
+            B.cc_get_U(h, -1, U)
+            _, k = B.cc_clusters(h, -1, lab)
+            assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, (tune, g)
+            assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (tune, g)
+        outs[tune] = U.cpu().numpy().astype(np.float64)
+        B.cc_destroy(h)
+    assert H.relerr(outs[0], outs[32]) <= 1e-5
+
+
 @pytest.mark.parametrize("name,kw,miss", [("genotype", dict(n=20, p=1000), 0.0),      # 4x4 tiles, one row block, ksplit > 1
                                           ("genotype", dict(n=52, p=5001), 0.0),      # the genotype shape, ragged p
                                           ("dense_weight", dict(n=150, p=200, n_clusters=4), 0.0),   # 8x8 tiles, ragged rows

@@ -1342,7 +1342,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) kd_small_ws(int n, int ld, int 
     const int nmine = blockIdx.x < nchunks ? (nchunks - 1 - blockIdx.x) / gridDim.x + 1 : 0;   // chunks this CTA walks
     double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
     if (!pair_role) {
-        const float inv = 1.f / (float)(n + 1), fn = (float)n;
+        const float inv = 1.f / (float)(n + 1), fn = (float)n, rfn = 1.f / (float)n;
         const int n4 = (n + 3) & ~3;
         const int pq = rt & 15, prg = rt >> 4, i0r = prg * 4;
         // sum_j s_ij (p_i - p_j) is evaluated as rowsum(S)_i p~_i - sum_j s_ij p~_j on rows centred by the column mean of
@@ -1398,7 +1398,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) kd_small_ws(int n, int ld, int 
                 float4 ub = ld4s(&csum[0][pq * 4]);
 #pragma unroll
                 for (int q = 1; q < 16; ++q) ub = ub + ld4s(&csum[q][pq * 4]);
-                ub = make_float4(ub.x / fn, ub.y / fn, ub.z / fn, ub.w / fn);
+                ub = rfn * ub;                 // (a reciprocal multiply: the eight fp32 divisions per chunk sat on the critical role)
                 float4 pi[4], g[4];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) { pi[q] = ld4s(&Ps[i0r + q][small_sw(i0r, pq)]); g[q] = f4(0.f); }
@@ -1447,7 +1447,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) kd_small_ws(int n, int ld, int 
                 float4 db = ld4s(&dsum[0][pq * 4]);
 #pragma unroll
                 for (int q = 1; q < 16; ++q) db = db + ld4s(&dsum[q][pq * 4]);
-                db = make_float4(db.x / fn, db.y / fn, db.z / fn, db.w / fn);
+                db = rfn * db;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     const int i = i0r + q;

@@ -1685,7 +1685,8 @@ __global__ void kd_lab_hook(int n, const float* __restrict__ S, int* lab, int* c
 // masked distances by reading S11), optional normalisation by the sum over i<j (S8).  64 x 64 pair tiles.
 template <bool MASKED>
 __global__ void __launch_bounds__(256) kd_weights(int n, int p, int ntile, float phi, const float* __restrict__ X,
-                                                  const uint8_t* __restrict__ mask, float* __restrict__ W) {
+                                                  const uint8_t* __restrict__ mask, float* __restrict__ W,
+                                                  int cols_per_slice, float* __restrict__ part) {
     __shared__ float Xi[PT][PCK + 1], Xj[PT][PCK + 1], Mi[MASKED ? PT : 1][PCK + 1], Mj[MASKED ? PT : 1][PCK + 1];
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
     int I = 0, rem = blockIdx.x;
@@ -1696,10 +1697,13 @@ __global__ void __launch_bounds__(256) kd_weights(int n, int p, int ntile, float
     for (int a = 0; a < 4; ++a)
 #pragma unroll
         for (int b = 0; b < 4; ++b) { acc[a][b] = 0.f; cnt[a][b] = 0.f; }
-    for (int c0 = 0; c0 < p; c0 += PCK) {
+    // few tiles and many columns (52 x 200,000: one tile): blockIdx.y slices the columns, the slices' partial sums go to
+    // `part` and kd_weights_fin adds them in slice order (one CTA walking all columns alone took 29 ms there)
+    const int cbeg = blockIdx.y * cols_per_slice, cend = min(p, cbeg + cols_per_slice);
+    for (int c0 = cbeg; c0 < cend; c0 += PCK) {
         for (int t = tid; t < PT * PCK; t += 256) {
             const int r = t / PCK, c = t % PCK, gc = c0 + c;
-            const bool vi = i0 + r < n && gc < p, vj = j0 + r < n && gc < p;
+            const bool vi = i0 + r < n && gc < cend, vj = j0 + r < n && gc < cend;
             Xi[r][c] = vi ? X[(size_t)(i0 + r) * p + gc] : 0.f;
             Xj[r][c] = vj ? X[(size_t)(j0 + r) * p + gc] : 0.f;
             if (MASKED) {
@@ -1732,6 +1736,16 @@ __global__ void __launch_bounds__(256) kd_weights(int n, int p, int ntile, float
         for (int b = 0; b < 4; ++b) {
             const int gi = i0 + ty * 4 + a, gj = j0 + tx + 16 * b;
             if (gi < n && gj < n) {
+                if (part) {
+                    const size_t nn = (size_t)n * n, o = (size_t)blockIdx.y * nn * (MASKED ? 2 : 1);
+                    part[o + (size_t)gi * n + gj] = acc[a][b];
+                    if (I != J) part[o + (size_t)gj * n + gi] = acc[a][b];
+                    if (MASKED) {
+                        part[o + nn + (size_t)gi * n + gj] = cnt[a][b];
+                        if (I != J) part[o + nn + (size_t)gj * n + gi] = cnt[a][b];
+                    }
+                    continue;
+                }
                 float d = acc[a][b];
                 if (MASKED) d = cnt[a][b] > 0.f ? d * (float)p / cnt[a][b] : 3.0e38f;
                 const float w = gi == gj ? 0.f : expf(-phi * d);
@@ -1739,6 +1753,21 @@ __global__ void __launch_bounds__(256) kd_weights(int n, int p, int ntile, float
                 if (I != J) W[(size_t)gj * n + gi] = w;
             }
         }
+}
+
+// Sum of the column slices of kd_weights in slice order, then the same last step: masked rescaling (S11), exp.
+template <bool MASKED>
+__global__ void __launch_bounds__(256) kd_weights_fin(int n, int p, int ksplit, float phi, const float* __restrict__ part,
+                                                      float* __restrict__ W) {
+    const size_t nn = (size_t)n * n, e = (size_t)blockIdx.x * 256 + threadIdx.x;
+    if (e >= nn) return;
+    float d = 0.f, c = 0.f;
+    for (int k = 0; k < ksplit; ++k) {
+        d += part[(size_t)k * nn * (MASKED ? 2 : 1) + e];
+        if (MASKED) c += part[(size_t)k * nn * 2 + nn + e];
+    }
+    if (MASKED) d = c > 0.f ? d * (float)p / c : 3.0e38f;
+    W[e] = (e / n == e % n) ? 0.f : expf(-phi * d);
 }
 
 __global__ void __launch_bounds__(CC_THREADS) kd_wsum(int n, const float* __restrict__ W, double* part, unsigned int* ticket,
@@ -2041,10 +2070,36 @@ extern "C" int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint
     cudaStream_t st = (cudaStream_t)stream;
     const int ntile = (int)((n + PT - 1) / PT);
     const unsigned grid = (unsigned)(ntile * (ntile + 1) / 2);
-    if (mask) kd_weights<true><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out);
-    else kd_weights<false><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out);
     cudaError_t e = cudaSuccess;
-    if (normalize) {
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // column slices when the pair tiles alone cannot fill the GPU: about two CTAs per SM, at least 8 column blocks per slice
+    long long ksplit = grid >= (unsigned)sms ? 1 : (2LL * sms + grid - 1) / grid;
+    const long long kmax = (p + 8LL * PCK - 1) / (8LL * PCK);
+    if (ksplit > kmax) ksplit = kmax;
+    if (ksplit <= 1) {
+        if (mask) kd_weights<true><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)p, nullptr);
+        else kd_weights<false><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)p, nullptr);
+    } else {
+        const long long cols = ((p + ksplit - 1) / ksplit + PCK - 1) / PCK * PCK;
+        ksplit = (p + cols - 1) / cols;
+        float* part = nullptr;
+        e = cc_dev_alloc((void**)&part, (size_t)ksplit * n * n * (mask ? 2 : 1) * sizeof(float), st);
+        if (e == cudaSuccess) {
+            const dim3 g2(grid, (unsigned)ksplit);
+            const unsigned gf = (unsigned)(((size_t)n * n + 255) / 256);
+            if (mask) {
+                kd_weights<true><<<g2, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)cols, part);
+                kd_weights_fin<true><<<gf, 256, 0, st>>>((int)n, (int)p, (int)ksplit, phi, part, W_out);
+            } else {
+                kd_weights<false><<<g2, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)cols, part);
+                kd_weights_fin<false><<<gf, 256, 0, st>>>((int)n, (int)p, (int)ksplit, phi, part, W_out);
+            }
+            cc_dev_free(part, st);
+        }
+    }
+    if (normalize && e == cudaSuccess) {
         double* red = nullptr;
         e = cc_dev_alloc((void**)&red, (size_t)(2 + 1024) * sizeof(double), st);
         if (e == cudaSuccess) {

@@ -100,7 +100,10 @@ def test_knn_weights_match_oracle(B, oracle, name, kw, k, phi, norm):
 
 @pytest.mark.parametrize("name,kw,phi,norm", [("genotype", dict(n=52, p=3001), 0.01, False),
                                               ("dense_weight", dict(n=200, p=64, n_clusters=4), 0.005, True),
-                                              ("expression", dict(n=70, p=333), 0.002, False)])
+                                              ("expression", dict(n=70, p=333), 0.002, False),
+                                              # few pair tiles, many columns: the column-sliced path (plain and masked)
+                                              ("genotype", dict(n=52, p=40000), 0.002, True),
+                                              ("expression", dict(n=30, p=5000), 0.0002, False)])
 def test_dense_weights_match_oracle(B, oracle, name, kw, phi, norm):
     """a0 for complete graphs against the oracle's eq. 8 with all pairs (incl. masked rule S11, S8)."""
     import torch

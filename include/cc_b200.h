@@ -59,7 +59,9 @@ typedef struct {
     int32_t proj_maxit; /*   cap on inner iterations per MM iteration (default 500); hitting it => CC_ENOCONV */
     int32_t min_it;   /* S3: never stop before this many MM iterations (default 10)                      */
     int32_t dense;    /* 0: graph given as CSR.  1: complete graph; `w` is an n x n row-major symmetric
-                             fp32 matrix (diagonal ignored, off-diagonal > 0), rowptr/col ignored        */
+                             fp32 matrix (diagonal ignored, off-diagonal >= 0), rowptr/col ignored.  The
+                             constraint set stays the complete graph: a zero entry is a pair of E that
+                             carries no penalty (its threshold is 0), not an absent pair                 */
     int32_t use_graph;/* 1 (default): one CUDA-graph launch per solve with device-side WHILE loops;
                          0: plain stream launches with a host loop (debugging)                           */
     int32_t hist_cap; /* capacity of the per-solve Phi_m / d_m history kept on the device (default 4096;
@@ -77,8 +79,12 @@ int cc_default_params(cc_params* prm);
 /* ---- a0: one-time k-NN + Gaussian weights, PAPER.md L127-L133 (eq. 8) -------------------------------
  * w_ij = 1{i ~_k j} exp(-phi ||x_i - x_j||^2), i ~_k j iff j is among the k nearest of i OR vice versa
  * (L127); self excluded, ties to the smaller index (S9).  With a mask, the squared distance is taken
- * over co-observed coordinates and scaled by p / #co-observed (S11).  normalize != 0 divides the
- * weights by their sum over pairs i<j (L133, S8).
+ * over co-observed coordinates and scaled by p / #co-observed (S11); rows without a common observed
+ * coordinate are at infinite distance and are never neighbours.  Which points are the k nearest is
+ * decided on fp64 distances of the fp32 inputs (an fp32 pass only shortlists), so the graph is the one
+ * the definition gives, ties included.  A pair whose weight underflows to 0 in fp32 is absent from the
+ * result (L40: a zero weight is no pair), in both directions, so the result always passes cc_create.
+ * normalize != 0 divides the weights by their sum over pairs i<j (L133, S8).
  * X (DEVICE, n*p fp32), mask (DEVICE n*p uint8 or NULL).  Outputs: *rowptr (int64[n+1]), *col
  * (int32[nnz]), *w (fp32[nnz]) are DEVICE arrays allocated by the library (cudaMalloc) and owned by
  * the caller, to be released with cc_free_graph; *nnz (HOST) receives the directed entry count.

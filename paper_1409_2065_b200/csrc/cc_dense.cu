@@ -1657,7 +1657,7 @@ __global__ void kd_check_w(int n, const float* __restrict__ W, int* flag) {
         const int i = (int)(e / n), j = (int)(e % n);
         if (i == j) continue;
         const float a = W[e];
-        if (!(a > 0.f) || isinf(a)) bad |= 64;                 // F_WBAD
+        if (!(a >= 0.f) || isinf(a)) bad |= 64;                // F_WBAD (a zero weight is allowed here: see cc_b200.h, prm.dense)
         if (a != W[(size_t)j * n + i]) bad |= 32;              // F_WASYM
     }
     if (bad) atomicOr(flag, bad);

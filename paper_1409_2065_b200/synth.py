@@ -187,6 +187,25 @@ def gamma_grid(lo: float, hi: float, n_gamma: int) -> np.ndarray:
     return np.exp(np.linspace(np.log(lo), np.log(hi), n_gamma))
 
 
+def tie_cases(seed: int = 0):
+    """Inputs with EXACT distance ties for the k-NN tie rule (reading S9): integer lattice points (many equal
+    squared distances, all exactly representable), a matrix with duplicated rows (distance 0 ties and equal
+    distances to both copies), and masked lattice rows with two rows that share no observed coordinate.
+    Returns a list of (name, X fp32, mask or None, k)."""
+    rng = np.random.default_rng(seed + 99)
+    g = np.stack(np.meshgrid(np.arange(6), np.arange(6), np.arange(3), indexing="ij"), -1).reshape(-1, 3).astype(np.float64)
+    lattice = g[rng.permutation(g.shape[0])]                      # 108 points, shuffled so that index order matters
+    base = rng.normal(size=(30, 5))
+    dup = np.concatenate([base, base[:12], base[3:9]], axis=0)    # rows 30..41 copy 0..11, rows 42..47 copy 3..8
+    dup = dup[rng.permutation(dup.shape[0])]
+    lat2 = rng.integers(0, 4, size=(40, 6)).astype(np.float64)
+    m2 = (rng.random(size=lat2.shape) >= 0.3).astype(np.uint8)
+    m2[0, :] = [1, 1, 1, 0, 0, 0]
+    m2[1, :] = [0, 0, 0, 1, 1, 1]                                 # rows 0 and 1 share no observed coordinate
+    m2[2, :] = 1
+    return [("lattice", _f32(lattice), None, 7), ("duplicates", _f32(dup), None, 5), ("masked_lattice", _f32(lat2), m2, 6)]
+
+
 def random_graph(n: int, avg_deg: float, seed: int, connected: bool = False):
     """Seeded random undirected pair list (i<j) with uniform(0.1,1) weights, for unit tests."""
     rng = np.random.default_rng(seed)

@@ -98,6 +98,76 @@ def test_knn_weights_match_oracle(B, oracle, name, kw, k, phi, norm):
     B.cc_destroy(h)
 
 
+def _oracle_csr(oracle, X32, mask, k, phi):
+    """The oracle's eq.-8 graph as the CSR the library must return: weights cast to fp32 once, pairs whose weight
+    is 0 in fp32 absent (S24)."""
+    n = X32.shape[0]
+    ei, ej, w, _ = oracle.knn_graph(X32.astype(np.float64), mask, k, phi)
+    w32 = w.astype(np.float32)
+    keep = w32 > 0
+    rp, cl, ww = oracle.to_csr(n, ei[keep], ej[keep], w32[keep].astype(np.float64))
+    return rp, cl, ww.astype(np.float32), int((~keep).sum())
+
+
+def test_knn_tie_rule_and_rows_with_few_candidates(B, oracle):
+    """Index output is held to identity.  (1) Exact ties (lattice points, duplicated rows): the smaller index wins on
+    both sides (S9) -- the fp32 pass cannot settle these rows and hands them to the exact pass.  (2) Masked rows with
+    fewer than k candidates at finite distance (disjoint observed sets): the row holds only those (advisor finding:
+    the fill used to write past the row)."""
+    import torch
+    for name, X32, mask, k in synth.tie_cases():
+        rp, cl, ww, _ = _oracle_csr(oracle, X32, mask, k, 0.25)
+        rowptr, col, wg = B.cc_knn_weights(X32.shape[0], X32.shape[1], _dev(torch, X32), _dev(torch, mask), k, 0.25)
+        assert np.array_equal(rowptr.cpu().numpy(), rp), name
+        assert np.array_equal(col.cpu().numpy(), cl), name
+        assert np.array_equal(wg.cpu().numpy(), ww), name          # same fp64 distance, same exp, one rounding to fp32
+    # two groups of rows that observe disjoint coordinates: 2 candidates at finite distance, k = 4
+    rng = np.random.default_rng(8)
+    X32 = rng.normal(size=(6, 4)).astype(np.float32)
+    mask = np.array([[1, 1, 0, 0]] * 3 + [[0, 0, 1, 1]] * 3, np.uint8)
+    rp, cl, ww, dropped = _oracle_csr(oracle, X32, mask, 4, 0.5)
+    assert dropped > 0 and rp[-1] == 12                             # the oracle lists infinite-distance pairs; weight 0
+    rowptr, col, wg = B.cc_knn_weights(6, 4, _dev(torch, X32), _dev(torch, mask), 4, 0.5)
+    assert np.array_equal(rowptr.cpu().numpy(), rp) and np.array_equal(col.cpu().numpy(), cl)
+    assert np.allclose(wg.cpu().numpy(), ww, rtol=1e-6)
+    # larger: random masks at 70 % missing leave many pairs without a common coordinate
+    X32 = rng.normal(size=(300, 5)).astype(np.float32)
+    mask = (rng.random(size=X32.shape) >= 0.7).astype(np.uint8)
+    mask[:, 0] |= (mask.sum(1) == 0).astype(np.uint8)
+    rp, cl, ww, _ = _oracle_csr(oracle, X32, mask, 12, 0.125)
+    rowptr, col, wg = B.cc_knn_weights(300, 5, _dev(torch, X32), _dev(torch, mask), 12, 0.125)
+    assert np.array_equal(rowptr.cpu().numpy(), rp) and np.array_equal(col.cpu().numpy(), cl)
+    assert np.allclose(wg.cpu().numpy(), ww, rtol=1e-6)
+
+
+def test_large_phi_underflowing_weights_end_to_end(B, oracle):
+    """raising phi sends most k-NN weights to 0.  A weight that is 0 in fp32 is an absent pair (S24):
+    cc_knn_weights drops those entries in both directions, so what it returns is what cc_create accepts, and the
+    solve on it follows the oracle's on the same graph."""
+    import torch
+    wl = synth.make("popres", n=500, phi=512.0)
+    rp, cl, ww, dropped = _oracle_csr(oracle, wl.X, None, wl.k, wl.phi)
+    assert dropped > 500 and rp[-1] > 1000                          # a real mix of underflowed and live pairs
+    X = _dev(torch, wl.X)
+    rowptr, col, wg = B.cc_knn_weights(wl.n, wl.p, X, None, wl.k, wl.phi)
+    assert np.array_equal(rowptr.cpu().numpy(), rp) and np.array_equal(col.cpu().numpy(), cl)
+    assert np.allclose(wg.cpu().numpy(), ww, rtol=1e-6, atol=0) and float(wg.min()) > 0.0
+    h = B.cc_create(wl.n, wl.p, X, None, rowptr, col, wg, None)     # used to fail with CC_EGRAPH (w <= 0)
+    up = cl > np.repeat(np.arange(wl.n), np.diff(rp))
+    ei, ej = np.repeat(np.arange(wl.n), np.diff(rp))[up].astype(np.int32), cl[up].astype(np.int32)
+    w64 = wg.cpu().numpy()[up].astype(np.float64)
+    ref = oracle.path(wl.X.astype(np.float64), None, ei, ej, w64, [0.5, 20.0], 60, proj_method=1)
+    U = torch.empty(wl.n, wl.p, device="cuda:0")
+    lab = torch.empty(wl.n, dtype=torch.int32, device="cuda:0")
+    for g, r in zip([0.5, 20.0], ref):
+        B.cc_solve(h, g, 0.0, 60)
+        B.cc_get_U(h, -1, U)
+        _, kc = B.cc_clusters(h, -1, lab)
+        assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= 1e-4
+        assert kc == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"])
+    B.cc_destroy(h)
+
+
 @pytest.mark.parametrize("name,kw,phi,norm", [("genotype", dict(n=52, p=3001), 0.01, False),
                                               ("dense_weight", dict(n=200, p=64, n_clusters=4), 0.005, True),
                                               ("expression", dict(n=70, p=333), 0.002, False),

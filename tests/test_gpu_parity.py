@@ -399,10 +399,43 @@ def test_dense_mode_rejects_bad_weights(B, torch_):
         B.cc_create(n, p, X, None, None, None, W, B.cc_default_params(dense=1))
     assert e.value.code == B.CC_EGRAPH
     W = torch.ones(n, n, device="cuda:0")
-    W[1, 2] = W[2, 1] = 0.0
+    W[1, 2] = W[2, 1] = -0.5
     with pytest.raises(B.CCError) as e:
         B.cc_create(n, p, X, None, None, None, W, B.cc_default_params(dense=1))
     assert e.value.code == B.CC_EGRAPH
+
+
+def test_dense_mode_zero_weights_are_unpenalised_pairs(B, torch_, oracle):
+    """Dense mode keeps the complete graph as the constraint set; a zero entry of W is a pair of E with no penalty
+    (threshold 0, v = b).  cc_dense_weights at a large phi produces such entries; the iteration with them must be
+    the oracle's iteration on the complete pair list with those zero weights."""
+    torch = torch_
+    wl = synth.make("dense_weight", n=90, p=24, n_clusters=3)
+    X64 = wl.X.astype(np.float64)
+    n = wl.n
+    ei, ej, w, d2 = oracle.complete_graph(X64, None, 3.0)
+    w32 = w.astype(np.float32)
+    assert 100 < int((w32 == 0).sum()) < len(ei) - 100              # a real mix
+    dev = torch.device("cuda:0")
+    X = torch.from_numpy(wl.X).to(dev)
+    W = B.cc_dense_weights(n, wl.p, X, None, 3.0)
+    Wref = np.zeros((n, n), np.float32); Wref[ei, ej] = w32; Wref = Wref + Wref.T
+    assert np.array_equal(W.cpu().numpy() == 0, Wref == 0)
+    W = torch.from_numpy(Wref).to(dev)
+    rp, cl, wc = oracle.to_csr(n, ei, ej, w32.astype(np.float64))
+    prob = {"X64": X64, "mask": None, "ei": ei, "ej": ej, "w64": w32.astype(np.float64), "n": n, "p": wl.p}
+    gammas = [3.0, 30.0, 300.0]
+    ref = H.oracle_path(oracle, prob, gammas, 60, proj_method=1)
+    h = B.cc_create(n, wl.p, X, None, None, None, W, B.cc_default_params(dense=1))
+    U = torch.empty(n, wl.p, device=dev)
+    lab = torch.empty(n, dtype=torch.int32, device=dev)
+    for g, r in zip(gammas, ref):
+        B.cc_solve(h, g, 0.0, 60)
+        B.cc_get_U(h, -1, U)
+        _, k = B.cc_clusters(h, -1, lab)
+        assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, g
+        assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (g, k, r["nclusters"])
+    B.cc_destroy(h)
 
 
 def test_two_points_closed_form_and_single_point(B, torch_):
@@ -601,41 +634,31 @@ def test_dense_n8192_against_oracle_small_p(B, torch_, oracle):
 
 
 def test_full_size_large_sparse_elementwise(B, torch_, oracle):
-    """configs[3] at full size (100,000 x 64, 856,602 pairs), in the launch configuration bench.py times: the graph
-    from cc_knn_weights against the oracle's brute-force graph, then every element of U after 2 x 4 iterations
-    (about 80 s, most of it the oracle's 10^10-pair neighbour search)."""
+    """configs[3] at full size (100,000 x 64, 856,602 pairs), in the launch configuration bench.py times.
+    (1) The graph from cc_knn_weights IS the oracle's brute-force graph: rowptr and col identical (index output is
+    held to identity: the fp32 tile pass only shortlists, the k nearest are decided in fp64 on the fp32 inputs).
+    (2) Every element of U after 2 x 4 iterations of the contract iteration (kappa = 1e-2) from the cold start.
+    (3) A run in which pairs really fuse, so that identical labels mean something at this size: kappa = 0.1
+    (a parameter of the iteration, S2; the same on both sides) makes the first thresholds gamma w kappa comparable
+    to the neighbour distances, 3 gammas x 6 iterations, thousands of fused pairs at the last gamma."""
     torch = torch_
     wl = synth.make("large_sparse")
     prob = H.build_problem(oracle, wl)
     dev = torch.device("cuda:0")
     X = torch.from_numpy(wl.X).to(dev)
     rowptr, col, w = B.cc_knn_weights(wl.n, wl.p, X, None, wl.k, prob["phi"])
-    # 10^10 candidate pairs: a few k-th / (k+1)-th neighbours are closer than fp32 can tell apart, and the kernel decides in
-    # fp32 where the oracle decides in fp64.  What is unique must agree; every other entry must be such a near-tie.
-    n = wl.n
-    rows_g = np.repeat(np.arange(n, dtype=np.int64), np.diff(rowptr.cpu().numpy()))
-    key_g = rows_g * n + col.cpu().numpy().astype(np.int64)
-    rows_o = np.repeat(np.arange(n, dtype=np.int64), np.diff(prob["rowptr"]))
-    key_o = rows_o * n + prob["col"].astype(np.int64)
-    extra = np.concatenate([np.setdiff1d(key_g, key_o), np.setdiff1d(key_o, key_g)])
-    assert extra.size <= 200, extra.size
-    if extra.size:
-        X64 = wl.X.astype(np.float64)
-        ii, jj = extra // n, extra % n
-        touched = np.unique(np.concatenate([ii, jj]))
-        _, d2k = oracle.knn(X64, None, wl.k + 1, rows=touched)
-        kth = dict(zip(touched.tolist(), d2k[:, wl.k - 1].tolist()))
-        kth1 = dict(zip(touched.tolist(), d2k[:, wl.k].tolist()))
-        dij = ((X64[ii] - X64[jj]) ** 2).sum(1)
-        for a, b2, dd2 in zip(ii.tolist(), jj.tolist(), dij.tolist()):
-            near = min(abs(dd2 - kth[a]) / kth[a], abs(dd2 - kth1[a]) / kth1[a],
-                       abs(dd2 - kth[b2]) / kth[b2], abs(dd2 - kth1[b2]) / kth1[b2])
-            assert near <= 1e-5, (a, b2, near)
-    print("full-size k-NN graph: directed entries that differ from the fp64 brute force (all near-ties):", extra.size)
+    assert np.array_equal(rowptr.cpu().numpy(), prob["rowptr"])
+    assert np.array_equal(col.cpu().numpy(), prob["col"])
+    assert np.abs(w.cpu().numpy() - prob["wcsr32"]).max() <= 1e-6 * prob["wcsr32"].max()
     gammas = [5.0, 80.0]
     ref = H.oracle_path(oracle, prob, gammas, 4, proj_method=1)
     out = _run_path(B, torch, prob, gammas, 4, ref)
     print("full-size large_sparse: relerr, clusters =", out)
+    gammas = [40.0, 70.0, 110.0]
+    ref = H.oracle_path(oracle, prob, gammas, 6, proj_method=1, kappa=0.1)
+    out = _run_path(B, torch, prob, gammas, 6, ref, kappa=0.1)
+    print("full-size large_sparse, kappa = 0.1: relerr, clusters =", out)
+    assert out[-1][1] < wl.n - 2000          # the comparison of labels is not vacuous
 
 
 # ----------------------------------------------------------------------------- f1: kappa continuation (S26)

@@ -353,6 +353,97 @@ def test_knn_masked_distance_rule(oracle):
     assert d[0] == np.inf and abs(d[1] - 2.0 * 4 / 2) < 1e-15 and abs(d[2] - (25 + 25 + 16) * 4 / 3) < 1e-13
 
 
+def _brute_knn(X, mask, k):
+    """k nearest by the definition: all squared distances (masked rule S11 by explicit loops), stable argsort
+    (equal distances keep the smaller index first, S9), self excluded."""
+    n, p = X.shape
+    D2 = np.full((n, n), np.inf)
+    for i in range(n):
+        for j in range(n):
+            if i == j:
+                continue
+            if mask is None:
+                D2[i, j] = float(((X[i] - X[j]) ** 2).sum())
+            else:
+                co = [c for c in range(p) if mask[i, c] and mask[j, c]]
+                if co:
+                    D2[i, j] = float(sum((X[i, c] - X[j, c]) ** 2 for c in co)) * p / len(co)
+    return np.argsort(D2, axis=1, kind="stable")[:, :k], D2
+
+
+def test_knn_tie_rule_smaller_index_first(oracle):
+    """Reading S9 (PAPER.md L127 does not say how ties are broken): equal distances go to the smaller index.
+    Lattice points and duplicated rows have many exact ties; turning the oracle's strict '<' into '<=' (or
+    scanning candidates in another order) changes these neighbour lists."""
+    O = oracle
+    n_ties = 0
+    for name, X32, mask, k in synth.tie_cases():
+        X = X32.astype(np.float64)
+        nn, D2 = _brute_knn(X, mask, k)
+        nbr, d2 = O.knn(X, mask, k)
+        assert np.array_equal(nbr, nn), name
+        assert np.array_equal(d2, np.take_along_axis(D2, nn, axis=1)), name
+        # the cases really have ties AT the cut: the k-th and (k+1)-th distances coincide for some rows
+        srt = np.sort(D2, axis=1)
+        n_ties += int((srt[:, k - 1] == srt[:, k]).sum())
+        # numpy restatement of the masked rule (used for the phi rule) agrees with the C rule
+        ii, jj = np.triu_indices(X.shape[0], 1)
+        d_np = O.pair_dist2(X, mask, ii, jj)
+        assert np.array_equal(d_np, D2[ii, jj]) or np.allclose(d_np, D2[ii, jj], rtol=1e-15), name
+    assert n_ties > 50
+
+
+def test_pair_dist2_masked_branch_matches_the_c_rule(oracle):
+    """oracle.pair_dist2 (numpy, used for the phi rule S10) restates orc_row_dist2's masked rule S11."""
+    O = oracle
+    rng = np.random.default_rng(3)
+    X = rng.normal(size=(25, 9))
+    mask = (rng.random(size=X.shape) >= 0.4).astype(np.uint8)
+    mask[3, :] = 0
+    mask[3, 0] = 1
+    mask[4, :] = 0
+    mask[4, 5] = 1                                   # rows 3 and 4 share no observed coordinate
+    for i in (0, 3, 4, 11):
+        d_c = O.row_dist2(X, mask, i)
+        jj = np.array([j for j in range(25) if j != i])
+        d_np = O.pair_dist2(X, mask, np.full(jj.size, i), jj)
+        assert np.allclose(d_np[np.isfinite(d_np)], d_c[jj][np.isfinite(d_c[jj])], rtol=1e-14)
+        assert np.array_equal(np.isinf(d_np), np.isinf(d_c[jj]))
+    assert np.isinf(O.row_dist2(X, mask, 3)[4])
+
+
+def test_S3_stop_rule_iteration_count(oracle):
+    """Reading S3: stop after iteration m (0-based) as soon as m + 1 >= min_it, m >= 1 and
+    Phi_{m-1} - Phi_m <= tol (1 + |Phi_{m-1}|).  The count is re-derived here from the Phi history of a
+    fixed-length run (tol = 0), so an off-by-one in either index of the rule fails."""
+    O = oracle
+    X, mask, ei, ej, w = _tiny(O, seed=21, n=18, p=3)
+    g = 1.5
+    rho, eps = O.default_rho_eps(X, mask, w, g)
+    U0, V0 = O.cold_start(X, mask, ei, ej)
+    full = O.mm(X, mask, ei, ej, w, g, rho, eps, U0, V0, 400)
+    phi = full["phi"]
+    dec = (phi[:-1] - phi[1:]) / (1.0 + np.abs(phi[:-1]))        # dec[m-1] belongs to iteration m
+    assert np.all(np.diff(dec[5:]) < 0)                           # decreasing: the first crossing is well defined
+
+    def expected(tol, min_it):
+        for m in range(1, len(phi)):
+            if m + 1 >= min_it and dec[m - 1] <= tol:
+                return m + 1
+        return len(phi)
+
+    for min_it in (0, 1, 2, 7, 10, 40):
+        for m_star in (12, 30):
+            tol = float(np.sqrt(dec[m_star - 1] * dec[m_star - 2]))   # between the decreases of iterations m*-1 and m*
+            r = O.mm(X, mask, ei, ej, w, g, rho, eps, U0, V0, 400, tol=tol, min_it=min_it)
+            want = expected(tol, min_it)
+            assert r["iters"] == want == max(m_star + 1, min_it, 2), (min_it, m_star, r["iters"], want)
+            assert np.array_equal(r["phi"], phi[:want])
+    # a tolerance that every decrease satisfies: min_it alone decides, but never before two iterations (m >= 1)
+    for min_it, want in ((0, 2), (1, 2), (2, 2), (3, 3), (9, 9)):
+        assert O.mm(X, mask, ei, ej, w, g, rho, eps, U0, V0, 400, tol=1e9, min_it=min_it)["iters"] == want
+
+
 # ---------------------------------------------------------------- golden fixture (oracle-written)
 def test_golden_tiny_path_is_reproducible(oracle):
     """tests/golden/tiny_path.json is written by tests/golden/make_golden.py, which calls only

@@ -15,12 +15,19 @@ undirected pair carried through one full MM iteration, projection sweeps include
 value   : |E| * iters * K / device time of the K steps, inputs resident in HBM.
 e2e     : the same work through the C ABI starting from pinned HOST buffers: per step H2D of X and the
           CSR graph, cc_create, cc_solve, cc_get_U into host memory, cc_destroy.
-roofline: the kernel with the largest share of device time; its duration is measured live inside the
-          timed region by the library's device-side %globaltimer marks (the kernels are nodes of a
-          CUDA graph with device-side WHILE loops, so host events cannot bracket them); bytes per
-          launch are the algorithmic no-reuse figures of DESIGN.md.
-cpu_baseline / --impl reference: the fp64 oracle (oracle/), as it stands, on the host cores, on a
-          bounded sample (the first `--cpu-n` points' worth of the same generator).
+roofline: the SWEEP (a1 right-hand side, a2 one inner projection sweep = k_cg_spmv +
+          k_cg_update, a3 pair norms, a5+a6 update) with the largest share of device time; durations are
+          measured live inside the timed region by the library's device-side %globaltimer marks (the
+          kernels are nodes of a CUDA graph with device-side WHILE loops, so host events cannot bracket
+          them); bytes per launch are SURVEY 8(d)'s no-reuse formulas (`bytes_per_launch`), the
+          implementation's own stream count is printed beside them (`impl_bytes`), and `per_iteration`
+          is the whole MM iteration against the same peak.  `traffic` / `l2_bytes` are ncu's DRAM and L2
+          bytes per launch of the dominant kernel from the capture named in profiles/r2_traffic.json.
+cpu_baseline: the fp64 oracle (oracle/), as it stands, on the host cores, SURVEY 8(d)'s protocol on a
+          bounded sample: the same generator at `--cpu-n` points, `--cpu-iters` MM iterations at the
+          first, middle and last gamma with the CG back-end on all cores, then one iteration at the
+          middle gamma on a single thread.  `--cpu-full` runs the protocol at the full size (minutes).
+--impl reference: the oracle timed step by step on the same bounded sample (driver contract).
 N > 1   : the path does not shard without a halo exchange: N independent
           replicas with different seeds, no collective on the data path, scaling "weak".
 """
@@ -56,8 +63,9 @@ def parse():
     ap.add_argument("--workload", default="large_sparse", choices=list(GRID))
     ap.add_argument("--iters", type=int, default=20, help="MM iterations per step")
     ap.add_argument("--n", type=int, default=0, help="override the number of points (0 = config size)")
-    ap.add_argument("--cpu-n", type=int, default=6000, help="points in the oracle's bounded sample")
+    ap.add_argument("--cpu-n", type=int, default=20000, help="points in the oracle's bounded sample (large_sparse)")
     ap.add_argument("--cpu-iters", type=int, default=3)
+    ap.add_argument("--cpu-full", action="store_true", help="cpu_baseline at the full configuration size (minutes)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-path", action="store_true", help="skip the full gamma-path wall time")
     ap.add_argument("--no-e2e", action="store_true")
@@ -113,12 +121,12 @@ def cpu_count_used(O):
     return int(O.num_threads())
 
 
-def oracle_sample(args, steps, warmup):
-    """Times the oracle on a bounded sample of the workload; returns (pair-updates/s, info dict)."""
+def _oracle_problem(args, full=False):
+    """The workload's generator (bounded sample unless `full`), graph and weights by the oracle's own eq.-8 code."""
     from oracle import oracle as O
     from paper_1409_2065_b200 import synth
     O.build()
-    wl = synth.make(args.workload, **CPU_SAMPLE[args.workload](args))
+    wl = synth.make(args.workload, **({} if full else CPU_SAMPLE[args.workload](args)))
     X = wl.X.astype(np.float64)
     if wl.phi_rule == "fixed":
         phi = wl.phi
@@ -130,6 +138,12 @@ def oracle_sample(args, steps, warmup):
         ei, ej, w, _ = O.knn_graph(X, wl.mask, wl.k, phi)
     else:
         ei, ej, w, _ = O.complete_graph(X, wl.mask, phi)
+    return O, wl, X, ei, ej, w
+
+
+def oracle_sample(args, steps, warmup):
+    """--impl reference: the oracle step by step on the bounded sample; returns (pair-updates/s, info, s per step)."""
+    O, wl, X, ei, ej, w = _oracle_problem(args)
     U, V = O.cold_start(X, wl.mask, ei, ej)
     times = []
     for s in range(warmup + steps):
@@ -149,29 +163,81 @@ def oracle_sample(args, steps, warmup):
     return val, info, tot / max(1, len(times))
 
 
-def alg_bytes(kernel, n, p, nnz, masked, dense=False):
-    """Algorithmic (no-reuse) bytes one launch of `kernel` must move: every gathered neighbour row is
-    counted once per directed entry, own rows and outputs once per node ('roofline')."""
+def oracle_protocol(args, full=False):
+    """cpu_baseline, SURVEY 8(d) "Timing the oracle beside it": `cpu_iters` MM iterations at the first, middle and last
+    gamma of the grid (warm-started in that order, CG back-end) on all cores, then one iteration at the middle gamma on
+    a single thread; core count read at run time.  Bounded sample of the workload unless `full`."""
+    from paper_1409_2065_b200 import synth
+    O, wl, X, ei, ej, w = _oracle_problem(args, full)
+    lo, hi, ng = GRID[args.workload]
+    grid = synth.gamma_grid(lo, hi, ng)
+    gs = [float(grid[0]), float(grid[ng // 2]), float(grid[-1])]
+    cores = cpu_count_used(O)
+    U, V = O.cold_start(X, wl.mask, ei, ej)
+    per_gamma, tot = [], 0.0
+    mid_state = None
+    for g in gs:
+        rho, eps = O.default_rho_eps(X, wl.mask, w, g)
+        if g == gs[1]:
+            mid_state = (U, V, rho, eps)
+        t0 = time.perf_counter()
+        r = O.mm(X, wl.mask, ei, ej, w, g, rho, eps, U, V, args.cpu_iters, proj_method=1)
+        dt = time.perf_counter() - t0
+        U, V = r["U"], r["V"]
+        tot += dt
+        per_gamma.append({"gamma": g, "s_per_iteration": dt / args.cpu_iters, "cg_iterations_per_iteration": r["proj_cycles"] / args.cpu_iters})
+    val = len(ei) * args.cpu_iters * len(gs) / tot
+    O.set_threads(1)
+    Um, Vm, rho, eps = mid_state
+    t0 = time.perf_counter()
+    O.mm(X, wl.mask, ei, ej, w, gs[1], rho, eps, Um, Vm, 1, proj_method=1)
+    t1 = time.perf_counter() - t0
+    O.set_threads(cores)
+    return {"value": val, "unit": "pair-updates/s", "cores": cores, "kind": "oracle",
+            "single_thread_value": len(ei) / t1, "per_gamma": per_gamma,
+            "sample": f"{args.workload} generator at n={wl.n}, p={wl.p} (|E|={len(ei)}){' = the full configuration' if full else ''}: "
+                      f"{args.cpu_iters} MM iterations at gamma = first/middle/last of the grid on {cores} threads, then 1 iteration "
+                      f"at the middle gamma on 1 thread; fp64, explicit V, CG projection to 1e-13"}
+
+
+def sweep_bytes(n, p, nnz, masked, dense=False):
+    """SURVEY 8(d) algorithmic bytes per sweep, "no-reuse" model: every gathered neighbour row counts once per
+    directed entry, own rows and outputs once per node; fp32.  Keys are the sweeps, values (bytes, kernels)."""
+    npb, E = 4 * n * p, nnz // 2
+    if dense and n <= 64:
+        # genotype-like: read U, A', write A + read X, U, A, write U (SURVEY 8(d) "Dense path": 7 node arrays)
+        return {"a9_small": (7 * npb, ("kd_proj",)), "a4_edges": (16 * n * n, ("kd_edges",)), "a5_update": (4 * npb + n * p, ("k_update",))}
+    if dense:
+        # dense-weight: W (n x n) once + ~10 node arrays per MM iteration (SURVEY 8(d)); per kernel the n x n it must touch
+        return {"a9_proj": (4 * n * n + 5 * npb, ("kd_proj",)), "a9_pairs": (4 * n * n // 2 + 2 * npb, ("kd_pairs",)),
+                "a4_edges": (8 * n * n, ("kd_edges",)), "a5_update": (4 * npb + n * p, ("k_update",))}
+    return {"a1_rhs": (nnz * (4 * p + 12) + 3 * npb, ("k_rhs",)),
+            "a2_sweep": (nnz * (4 * p + 4) + 7 * npb, ("k_cg_spmv", "k_cg_update")),
+            "a3_norms": (E * (8 * p + 12) + 2 * npb, ("k_norm",)),
+            "a5_update": (4 * npb + n * p, ("k_update",))}
+
+
+def impl_bytes(kernel, n, p, nnz, masked, dense=False):
+    """What the kernels as written stream per launch (own count, for comparison with sweep_bytes)."""
     row, npb = 4 * p, 4 * n * p
     return {
-        "k_rhs": nnz * (2 * row + 8) + 5 * npb + 4 * n,
+        "k_rhs": nnz * (row + 8) + 5 * npb + 4 * n,          # z_j for every entry; a'_j only for unfused pairs (not counted)
         "k_cg_spmv": nnz * (row + 4) + 5 * npb + 4 * n,      # gather + own uc, p, s in; p, s out
         "k_cg_update": 6 * npb + 4 * n,                      # p, s, A, uc in; A, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
         "k_update": (5 * npb if dense else 8 * npb + 16 * nnz) + (n * p if masked else 0),
-        # dense mode (nnz = n(n-1)): matrices are n x n fp32
-        "kd_proj": 4 * n * n + 5 * npb + (n * p if masked else 0),
+        "kd_proj": (4 * npb if n <= 64 else 8 * n * n + 5 * npb) + (n * p if masked else 0),
         "kd_pairs": 2 * npb + (n * n // 2) * 12 + 4 * n * n,
         "kd_edges": 16 * n * n,
-        "kd_small": 4 * npb + (n * p if masked else 0),          # U, A', X in; A out (S and the slices are negligible)
     }[kernel]
 
 
-def alg_flops(kernel, n, p):
-    """Floating-point operations one launch must do (FMA = 2): the contraction S.A' and the direct pair
-    differences (sub, sub, 3 FMA per pair and column).  Zero for the streaming kernels."""
-    return {"kd_proj": 2.0 * n * n * p, "kd_pairs": 8.0 * (n * (n - 1) / 2) * p,
-            "kd_small": 3.0 * n * n * p + 8.0 * (n * (n - 1) / 2) * p}.get(kernel, 0.0)
+def alg_flops(kernel, n, p, dense_small):
+    """Algorithmic floating-point operations per launch (FMA = 2): the contraction S.A' 2 n^2 p, the pair
+    norms 6p per unordered pair; n <= 64: Gram-equivalent 2 n^2 p / 2 + contraction 2 n^2 p."""
+    if dense_small:
+        return {"kd_proj": 2.0 * n * n * p + 1.0 * n * n * p}.get(kernel, 0.0)
+    return {"kd_proj": 2.0 * n * n * p, "kd_pairs": 2.0 * (n * (n - 1) / 2) * p}.get(kernel, 0.0)
 
 
 def aggregate(dist, dev, times_ms, units):
@@ -247,7 +313,7 @@ def run_ours(args):
     if not dense:
         rowptr_h, col_h, w_h = rowptr.cpu().pin_memory(), col.cpu().pin_memory(), w.cpu().pin_memory()
     E = nnz // 2
-    prm = B.cc_default_params(use_graph=0 if args.eager else 1, dense=1 if dense else 0, reserved0=int(os.environ.get('CC_TUNE', '0')))
+    prm = B.cc_default_params(use_graph=0 if args.eager else 1, dense=1 if dense else 0)
     h = B.cc_create(n, p, X, M, rowptr, col, w, prm)
     for s in range(args.warmup):
         B.cc_solve(h, gamma_for_step(args.workload, s), 0.0, args.iters)
@@ -275,8 +341,6 @@ def run_ours(args):
     launches = B.cc_get_counts(h)["launches"] - launches0
     cg_per_it = prof["k_cg_spmv"]["calls"] / max(1, iters_done)
     prof = {k: v for k, v in prof.items() if v["calls"]}
-    if dense and n <= 64 and "kd_proj" in prof:      # n <= 64 runs the fused kd_small kernel in that timer slot
-        prof["kd_small"] = prof.pop("kd_proj")
 
     # ---- full gamma path (rank 0, N = 1): the other half of BASELINE.json's metric
     path = None
@@ -361,49 +425,94 @@ def run_ours(args):
         return
 
     peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    peaks = json.load(open(peaks_path)) if os.path.exists(peaks_path) else {}
+    if "hbm_gbs" in peaks:
+        peak, peak_src = float(peaks["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
     else:
         peak, peak_src = 6650.0, "B200_PROFILING.md fallback (of fallback)"
+    # TF32 tensor peak = measured bf16 cuBLAS peak x the nominal tf32/bf16 ratio (1.1 / 2.25), B200_PROFILING.md; the
+    # sustained figure, because the kernel is timed inside a long step
+    bf16 = float(peaks.get("bf16_tflops_sustained", peaks.get("bf16_tflops", 1400.0)))
+    tf32_peak = bf16 * 1.1 / 2.25
+    masked = M is not None
+    dense_small = dense and n <= 64
     tot_ns = sum(v["ns"] for v in prof.values()) or 1.0
-    top = max(prof, key=lambda k: prof[k]["ns"])
     per_kernel = {}
     for k, v in prof.items():
-        if v["calls"]:
-            dur = v["ns"] / v["calls"]
-            gbs = alg_bytes(k, n, p, nnz, M is not None, dense) / dur
-            tfl = alg_flops(k, n, p) / dur / 1e3
-            per_kernel[k] = {"share": v["ns"] / tot_ns, "us_per_launch": dur / 1e3, "launches": v["calls"],
-                             "alg_gbs": gbs, "frac": gbs / peak, "alg_tflops": tfl, "frac_fp32_alu": tfl / FP32_PEAK_TFLOPS}
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.txt")
+        dur = v["ns"] / v["calls"]
+        per_kernel[k] = {"share": v["ns"] / tot_ns, "us_per_launch": dur / 1e3, "launches": v["calls"],
+                         "impl_bytes": impl_bytes(k, n, p, nnz, masked, dense),
+                         "impl_gbs": impl_bytes(k, n, p, nnz, masked, dense) / dur}
+        fl = alg_flops(k, n, p, dense_small)
+        if fl:
+            per_kernel[k].update(alg_flops=fl, alg_tflops=fl / dur / 1e3)
+    # sweeps of SURVEY 8(d): bytes by its formulas, time = the sweep's kernels together, per launch of the first one
+    sweeps = {}
+    for name, (nbytes, kernels) in sweep_bytes(n, p, nnz, masked, dense).items():
+        if not all(k in prof for k in kernels):
+            continue
+        calls = prof[kernels[0]]["calls"]
+        ns = sum(prof[k]["ns"] for k in kernels)
+        sweeps[name] = {"kernels": list(kernels), "bytes_per_launch": nbytes, "us_per_launch": ns / calls / 1e3,
+                        "launches": calls, "share": ns / tot_ns, "alg_gbs": nbytes / (ns / calls), "frac": nbytes / (ns / calls) / peak}
+    it_us = 1e3 * ms / max(1, iters_done)
+    persistent = not sweeps           # small n: the whole solve is one persistent kernel (cc_persist.cu), no per-kernel marks
+    if persistent:
+        # SURVEY 8(d) bytes of one MM iteration with the projection by the precomputed inverse (Minv n x n + uc in, A out)
+        sb = sweep_bytes(n, p, nnz, masked, dense)
+        it_bytes = sb["a1_rhs"][0] + sb["a3_norms"][0] + sb["a5_update"][0] + 4 * n * n + 3 * 4 * n * p
+        sweeps["mm_iteration"] = {"kernels": ["k_mm_persist"], "bytes_per_launch": it_bytes, "us_per_launch": it_us,
+                                  "launches": iters_done, "share": 1.0, "alg_gbs": it_bytes / (it_us * 1e3),
+                                  "frac": it_bytes / (it_us * 1e3) / peak}
+    top = max(sweeps, key=lambda k: sweeps[k]["share"])
+    topk = sweeps[top]["kernels"][0]
+    it_bytes = sum(v["bytes_per_launch"] * v["launches"] for v in sweeps.values()) / max(1, iters_done)
+    per_iteration = {"bytes": it_bytes, "us": it_us, "alg_gbs": it_bytes / (it_us * 1e3), "frac": it_bytes / (it_us * 1e3) / peak,
+                     "note": "sum over the sweeps of SURVEY 8(d) bytes x launches / MM iterations, over the event-timed step"}
+    # DRAM and L2 bytes per launch of the dominant kernel: from the committed ncu capture (provenance in the file)
+    traffic = l2_bytes = tsrc = None
+    tpath = os.path.join(ROOT, "profiles", "r2_traffic.json")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(args.workload, {}).get(top)
-    alu_bound = per_kernel[top]["frac_fp32_alu"] > per_kernel[top]["frac"]
-    # kd_proj at n >= 128 runs on tcgen05 (kind::tf32, 3xTF32): report it against the TF32 tensor peak =
-    # measured bf16 cuBLAS peak x the nominal tf32/bf16 ratio (1.1 / 2.25), B200_PROFILING.md
-    if "kd_proj" in per_kernel and dense and n >= 128 and n % 4 == 0:
-        pk = json.load(open(peaks_path)).get("bf16_tflops", 1590.0) if os.path.exists(peaks_path) else 1590.0
+        tj = json.load(open(tpath))
+        ent = tj.get(args.workload, {}).get(topk)
+        if ent:
+            traffic, l2_bytes = ent.get("dram_bytes"), ent.get("lts_bytes")
+            tsrc = {"capture": ent.get("capture"), "date": ent.get("date"), "command": tj.get("_command")}
+    if dense and not dense_small and "kd_proj" in per_kernel:
+        # dense-weight: the bound is the tensor pipe; useful flops = 2 n^2 p (contraction) + n^2 p (pair Grams,
+        # symmetric) = 6p per unordered pair; 3xTF32 issues three MMAs per useful product (10 per K step in the pair kernel)
+        tens = {k: per_kernel[k] for k in ("kd_proj", "kd_pairs") if k in per_kernel}
+        fl_it = sum(v["alg_flops"] * v["launches"] for v in tens.values()) / max(1, iters_done)
+        for k, v in tens.items():
+            v["frac_tensor_useful"] = v["alg_tflops"] / tf32_peak
+        tk = max(tens, key=lambda k: tens[k]["share"])
+        roofline = {"bound": "tensor", "kernel": tk, "achieved": tens[tk]["alg_tflops"], "peak": tf32_peak, "unit": "TFLOP/s",
+                    "frac": tens[tk]["alg_tflops"] / tf32_peak, "traffic": traffic, "l2_bytes": l2_bytes, "traffic_source": tsrc,
+                    "peak_source": "TF32 = MEASURED_PEAKS.json bf16_tflops_sustained x 1.1/2.25 (nominal ratio; of measured)",
+                    "flops_per_launch": tens[tk]["alg_flops"],
+                    "per_iteration": {"flops": fl_it, "us": it_us, "alg_tflops": fl_it / it_us / 1e6, "frac": fl_it / it_us / 1e6 / tf32_peak,
+                                      "hbm": per_iteration},
+                    "note": "useful (algorithmic) flops; the 3xTF32 split issues 3 MMAs per product, so the tensor pipe is about 3x busier than frac says"}
+    elif dense_small:
+        # genotype-like: near the ridge: report against HBM (7 node arrays per iteration) and print the FP32 figure beside it
         v = per_kernel["kd_proj"]
-        v["bound"] = "tensor"
-        v["tf32_peak_tflops"] = pk * 1.1 / 2.25
-        v["frac_tensor"] = v["alg_tflops"] / v["tf32_peak_tflops"]
-        v["frac_tensor_3x"] = 3.0 * v["frac_tensor"]      # three TF32 MMAs are issued per useful product
-        if "kd_pairs" in per_kernel:                     # kd_pairs_tc: 10 TF32 MMAs of 2*128*128*8 flop per K step and tile
-            v2 = per_kernel["kd_pairs"]
-            v2["bound"] = "tensor"
-            v2["tf32_peak_tflops"] = v["tf32_peak_tflops"]
-            nt = (n + 127) // 128
-            v2["mma_tflops"] = 10.0 * 2 * 128 * 128 * p * (nt * (nt + 1) // 2) / (v2["us_per_launch"] * 1e6)
-            v2["frac_tensor_issued"] = v2["mma_tflops"] / v2["tf32_peak_tflops"]
-    roofline = {"bound": "alu" if alu_bound else "hbm", "kernel": top,
-                "achieved": per_kernel[top]["alg_tflops" if alu_bound else "alg_gbs"],
-                "peak": FP32_PEAK_TFLOPS if alu_bound else peak, "unit": "TFLOP/s" if alu_bound else "GB/s",
-                "frac": per_kernel[top]["frac_fp32_alu" if alu_bound else "frac"], "traffic": traffic,
-                "peak_source": "148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (guide unit counts; FFMA path)" if alu_bound else peak_src,
-                "bytes_per_launch": alg_bytes(top, n, p, nnz, M is not None, dense), "flops_per_launch": alg_flops(top, n, p),
-                "timing": "device %globaltimer marks inside the timed region (kernel + launch gap)",
-                "kernels": per_kernel, "device_ms_sum": tot_ns / 1e6}
+        roofline = {"bound": "hbm", "kernel": "kd_small_ws", "achieved": sweeps[top]["alg_gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": sweeps[top]["frac"], "traffic": traffic, "l2_bytes": l2_bytes, "traffic_source": tsrc, "peak_source": peak_src,
+                    "bytes_per_launch": sweeps[top]["bytes_per_launch"], "alg_tflops": v.get("alg_tflops"),
+                    "frac_fp32_alu": v.get("alg_tflops", 0.0) / FP32_PEAK_TFLOPS, "per_iteration": per_iteration}
+    else:
+        roofline = {"bound": "hbm", "kernel": "+".join(sweeps[top]["kernels"]), "sweep": top, "achieved": sweeps[top]["alg_gbs"],
+                    "peak": peak, "unit": "GB/s", "frac": sweeps[top]["frac"], "traffic": traffic, "l2_bytes": l2_bytes,
+                    "traffic_source": tsrc, "peak_source": peak_src, "bytes_per_launch": sweeps[top]["bytes_per_launch"],
+                    "per_iteration": per_iteration,
+                    "note": ("latency-bound configuration (SURVEY 8(d): roofline % is not meaningful here): the state lives in shared "
+                             "memory for the whole solve, one MM iteration = two grid barriers; the figure to read is us per iteration")
+                            if persistent else
+                            ("bytes are SURVEY 8(d)'s no-reuse algorithmic figures; the gathered arrays are L2-resident, so a fraction "
+                             "near or above 1 of the HBM copy peak reads as an L2-served gather (see traffic vs l2_bytes), not as HBM "
+                             "bandwidth")}
+    roofline.update(timing="device %globaltimer marks inside the timed region (kernel + launch gap)", sweeps=sweeps,
+                    kernels=per_kernel, device_ms_sum=tot_ns / 1e6)
 
     line = {"metric": "pair-updates/sec per MM iteration", "value": units / (ms / 1e3), "unit": "pair-updates/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
@@ -426,8 +535,7 @@ def run_ours(args):
         line["path"] = path
     if not args.no_cpu and world == 1:
         try:
-            _, info, _ = oracle_sample(args, 1, 0)
-            line["cpu_baseline"] = info
+            line["cpu_baseline"] = oracle_protocol(args, full=args.cpu_full)
         except Exception as ex:  # the baseline is reported, never required for the GPU number
             line["cpu_baseline"] = {"value": None, "unit": "pair-updates/s", "cores": os.cpu_count(), "kind": "oracle",
                                     "sample": f"failed: {ex}"}

@@ -138,17 +138,23 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
         return CC_OK;
     }
     CC_CUDA(h, cudaMemcpyAsync(h->sc, S, sizeof(cc_scal), cudaMemcpyHostToDevice, h->stream));
-    if (h->prm.use_graph) {
+    if (h->pt_slabs) {
+        // small n: the whole MM loop is one persistent kernel (cc_persist.cu)
+        int rc = ccp_solve(h);
+        if (rc != CC_OK) return rc;
+        CC_CUDA(h, cudaMemcpyAsync(S, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
+        CC_CUDA(h, cudaStreamSynchronize(h->stream));
+    } else if (h->prm.use_graph) {
         int rc = h->dense ? ccd_build_graph(h) : ccs_build_graph(h);
         if (rc != CC_OK) return rc;
         CC_CUDA(h, cudaGraphLaunch(h->gexec, h->stream));
         CC_CUDA(h, cudaMemcpyAsync(S, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
         CC_CUDA(h, cudaStreamSynchronize(h->stream));
-        h->launches += h->dense ? (h->dn_small ? 3LL : (h->dn_tc ? 10LL : 8LL)) * S->mm_iter : (h->Minv ? 4LL * S->mm_iter : 3LL * S->mm_iter + 2LL * S->cg_total);
     } else {
         int rc = h->dense ? ccd_solve_eager(h, maxit) : ccs_solve_eager(h, maxit);
         if (rc != CC_OK) return rc;
     }
+    h->launches += (long long)S->nlaunch;      // counted on the device: every kernel of the iteration that executed
     for (int k = 0; k < 8; ++k) { h->prof_ns[k] += S->prof_ns[k]; h->prof_calls[k] += S->prof_calls[k]; }
     if (iters_out) *iters_out = S->mm_iter;
     if (phi_out) *phi_out = S->phi;

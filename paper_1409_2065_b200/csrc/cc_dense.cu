@@ -21,7 +21,9 @@ namespace {
 
 // ---- column means of two node arrays, deterministic two-stage ------------------------------------
 __global__ void kd_colsum1(int n, int ld, int nslice, const float* __restrict__ U, const float* __restrict__ Ap,
-                           double* __restrict__ ps) {
+                           double* __restrict__ ps, cc_scal* sc) {
+    if (!sc->mm_active) return;
+    count_launch(sc);
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     const int sl = blockIdx.y;
     if (c >= ld) return;
@@ -36,8 +38,9 @@ __global__ void kd_colsum1(int n, int ld, int nslice, const float* __restrict__ 
 }
 
 __global__ void kd_colsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ ubar,
-                           float* __restrict__ abar, const cc_scal* sc) {
+                           float* __restrict__ abar, cc_scal* sc) {
     if (!sc->mm_active) return;
+    count_launch(sc);
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ld) return;
     double su = 0.0, sa = 0.0;
@@ -53,8 +56,9 @@ __global__ void kd_colsum2(int n, int ld, int nslice, const double* __restrict__
 // contraction leaves a residual of ~5e-7 (relative) per iteration in the column sums, which would add up along a
 // path of thousands of iterations.  k_update subtracts dbar from A, restoring the invariant every iteration.
 __global__ void kd_dsum1(int n, int ld, int nslice, const float* __restrict__ A, const float* __restrict__ U,
-                         double* __restrict__ ps, const cc_scal* sc) {
+                         double* __restrict__ ps, cc_scal* sc) {
     if (!sc->mm_active) return;
+    count_launch(sc);
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     const int sl = blockIdx.y;
     if (c >= ld) return;
@@ -64,8 +68,9 @@ __global__ void kd_dsum1(int n, int ld, int nslice, const float* __restrict__ A,
     ps[(size_t)sl * ld + c] = s;
 }
 
-__global__ void kd_dsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ dbar, const cc_scal* sc) {
+__global__ void kd_dsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ dbar, cc_scal* sc) {
     if (!sc->mm_active) return;
+    count_launch(sc);
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ld) return;
     double s = 0.0;
@@ -454,8 +459,9 @@ constexpr int TC2_SMEM = TC_NST * 2 * TC_SIDE + 1024;
 
 __global__ void __launch_bounds__(TC_THREADS) kd_prep_proj(int n, int ld, int nkb, const float* __restrict__ Ap,
                                                            const float* __restrict__ abar, uint8_t* __restrict__ Bpre,
-                                                           const cc_scal* sc) {
+                                                           cc_scal* sc) {
     if (!sc->mm_active) return;
+    count_launch(sc);
     const int kb = blockIdx.x, ct = blockIdx.y, tid = threadIdx.x;
     const int nl = tid & 127, kc0 = tid >> 7, gc = ct * TC_N + nl;
     const bool ok = gc < ld;
@@ -864,8 +870,9 @@ constexpr int PK2_SMEM = PK_NST * 2 * PK_SIDE + 1024;
 __global__ void __launch_bounds__(TC_THREADS) kd_prep_pairs(int n, int ld, int nkb, const float* __restrict__ A,
                                                             const float* __restrict__ Ap, const float* __restrict__ abar,
                                                             uint8_t* __restrict__ pre, float* __restrict__ nrm_part,
-                                                            int npad, const cc_scal* sc) {
+                                                            int npad, cc_scal* sc) {
     if (!sc->mm_active) return;
+    count_launch(sc);
     const int T = blockIdx.y, kb = blockIdx.x;
     const int tid = threadIdx.x, r = tid >> 2, kc = tid & 3;
     const int gi = T * TC_M + r, gc = kb * PK + kc * 4;
@@ -1795,7 +1802,7 @@ static const int kSliceDense = 32;
 
 void ccd_colmeans(cc_handle* h) {
     dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)kSliceDense);
-    kd_colsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->U, h->Ap, h->colps);
+    kd_colsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->U, h->Ap, h->colps, h->sc);
     kd_colsum2<<<(unsigned)((h->ld + 127) / 128), 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->colps,
                                                                       h->ubar, h->abar, h->sc);
 }
@@ -2019,7 +2026,6 @@ int ccd_solve_eager(cc_handle* h, int maxit) {
     for (int it = 0; it < maxit; ++it) {
         ccs_begin_iter(h);
         ccd_iteration(h);
-        h->launches += 7;
         CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
         CC_CUDA(h, cudaStreamSynchronize(h->stream));
         if (!h->sc_host->mm_active || h->sc_host->stop_pending) break;

@@ -100,6 +100,13 @@ __device__ __forceinline__ void prof_mark(S* sc, int id) {
     const unsigned long long now = global_ns();
     if (sc->t_last) { sc->prof_ns[id] += now - sc->t_last; sc->prof_calls[id] += 1; }
     sc->t_last = now;
+    atomicAdd(&sc->nlaunch, 1ULL);
+}
+
+// The kernels that carry no timer count themselves here (one thread of the grid calls it).
+template <typename S>
+__device__ __forceinline__ void count_launch(S* sc) {
+    if (blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) atomicAdd(&sc->nlaunch, 1ULL);
 }
 
 

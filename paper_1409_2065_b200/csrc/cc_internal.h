@@ -47,6 +47,7 @@ struct cc_scal {
     unsigned long long t_last;
     unsigned long long prof_ns[8];
     unsigned long long prof_calls[8];
+    unsigned long long nlaunch;   // kernels of this solve that executed (each counts itself on the device)
 };
 
 // Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
@@ -118,6 +119,11 @@ struct cc_handle {
     long long launches;
     unsigned long long prof_ns[8], prof_calls[8];   // accumulated over solves (cc_get_profile)
     int grid_nodes, grid_rows, grid_edges;   // launch sizes, fixed per handle (determinism)
+    // persistent single-kernel solve (cc_persist.cu): 0 slabs = not used by this handle
+    int pt_slabs, pt_sw, pt_minv_smem;
+    size_t pt_smem;
+    float* pt_nbpart;                 // pt_slabs x nnz partial squared norms
+    double* pt_spart;                 // pt_slabs x 4 partial scalars
     char err[256];
 };
 
@@ -133,6 +139,10 @@ void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out);
 int ccs_solve_eager(cc_handle* h, int maxit);
 int ccs_build_graph(cc_handle* h);
 int ccs_setup_inverse(cc_handle* h);
+
+// ---- cc_persist.cu: one persistent kernel per solve for small-n problems (n <= CC_INV_NMAX, state in shared memory)
+int ccp_setup(cc_handle* h);
+int ccp_solve(cc_handle* h);
 
 // ---- cc_dense.cu (a9) ------------------------------------------------------------------------------
 int ccd_setup(cc_handle* h, const float* W);

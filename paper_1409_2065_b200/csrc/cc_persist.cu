@@ -1,0 +1,387 @@
+// cc_persist.cu -- the whole MM loop of one cc_solve as ONE persistent kernel, for problems whose projection uses
+// the precomputed inverse (n <= CC_INV_NMAX) and whose state fits in shared memory: `tiny`, `expression`, and the
+// small instances of every test.  PAPER.md L202 is this regime: the paper's own GPU code lost to its CPU code on
+// POPRES because of per-step overheads; here a kernel node inside the CUDA graph's WHILE loops costs ~5 us and an
+// MM iteration was four of them (30 us on `tiny`, 57 us on `expression`).
+//
+// Decomposition: the columns are cut into slabs of `sw` columns, one CTA per slab, all CTAs co-resident (cooperative
+// launch).  Every step of the iteration is separable over columns -- the right-hand side (L100), the projection
+// A = U + Minv (D^-1 r0) (L90-L103), the U update (L82, L116) -- except the pair norms ||b_ij||^2 (a sum over the
+// columns, L84/L86) and the scalars dist^2, loss, penalty (L76, L64-L66).  So a CTA keeps its slab of X, U, A', A in
+// shared memory for the whole solve and one MM iteration needs two grid-wide barriers:
+//   phase 1 (local)  r0, A, the slab's share of every ||b_ij||^2 and of dist^2 / loss / penalty  -> global partials
+//   ---- barrier A ----
+//   phase 2          every CTA adds the scalar partials in the same fixed order -> d_m, Phi_m, stop rule (S3), the
+//                    update coefficients; each CTA adds the norm partials of ITS share of the pairs, shrinks them
+//                    (L86-L88) and writes s, ||v||; U update of the slab, A' <- A
+//   ---- barrier B ----   (the new shrink factors are visible to everybody)
+// No atomics on data, every sum in a fixed order: results are reproducible run to run.  With one slab (`tiny`) the
+// barriers are plain __syncthreads.
+#include <cstdio>
+
+#include "cc_device.cuh"
+#include "cc_internal.h"
+
+namespace {
+
+constexpr int PT_THREADS = 512;
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// Grid-wide barrier over co-resident CTAs: a monotone arrival counter (zeroed by the host with the control block).
+__device__ __forceinline__ void grid_barrier(unsigned* ctr, unsigned& target, unsigned nblk) {
+    __syncthreads();
+    if (nblk > 1) {
+        if (threadIdx.x == 0) {
+            target += nblk;
+            __threadfence();                    // release the CTA's writes (cumulative over the __syncthreads above)
+            atomicAdd(ctr, 1u);
+            while (ld_acquire_u32(ctr) < target) { }
+            __threadfence();
+        }
+        __syncthreads();
+    }
+}
+
+// block-wide sums of NV doubles, fixed order; the totals are valid in thread 0
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double (*sm)[PT_THREADS / 32]) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        double x = v[k];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+        if (lane == 0) sm[k][wid] = x;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            double x = 0.0;
+            for (int w2 = 0; w2 < PT_THREADS / 32; ++w2) x += sm[k][w2];
+            v[k] = x;
+        }
+    }
+}
+
+struct pt_ctl {
+    float cu, ca, cthr;
+    int stop;
+};
+
+template <bool MINV_SMEM>
+__global__ void __launch_bounds__(PT_THREADS, 1)
+k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, const int* __restrict__ rowup,
+             const int* __restrict__ col, const int* __restrict__ peer, const float* __restrict__ w, float* s, float* vn,
+             float* nb2, const float* __restrict__ dinv, const float* __restrict__ Minv, const float* __restrict__ X,
+             const uint8_t* __restrict__ mask, float* U, float* A, float* Ap, cc_scal* sc, float* nbpart, double* spart,
+             double* hist_phi, double* hist_d) {
+    extern __shared__ __align__(16) unsigned char pt_smem[];
+    __shared__ double red_s[3][PT_THREADS / 32];
+    __shared__ pt_ctl ctl;
+    const int tid = threadIdx.x, c = blockIdx.x, nslab = gridDim.x;
+    const int c0 = c * sw;
+    const int wq = (min(sw, ld - c0)) >> 2;              // float4 quads of this slab (ld and sw are multiples of 4)
+    const int npairs = nnz >> 1;
+    // ---- carve shared memory
+    float* Xs = reinterpret_cast<float*>(pt_smem);
+    float* Us = Xs + (size_t)n * sw;
+    float* Ps = Us + (size_t)n * sw;                     // A' (the previous projection)
+    float* As = Ps + (size_t)n * sw;
+    float* Cs = As + (size_t)n * sw;                     // D^-1 r0
+    float* ss = Cs + (size_t)n * sw;                     // shrink factors, all directed entries
+    float* Mv = ss + ((nnz + 3) & ~3);                   // Minv (n x n) when it fits
+    int* plist = reinterpret_cast<int*>(Mv + (MINV_SMEM ? (size_t)n * n : 0));   // upper entries (col > row), in order
+    unsigned short* cols = reinterpret_cast<unsigned short*>(plist + npairs);
+    unsigned short* rows = cols + nnz;
+    uint8_t* Ms = reinterpret_cast<uint8_t*>(rows + nnz);    // mask slab, if any (nnz is even: 4-byte aligned)
+
+    // ---- one-time loads
+    for (int it = tid; it < n * wq; it += PT_THREADS) {
+        const int i = it / wq, q = it - i * wq;
+        const size_t g = (size_t)i * ld + c0 + 4 * q;
+        const int o = i * sw + 4 * q;
+        st4(Xs + o, ld4s(X + g));
+        st4(Us + o, ld4s(U + g));
+        st4(Ps + o, ld4s(Ap + g));
+        if (mask) *reinterpret_cast<uchar4*>(Ms + o) = *reinterpret_cast<const uchar4*>(mask + g);
+    }
+    if (MINV_SMEM)
+        for (int t = tid; t < n * n; t += PT_THREADS) Mv[t] = Minv[t];
+    for (int i = tid; i < n; i += PT_THREADS) {
+        const int rs = rowptr[i], re = rowptr[i + 1];
+        for (int e = rs; e < re; ++e) {
+            cols[e] = (unsigned short)col[e];
+            rows[e] = (unsigned short)i;
+        }
+    }
+    __syncthreads();
+    // upper entries in entry order: entry e is upper iff cols[e] > rows[e]; its slot = number of upper entries before it.
+    // One thread per row counts its lower entries; a serial prefix over n <= 384 rows by thread 0 is cheap and runs once.
+    __shared__ int pbase[CC_INV_NMAX + 1];
+    if (tid == 0) {
+        int acc = 0;
+        for (int i = 0; i < n; ++i) { pbase[i] = acc; acc += rowptr[i + 1] - rowup[i]; }
+        pbase[n] = acc;
+    }
+    __syncthreads();
+    for (int i = tid; i < n; i += PT_THREADS) {
+        const int ru = rowup[i], re = rowptr[i + 1];
+        for (int e = ru; e < re; ++e) plist[pbase[i] + (e - ru)] = e;
+    }
+    for (int e = tid; e < nnz; e += PT_THREADS) ss[e] = s[e];
+    __syncthreads();
+
+    // ---- control (identical in every CTA)
+    const double gamma = sc->gamma, rho = sc->rho, eps = sc->eps, tol = sc->tol;
+    const int maxit = sc->mm_maxit, min_it = sc->mm_min_it, hist_cap = sc->hist_cap;
+    unsigned* bar = &sc->ticket[7];
+    unsigned target = 0;
+    double phi_prev = 0.0, phi = 0.0, d = sqrt(eps), dist2_t = 0.0, loss_t = 0.0, pen_t = 0.0;
+    // this CTA's share of the pairs (phase 2): a contiguous range of plist
+    const int k0 = (int)((long long)npairs * c / nslab), k1 = (int)((long long)npairs * (c + 1) / nslab);
+    int m = 0;
+    for (; m < maxit; ++m) {
+        // ===== phase 1a: D^-1 r0,  r0_i = sum_j [ s_ij (a'_i - a'_j) - (u_i - u_j) ]   (L100 minus (I+L) u, warm start z = u)
+        for (int it = tid; it < n * wq; it += PT_THREADS) {
+            const int i = it / wq, q = it - i * wq;
+            const int o = i * sw + 4 * q;
+            const float4 api = ld4s(Ps + o), ui = ld4s(Us + o);
+            float4 acc = f4(0.f);
+            const int rs = rowptr[i], re = rowptr[i + 1];
+            for (int e = rs; e < re; ++e) {
+                const int oj = (int)cols[e] * sw + 4 * q;
+                acc = fma4(ss[e], api - ld4s(Ps + oj), acc);
+                acc = acc - (ui - ld4s(Us + oj));
+            }
+            st4(Cs + o, __ldg(dinv + i) * acc);
+        }
+        __syncthreads();
+        // ===== phase 1b: A = U + Minv (D^-1 r0)   (the projection, L90-L103, by the inverse formed once in cc_create)
+        for (int it = tid; it < n * wq; it += PT_THREADS) {
+            const int i = it / wq, q = it - i * wq;
+            float4 acc0 = f4(0.f), acc1 = f4(0.f);
+            int j = 0;
+            for (; j + 1 < n; j += 2) {
+                acc0 = fma4(MINV_SMEM ? Mv[i * n + j] : __ldg(Minv + (size_t)i * n + j), ld4s(Cs + j * sw + 4 * q), acc0);
+                acc1 = fma4(MINV_SMEM ? Mv[i * n + j + 1] : __ldg(Minv + (size_t)i * n + j + 1), ld4s(Cs + (j + 1) * sw + 4 * q), acc1);
+            }
+            if (j < n) acc0 = fma4(MINV_SMEM ? Mv[i * n + j] : __ldg(Minv + (size_t)i * n + j), ld4s(Cs + j * sw + 4 * q), acc0);
+            const int o = i * sw + 4 * q;
+            st4(As + o, ld4s(Us + o) + (acc0 + acc1));
+        }
+        __syncthreads();
+        // ===== phase 1c: the slab's share of ||u - a||^2, the loss, every ||b_ij||^2 and ||v_ij - b_ij||^2, the penalty
+        double red[3] = {0.0, 0.0, 0.0};      // dist^2, loss, penalty
+        {
+            float dl = 0.f, ls = 0.f;
+            for (int it = tid; it < n * wq; it += PT_THREADS) {
+                const int i = it / wq, q = it - i * wq;
+                const int o = i * sw + 4 * q;
+                const float4 u = ld4s(Us + o);
+                const float4 t = u - ld4s(As + o);
+                float4 qx = ld4s(Xs + o) - u;
+                if (mask) {
+                    const uchar4 mk = *reinterpret_cast<const uchar4*>(Ms + o);
+                    qx.x = mk.x ? qx.x : 0.f; qx.y = mk.y ? qx.y : 0.f; qx.z = mk.z ? qx.z : 0.f; qx.w = mk.w ? qx.w : 0.f;
+                }
+                dl += dot4(t, t);
+                ls += dot4(qx, qx);
+            }
+            red[0] += (double)dl;
+            red[1] += (double)ls;
+        }
+        for (int k = tid; k < npairs; k += PT_THREADS) {
+            const int e = plist[k];
+            const int oi = (int)rows[e] * sw, oj = (int)cols[e] * sw;
+            const float se = ss[e];
+            float nbp = 0.f, dv = 0.f;
+            for (int q = 0; q < wq; ++q) {
+                const float4 b = ld4s(As + oi + 4 * q) - ld4s(As + oj + 4 * q);
+                const float4 bp = ld4s(Ps + oi + 4 * q) - ld4s(Ps + oj + 4 * q);
+                const float4 vb = fma4(se, bp, f4(0.f)) - b;
+                nbp += dot4(b, b);
+                dv += dot4(vb, vb);
+            }
+            if (nslab > 1) __stcg(nbpart + (size_t)c * nnz + e, nbp);
+            else nbpart[e] = nbp;
+            red[0] += (double)dv;
+        }
+        for (int k = k0 + tid; k < k1; k += PT_THREADS) {
+            const int e = plist[k];
+            red[2] += (double)(__ldg(w + e) * __ldcg(vn + e));
+        }
+        block_sum<3>(red, red_s);
+        if (tid == 0) {
+            __stcg(spart + (size_t)c * 4 + 0, red[0]);
+            __stcg(spart + (size_t)c * 4 + 1, red[1]);
+            __stcg(spart + (size_t)c * 4 + 2, red[2]);
+        }
+        grid_barrier(bar, target, nslab);
+        // ===== phase 2: scalars (every CTA, same order), stop rule S3, coefficients
+        if (tid < 32) {
+            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
+            for (int b = tid; b < nslab; b += 32) {
+                a0 += __ldcg(spart + (size_t)b * 4 + 0);
+                a1 += __ldcg(spart + (size_t)b * 4 + 1);
+                a2 += __ldcg(spart + (size_t)b * 4 + 2);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                a0 += __shfl_xor_sync(0xffffffffu, a0, o);
+                a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+                a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+            }
+            if (tid == 0) {
+                dist2_t = a0; loss_t = a1; pen_t = a2;
+                d = sqrt(a0 + eps);                                  // L76
+                phi = 0.5 * a1 + gamma * a2 + rho * d;               // L64-L66, L109
+                int stop = (m + 1 >= maxit) ? 1 : 0;
+                if (tol > 0.0 && m + 1 >= min_it && m >= 1 && phi_prev - phi <= tol * (1.0 + fabs(phi_prev))) stop = 1;
+                phi_prev = phi;
+                ctl.cu = (float)(d / (d + rho));
+                ctl.ca = (float)(rho / (d + rho));
+                ctl.cthr = (float)(gamma * d / rho);
+                ctl.stop = stop;
+                if (c == 0 && m < hist_cap) { hist_phi[m] = phi; hist_d[m] = d; }
+            }
+        }
+        __syncthreads();
+        const float cu = ctl.cu, ca = ctl.ca, cthr = ctl.cthr;
+        const int stop = ctl.stop;
+        // ===== phase 2: this CTA's pairs -- add the slabs' partial norms in order, block soft-threshold (L86-L88, S6)
+        for (int k = k0 + tid; k < k1; k += PT_THREADS) {
+            const int e = plist[k], pe = __ldg(peer + e);
+            float q = 0.f;
+            if (nslab > 1) {
+                int b = 0;
+                for (; b + 4 <= nslab; b += 4) {
+                    const float v0 = __ldcg(nbpart + (size_t)b * nnz + e), v1 = __ldcg(nbpart + (size_t)(b + 1) * nnz + e);
+                    const float v2 = __ldcg(nbpart + (size_t)(b + 2) * nnz + e), v3 = __ldcg(nbpart + (size_t)(b + 3) * nnz + e);
+                    q = (((q + v0) + v1) + v2) + v3;
+                }
+                for (; b < nslab; ++b) q += __ldcg(nbpart + (size_t)b * nnz + e);
+            } else {
+                q = nbpart[e];
+            }
+            const float nb = sqrtf(q);
+            const float thr = cthr * __ldg(w + e);
+            const float sn = nb <= thr ? 0.f : 1.f - thr / nb;
+            s[e] = sn; s[pe] = sn;
+            vn[e] = sn * nb; vn[pe] = sn * nb;
+            nb2[e] = q; nb2[pe] = q;
+        }
+        // ===== phase 2: U update (L82, L116), A' <- A
+        for (int it = tid; it < n * wq; it += PT_THREADS) {
+            const int i = it / wq, q = it - i * wq;
+            const int o = i * sw + 4 * q;
+            const float4 a = ld4s(As + o), u = ld4s(Us + o);
+            float4 y = ld4s(Xs + o);
+            if (mask) {
+                const uchar4 mk = *reinterpret_cast<const uchar4*>(Ms + o);
+                y.x = mk.x ? y.x : u.x; y.y = mk.y ? y.y : u.y; y.z = mk.z ? y.z : u.z; y.w = mk.w ? y.w : u.w;
+            }
+            st4(Us + o, fma4(cu, y, ca * a));
+            st4(Ps + o, a);
+        }
+        grid_barrier(bar, target, nslab);
+        if (stop) { ++m; break; }
+        for (int e = tid; e < nnz; e += PT_THREADS) ss[e] = __ldcg(s + e);
+        __syncthreads();
+    }
+    // ---- state back to global memory (what cc_get_U, cc_clusters and the next solve read)
+    for (int it = tid; it < n * wq; it += PT_THREADS) {
+        const int i = it / wq, q = it - i * wq;
+        const size_t g = (size_t)i * ld + c0 + 4 * q;
+        const int o = i * sw + 4 * q;
+        st4(U + g, ld4s(Us + o));
+        st4(Ap + g, ld4s(Ps + o));
+        if (m > 0) st4(A + g, ld4s(As + o));
+    }
+    if (c == 0 && tid == 0) {
+        sc->mm_iter = m;
+        sc->dist2 = dist2_t; sc->loss = loss_t; sc->pen = pen_t;
+        sc->d = d; sc->d_prev = d;
+        sc->phi = phi; sc->phi_prev = phi_prev;
+        sc->cu = ctl.cu; sc->ca = ctl.ca; sc->cthr = ctl.cthr;
+        sc->stop_pending = 1;
+        sc->mm_active = 0;
+        atomicAdd(&sc->nlaunch, 1ULL);
+    }
+}
+
+}  // namespace
+
+// ---- host side -----------------------------------------------------------------------------------------------------
+static size_t persist_smem(const cc_handle* h, int sw, int minv_in_smem) {
+    const size_t n = (size_t)h->n, nnz = (size_t)h->nnz;
+    size_t b = 5 * n * sw * sizeof(float) + ((nnz + 3) & ~(size_t)3) * sizeof(float);
+    if (minv_in_smem) b += n * n * sizeof(float);
+    b += (nnz / 2) * sizeof(int) + 2 * nnz * sizeof(unsigned short);
+    if (h->mask) b += n * sw;
+    return b + 16;
+}
+
+// Decide whether this handle runs the persistent kernel, and with which slab width.  Called once from cc_create after
+// the inverse exists.  Leaves h->pt_slabs = 0 when the handle stays on the CUDA-graph path.
+int ccp_setup(cc_handle* h) {
+    h->pt_slabs = 0;
+    if (h->dense || !h->Minv || !h->prm.use_graph || h->n > 65535) return CC_OK;
+    int dev = 0, coop = 0, maxsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) {
+        cudaGetLastError();
+        return CC_OK;
+    }
+    cudaDeviceGetAttribute(&maxsm, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    // slab width: enough columns that the n x n x sw products of the projection outweigh a barrier (~64k FMA), and at
+    // least ld / #SM so that the slabs fit the GPU in one co-resident wave
+    const long long n = h->n, ld = h->ld;
+    long long sw = (65536 + n * n - 1) / (n * n);
+    const long long per_sm = (ld + h->sms - 1) / h->sms;
+    if (sw < per_sm) sw = per_sm;
+    sw = (sw + 3) / 4 * 4;
+    if (sw > ld) sw = ld;
+    for (;; sw += 4) {            // shrink nothing: a wider slab only lowers the CTA count; stop when it cannot fit
+        const int nslab = (int)((ld + sw - 1) / sw);
+        int minv_smem = 1;
+        size_t need = persist_smem(h, (int)sw, 1);
+        if (need > (size_t)maxsm) { minv_smem = 0; need = persist_smem(h, (int)sw, 0); }
+        if (need > (size_t)maxsm) return CC_OK;            // does not fit at the narrowest admissible slab: graph path
+        if (nslab > h->sms) { if (sw >= ld) return CC_OK; continue; }
+        const void* fn = minv_smem ? (const void*)k_mm_persist<true> : (const void*)k_mm_persist<false>;
+        if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need) != cudaSuccess) {
+            cudaGetLastError();
+            return CC_OK;
+        }
+        int occ = 0;
+        if ((minv_smem ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<true>, PT_THREADS, need)
+                       : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<false>, PT_THREADS, need)) != cudaSuccess || occ < 1) {
+            cudaGetLastError();
+            return CC_OK;
+        }
+        h->pt_slabs = nslab;
+        h->pt_sw = (int)sw;
+        h->pt_minv_smem = minv_smem;
+        h->pt_smem = need;
+        break;
+    }
+    cudaError_t e = cc_dev_alloc((void**)&h->pt_nbpart, (size_t)h->pt_slabs * (h->nnz ? h->nnz : 1) * sizeof(float), h->stream);
+    if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->pt_spart, (size_t)h->pt_slabs * 4 * sizeof(double), h->stream);
+    if (e != cudaSuccess) { cudaGetLastError(); h->pt_slabs = 0; }
+    return CC_OK;
+}
+
+int ccp_solve(cc_handle* h) {
+    int n = (int)h->n, ld = (int)h->ld, sw = h->pt_sw, nnz = (int)h->nnz;
+    void* args[] = {&n, &ld, &sw, &nnz, &h->rowptr, &h->rowup, &h->col, &h->peer, &h->w, &h->s, &h->vn, &h->nb2,
+                    &h->dinv, &h->Minv, &h->X, &h->mask, &h->U, &h->A, &h->Ap, &h->sc, &h->pt_nbpart, &h->pt_spart,
+                    &h->hist_phi, &h->hist_d};
+    CC_CUDA(h, cudaLaunchCooperativeKernel(h->pt_minv_smem ? (const void*)k_mm_persist<true> : (const void*)k_mm_persist<false>, dim3((unsigned)h->pt_slabs), dim3(PT_THREADS), args,
+                                           h->pt_smem, h->stream));
+    return CC_OK;
+}

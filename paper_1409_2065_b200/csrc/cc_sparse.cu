@@ -515,6 +515,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
 // One thread: eager-mode bookkeeping between iterations (the WHILE node does this in graph mode).
 __global__ void k_begin_iter(cc_scal* sc) {
     if (sc->stop_pending) sc->mm_active = 0;
+    else count_launch(sc);
 }
 
 // Cold start of the pair state (S4: V0 = D U0, i.e. s = 1, ||v_ij|| = ||u0_i - u0_j||), and the pair
@@ -641,8 +642,7 @@ int ccs_solve_eager(cc_handle* h, int maxit) {
     for (int it = 0; it < maxit; ++it) {
         ccs_begin_iter(h);
         ccs_rhs(h);
-        h->launches += 2;
-        if (h->Minv) { ccs_apply_inv(h); h->launches += 1; }
+        if (h->Minv) ccs_apply_inv(h);
         for (; !h->Minv;) {
             CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
             CC_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -651,11 +651,9 @@ int ccs_solve_eager(cc_handle* h, int maxit) {
                 ccs_cg_spmv(h);
                 ccs_cg_update(h);
             }
-            h->launches += 2;  // counted below from cg_total for the ones that did work
         }
         ccs_norm(h);
         ccs_update(h);
-        h->launches += 2;
         CC_CUDA(h, cudaMemcpyAsync(h->sc_host, h->sc, sizeof(cc_scal), cudaMemcpyDeviceToHost, h->stream));
         CC_CUDA(h, cudaStreamSynchronize(h->stream));
         if (!h->sc_host->mm_active || h->sc_host->stop_pending) break;

@@ -211,6 +211,33 @@ def test_graph_and_eager_launch_modes_are_bit_identical_and_deterministic(B, tor
     assert np.array_equal(outs[0], outs[2])
 
 
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("expression", dict(n=40, p=301)), ("expression", dict(n=100, p=2000))])
+def test_persistent_kernel_and_stream_kernels_agree(B, torch_, oracle, name, kw):
+    """Small n: cc_solve runs the whole MM loop as one persistent kernel (column slabs in shared memory, two grid
+    barriers per iteration); prm.use_graph = 0 drives the separate stream kernels from the host.  Different summation
+    orders, same iteration: both within the tolerance of the oracle, and within 1e-5 of each other, labels equal."""
+    torch = torch_
+    wl = synth.make(name, **kw)
+    prob = H.build_problem(oracle, wl)
+    gammas, iters = ([1.0, 100.0, 1000.0], 120) if name == "tiny" else ([0.5, 5.0, 50.0], 60)
+    ref = H.oracle_path(oracle, prob, gammas, iters)
+    outs, labs = [], []
+    for use_graph in (1, 0):
+        h = H.gpu_create(B, torch, prob, use_graph=use_graph)
+        U = torch.empty(wl.n, wl.p, device="cuda:0")
+        lab = torch.empty(wl.n, dtype=torch.int32, device="cuda:0")
+        for g, r in zip(gammas, ref):
+            it, _, _ = B.cc_solve(h, g, 0.0, iters)
+            assert it == iters
+            B.cc_get_U(h, -1, U)
+            _, k = B.cc_clusters(h, -1, lab)
+            assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, (use_graph, g)
+            assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (use_graph, g)
+        outs.append(U.cpu().numpy().astype(np.float64))
+        B.cc_destroy(h)
+    assert H.relerr(outs[0], outs[1]) <= 1e-5
+
+
 def test_stop_rule_matches_oracle(B, torch_, oracle):
     """tol > 0 (reading S3): the GPU stops at (nearly) the oracle's iteration."""
     torch = torch_
@@ -600,6 +627,41 @@ def test_full_size_dense_weight_properties(B, torch_):
         outs.append(U.double())
         B.cc_destroy(h)
     assert ((outs[0] - outs[1]).norm() / outs[1].norm()).item() <= 1e-5
+
+
+def test_dense_weight_p256_against_oracle(B, torch_, oracle):
+    """configs[4]'s generator at its real width p = 256 (16 K steps per tensor-core tile pass) and n = 2048 (16 row
+    tiles, 136 pair tiles): the oracle's explicit V still fits (2.1 M pairs x 256 x 8 B = 4.3 GB).  Element-wise
+    against the oracle along a short path; kappa = 0.1 (a parameter of the iteration, the same on both sides) lets
+    the short run reach fusion, so that the labels are compared on fused pairs too."""
+    torch = torch_
+    n, p = 2048, 256
+    wl = synth.make("dense_weight", n=n, p=p, n_clusters=32)
+    prob = H.build_problem(oracle, wl)
+    assert len(prob["ei"]) == n * (n - 1) // 2
+    gammas = [80.0, 160.0, 320.0]
+    ref = H.oracle_path(oracle, prob, gammas, 4, proj_method=1, kappa=0.1)
+    dev = torch.device("cuda:0")
+    W = np.zeros((n, n), np.float32)
+    W[prob["ei"], prob["ej"]] = prob["w64"].astype(np.float32)
+    W = W + W.T
+    h = B.cc_create(n, p, torch.from_numpy(wl.X).to(dev), None, None, None, torch.from_numpy(W).to(dev),
+                    B.cc_default_params(dense=1, kappa=0.1))
+    U = torch.empty(n, p, device=dev)
+    lab = torch.empty(n, dtype=torch.int32, device=dev)
+    ks = []
+    for g, r in zip(gammas, ref):
+        B.cc_solve(h, g, 0.0, 4)
+        B.cc_get_U(h, -1, U)
+        _, k = B.cc_clusters(h, -1, lab)
+        ph, dd = B.cc_get_history(h)
+        assert H.relerr(U.cpu().numpy().astype(np.float64), r["U"]) <= TOL, g
+        assert k == r["nclusters"] and np.array_equal(lab.cpu().numpy(), r["labels"]), (g, k, r["nclusters"])
+        assert np.allclose(ph, r["phi"], rtol=1e-4) and np.allclose(dd, r["d"], rtol=5e-4), g
+        ks.append(k)
+    B.cc_destroy(h)
+    print("dense p=256 n=2048: clusters along the path", ks)
+    assert ks[-1] < n
 
 
 def test_dense_n8192_against_oracle_small_p(B, torch_, oracle):

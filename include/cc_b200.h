@@ -235,8 +235,13 @@ int cc_get_stats(cc_handle* h, double* rho, double* eps, int64_t* proj_iters, do
  * 1 k_cg_spmv (a2), 2 k_cg_update (a2), 3 k_norm (a3+a6), 4 k_update (a5+a4); dense mode (a9): 5 kd_proj
  * (with the column means), 6 kd_pairs, 7 kd_edges.  Measured on the device:
  * the block that finishes a kernel last reads %globaltimer and the interval since the previous kernel
- * finished (= this kernel plus its launch gap) is charged to it.  Either pointer may be NULL. */
+ * finished (= this kernel plus its launch gap) is charged to it.  Either pointer may be NULL.
+ * Handles that run the persistent single-kernel solve (small n, see cc_solve) report its PHASES per MM iteration
+ * instead, and only after cc_reset_profile has been called once (reading the timer costs about 0.5 us a lap, several
+ * laps per iteration, so it is off by default): 0 right-hand side, 2 projection by the inverse, 3 pair norms and
+ * partial sums, 4 shrink and U update, 5 / 6 the two grid barriers.  Diagnostics only; not part of the iteration. */
 int cc_get_profile(cc_handle* h, double* ns_out, int64_t* calls_out);
+/* Zero the accumulated times (and switch the persistent kernel's phase timing on for this handle). */
 int cc_reset_profile(cc_handle* h);
 
 /* Back to the cold start (S4); snapshots are dropped. */

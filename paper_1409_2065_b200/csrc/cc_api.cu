@@ -132,6 +132,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
     S->mm_active = 1;
     S->cg_maxit = h->prm.proj_maxit;
     S->hist_cap = h->prm.hist_cap;
+    S->prof_phases = h->pt_prof;
     if (maxit == 0) {
         if (iters_out) *iters_out = 0;
         if (phi_out) *phi_out = NAN;
@@ -343,6 +344,7 @@ int cc_reset_profile(cc_handle* h) {
     if (!h) return CC_EINVAL;
     memset(h->prof_ns, 0, sizeof(h->prof_ns));
     memset(h->prof_calls, 0, sizeof(h->prof_calls));
+    h->pt_prof = 1;      // from now on the persistent kernel times its phases too (see cc_b200.h)
     return CC_OK;
 }
 

@@ -48,6 +48,8 @@ struct cc_scal {
     unsigned long long prof_ns[8];
     unsigned long long prof_calls[8];
     unsigned long long nlaunch;   // kernels of this solve that executed (each counts itself on the device)
+    int32_t prof_phases;          // persistent kernel: time its phases (reading %globaltimer costs ~0.5 us a lap; off by default)
+    int32_t pad1;
 };
 
 // Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
@@ -120,7 +122,7 @@ struct cc_handle {
     unsigned long long prof_ns[8], prof_calls[8];   // accumulated over solves (cc_get_profile)
     int grid_nodes, grid_rows, grid_edges;   // launch sizes, fixed per handle (determinism)
     // persistent single-kernel solve (cc_persist.cu): 0 slabs = not used by this handle
-    int pt_slabs, pt_sw, pt_minv_smem;
+    int pt_slabs, pt_sw, pt_minv_smem, pt_prof;
     size_t pt_smem;
     float* pt_nbpart;                 // pt_slabs x nnz partial squared norms
     double* pt_spart;                 // pt_slabs x 4 partial scalars

@@ -76,7 +76,7 @@ struct pt_ctl {
 
 template <bool MINV_SMEM>
 __global__ void __launch_bounds__(PT_THREADS, 1)
-k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, const int* __restrict__ rowup,
+k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ rowptr, const int* __restrict__ rowup,
              const int* __restrict__ col, const int* __restrict__ peer, const float* __restrict__ w, float* s, float* vn,
              float* nb2, const float* __restrict__ dinv, const float* __restrict__ Minv, const float* __restrict__ X,
              const uint8_t* __restrict__ mask, float* U, float* A, float* Ap, cc_scal* sc, float* nbpart, double* spart,
@@ -89,30 +89,42 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
     const int wq = (min(sw, ld - c0)) >> 2;              // float4 quads of this slab (ld and sw are multiples of 4)
     const int npairs = nnz >> 1;
     // ---- carve shared memory
+    // rows of a slab are `rs_` floats apart: sw, or sw + 4 when sw / 4 is even, so that rs_ / 4 is odd and rows r .. r+7 at
+    // the same quad fall into 8 different 16-byte bank groups (the pair loop reads rows scattered over the slab)
     float* Xs = reinterpret_cast<float*>(pt_smem);
-    float* Us = Xs + (size_t)n * sw;
-    float* Ps = Us + (size_t)n * sw;                     // A' (the previous projection)
-    float* As = Ps + (size_t)n * sw;
-    float* Cs = As + (size_t)n * sw;                     // D^-1 r0
-    float* ss = Cs + (size_t)n * sw;                     // shrink factors, all directed entries
-    float* Mv = ss + ((nnz + 3) & ~3);                   // Minv (n x n) when it fits
-    int* plist = reinterpret_cast<int*>(Mv + (MINV_SMEM ? (size_t)n * n : 0));   // upper entries (col > row), in order
+    float* Us = Xs + (size_t)n * rs_;
+    float* Ps = Us + (size_t)n * rs_;                    // A' (the previous projection)
+    float* As = Ps + (size_t)n * rs_;
+    float* Cs = As + (size_t)n * rs_;                    // D^-1 r0
+    float* ss = Cs + (size_t)n * rs_;                    // shrink factors, all directed entries
+    const int n4 = (n + 3) & ~3;
+    float* Mv = ss + ((nnz + 3) & ~3);                   // Minv TRANSPOSED, n rows of n4 floats (rows i >= n of a column: 0), when it fits
+    int* plist = reinterpret_cast<int*>(Mv + (MINV_SMEM ? (size_t)n * n4 : 0));   // upper entries (col > row), in order
     unsigned short* cols = reinterpret_cast<unsigned short*>(plist + npairs);
     unsigned short* rows = cols + nnz;
     uint8_t* Ms = reinterpret_cast<uint8_t*>(rows + nnz);    // mask slab, if any (nnz is even: 4-byte aligned)
+    // one slab (the whole problem in this CTA): per-pair ||b||^2, ||v|| and w live in shared memory too and the loop never
+    // touches global memory; s, ||v||, ||b||^2 go back once, after the last iteration
+    const bool single = gridDim.x == 1;
+    float* nbs = reinterpret_cast<float*>(Ms + (mask ? (size_t)n * rs_ : 0));
+    float* vns = nbs + npairs;
+    float* wps = vns + npairs;
 
     // ---- one-time loads
     for (int it = tid; it < n * wq; it += PT_THREADS) {
         const int i = it / wq, q = it - i * wq;
         const size_t g = (size_t)i * ld + c0 + 4 * q;
-        const int o = i * sw + 4 * q;
+        const int o = i * rs_ + 4 * q;
         st4(Xs + o, ld4s(X + g));
         st4(Us + o, ld4s(U + g));
         st4(Ps + o, ld4s(Ap + g));
         if (mask) *reinterpret_cast<uchar4*>(Ms + o) = *reinterpret_cast<const uchar4*>(mask + g);
     }
     if (MINV_SMEM)
-        for (int t = tid; t < n * n; t += PT_THREADS) Mv[t] = Minv[t];
+        for (int t = tid; t < n * n4; t += PT_THREADS) {
+            const int j = t / n4, i = t - j * n4;
+            Mv[t] = i < n ? Minv[(size_t)i * n + j] : 0.f;
+        }
     for (int i = tid; i < n; i += PT_THREADS) {
         const int rs = rowptr[i], re = rowptr[i + 1];
         for (int e = rs; e < re; ++e) {
@@ -123,7 +135,10 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
     __syncthreads();
     // upper entries in entry order: entry e is upper iff cols[e] > rows[e]; its slot = number of upper entries before it.
     // One thread per row counts its lower entries; a serial prefix over n <= 384 rows by thread 0 is cheap and runs once.
-    __shared__ int pbase[CC_INV_NMAX + 1];
+    __shared__ int pbase[CC_INV_NMAX + 1], rp_s[CC_INV_NMAX + 1];
+    __shared__ float dinv_s[CC_INV_NMAX];
+    for (int i = tid; i <= n; i += PT_THREADS) rp_s[i] = rowptr[i];
+    for (int i = tid; i < n; i += PT_THREADS) dinv_s[i] = dinv[i];
     if (tid == 0) {
         int acc = 0;
         for (int i = 0; i < n; ++i) { pbase[i] = acc; acc += rowptr[i + 1] - rowup[i]; }
@@ -136,6 +151,10 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
     }
     for (int e = tid; e < nnz; e += PT_THREADS) ss[e] = s[e];
     __syncthreads();
+    if (single) {
+        for (int k = tid; k < npairs; k += PT_THREADS) { vns[k] = vn[plist[k]]; wps[k] = w[plist[k]]; nbs[k] = nb2[plist[k]]; }
+        __syncthreads();
+    }
 
     // ---- control (identical in every CTA)
     const double gamma = sc->gamma, rho = sc->rho, eps = sc->eps, tol = sc->tol;
@@ -145,44 +164,117 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
     double phi_prev = 0.0, phi = 0.0, d = sqrt(eps), dist2_t = 0.0, loss_t = 0.0, pen_t = 0.0;
     // this CTA's share of the pairs (phase 2): a contiguous range of plist
     const int k0 = (int)((long long)npairs * c / nslab), k1 = (int)((long long)npairs * (c + 1) / nslab);
+    // per-phase device time of this solve, read by CTA 0 (it waits for the slowest CTA at the barriers), into the
+    // control block's timer slots: 0 right-hand side, 2 projection, 3 norms + scalars, 4 shrink + update, 5 / 6 the two barriers
+    const bool timing = c == 0 && tid == 0 && sc->prof_phases;
+    unsigned long long tph[6] = {0, 0, 0, 0, 0, 0}, tlast = timing ? global_ns() : 0ULL;
+    auto lap = [&](int k) {
+        if (timing) { const unsigned long long now = global_ns(); tph[k] += now - tlast; tlast = now; }
+    };
+    int JS = 1;                                           // j-split of the projection (power of two <= 8)
+    while (JS < 8 && ((n4 >> 2) * ((wq + 1) >> 1)) * JS * 2 <= PT_THREADS) JS *= 2;      // 32 / JS tiles per warp
     int m = 0;
     for (; m < maxit; ++m) {
-        // ===== phase 1a: D^-1 r0,  r0_i = sum_j [ s_ij (a'_i - a'_j) - (u_i - u_j) ]   (L100 minus (I+L) u, warm start z = u)
+        // ===== phase 1a: D^-1 r0 with the warm start z = a' (any z gives the same projection, S5):
+        //   r0_i = sum_j s_ij (a'_i - a'_j) - sum_j (z_i - z_j) - (z_i - u_i) = sum_j (s_ij - 1)(a'_i - a'_j) - (a'_i - u_i)
+        // (L100's right-hand side minus (I+L) z).  One row gather per entry; z = u would need a'_j and u_j.
         for (int it = tid; it < n * wq; it += PT_THREADS) {
             const int i = it / wq, q = it - i * wq;
-            const int o = i * sw + 4 * q;
-            const float4 api = ld4s(Ps + o), ui = ld4s(Us + o);
+            const int o = i * rs_ + 4 * q;
+            const float4 api = ld4s(Ps + o);
             float4 acc = f4(0.f);
-            const int rs = rowptr[i], re = rowptr[i + 1];
-            for (int e = rs; e < re; ++e) {
-                const int oj = (int)cols[e] * sw + 4 * q;
-                acc = fma4(ss[e], api - ld4s(Ps + oj), acc);
-                acc = acc - (ui - ld4s(Us + oj));
+            const int rs = rp_s[i], re = rp_s[i + 1];
+            for (int e = rs; e < re; e += 4) {        // batches of 4 entries: the four 16-byte loads before the arithmetic
+                int oj[4];
+                float sv[4];
+                float4 pj[4];
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {          // past the row's end: the row itself contributes exact zeros
+                    oj[b] = (e + b < re ? (int)cols[e + b] : i) * rs_ + 4 * q;
+                    sv[b] = e + b < re ? ss[e + b] - 1.f : 0.f;
+                }
+#pragma unroll
+                for (int b = 0; b < 4; ++b) pj[b] = ld4s(Ps + oj[b]);
+#pragma unroll
+                for (int b = 0; b < 4; ++b) acc = fma4(sv[b], api - pj[b], acc);
             }
-            st4(Cs + o, __ldg(dinv + i) * acc);
+            acc = acc - (api - ld4s(Us + o));
+            st4(Cs + o, dinv_s[i] * acc);
         }
         __syncthreads();
-        // ===== phase 1b: A = U + Minv (D^-1 r0)   (the projection, L90-L103, by the inverse formed once in cc_create)
-        for (int it = tid; it < n * wq; it += PT_THREADS) {
-            const int i = it / wq, q = it - i * wq;
-            float4 acc0 = f4(0.f), acc1 = f4(0.f);
-            int j = 0;
-            for (; j + 1 < n; j += 2) {
-                acc0 = fma4(MINV_SMEM ? Mv[i * n + j] : __ldg(Minv + (size_t)i * n + j), ld4s(Cs + j * sw + 4 * q), acc0);
-                acc1 = fma4(MINV_SMEM ? Mv[i * n + j + 1] : __ldg(Minv + (size_t)i * n + j + 1), ld4s(Cs + (j + 1) * sw + 4 * q), acc1);
+        lap(0);
+        // ===== phase 1b: A = z + Minv (D^-1 r0), z = a'   (the projection, L90-L103, by the inverse formed once in cc_create)
+        if constexpr (MINV_SMEM) {
+            // register tile of 4 rows x 4 columns per thread; the sum over j is split over JS adjacent lanes (j = jp, jp + JS, ...)
+            // and combined by a fixed shuffle tree, so that small problems still occupy the CTA.  Per j step: one 16-byte
+            // load of D^-1 r0 and one of the transposed inverse for 16 FFMA (the one-row form was bound by shared-memory
+            // wavefronts: 12.7 us of a 27.7 us iteration on `expression`).
+            const int nrg = n4 >> 2, nqp = (wq + 1) >> 1, ntile = nrg * nqp;
+            // lanes of a warp: jp = lane / (32 / JS) (so the 8 lanes that share a shared-memory wavefront read the same row j
+            // of D^-1 r0 and of the inverse), tile = warp-slot * (32 / JS) + lane % (32 / JS); the partial sums of a tile sit
+            // in lanes 32 / JS apart and are combined by xor-shuffles over those strides
+            const int lpt = 32 / JS, lane = tid & 31, wid = tid >> 5;
+            const int tiles_per_pass = (PT_THREADS / 32) * lpt;
+            for (int base = 0; base < ntile; base += tiles_per_pass) {
+                const int tile_ = base + wid * lpt + (lane % lpt);
+                const bool valid = tile_ < ntile;
+                const int jp = lane / lpt, tile = valid ? tile_ : 0;
+                const int rg = tile / nqp, q = 2 * (tile - rg * nqp);
+                const bool two = q + 1 < wq;                     // the last quad of an odd slab stands alone
+                const int q1 = two ? q + 1 : q;
+                float4 a0 = f4(0.f), a1 = f4(0.f), a2 = f4(0.f), a3 = f4(0.f), b0 = f4(0.f), b1 = f4(0.f), b2 = f4(0.f), b3 = f4(0.f);
+                if (valid) {
+#pragma unroll 2
+                    for (int j = jp; j < n; j += JS) {
+                        const float4 cv = ld4s(Cs + j * rs_ + 4 * q), dv4 = ld4s(Cs + j * rs_ + 4 * q1);
+                        const float4 mv = ld4s(Mv + j * n4 + 4 * rg);
+                        a0 = fma4(mv.x, cv, a0); a1 = fma4(mv.y, cv, a1); a2 = fma4(mv.z, cv, a2); a3 = fma4(mv.w, cv, a3);
+                        b0 = fma4(mv.x, dv4, b0); b1 = fma4(mv.y, dv4, b1); b2 = fma4(mv.z, dv4, b2); b3 = fma4(mv.w, dv4, b3);
+                    }
+                }
+                float4* acc[8] = {&a0, &a1, &a2, &a3, &b0, &b1, &b2, &b3};
+                for (int o = 16; o >= lpt; o >>= 1) {
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) {
+                        acc[r]->x += __shfl_xor_sync(0xffffffffu, acc[r]->x, o); acc[r]->y += __shfl_xor_sync(0xffffffffu, acc[r]->y, o);
+                        acc[r]->z += __shfl_xor_sync(0xffffffffu, acc[r]->z, o); acc[r]->w += __shfl_xor_sync(0xffffffffu, acc[r]->w, o);
+                    }
+                }
+                if (valid && jp == 0) {
+                    const int i0 = 4 * rg;
+#pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        if (i0 + r < n) {
+                            const int o = (i0 + r) * rs_ + 4 * q;
+                            st4(As + o, ld4s(Ps + o) + *acc[r]);
+                            if (two) st4(As + o + 4, ld4s(Ps + o + 4) + *acc[4 + r]);
+                        }
+                    }
+                }
             }
-            if (j < n) acc0 = fma4(MINV_SMEM ? Mv[i * n + j] : __ldg(Minv + (size_t)i * n + j), ld4s(Cs + j * sw + 4 * q), acc0);
-            const int o = i * sw + 4 * q;
-            st4(As + o, ld4s(Us + o) + (acc0 + acc1));
+        } else {
+            for (int it = tid; it < n * wq; it += PT_THREADS) {
+                const int i = it / wq, q = it - i * wq;
+                float4 acc0 = f4(0.f), acc1 = f4(0.f);
+                int j = 0;
+                for (; j + 1 < n; j += 2) {
+                    acc0 = fma4(__ldg(Minv + (size_t)i * n + j), ld4s(Cs + j * rs_ + 4 * q), acc0);
+                    acc1 = fma4(__ldg(Minv + (size_t)i * n + j + 1), ld4s(Cs + (j + 1) * rs_ + 4 * q), acc1);
+                }
+                if (j < n) acc0 = fma4(__ldg(Minv + (size_t)i * n + j), ld4s(Cs + j * rs_ + 4 * q), acc0);
+                const int o = i * rs_ + 4 * q;
+                st4(As + o, ld4s(Ps + o) + (acc0 + acc1));
+            }
         }
         __syncthreads();
+        lap(1);
         // ===== phase 1c: the slab's share of ||u - a||^2, the loss, every ||b_ij||^2 and ||v_ij - b_ij||^2, the penalty
         double red[3] = {0.0, 0.0, 0.0};      // dist^2, loss, penalty
         {
             float dl = 0.f, ls = 0.f;
             for (int it = tid; it < n * wq; it += PT_THREADS) {
                 const int i = it / wq, q = it - i * wq;
-                const int o = i * sw + 4 * q;
+                const int o = i * rs_ + 4 * q;
                 const float4 u = ld4s(Us + o);
                 const float4 t = u - ld4s(As + o);
                 float4 qx = ld4s(Xs + o) - u;
@@ -198,9 +290,10 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
         }
         for (int k = tid; k < npairs; k += PT_THREADS) {
             const int e = plist[k];
-            const int oi = (int)rows[e] * sw, oj = (int)cols[e] * sw;
+            const int oi = (int)rows[e] * rs_, oj = (int)cols[e] * rs_;
             const float se = ss[e];
             float nbp = 0.f, dv = 0.f;
+#pragma unroll 3
             for (int q = 0; q < wq; ++q) {
                 const float4 b = ld4s(As + oi + 4 * q) - ld4s(As + oj + 4 * q);
                 const float4 bp = ld4s(Ps + oi + 4 * q) - ld4s(Ps + oj + 4 * q);
@@ -208,34 +301,40 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
                 nbp += dot4(b, b);
                 dv += dot4(vb, vb);
             }
-            if (nslab > 1) __stcg(nbpart + (size_t)c * nnz + e, nbp);
-            else nbpart[e] = nbp;
+            if (single) { nbs[k] = nbp; red[2] += (double)(wps[k] * vns[k]); }
+            else __stcg(nbpart + (size_t)c * nnz + e, nbp);
             red[0] += (double)dv;
         }
-        for (int k = k0 + tid; k < k1; k += PT_THREADS) {
-            const int e = plist[k];
-            red[2] += (double)(__ldg(w + e) * __ldcg(vn + e));
-        }
+        if (!single)
+            for (int k = k0 + tid; k < k1; k += PT_THREADS) {
+                const int e = plist[k];
+                red[2] += (double)(__ldg(w + e) * __ldcg(vn + e));
+            }
         block_sum<3>(red, red_s);
-        if (tid == 0) {
+        if (tid == 0 && !single) {
             __stcg(spart + (size_t)c * 4 + 0, red[0]);
             __stcg(spart + (size_t)c * 4 + 1, red[1]);
             __stcg(spart + (size_t)c * 4 + 2, red[2]);
         }
+        lap(2);
         grid_barrier(bar, target, nslab);
+        lap(4);
         // ===== phase 2: scalars (every CTA, same order), stop rule S3, coefficients
         if (tid < 32) {
-            double a0 = 0.0, a1 = 0.0, a2 = 0.0;
-            for (int b = tid; b < nslab; b += 32) {
-                a0 += __ldcg(spart + (size_t)b * 4 + 0);
-                a1 += __ldcg(spart + (size_t)b * 4 + 1);
-                a2 += __ldcg(spart + (size_t)b * 4 + 2);
-            }
+            double a0 = red[0], a1 = red[1], a2 = red[2];        // one slab: thread 0 holds the totals already
+            if (!single) {
+                a0 = a1 = a2 = 0.0;
+                for (int b = tid; b < nslab; b += 32) {
+                    a0 += __ldcg(spart + (size_t)b * 4 + 0);
+                    a1 += __ldcg(spart + (size_t)b * 4 + 1);
+                    a2 += __ldcg(spart + (size_t)b * 4 + 2);
+                }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                a0 += __shfl_xor_sync(0xffffffffu, a0, o);
-                a1 += __shfl_xor_sync(0xffffffffu, a1, o);
-                a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+                for (int o = 16; o > 0; o >>= 1) {
+                    a0 += __shfl_xor_sync(0xffffffffu, a0, o);
+                    a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+                    a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+                }
             }
             if (tid == 0) {
                 dist2_t = a0; loss_t = a1; pen_t = a2;
@@ -255,31 +354,39 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
         const float cu = ctl.cu, ca = ctl.ca, cthr = ctl.cthr;
         const int stop = ctl.stop;
         // ===== phase 2: this CTA's pairs -- add the slabs' partial norms in order, block soft-threshold (L86-L88, S6)
-        for (int k = k0 + tid; k < k1; k += PT_THREADS) {
-            const int e = plist[k], pe = __ldg(peer + e);
-            float q = 0.f;
-            if (nslab > 1) {
-                int b = 0;
-                for (; b + 4 <= nslab; b += 4) {
-                    const float v0 = __ldcg(nbpart + (size_t)b * nnz + e), v1 = __ldcg(nbpart + (size_t)(b + 1) * nnz + e);
-                    const float v2 = __ldcg(nbpart + (size_t)(b + 2) * nnz + e), v3 = __ldcg(nbpart + (size_t)(b + 3) * nnz + e);
-                    q = (((q + v0) + v1) + v2) + v3;
+        if (nslab > 1) {
+            // a warp per pair: the lanes add the slabs' partials b = lane, lane + 32, ... then combine in a fixed tree
+            const int lane = tid & 31, wid = tid >> 5;
+            for (int k = k0 + wid; k < k1; k += PT_THREADS / 32) {
+                const int e = plist[k];
+                float q = 0.f;
+                for (int b = lane; b < nslab; b += 32) q += __ldcg(nbpart + (size_t)b * nnz + e);
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+                if (lane == 0) {
+                    const int pe = __ldg(peer + e);
+                    const float nb = sqrtf(q);
+                    const float thr = cthr * __ldg(w + e);
+                    const float sn = nb <= thr ? 0.f : 1.f - thr / nb;
+                    s[e] = sn; s[pe] = sn;
+                    vn[e] = sn * nb; vn[pe] = sn * nb;
+                    nb2[e] = q; nb2[pe] = q;
                 }
-                for (; b < nslab; ++b) q += __ldcg(nbpart + (size_t)b * nnz + e);
-            } else {
-                q = nbpart[e];
             }
-            const float nb = sqrtf(q);
-            const float thr = cthr * __ldg(w + e);
-            const float sn = nb <= thr ? 0.f : 1.f - thr / nb;
-            s[e] = sn; s[pe] = sn;
-            vn[e] = sn * nb; vn[pe] = sn * nb;
-            nb2[e] = q; nb2[pe] = q;
+        } else {
+            for (int k = tid; k < npairs; k += PT_THREADS) {
+                const int e = plist[k], pe = __ldg(peer + e);
+                const float nb = sqrtf(nbs[k]);
+                const float thr = cthr * wps[k];
+                const float sn = nb <= thr ? 0.f : 1.f - thr / nb;
+                ss[e] = sn; ss[pe] = sn;
+                vns[k] = sn * nb;
+            }
         }
         // ===== phase 2: U update (L82, L116), A' <- A
         for (int it = tid; it < n * wq; it += PT_THREADS) {
             const int i = it / wq, q = it - i * wq;
-            const int o = i * sw + 4 * q;
+            const int o = i * rs_ + 4 * q;
             const float4 a = ld4s(As + o), u = ld4s(Us + o);
             float4 y = ld4s(Xs + o);
             if (mask) {
@@ -289,16 +396,28 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
             st4(Us + o, fma4(cu, y, ca * a));
             st4(Ps + o, a);
         }
+        lap(3);
         grid_barrier(bar, target, nslab);
+        lap(5);
         if (stop) { ++m; break; }
-        for (int e = tid; e < nnz; e += PT_THREADS) ss[e] = __ldcg(s + e);
-        __syncthreads();
+        if (!single) {
+            for (int e = tid; e < nnz; e += PT_THREADS) ss[e] = __ldcg(s + e);
+            __syncthreads();
+        }
+    }
+    if (single && m > 0) {
+        for (int k = tid; k < npairs; k += PT_THREADS) {
+            const int e = plist[k], pe = peer[e];
+            s[e] = ss[e]; s[pe] = ss[e];
+            vn[e] = vns[k]; vn[pe] = vns[k];
+            nb2[e] = nbs[k]; nb2[pe] = nbs[k];
+        }
     }
     // ---- state back to global memory (what cc_get_U, cc_clusters and the next solve read)
     for (int it = tid; it < n * wq; it += PT_THREADS) {
         const int i = it / wq, q = it - i * wq;
         const size_t g = (size_t)i * ld + c0 + 4 * q;
-        const int o = i * sw + 4 * q;
+        const int o = i * rs_ + 4 * q;
         st4(U + g, ld4s(Us + o));
         st4(Ap + g, ld4s(Ps + o));
         if (m > 0) st4(A + g, ld4s(As + o));
@@ -312,18 +431,23 @@ k_mm_persist(int n, int ld, int sw, int nnz, const int* __restrict__ rowptr, con
         sc->stop_pending = 1;
         sc->mm_active = 0;
         atomicAdd(&sc->nlaunch, 1ULL);
+        const int slot[6] = {0, 2, 3, 4, 5, 6};
+        for (int k = 0; k < 6; ++k) { sc->prof_ns[slot[k]] += tph[k]; sc->prof_calls[slot[k]] += (unsigned long long)m; }
     }
 }
 
 }  // namespace
 
 // ---- host side -----------------------------------------------------------------------------------------------------
+static int persist_stride(int sw) { return ((sw >> 2) & 1) ? sw : sw + 4; }
+
 static size_t persist_smem(const cc_handle* h, int sw, int minv_in_smem) {
-    const size_t n = (size_t)h->n, nnz = (size_t)h->nnz;
-    size_t b = 5 * n * sw * sizeof(float) + ((nnz + 3) & ~(size_t)3) * sizeof(float);
-    if (minv_in_smem) b += n * n * sizeof(float);
+    const size_t n = (size_t)h->n, nnz = (size_t)h->nnz, rs = (size_t)persist_stride(sw);
+    size_t b = 5 * n * rs * sizeof(float) + ((nnz + 3) & ~(size_t)3) * sizeof(float);
+    if (minv_in_smem) b += n * ((n + 3) & ~(size_t)3) * sizeof(float);
     b += (nnz / 2) * sizeof(int) + 2 * nnz * sizeof(unsigned short);
-    if (h->mask) b += n * sw;
+    if (h->mask) b += n * rs;
+    if ((h->ld + sw - 1) / sw == 1) b += 3 * (nnz / 2) * sizeof(float);      // one slab: per-pair arrays
     return b + 16;
 }
 
@@ -377,8 +501,8 @@ int ccp_setup(cc_handle* h) {
 }
 
 int ccp_solve(cc_handle* h) {
-    int n = (int)h->n, ld = (int)h->ld, sw = h->pt_sw, nnz = (int)h->nnz;
-    void* args[] = {&n, &ld, &sw, &nnz, &h->rowptr, &h->rowup, &h->col, &h->peer, &h->w, &h->s, &h->vn, &h->nb2,
+    int n = (int)h->n, ld = (int)h->ld, sw = h->pt_sw, rs = persist_stride(h->pt_sw), nnz = (int)h->nnz;
+    void* args[] = {&n, &ld, &sw, &rs, &nnz, &h->rowptr, &h->rowup, &h->col, &h->peer, &h->w, &h->s, &h->vn, &h->nb2,
                     &h->dinv, &h->Minv, &h->X, &h->mask, &h->U, &h->A, &h->Ap, &h->sc, &h->pt_nbpart, &h->pt_spart,
                     &h->hist_phi, &h->hist_d};
     CC_CUDA(h, cudaLaunchCooperativeKernel(h->pt_minv_smem ? (const void*)k_mm_persist<true> : (const void*)k_mm_persist<false>, dim3((unsigned)h->pt_slabs), dim3(PT_THREADS), args,

@@ -67,10 +67,7 @@ typedef struct {
     int32_t hist_cap; /* capacity of the per-solve Phi_m / d_m history kept on the device (default 4096;
                          iterations beyond it are not recorded)                                          */
     int32_t max_snapshots; /* how many per-gamma snapshots of U cc_path may keep (default 64)            */
-    int32_t reserved0; /* 0 (default).  Debug selector used by the A/B tests and benches: 4 = dense mode on the FP32-FFMA
-                          kernels only, 8 = FFMA pair kernel with the tensor-core contraction, 16 = the thread-staged
-                          (non-TMA) tensor-core kernels, 32 = the phase-alternating fused kernel for n <= 64 instead of the
-                          warp-specialised one.  Results agree within the parity tolerance in every setting. */
+    int32_t reserved; /* must be 0 */
 } cc_params;
 
 /* Fill *prm with the defaults above.  HOST pointer. */

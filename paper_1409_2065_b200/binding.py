@@ -33,7 +33,7 @@ class cc_params(ctypes.Structure):
     _fields_ = [("rho_scale", ctypes.c_double), ("rho_abs", ctypes.c_double), ("kappa", ctypes.c_double),
                 ("eps_abs", ctypes.c_double), ("proj_tol", ctypes.c_double), ("proj_maxit", ctypes.c_int32),
                 ("min_it", ctypes.c_int32), ("dense", ctypes.c_int32), ("use_graph", ctypes.c_int32),
-                ("hist_cap", ctypes.c_int32), ("max_snapshots", ctypes.c_int32), ("reserved0", ctypes.c_int32)]
+                ("hist_cap", ctypes.c_int32), ("max_snapshots", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 _vp, _i64, _i32, _dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double

@@ -61,7 +61,7 @@ int cc_create(cc_handle** out, int64_t n, int64_t p, const float* X, const uint8
         snprintf(g_err, sizeof(g_err), "cc_create: bad size or NULL pointer (n=%lld p=%lld)", (long long)n, (long long)p);
         return CC_EINVAL;
     }
-    if (P.proj_maxit < 1 || P.hist_cap < 0 || P.max_snapshots < 0 || !(P.proj_tol > 0.0) ||
+    if (P.reserved != 0 || P.proj_maxit < 1 || P.hist_cap < 0 || P.max_snapshots < 0 || !(P.proj_tol > 0.0) ||
         (P.rho_abs <= 0.0 && !(P.rho_scale > 0.0)) || (P.eps_abs <= 0.0 && !(P.kappa > 0.0))) {
         snprintf(g_err, sizeof(g_err), "cc_create: bad cc_params");
         return CC_EINVAL;
@@ -126,7 +126,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
     S->xscale = sqrt(h->xss);
     S->proj_tol = h->prm.proj_tol;
     S->d = S->d_prev = sqrt(S->eps);
-    S->cthr = (float)(gamma * S->d / S->rho);   // threshold factor of a feasible start (kd_pairs_tc's recompute rule)
+    S->cthr = h->dense && h->dn_tc ? h->dn_cthr : (float)(gamma * S->d / S->rho);   // tensor-core dense path: the factor that made the current (implicit) S
     S->mm_maxit = maxit;
     S->mm_min_it = h->prm.min_it;
     S->mm_active = 1;
@@ -156,6 +156,7 @@ int cc_solve(cc_handle* h, double gamma, double tol, int32_t maxit, int32_t* ite
         if (rc != CC_OK) return rc;
     }
     h->launches += (long long)S->nlaunch;      // counted on the device: every kernel of the iteration that executed
+    if (h->dense && h->dn_tc) h->dn_cthr = S->cthr;
     for (int k = 0; k < 8; ++k) { h->prof_ns[k] += S->prof_ns[k]; h->prof_calls[k] += S->prof_calls[k]; }
     if (iters_out) *iters_out = S->mm_iter;
     if (phi_out) *phi_out = S->phi;

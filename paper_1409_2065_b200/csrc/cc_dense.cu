@@ -191,16 +191,16 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
     }
 }
 
-// ---- kd_proj_tc: the contraction S (A' - abar) on the 5th-generation tensor cores ------------------------
-// tcgen05.mma kind::tf32, M = 128 rows x N = 128 columns per CTA, fp32 accumulator in TMEM (128 lanes x 128
-// columns), K walked in blocks of 32.  fp32 accuracy is kept with the 3xTF32 split: x = hi + lo with hi = x
-// rounded to TF32 (10 mantissa bits) and lo = x - hi rounded to TF32;
-// S A' ~= S_hi B_hi + S_hi B_lo + S_lo B_hi, three MMAs per K step into the same accumulator (the dropped
-// lo*lo term is 2^-22 relative).  Operands are split while they are staged into shared memory by the CTA's
-// threads (generic proxy) in the canonical K-major no-swizzle layout -- core matrices of 8 rows x 16 bytes,
-// SBO between 8-row groups, LBO between K cores -- then fence.proxy.async hands them to the tensor core.
-// A' is transposed on the way in (B operand is N x K, K-major).  Two shared-memory stages: the MMAs of
-// block kb run while the threads stage block kb+1; tcgen05.commit on an mbarrier frees a stage.
+// ---- the contraction S (A' - abar) on the 5th-generation tensor cores: common pieces ---------------------------
+// tcgen05.mma kind::tf32, M = 128 rows x N = 128 columns per CTA, fp32 accumulators in TMEM, K walked in blocks
+// of 32.  fp32 accuracy is kept with the 3xTF32 split: x = hi + lo with hi = x rounded to TF32 (10 mantissa bits)
+// and lo = x - hi rounded to TF32;  S A' ~= S_hi B_hi + S_hi B_lo + S_lo B_hi, three MMAs per K step into the same
+// accumulator (the dropped lo*lo term is 2^-22 relative).  Operands sit in shared memory in the canonical K-major
+// no-swizzle layout -- core matrices of 8 rows x 16 bytes, SBO between 8-row groups, LBO between K cores.
+// The tensor core's fp32 accumulation truncates; over K = n terms that is a systematic bias (measured: U drifts 5e-8
+// per MM iteration at n = 4096 against 2e-9 for FFMA, and the U update accumulates a bias by 1/kappa).  So the K blocks
+// rotate over FOUR TMEM accumulators (all 512 columns) and every TC_CH K blocks they are drained with tcgen05.ld into
+// fp32 registers (round-to-nearest adds) and restarted: no accumulator ever sums more than TC_CH / 4 K blocks (128 terms).
 constexpr int TC_M = 128, TC_N = 128, TC_K = 32;
 constexpr int TC_THREADS = 512, TC_WARPS = TC_THREADS / 32;
 constexpr int TC_CH = 16;                           // K blocks per accumulator chunk (512 terms)
@@ -209,7 +209,6 @@ constexpr int TC_BPASS = (TC_K / 4) / (TC_THREADS / 128);   // B K-cores per thr
 constexpr int TC_SBO = 128;                         // bytes between 8-row groups (one core matrix)
 constexpr int TC_LBO = (TC_M / 8) * 128 + 16;       // bytes between K cores; +16 spreads the staging stores over banks
 constexpr int TC_TILE = (TC_K / 4) * TC_LBO;        // bytes of one 128 x 32 operand tile
-constexpr int TC_SMEM = 2 * 4 * TC_TILE + 1024;     // 2 stages x {A_hi, A_lo, B_hi, B_lo} + alignment slack
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -255,25 +254,76 @@ __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
     lo = rna_tf32(x - hi);
 }
 
-__global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const float* __restrict__ S, const float* __restrict__ Ap,
-                                                     const float* __restrict__ U, const float* __restrict__ X,
-                                                     const uint8_t* __restrict__ mask, const float* __restrict__ ubar,
-                                                     const float* __restrict__ abar, float* __restrict__ A, cc_scal* sc,
-                                                     double* part) {
+// ---- kd_prep_proj: the B operand (A' - abar)^T, split hi/lo ONCE per iteration, already in the tile layout (one
+// contiguous TC_SIDE block per column tile and K block), so that kd_proj_tc3 fetches it with one TMA bulk copy per K block
+constexpr int TC_SIDE = 2 * TC_TILE;                // hi + lo of one operand for one K block
+
+__global__ void __launch_bounds__(TC_THREADS) kd_prep_proj(int n, int ld, int nkb, const float* __restrict__ Ap,
+                                                           const float* __restrict__ abar, uint8_t* __restrict__ Bpre,
+                                                           cc_scal* sc) {
+    if (!sc->mm_active) return;
+    count_launch(sc);
+    const int kb = blockIdx.x, ct = blockIdx.y, tid = threadIdx.x;
+    const int nl = tid & 127, kc0 = tid >> 7, gc = ct * TC_N + nl;
+    const bool ok = gc < ld;
+    const float mean = ok ? __ldg(abar + gc) : 0.f;
+    uint8_t* base = Bpre + ((size_t)ct * nkb + kb) * TC_SIDE;
+#pragma unroll
+    for (int pass = 0; pass < TC_BPASS; ++pass) {
+        const int kc = kc0 + (TC_THREADS / 128) * pass;
+        float v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int gk = kb * TC_K + kc * 4 + q;
+            v[q] = (ok && gk < n) ? __ldg(Ap + (size_t)gk * ld + gc) - mean : 0.f;
+        }
+        float4 h, l;
+        split_tf32(v[0], h.x, l.x); split_tf32(v[1], h.y, l.y); split_tf32(v[2], h.z, l.z); split_tf32(v[3], h.w, l.w);
+        const int off = kc * TC_LBO + (nl >> 3) * TC_SBO + (nl & 7) * 16;
+        *reinterpret_cast<float4*>(base + off) = h;
+        *reinterpret_cast<float4*>(base + TC_TILE + off) = l;
+    }
+}
+
+// The block soft-threshold factor of a pair from ||b|| and its threshold (||b|| <= thr gives
+// exactly 0, which covers b = 0).  On the tensor-core path S is never stored: the contraction (kd_proj_tc3), the pair
+// epilogue (kd_pairs_tc2) and the cluster read-out all recompute s_ij from the stored ||b_ij||, W_ij and the
+// threshold factor with THIS function, so they see bit-identical factors.
+__device__ __forceinline__ float shrink_factor(float nb, float thr) { return nb <= thr ? 0.f : 1.f - __fdividef(thr, nb); }
+
+// ---- kd_proj_tc3: shrink -> S tile -> S (A' - abar) in one kernel; S never reaches HBM ---------------
+// One CTA = 128 rows x 128 columns of S (A' - abar), K = all n columns of S walked in blocks of 32.  Per K block the
+// CTA's 512 threads read the 128 x 32 tiles of ||b|| and W (fp32, 8 lanes per 128-byte row segment), form
+// s = shrink_factor(||b||, cthr W), add the row sums of S (the flash-attention style running `l`), split s into TF32
+// hi + lo and store both in the tensor core's K-major core-matrix layout (two stages); the B operand (A' - abar)^T,
+// pre-split once per iteration by kd_prep_proj, arrives by TMA bulk copies (three stages, one K block ahead).  One thread
+// issues the 12 tcgen05.mma of the K block (3xTF32) after the CTA barrier.  Accumulators: four rotating 128-column TMEM
+// accumulators drained into fp32 registers every TC_CH K blocks (see the note on truncating accumulation above).
+// The loads of the next K block's ||b|| and W are in flight across the fence, the barrier and the MMA issue.
+constexpr int F_AST = 2, F_BST = 3;
+constexpr int F_SMEM = (F_AST + F_BST) * TC_SIDE + 1024;
+
+__global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc3(int n, int ld, int nkb, const float* __restrict__ NB,
+                                                      const float* __restrict__ W, const uint8_t* __restrict__ Bpre,
+                                                      const float* __restrict__ Ap, const float* __restrict__ U,
+                                                      const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                      const float* __restrict__ ubar, const float* __restrict__ abar,
+                                                      float* __restrict__ A, cc_scal* sc, double* part) {
     if (!sc->mm_active) return;
     extern __shared__ uint8_t tc_smem_raw[];
-    __shared__ __align__(8) uint64_t mbar[2], mbar_acc;
+    __shared__ __align__(8) uint64_t fullB[F_BST], freeA[F_AST], mbar_acc;
     __shared__ uint32_t tmem_base_s;
     __shared__ float rs_s[TC_M];
     __shared__ int fail_s;
     uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
+    uint8_t* smB = sm + (size_t)F_AST * TC_SIDE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int i0 = blockIdx.y * TC_M, c0 = blockIdx.x * TC_N;
-
+    const int It = blockIdx.y, Ct = blockIdx.x, i0 = It * TC_M, c0 = Ct * TC_N;
+    const float cthr = sc->cthr;
     if (tid == 0) {
         fail_s = 0;
-        for (int b = 0; b < 2; ++b)
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar[b])));
+        for (int b = 0; b < F_BST; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&fullB[b])));
+        for (int b = 0; b < F_AST; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&freeA[b])));
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar_acc)));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -285,112 +335,99 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_d = tmem_base_s;
-    // instruction descriptor (cute::UMMA::InstrDescriptor): D = F32, A = B = TF32, both K-major, N >> 3, M >> 4
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
-
-    // The tensor core's fp32 accumulation truncates; over K = n terms that is a systematic bias (measured: U drifts
-    // 5e-8 per MM iteration at n = 4096 against 2e-9 for FFMA).  So the TMEM accumulator is drained every TC_CH K blocks
-    // into fp32 registers (round-to-nearest adds) and restarted, and inside a chunk the K blocks rotate over FOUR
-    // TMEM accumulators (all 512 columns), so no accumulator ever sums more than TC_CH / 4 K blocks (128 terms).
-    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);   // accumulator columns per warp (its lane quadrant x this column group)
+    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);
     float accr[TC_CPW];
 #pragma unroll
     for (int q = 0; q < TC_CPW; ++q) accr[q] = 0.f;
-    auto drain = [&](int nacc) {
-        for (int ac = 0; ac < nacc; ++ac)
-#pragma unroll
-        for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
-            uint32_t v[16];
-            const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
-            asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                           "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                         : "r"(taddr));
-            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-            for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
-        }
-    };
-    int nchunk_done = 0;
     float rsum[TC_APASS];
 #pragma unroll
     for (int q = 0; q < TC_APASS; ++q) rsum[q] = 0.f;
-    const int nkb = (n + TC_K - 1) / TC_K;
-    // per-thread staging roles (fixed over the K loop)
-    const int a_kc = lane & 7;                       // A: 8 lanes walk one row's 128 bytes
-    const int b_nl = tid & 127, b_kc0 = tid >> 7;    // B: row = column c0 + b_nl of A', K cores b_kc0 + (TC_THREADS/128) pass
-    const int b_gc = c0 + b_nl;
-    const bool b_ok = b_gc < ld;
-    const float b_mean = b_ok ? __ldg(abar + b_gc) : 0.f;
-    float4 va[TC_APASS];
-    float vb[TC_BPASS][4];
-    auto load_block = [&](int k0) {                  // global -> registers (raw fp32), one K block ahead of the stores
+    const uint8_t* srcB = Bpre + (size_t)Ct * nkb * TC_SIDE;
+    auto issue_B = [&](int kb) {      // one thread: TMA bulk copy of K block kb's B operand (hi + lo) into its stage
+        const int st = kb % F_BST;
+        const uint32_t bar = smem_u32(&fullB[st]);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(TC_SIDE) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     :: "r"(smem_u32(smB + (size_t)st * TC_SIDE)), "l"(srcB + (size_t)kb * TC_SIDE), "r"(TC_SIDE), "r"(bar) : "memory");
+    };
+    // staging role of a thread (fixed over the K loop): rows pass * 64 + warp * 4 + lane / 8, K core lane % 8
+    const int a_kc = lane & 7;
+    float4 vnb[TC_APASS], vw[TC_APASS];
+    auto load_block = [&](int k0) {
 #pragma unroll
         for (int pass = 0; pass < TC_APASS; ++pass) {
             const int gi = i0 + pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3), gk = k0 + a_kc * 4;
-            va[pass] = (gi < n && gk < n) ? __ldg(reinterpret_cast<const float4*>(S + (size_t)gi * n + gk)) : f4(0.f);
-        }
-#pragma unroll
-        for (int pass = 0; pass < TC_BPASS; ++pass) {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int gk2 = k0 + (b_kc0 + (TC_THREADS / 128) * pass) * 4 + q;
-                vb[pass][q] = (b_ok && gk2 < n) ? __ldg(Ap + (size_t)gk2 * ld + b_gc) - b_mean : 0.f;
-            }
+            const bool ok = gi < n && gk < n;          // n is a multiple of 4 on this path: a quad is inside or outside
+            vnb[pass] = ok ? __ldg(reinterpret_cast<const float4*>(NB + (size_t)gi * n + gk)) : f4(0.f);
+            vw[pass] = ok ? __ldg(reinterpret_cast<const float4*>(W + (size_t)gi * n + gk)) : f4(0.f);
         }
     };
+    if (tid == 32 && nkb > 0) issue_B(0);
     if (nkb > 0) load_block(0);
+    int nchunk_done = 0;
     for (int kb = 0; kb < nkb; ++kb) {
-        const int st = kb & 1;
-        uint8_t* a_hi = sm + (size_t)(st * 4 + 0) * TC_TILE;
-        uint8_t* a_lo = sm + (size_t)(st * 4 + 1) * TC_TILE;
-        uint8_t* b_hi = sm + (size_t)(st * 4 + 2) * TC_TILE;
-        uint8_t* b_lo = sm + (size_t)(st * 4 + 3) * TC_TILE;
-        if (kb >= 2 && !mbar_wait(smem_u32(&mbar[st]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
+        const int stA = kb & 1;
+        uint8_t* a_hi = sm + (size_t)stA * TC_SIDE;
+        uint8_t* a_lo = a_hi + TC_TILE;
+        // the MMAs of K block kb - 2 are done: its A stage and its B stage (= the one block kb + 1 will use) are free
+        if (kb >= 2 && !mbar_wait(smem_u32(&freeA[stA]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
+        if (tid == 32 && kb + 1 < nkb) issue_B(kb + 1);
 #pragma unroll
         for (int pass = 0; pass < TC_APASS; ++pass) {
             const int r = pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3);
-            const float4 v = va[pass];
-            rsum[pass] += (v.x + v.y) + (v.z + v.w);
+            const float4 nb4 = vnb[pass], w4 = vw[pass];
+            // out-of-range and diagonal entries have ||b|| = 0 <= thr: s = 0
+            const float s0 = shrink_factor(nb4.x, cthr * w4.x), s1 = shrink_factor(nb4.y, cthr * w4.y);
+            const float s2 = shrink_factor(nb4.z, cthr * w4.z), s3 = shrink_factor(nb4.w, cthr * w4.w);
+            rsum[pass] += (s0 + s1) + (s2 + s3);
             float4 h, l;
-            split_tf32(v.x, h.x, l.x); split_tf32(v.y, h.y, l.y); split_tf32(v.z, h.z, l.z); split_tf32(v.w, h.w, l.w);
+            split_tf32(s0, h.x, l.x); split_tf32(s1, h.y, l.y); split_tf32(s2, h.z, l.z); split_tf32(s3, h.w, l.w);
             const int off = a_kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
             *reinterpret_cast<float4*>(a_hi + off) = h;
             *reinterpret_cast<float4*>(a_lo + off) = l;
         }
-#pragma unroll
-        for (int pass = 0; pass < TC_BPASS; ++pass) {
-            float4 h, l;
-            split_tf32(vb[pass][0], h.x, l.x); split_tf32(vb[pass][1], h.y, l.y);
-            split_tf32(vb[pass][2], h.z, l.z); split_tf32(vb[pass][3], h.w, l.w);
-            const int off = (b_kc0 + (TC_THREADS / 128) * pass) * TC_LBO + (b_nl >> 3) * TC_SBO + (b_nl & 7) * 16;
-            *reinterpret_cast<float4*>(b_hi + off) = h;
-            *reinterpret_cast<float4*>(b_lo + off) = l;
-        }
-        if (kb + 1 < nkb) load_block((kb + 1) * TC_K);   // in flight across the fence, the barrier and the MMA issue
+        if (kb + 1 < nkb) load_block((kb + 1) * TC_K);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
         __syncthreads();
         if (tid == 0) {
+            const int stB = kb % F_BST;
+            if (!mbar_wait(smem_u32(&fullB[stB]), (uint32_t)((kb / F_BST) & 1))) fail_s = 1;
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t sA = smem_u32(a_hi), sB = smem_u32(smB + (size_t)stB * TC_SIDE);
+            const uint32_t td = tmem_d + (uint32_t)((kb & 3) * TC_N);     // rotate over the four accumulators
 #pragma unroll
             for (int ks = 0; ks < TC_K / 8; ++ks) {
                 const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
-                const uint64_t dah = tc_desc(smem_u32(a_hi) + koff), dal = tc_desc(smem_u32(a_lo) + koff);
-                const uint64_t dbh = tc_desc(smem_u32(b_hi) + koff), dbl = tc_desc(smem_u32(b_lo) + koff);
-                const uint32_t td = tmem_d + (uint32_t)((kb & 3) * TC_N);     // rotate over the four accumulators
+                const uint64_t dah = tc_desc(sA + koff), dal = tc_desc(sA + TC_TILE + koff);
+                const uint64_t dbh = tc_desc(sB + koff), dbl = tc_desc(sB + TC_TILE + koff);
                 tc_mma(td, dah, dbh, idesc, ((kb % TC_CH) >= 4 || ks > 0) ? 1u : 0u);
                 tc_mma(td, dah, dbl, idesc, 1u);
                 tc_mma(td, dal, dbh, idesc, 1u);
             }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar[st])) : "memory");
+            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&freeA[stA])) : "memory");
             if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb)
                 asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar_acc)) : "memory");
         }
-        if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb) {      // chunk boundary: wait for the MMAs, drain, restart the accumulator
+        if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb) {      // chunk boundary: wait for the MMAs, drain, restart the accumulators
+            __syncwarp();
             if (!mbar_wait(smem_u32(&mbar_acc), (uint32_t)(nchunk_done & 1))) fail_s = 1;
             ++nchunk_done;
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            drain(min(4, (kb % TC_CH) + 1));
+            const int nacc = min(4, (kb % TC_CH) + 1);
+            for (int ac = 0; ac < nacc; ++ac)
+#pragma unroll
+                for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
+                    uint32_t v[16];
+                    const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                                 : "r"(taddr));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                    for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
+                }
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncthreads();
         }
@@ -405,7 +442,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
         if ((lane & 7) == 0) rs_s[pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3)] = v;
     }
     __syncthreads();
-    // epilogue: warp w reads TMEM lanes 32 (w % 4) .. +31 (its rows) and the column group w / 4
+    // epilogue: warp w reads its rows (TMEM lanes 32 (w % 4) ..) and the column group w / 4:
+    // a = u + [rowsum(S) (a' - abar) - S(A' - abar) - n (u - ubar)] / (n+1)      (closed-form projection, pin P3)
     const float inv = 1.f / (float)(n + 1), fn = (float)n;
     double red[2] = {0.0, 0.0};
     const int row = (warp & 3) * 32 + lane, gi = i0 + row;
@@ -449,174 +487,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc(int n, int ld, const
     }
 }
 
-// ---- kd_proj_tc2: the contraction fed by TMA bulk copies ---------------------------------------------------------
-// The A operand (S, split hi/lo, tile layout) and the row sums of S are written by kd_edges when it produces S; the B
-// operand ((A' - abar)^T, split hi/lo, tile layout) by kd_prep_proj.  One thread issues two cp.async.bulk per K block,
-// one thread the 12 MMAs; all threads meet every TC_CH K blocks to drain the four rotating accumulators.
-constexpr int TC_SIDE = 2 * TC_TILE;                // hi + lo of one operand for one K block
-constexpr int TC_NST = 3;
-constexpr int TC2_SMEM = TC_NST * 2 * TC_SIDE + 1024;
-
-__global__ void __launch_bounds__(TC_THREADS) kd_prep_proj(int n, int ld, int nkb, const float* __restrict__ Ap,
-                                                           const float* __restrict__ abar, uint8_t* __restrict__ Bpre,
-                                                           cc_scal* sc) {
-    if (!sc->mm_active) return;
-    count_launch(sc);
-    const int kb = blockIdx.x, ct = blockIdx.y, tid = threadIdx.x;
-    const int nl = tid & 127, kc0 = tid >> 7, gc = ct * TC_N + nl;
-    const bool ok = gc < ld;
-    const float mean = ok ? __ldg(abar + gc) : 0.f;
-    uint8_t* base = Bpre + ((size_t)ct * nkb + kb) * TC_SIDE;
-#pragma unroll
-    for (int pass = 0; pass < TC_BPASS; ++pass) {
-        const int kc = kc0 + (TC_THREADS / 128) * pass;
-        float v[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int gk = kb * TC_K + kc * 4 + q;
-            v[q] = (ok && gk < n) ? __ldg(Ap + (size_t)gk * ld + gc) - mean : 0.f;
-        }
-        float4 h, l;
-        split_tf32(v[0], h.x, l.x); split_tf32(v[1], h.y, l.y); split_tf32(v[2], h.z, l.z); split_tf32(v[3], h.w, l.w);
-        const int off = kc * TC_LBO + (nl >> 3) * TC_SBO + (nl & 7) * 16;
-        *reinterpret_cast<float4*>(base + off) = h;
-        *reinterpret_cast<float4*>(base + TC_TILE + off) = l;
-    }
-}
-
-__global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc2(int n, int ld, int nkb, const uint8_t* __restrict__ Spre,
-                                                      const uint8_t* __restrict__ Bpre, const float* __restrict__ rs_S,
-                                                      const float* __restrict__ Ap, const float* __restrict__ U,
-                                                      const float* __restrict__ X, const uint8_t* __restrict__ mask,
-                                                      const float* __restrict__ ubar, const float* __restrict__ abar,
-                                                      float* __restrict__ A, cc_scal* sc, double* part) {
-    if (!sc->mm_active) return;
-    extern __shared__ uint8_t tc_smem_raw[];
-    __shared__ __align__(8) uint64_t full[TC_NST], empty[TC_NST], mbar_acc;
-    __shared__ uint32_t tmem_base_s;
-    __shared__ int fail_s;
-    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int It = blockIdx.y, Ct = blockIdx.x, i0 = It * TC_M, c0 = Ct * TC_N;
-    if (tid == 0) {
-        fail_s = 0;
-        for (int b = 0; b < TC_NST; ++b) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&full[b])));
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&empty[b])));
-        }
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar_acc)));
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(4 * TC_N));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t tmem_d = tmem_base_s;
-    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
-    constexpr int TC_CPW = TC_N / (TC_WARPS / 4);
-    float accr[TC_CPW];
-#pragma unroll
-    for (int q = 0; q < TC_CPW; ++q) accr[q] = 0.f;
-    const uint8_t* srcA = Spre + (size_t)It * nkb * TC_SIDE;
-    const uint8_t* srcB = Bpre + (size_t)Ct * nkb * TC_SIDE;
-    const int nch = (nkb + TC_CH - 1) / TC_CH;
-    for (int ch = 0; ch < nch; ++ch) {
-        const int kb0 = ch * TC_CH, kb1 = min(nkb, kb0 + TC_CH);
-        if (tid == 32) {
-            for (int kb = kb0; kb < kb1; ++kb) {
-                const int st = kb % TC_NST;
-                if (kb >= TC_NST && !mbar_wait(smem_u32(&empty[st]), (uint32_t)((kb / TC_NST - 1) & 1))) fail_s = 1;
-                const uint32_t bar = smem_u32(&full[st]);
-                const uint32_t dA = smem_u32(sm + (size_t)st * 2 * TC_SIDE), dB = dA + TC_SIDE;
-                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(2 * TC_SIDE) : "memory");
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                             :: "r"(dA), "l"(srcA + (size_t)kb * TC_SIDE), "r"(TC_SIDE), "r"(bar) : "memory");
-                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                             :: "r"(dB), "l"(srcB + (size_t)kb * TC_SIDE), "r"(TC_SIDE), "r"(bar) : "memory");
-            }
-        } else if (tid == 0) {
-            for (int kb = kb0; kb < kb1; ++kb) {
-                const int st = kb % TC_NST;
-                if (!mbar_wait(smem_u32(&full[st]), (uint32_t)((kb / TC_NST) & 1))) fail_s = 1;
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const uint32_t sA = smem_u32(sm + (size_t)st * 2 * TC_SIDE), sB = sA + TC_SIDE;
-                const uint32_t td = tmem_d + (uint32_t)((kb & 3) * TC_N);
-#pragma unroll
-                for (int ks = 0; ks < TC_K / 8; ++ks) {
-                    const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
-                    const uint64_t dah = tc_desc(sA + koff), dal = tc_desc(sA + TC_TILE + koff);
-                    const uint64_t dbh = tc_desc(sB + koff), dbl = tc_desc(sB + TC_TILE + koff);
-                    tc_mma(td, dah, dbh, idesc, ((kb - kb0) >= 4 || ks > 0) ? 1u : 0u);
-                    tc_mma(td, dah, dbl, idesc, 1u);
-                    tc_mma(td, dal, dbh, idesc, 1u);
-                }
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&empty[st])) : "memory");
-            }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar_acc)) : "memory");
-        }
-        __syncwarp();
-        if (!mbar_wait(smem_u32(&mbar_acc), (uint32_t)(ch & 1))) fail_s = 1;
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const int nacc = min(4, kb1 - kb0);
-        for (int ac = 0; ac < nacc; ++ac)
-#pragma unroll
-            for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
-                uint32_t v[16];
-                const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
-                asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                               "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                             : "r"(taddr));
-                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
-            }
-        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-        __syncthreads();
-    }
-    const float inv = 1.f / (float)(n + 1), fn = (float)n;
-    double red[2] = {0.0, 0.0};
-    const int row = (warp & 3) * 32 + lane, gi = i0 + row;
-    const float rs = gi < n ? __ldg(rs_S + gi) : 0.f;
-#pragma unroll
-    for (int cb = (warp >> 2) * TC_CPW, h2 = 0; h2 < TC_CPW / 16; cb += 16, ++h2) {
-        if (gi < n) {
-#pragma unroll
-            for (int q4 = 0; q4 < 4; ++q4) {
-                const int gc = c0 + cb + q4 * 4;
-                if (gc >= ld) continue;
-                const size_t o = (size_t)gi * ld + gc;
-                const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
-                const float4 sa = make_float4(accr[h2 * 16 + q4 * 4 + 0], accr[h2 * 16 + q4 * 4 + 1],
-                                              accr[h2 * 16 + q4 * 4 + 2], accr[h2 * 16 + q4 * 4 + 3]);
-                // the two large terms (magnitude ~n) are combined in fp64
-                const float4 sg = make_float4((float)((double)rs * ap.x - sa.x), (float)((double)rs * ap.y - sa.y),
-                                              (float)((double)rs * ap.z - sa.z), (float)((double)rs * ap.w - sa.w));
-                const float4 g = sg - fn * (u - ub);
-                const float4 dl = inv * g;
-                st4(A + o, u + dl);
-                float4 q = ld4s(X + o) - u;
-                if (mask) {
-                    const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + o);
-                    q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
-                }
-                red[0] += (double)dot4(dl, dl);
-                red[1] += (double)dot4(q, q);
-            }
-        }
-    }
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(4 * TC_N));
-    if (tid == 0 && fail_s) sc->cg_failed = 2;
-    double tot[2];
-    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[0], tot)) {
-        sc->dist2 = tot[0];
-        sc->loss = tot[1];
-        prof_mark(sc, 5);
-    }
-}
 
 // ---- kd_pairs_tc: pair norms on the tensor cores, with a direct fp32 recompute where a Gram block is not enough ---
 // For a 128 x 128 tile of pairs (I <= J), with alpha = a - abar (any common shift cancels) and e = a' - a:
@@ -632,17 +502,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc2(int n, int ld, int 
 // in fp32 (one warp per pair), so the fused / not-fused decision never sees Gram rounding.
 constexpr int PK = 16;                               // K block: 16 columns = 4 K cores = 2 MMA K steps
 constexpr int PK_TILE = (PK / 4) * TC_LBO;           // bytes of one 128 x 16 operand tile
-constexpr int PK_SMEM = 2 * 8 * PK_TILE + 1024;      // 2 stages x {alpha,e} x {I,J} x {hi,lo}
 #define CC_RECOMP_REL 1.0e-2f
 
 // Epilogue shared by the two staging variants of kd_pairs_tc: combine the four Gram accumulators, flag and recompute.
 __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, int i0, int j0, uint32_t tmem_d,
-                                                  float (*nrm)[3][TC_M], unsigned int (*flag_s)[4], const int* fail_p,
-                                                  const float* __restrict__ A, const float* __restrict__ Ap,
-                                                  const float* __restrict__ S, const float* __restrict__ W,
-                                                  const float* __restrict__ VN, float* __restrict__ NB2, cc_scal* sc,
-                                                  double* part, double* hist_phi, double* hist_d,
-                                                  cudaGraphConditionalHandle outer) {
+                                                  float (*nrm)[3][TC_M], unsigned int (*flag_s)[4], float* svbuf,
+                                                  const int* fail_p, const float* __restrict__ A,
+                                                  const float* __restrict__ Ap, const float* __restrict__ W,
+                                                  float* NB, float cthr, cc_scal* sc, double* part, double* hist_phi,
+                                                  double* hist_d, cudaGraphConditionalHandle outer) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // epilogue: warp w owns TMEM lanes 32 (w % 4) .. (its rows) and the 32-column group w / 4 of all four accumulators
     const int row = (warp & 3) * 32 + lane, gi = i0 + row, grp = warp >> 2;
@@ -653,12 +521,17 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
     for (int half = 0; half < 2; ++half) {
         const int cb = grp * 32 + half * 16;
         uint32_t g[4][16];
-        float sq[16], nbrow[16];   // this row's 16 shrink factors (four float4 loads, issued before the accumulators are read) and results
+        // this row's 16 previous ||b|| (the pairs' state: v = s b', ||v|| = s ||b'||) and weights: eight float4 loads issued
+        // before the accumulators are read; the new ||b|| go to the same places afterwards (in-place: only this tile reads them)
+        float nbp[16], wq[16], nbrow[16];
 #pragma unroll
         for (int q4 = 0; q4 < 4; ++q4) {
             const int gj = j0 + cb + q4 * 4;
-            const float4 v = (gi < n && gj < n) ? __ldg(reinterpret_cast<const float4*>(S + (size_t)gi * n + gj)) : f4(0.f);
-            sq[q4 * 4 + 0] = v.x; sq[q4 * 4 + 1] = v.y; sq[q4 * 4 + 2] = v.z; sq[q4 * 4 + 3] = v.w;
+            const bool ok = gi < n && gj < n;
+            const float4 v = ok ? *reinterpret_cast<const float4*>(NB + (size_t)gi * n + gj) : f4(0.f);
+            const float4 u = ok ? __ldg(reinterpret_cast<const float4*>(W + (size_t)gi * n + gj)) : f4(0.f);
+            nbp[q4 * 4 + 0] = v.x; nbp[q4 * 4 + 1] = v.y; nbp[q4 * 4 + 2] = v.z; nbp[q4 * 4 + 3] = v.w;
+            wq[q4 * 4 + 0] = u.x; wq[q4 * 4 + 1] = u.y; wq[q4 * 4 + 2] = u.z; wq[q4 * 4 + 3] = u.w;
         }
 #pragma unroll
         for (int a = 0; a < 4; ++a) {
@@ -677,19 +550,23 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                 if (gj >= n || (I == J && gi >= gj)) { nbrow[q] = 0.f; continue; }   // diagonal tiles: pairs i < j only, mirrored
                 const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
                 const size_t o = (size_t)gi * n + gj;
+                // the factor of v_m = s b' (L86), recomputed as kd_proj_tc3 did, and this pair's share of the penalty of Phi_m
+                const float sv = shrink_factor(nbp[q], cthr * wq[q]);
+                red[1] += (double)(wq[q] * (sv * nbp[q]));
+                svbuf[row * TC_N + cl] = sv;
                 float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
                 // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
-                nbrow[q] = fmaxf(nb2, 0.f);
+                const float nbn = sqrtf(fmaxf(nb2, 0.f));
+                nbrow[q] = nbn;
                 if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
                     myflags |= 1u << (half * 16 + q);               // recomputed directly below
                 } else {
                     const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));
                     const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
-                    const float sv = sq[q], om = 1.f - sv;
+                    const float om = 1.f - sv;
                     const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
-                    if (I == J) NB2[o] = nb2;                      // diagonal tiles: guarded scalar stores (i < j only)
-                    else nbrow[q] = nb2;
-                    NB2[(size_t)gj * n + gi] = nb2;
+                    if (I == J) NB[o] = nbn;                       // diagonal tiles: guarded scalar stores (i < j only)
+                    NB[(size_t)gj * n + gi] = nbn;
                     red[0] += (double)dv;
                 }
             }
@@ -700,7 +577,7 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                 for (int q4 = 0; q4 < 4; ++q4) {
                     const int gj = j0 + cb + q4 * 4;
                     if (gj < n)
-                        st4(NB2 + (size_t)gi * n + gj, make_float4(nbrow[q4 * 4 + 0], nbrow[q4 * 4 + 1], nbrow[q4 * 4 + 2], nbrow[q4 * 4 + 3]));
+                        st4(NB + (size_t)gi * n + gj, make_float4(nbrow[q4 * 4 + 0], nbrow[q4 * 4 + 1], nbrow[q4 * 4 + 2], nbrow[q4 * 4 + 3]));
                 }
             }
         }
@@ -719,7 +596,7 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                 m &= m - 1;
                 const int gj2 = j0 + gq * 32 + b;
                 const size_t o = (size_t)gi2 * n + gj2;
-                const float sv = __ldg(S + o);
+                const float sv = svbuf[rr * TC_N + gq * 32 + b];
                 float nbv = 0.f, dvv = 0.f;
                 for (int c = lane * 4; c < ld; c += 128) {
                     const float4 bb = ld4s(A + (size_t)gi2 * ld + c) - ld4s(A + (size_t)gj2 * ld + c);
@@ -734,8 +611,9 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                     dvv += __shfl_xor_sync(0xffffffffu, dvv, of);
                 }
                 if (lane == 0) {
-                    NB2[o] = nbv;
-                    NB2[(size_t)gj2 * n + gi2] = nbv;
+                    const float nbn = sqrtf(nbv);
+                    NB[o] = nbn;
+                    NB[(size_t)gj2 * n + gi2] = nbn;
                     red[0] += (double)dvv;
                 }
             }
@@ -744,117 +622,9 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
     if (tid == 0 && *fail_p) sc->cg_failed = 2;
     double tot[2];
     if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[3], tot)) {
-        finish_iteration(sc, sc->dist2 + tot[0], sc->loss, sc->pen_next, hist_phi, hist_d, outer);   // penalty: kd_edges
+        finish_iteration(sc, sc->dist2 + tot[0], sc->loss, tot[1], hist_phi, hist_d, outer);
         prof_mark(sc, 6);
     }
-}
-
-__global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc(int n, int ld, int ntile, const float* __restrict__ A,
-                                                      const float* __restrict__ Ap, const float* __restrict__ abar,
-                                                      const float* __restrict__ S, const float* __restrict__ W,
-                                                      const float* __restrict__ VN, float* __restrict__ NB2, cc_scal* sc,
-                                                      double* part, double* hist_phi, double* hist_d,
-                                                      cudaGraphConditionalHandle outer) {
-    if (!sc->mm_active) return;
-    extern __shared__ uint8_t tc_smem_raw[];
-    __shared__ __align__(8) uint64_t mbar[2];
-    __shared__ uint32_t tmem_base_s;
-    __shared__ float nrm[2][3][TC_M];                // [I/J][|alpha|^2, alpha.e, |e|^2][row]
-    __shared__ unsigned int flag_s[TC_M][4];         // recompute mask: row x 128 columns
-    __shared__ int fail_s;
-    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
-    const int tid = threadIdx.x, warp = tid >> 5;
-    int I = 0, rem = blockIdx.x;
-    while (rem >= ntile - I) { rem -= ntile - I; ++I; }
-    const int J = I + rem, i0 = I * TC_M, j0 = J * TC_M;
-
-    if (tid == 0) {
-        fail_s = 0;
-        for (int b = 0; b < 2; ++b)
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar[b])));
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(512));
-        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-    }
-    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-    __syncthreads();
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    const uint32_t tmem_d = tmem_base_s;
-    const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
-
-    // staging role: row r of both tiles, K core kc (4 lanes cover one row's 64 bytes of a K block)
-    const int r = tid >> 2, kc = tid & 3;
-    const int gI = i0 + r, gJ = j0 + r;
-    float nI[3] = {0.f, 0.f, 0.f}, nJ[3] = {0.f, 0.f, 0.f};
-    float4 aI, pI, aJ, pJ, mb;
-    const int nkb = (ld + PK - 1) / PK;
-    auto load_block = [&](int k0) {
-        const int gc = k0 + kc * 4;
-        const bool okc = gc < ld;
-        mb = okc ? ld4s(abar + gc) : f4(0.f);
-        aI = (okc && gI < n) ? ld4s(A + (size_t)gI * ld + gc) : mb;     // out-of-range rows/columns: alpha = e = 0
-        pI = (okc && gI < n) ? ld4s(Ap + (size_t)gI * ld + gc) : mb;
-        aJ = (okc && gJ < n) ? ld4s(A + (size_t)gJ * ld + gc) : mb;
-        pJ = (okc && gJ < n) ? ld4s(Ap + (size_t)gJ * ld + gc) : mb;
-    };
-    auto stage_side = [&](uint8_t* base, const float4& a, const float4& pp, float (&nr)[3]) {
-        const float4 al = a - mb, e = pp - a;
-        nr[0] += dot4(al, al); nr[1] += dot4(al, e); nr[2] += dot4(e, e);
-        float4 h, l;
-        const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
-        split_tf32(al.x, h.x, l.x); split_tf32(al.y, h.y, l.y); split_tf32(al.z, h.z, l.z); split_tf32(al.w, h.w, l.w);
-        *reinterpret_cast<float4*>(base + 0 * PK_TILE + off) = h;
-        *reinterpret_cast<float4*>(base + 1 * PK_TILE + off) = l;
-        split_tf32(e.x, h.x, l.x); split_tf32(e.y, h.y, l.y); split_tf32(e.z, h.z, l.z); split_tf32(e.w, h.w, l.w);
-        *reinterpret_cast<float4*>(base + 2 * PK_TILE + off) = h;
-        *reinterpret_cast<float4*>(base + 3 * PK_TILE + off) = l;
-    };
-    if (nkb > 0) load_block(0);
-    for (int kb = 0; kb < nkb; ++kb) {
-        const int st = kb & 1;
-        uint8_t* sI = sm + (size_t)(st * 8 + 0) * PK_TILE;   // alpha_hi, alpha_lo, e_hi, e_lo of tile I
-        uint8_t* sJ = sm + (size_t)(st * 8 + 4) * PK_TILE;   // the same of tile J
-        if (kb >= 2 && !mbar_wait(smem_u32(&mbar[st]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
-        stage_side(sI, aI, pI, nI);
-        stage_side(sJ, aJ, pJ, nJ);
-        if (kb + 1 < nkb) load_block((kb + 1) * PK);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncthreads();
-        if (tid == 0) {
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-#pragma unroll
-            for (int ks = 0; ks < PK / 8; ++ks) {
-                const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
-                const uint32_t bI = smem_u32(sI) + koff, bJ = smem_u32(sJ) + koff;
-                const uint64_t Iah = tc_desc(bI), Ial = tc_desc(bI + PK_TILE), Ieh = tc_desc(bI + 2 * PK_TILE), Iel = tc_desc(bI + 3 * PK_TILE);
-                const uint64_t Jah = tc_desc(bJ), Jal = tc_desc(bJ + PK_TILE), Jeh = tc_desc(bJ + 2 * PK_TILE), Jel = tc_desc(bJ + 3 * PK_TILE);
-                const uint32_t acc = (kb > 0 || ks > 0) ? 1u : 0u;
-                tc_mma(tmem_d + 0 * TC_N, Iah, Jah, idesc, acc); tc_mma(tmem_d + 0 * TC_N, Iah, Jal, idesc, 1u); tc_mma(tmem_d + 0 * TC_N, Ial, Jah, idesc, 1u);
-                tc_mma(tmem_d + 1 * TC_N, Iah, Jeh, idesc, acc); tc_mma(tmem_d + 1 * TC_N, Iah, Jel, idesc, 1u); tc_mma(tmem_d + 1 * TC_N, Ial, Jeh, idesc, 1u);
-                tc_mma(tmem_d + 2 * TC_N, Ieh, Jah, idesc, acc); tc_mma(tmem_d + 2 * TC_N, Ieh, Jal, idesc, 1u); tc_mma(tmem_d + 2 * TC_N, Iel, Jah, idesc, 1u);
-                tc_mma(tmem_d + 3 * TC_N, Ieh, Jeh, idesc, acc);
-            }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar[st])) : "memory");
-        }
-    }
-    // row norms: 4 lanes per row
-#pragma unroll
-    for (int q = 0; q < 3; ++q) {
-        float v = nI[q], u = nJ[q];
-        v += __shfl_xor_sync(0xffffffffu, v, 1); v += __shfl_xor_sync(0xffffffffu, v, 2);
-        u += __shfl_xor_sync(0xffffffffu, u, 1); u += __shfl_xor_sync(0xffffffffu, u, 2);
-        if (kc == 0) { nrm[0][q][r] = v; nrm[1][q][r] = u; }
-    }
-    if (tid < TC_M * 4) flag_s[tid >> 2][tid & 3] = 0u;
-    {
-        const int kl = nkb - 1;
-        if (nkb > 0 && !mbar_wait(smem_u32(&mbar[kl & 1]), (uint32_t)((kl >> 1) & 1))) fail_s = 1;
-    }
-    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    __syncthreads();
-    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, &fail_s, A, Ap, S, W, VN, NB2, sc, part, hist_phi, hist_d, outer);
 }
 
 // ---- kd_pairs_tc, bulk-copy variant ------------------------------------------------------------------------------
@@ -904,11 +674,11 @@ __global__ void __launch_bounds__(TC_THREADS) kd_prep_pairs(int n, int ld, int n
 __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int ntile, int nkb, const uint8_t* __restrict__ pre,
                                                        const float* __restrict__ nrm_part, int npad,
                                                        const float* __restrict__ A, const float* __restrict__ Ap,
-                                                       const float* __restrict__ S, const float* __restrict__ W,
-                                                       const float* __restrict__ VN, float* __restrict__ NB2, cc_scal* sc,
+                                                       const float* __restrict__ W, float* NB, cc_scal* sc,
                                                        double* part, double* hist_phi, double* hist_d,
                                                        cudaGraphConditionalHandle outer) {
     if (!sc->mm_active) return;
+    const float cthr = sc->cthr;     // the factor that made the current S; the last block replaces it after every block is done
     extern __shared__ uint8_t tc_smem_raw[];
     __shared__ __align__(8) uint64_t full[PK_NST], empty[PK_NST], done;
     __shared__ uint32_t tmem_base_s;
@@ -993,7 +763,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int
     if (nkb > 0 && !mbar_wait(smem_u32(&done), 0u)) fail_s = 1;
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     __syncthreads();
-    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, &fail_s, A, Ap, S, W, VN, NB2, sc, part, hist_phi, hist_d, outer);
+    // every MMA is complete: the operand stages are free and serve as the 128 x 128 buffer of shrink factors
+    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, reinterpret_cast<float*>(sm), &fail_s, A, Ap, W, NB, cthr, sc, part,
+                      hist_phi, hist_d, outer);
 }
 
 // ---- kd_pairs --------------------------------------------------------------------------------------
@@ -1099,205 +871,12 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
 // 1'(A-U)) are partial sums left in shared memory by the previous phase and added up by every thread that
 // needs them, in a fixed order.  History at 52 x 200,000: scalar shared loads, 8 barriers 330 us; float4 217 us.
 constexpr int SM_N = 64, SM_C = 64, SM_Q = SM_C / 4;
-constexpr int SMALL_SMEM = (SM_N * (SM_N + 4) + 3 * SM_N * SM_C + 2 * 16 * SM_C) * (int)sizeof(float);
 
 // Column quad q of row r sits at float offset small_sw(r, q) of the row (row stride 64 floats): the quad index is
 // XORed with twice the row's 4-row tile index, so that the pair phase -- a quarter warp reads rows 4tx+a of four
 // consecutive tiles tx at two column quads -- hits 8 distinct 16-byte bank groups (a plain padded stride cannot:
 // rows 8 apart always collide), while a row's 16 quads stay a permutation of themselves.
 __device__ __forceinline__ int small_sw(int r, int q) { return (q ^ (((r >> 2) << 1) & 15)) << 2; }
-
-__global__ void __launch_bounds__(256, 2) kd_small(int n, int ld, int cs_per_tile, const float* __restrict__ S,
-                                                   const float* __restrict__ Ap, const float* __restrict__ U,
-                                                   const float* __restrict__ X, const uint8_t* __restrict__ mask,
-                                                   const float* __restrict__ W, const float* __restrict__ VN,
-                                                   float* __restrict__ A, float* __restrict__ NB2, cc_scal* sc, double* part,
-                                                   double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer,
-                                                   int init_only) {
-    if (!init_only && !sc->mm_active) return;
-    extern __shared__ __align__(16) float sm_small[];
-    float (*SsT)[SM_N + 4] = reinterpret_cast<float (*)[SM_N + 4]>(sm_small);   // S transposed: rows i of column j contiguous
-    float (*Us)[SM_C] = reinterpret_cast<float (*)[SM_C]>(sm_small + SM_N * (SM_N + 4));
-    float (*Ps)[SM_C] = Us + SM_N;
-    float (*As)[SM_C] = Ps + SM_N;
-    float (*csum)[SM_C] = As + SM_N;       // 16 partial column sums of U (one per row slot of the loading threads)
-    float (*dsum)[SM_C] = csum + 16;       // 16 partial column sums of A - U (one per 4-row group of the projection)
-    __shared__ unsigned char t_ty[136], t_tx[136];
-    __shared__ int ntiles_s;
-    const int tid = threadIdx.x;
-    if (tid == 0) {
-        int k = 0;
-        const int nt4 = (n + 3) / 4;
-        for (int ty = 0; ty < nt4; ++ty)
-            for (int tx = ty; tx < nt4; ++tx) { t_ty[k] = (unsigned char)ty; t_tx[k] = (unsigned char)tx; ++k; }
-        ntiles_s = k;
-    }
-    for (int t = tid; t < SM_N * SM_N; t += 256) {
-        const int i = t / SM_N, j = t % SM_N;
-        const float v = (!init_only && i < n && j < n) ? S[(size_t)i * n + j] : 0.f;
-        SsT[j][i] = v;
-    }
-    __syncthreads();
-    const int ntiles = ntiles_s;
-    const bool pair_thread = tid < ntiles * cs_per_tile;
-    const int tile = pair_thread ? tid / cs_per_tile : 0, cph = tid % cs_per_tile;
-    const int ty = t_ty[tile], tx = t_tx[tile];
-    float sv[4][4], nb[4][4], dv[4][4];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-        for (int b = 0; b < 4; ++b) { sv[a][b] = SsT[tx * 4 + b][ty * 4 + a]; nb[a][b] = 0.f; dv[a][b] = 0.f; }
-    double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
-    const float inv = 1.f / (float)(n + 1), fn = (float)n;
-    const int nchunks = (ld + SM_C - 1) / SM_C;
-    const int n4 = (n + 3) & ~3;
-    const int pq = tid & 15, prg = tid >> 4;       // column quad; row slot of the loads = group of 4 rows of the projection
-    for (int chunk = blockIdx.x; chunk < nchunks; chunk += gridDim.x) {
-        const int c0 = chunk * SM_C;
-        const bool inside = c0 + pq * 4 < ld;      // ld is a multiple of 4: a quad is inside or outside as a whole
-        {
-            // rows prg, prg+16, prg+32, prg+48 of quad pq: all 8 loads are issued before the first store; rows >= n and
-            // quads outside the matrix are zero
-            float4 uu[4], pp[4];
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int r = prg + 16 * k;
-                const bool ok = r < n && inside;
-                uu[k] = ok ? ld4s(U + (size_t)r * ld + c0 + pq * 4) : f4(0.f);
-                pp[k] = (ok && !init_only) ? ld4s(Ap + (size_t)r * ld + c0 + pq * 4) : uu[k];
-            }
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int r = prg + 16 * k, o = small_sw(r, pq);
-                st4(&Us[r][o], uu[k]);
-                st4(&Ps[r][o], pp[k]);
-                if (init_only) st4(&As[r][o], uu[k]);
-            }
-            st4(&csum[prg][pq * 4], (uu[0] + uu[1]) + (uu[2] + uu[3]));
-        }
-        __syncthreads();
-        if (!init_only) {
-            float dua = 0.f, los = 0.f;
-            const int i0r = prg * 4;
-            float4 dsl = f4(0.f);
-            if (i0r < n) {
-                // column means of U from the 16 partial sums, in a fixed order
-                float4 ub = ld4s(&csum[0][pq * 4]);
-#pragma unroll
-                for (int k = 1; k < 16; ++k) ub = ub + ld4s(&csum[k][pq * 4]);
-                ub = make_float4(ub.x / fn, ub.y / fn, ub.z / fn, ub.w / fn);
-                float4 pi[4], g[4];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) { pi[k] = ld4s(&Ps[i0r + k][small_sw(i0r, pq)]); g[k] = f4(0.f); }
-                // rows j >= n of P and of S^T are zero, so the padded tail of the last 4-row tile adds exact zeros
-                for (int j4 = 0; j4 < n4; j4 += 4) {
-                    const int o = small_sw(j4, pq);
-#pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        const float4 pj = ld4s(&Ps[j4 + jj][o]);
-                        const float4 s4 = ld4s(&SsT[j4 + jj][i0r]);
-                        g[0] = fma4(s4.x, pi[0] - pj, g[0]);
-                        g[1] = fma4(s4.y, pi[1] - pj, g[1]);
-                        g[2] = fma4(s4.z, pi[2] - pj, g[2]);
-                        g[3] = fma4(s4.w, pi[3] - pj, g[3]);
-                    }
-                }
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int i = i0r + k;
-                    if (i < n) {
-                        const float4 u = ld4s(&Us[i][small_sw(i0r, pq)]);
-                        float4 dl;
-                        dl.x = inv * (g[k].x - fn * (u.x - ub.x)); dl.y = inv * (g[k].y - fn * (u.y - ub.y));
-                        dl.z = inv * (g[k].z - fn * (u.z - ub.z)); dl.w = inv * (g[k].w - fn * (u.w - ub.w));
-                        const float4 a = u + dl;
-                        st4(&As[i][small_sw(i0r, pq)], a);
-                        dsl = dsl + (a - u);               // the stored difference, not dl: this is what must sum to zero
-                        if (inside) {
-                            const size_t o = (size_t)i * ld + c0 + pq * 4;
-                            dua += dot4(dl, dl);
-                            float4 q = ld4s(X + o) - u;
-                            if (mask) {
-                                const uchar4 mk = *reinterpret_cast<const uchar4*>(mask + o);
-                                q.x = mk.x ? q.x : 0.f; q.y = mk.y ? q.y : 0.f; q.z = mk.z ? q.z : 0.f; q.w = mk.w ? q.w : 0.f;
-                            }
-                            los += dot4(q, q);
-                        }
-                    }
-                }
-            }
-            st4(&dsum[prg][pq * 4], dsl);
-            red[0] += (double)dua;
-            red[1] += (double)los;
-            __syncthreads();
-            // 1'(A - U) = 0 holds exactly for the projection; remove the fp32 residual of this chunk's columns
-            if (i0r < n) {
-                float4 db = ld4s(&dsum[0][pq * 4]);
-#pragma unroll
-                for (int k = 1; k < 16; ++k) db = db + ld4s(&dsum[k][pq * 4]);
-                db = make_float4(db.x / fn, db.y / fn, db.z / fn, db.w / fn);
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                    const int i = i0r + k;
-                    float* as = &As[i][small_sw(i0r, pq)];
-                    const float4 a2 = i < n ? ld4s(as) - db : f4(0.f);     // rows n .. 4 ceil(n/4) - 1 feed the last pair tiles: zero
-                    st4(as, a2);
-                    if (i < n && inside) st4(A + (size_t)i * ld + c0 + pq * 4, a2);
-                }
-            }
-            __syncthreads();
-        }
-        if (pair_thread) {
-            const int gy = (ty << 1) & 15, gx = (tx << 1) & 15;
-            for (int cq = cph; cq < SM_Q; cq += cs_per_tile) {
-                const int oy = (cq ^ gy) << 2, ox = (cq ^ gx) << 2;
-                float4 ai[4], aj[4], pi[4], pj[4];
-#pragma unroll
-                for (int a = 0; a < 4; ++a) {
-                    ai[a] = ld4s(&As[ty * 4 + a][oy]); pi[a] = ld4s(&Ps[ty * 4 + a][oy]);
-                    aj[a] = ld4s(&As[tx * 4 + a][ox]); pj[a] = ld4s(&Ps[tx * 4 + a][ox]);
-                }
-#pragma unroll
-                for (int a = 0; a < 4; ++a)
-#pragma unroll
-                    for (int b = 0; b < 4; ++b) {
-                        const float4 bb = ai[a] - aj[b];
-                        const float4 dp = pi[a] - pj[b];
-                        const float4 tt = make_float4(fmaf(sv[a][b], dp.x, -bb.x), fmaf(sv[a][b], dp.y, -bb.y),
-                                                      fmaf(sv[a][b], dp.z, -bb.z), fmaf(sv[a][b], dp.w, -bb.w));
-                        nb[a][b] = fmaf(bb.w, bb.w, fmaf(bb.z, bb.z, fmaf(bb.y, bb.y, fmaf(bb.x, bb.x, nb[a][b]))));
-                        dv[a][b] = fmaf(tt.w, tt.w, fmaf(tt.z, tt.z, fmaf(tt.y, tt.y, fmaf(tt.x, tt.x, dv[a][b]))));
-                    }
-            }
-        }
-        __syncthreads();
-    }
-    if (pair_thread) {
-        float* out = NB2 + (size_t)(blockIdx.x * cs_per_tile + cph) * n * n;
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                const int gi = ty * 4 + a, gj = tx * 4 + b;
-                if (gi < n && gj < n && gi != gj) {
-                    out[(size_t)gi * n + gj] = nb[a][b];
-                    if (ty != tx) out[(size_t)gj * n + gi] = nb[a][b];
-                    if (gi < gj) {
-                        red[2] += (double)dv[a][b];
-                        if (blockIdx.x == 0 && cph == 0 && !init_only)
-                            red[3] += (double)(W[(size_t)gi * n + gj] * VN[(size_t)gi * n + gj]);
-                    }
-                }
-            }
-    }
-    double tot[4];
-    if (grid_reduce<4>(red, part, &sc->ticket[3], tot)) {
-        if (!init_only) {
-            finish_iteration(sc, tot[0] + tot[2], tot[1], tot[3], hist_phi, hist_d, outer);
-            prof_mark(sc, 5);
-        }
-    }
-}
 
 // ---- kd_small_ws: the same iteration, warp-specialised -------------------------------------------------------
 // kd_small alternates phases inside a CTA (load | projection | fix | pairs) and ncu showed a quarter of warp time
@@ -1533,13 +1112,11 @@ __global__ void __launch_bounds__(WS_THREADS, 1) kd_small_ws(int n, int ld, int 
     }
 }
 
-// ---- kd_edges: block soft-threshold over the n x n matrices ------------------
-// (measured on B200, n = 8192: 4 columns per thread at 4 blocks/SM 345 us, 8 at 3 blocks/SM 383 us, 16 at 3 404 us;
-// streaming-store hints made no difference)
-constexpr int CPT = 4;   // columns per thread and loop step in the streaming case
+// ---- kd_edges: block soft-threshold over the n x n matrices; the FFMA / n <= 64 paths only
+// (the tensor-core path never stores S: see shrink_factor)
 __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, double* part,
-                                                int init_only, uint8_t* __restrict__ Spre, float* __restrict__ rs_out, int nkb32) {
+                                                int init_only) {
     if (!init_only && !sc->mm_active) return;
     const size_t nn = (size_t)n * n;
     const float cthr = sc->cthr;
@@ -1548,72 +1125,6 @@ __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const floa
     // over the slices and combine with a fixed shuffle tree (deterministic either way)
     const bool warp_per = ksplit >= 32;
     const int lane = threadIdx.x & 31;
-    if (!warp_per && (n & 3) == 0) {
-        // streaming case (large n): a block walks groups of 8 rows; thread = (row r8 of the group, column quad cq).  A warp
-        // then reads / writes 64-byte row segments of the n x n matrices and, for the pre-split copy, whole 128-byte
-        // core matrices (8 rows x 16 bytes) of kd_proj_tc2's operand layout.
-        const int r8 = threadIdx.x & 7, cq = threadIdx.x >> 3;
-        __shared__ float rs_part[8][33];
-        for (int ig = blockIdx.x; ig * 8 < n; ig += gridDim.x) {
-            const int i = ig * 8 + r8;
-            float rsum = 0.f;
-            if (i < n) {
-                for (int j0 = cq * CPT; j0 < n; j0 += 32 * CPT) {      // CPT columns per thread: a warp covers 4 x 4*CPT-byte row segments of 8 rows
-                    // all loads of the thread's columns are issued before any arithmetic
-                    float4 qv[CPT / 4], wq[CPT / 4];
-#pragma unroll
-                    for (int hq = 0; hq < CPT / 4; ++hq) {
-                        const int j = j0 + hq * 4;
-                        const size_t e = (size_t)i * n + (j < n ? j : 0);
-                        qv[hq] = __ldcs(reinterpret_cast<const float4*>(NB2 + e));      // streamed once: evict-first
-                        wq[hq] = __ldg(reinterpret_cast<const float4*>(W + e));
-                    }
-#pragma unroll
-                    for (int hq = 0; hq < CPT / 4; ++hq) {
-                        const int j = j0 + hq * 4;
-                        if (j >= n) break;
-                        const size_t e = (size_t)i * n + j;
-                        float4 q = qv[hq];
-                        for (int k = 1; k < ksplit; ++k) q = q + ld4s(NB2 + (size_t)k * nn + e);
-                        const float4 wv = wq[hq];
-                        float qa[4] = {q.x, q.y, q.z, q.w}, wa[4] = {wv.x, wv.y, wv.z, wv.w}, sa[4], va[4];
-#pragma unroll
-                        for (int t = 0; t < 4; ++t) {
-                            const float nb = sqrtf(qa[t]);
-                            const float thr = cthr * wa[t];
-                            float sn = init_only ? 1.f : (nb <= thr ? 0.f : 1.f - thr / nb);
-                            if (j + t == i) sn = 0.f;
-                            sa[t] = sn;
-                            va[t] = j + t == i ? 0.f : sn * nb;
-                            if (j + t > i) pen[0] += (double)(wa[t] * va[t]);
-                        }
-                        st4(S + e, make_float4(sa[0], sa[1], sa[2], sa[3]));
-                        if (VN) st4(VN + e, make_float4(va[0], va[1], va[2], va[3]));
-                        if (Spre) {
-                            rsum += (sa[0] + sa[1]) + (sa[2] + sa[3]);
-                            float4 hh, ll;
-                            split_tf32(sa[0], hh.x, ll.x); split_tf32(sa[1], hh.y, ll.y); split_tf32(sa[2], hh.z, ll.z); split_tf32(sa[3], hh.w, ll.w);
-                            const int r = i & (TC_M - 1), kb = j >> 5, kc = (j & 31) >> 2;
-                            uint8_t* base = Spre + ((size_t)(i / TC_M) * nkb32 + kb) * (2 * TC_TILE);
-                            const int off = kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
-                            *reinterpret_cast<float4*>(base + off) = hh;
-                            *reinterpret_cast<float4*>(base + TC_TILE + off) = ll;
-                        }
-                    }
-                }
-            }
-            if (Spre) {   // row sums of S in fp32, fixed order over the 32 column-quad threads of each row
-                rs_part[r8][cq] = rsum;
-                __syncthreads();
-                if (threadIdx.x < 8 && ig * 8 + threadIdx.x < n) {
-                    float t = 0.f;
-                    for (int c = 0; c < 32; ++c) t += rs_part[threadIdx.x][c];
-                    rs_out[ig * 8 + threadIdx.x] = t;
-                }
-                __syncthreads();
-            }
-        }
-    } else {
     const long long nwork = (long long)gridDim.x * (warp_per ? blockDim.x / 32 : blockDim.x);
     for (long long e = warp_per ? (long long)blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32
                                 : (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1640,9 +1151,8 @@ __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const floa
             }
         }
         S[e] = sn;
-        if (VN) VN[e] = vn;
+        VN[e] = vn;
         if (j > i) pen[0] += (double)(W[e] * vn);
-    }
     }
     double ptot[1];
     if (grid_reduce<1>(pen, part, &sc->ticket[7], ptot)) sc->pen_next = ptot[0];
@@ -1654,6 +1164,13 @@ __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const floa
             prof_mark(sc, 7);
         }
     }
+}
+
+// tensor-core path, cold start: the pair state is ||b|| itself (S4: V0 = D U0, so ||v|| = ||b|| and s = 1, which the
+// threshold factor 0 reproduces); kd_pairs wrote ||u0_i - u0_j||^2
+__global__ void kd_nb_sqrt(long long nn, float* __restrict__ NB) {
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += (long long)gridDim.x * blockDim.x)
+        NB[e] = sqrtf(NB[e]);
 }
 
 // dense-mode validation of W: symmetric, finite, > 0 off the diagonal
@@ -1679,6 +1196,24 @@ __global__ void kd_lab_hook(int n, const float* __restrict__ S, int* lab, int* c
     int m = li;
     for (int j = lane; j < n; j += 32)
         if (j != i && S[(size_t)i * n + j] == 0.f) m = min(m, lab[j]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if (lane == 0 && m < li) {
+        atomicMin(&lab[li], m);
+        atomicMin(&lab[i], m);
+        *changed = 1;
+    }
+}
+
+// the same on the tensor-core path, where S is implicit: s_ij = 0 iff ||b_ij|| <= cthr w_ij (shrink_factor's own test)
+__global__ void kd_lab_hook_nb(int n, const float* __restrict__ NB, const float* __restrict__ W, float cthr, int* lab, int* changed) {
+    const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // one warp per row
+    const int lane = threadIdx.x & 31;
+    if (i >= n) return;
+    const int li = lab[i];
+    int m = li;
+    for (int j = lane; j < n; j += 32)
+        if (j != i && shrink_factor(NB[(size_t)i * n + j], cthr * W[(size_t)i * n + j]) == 0.f) m = min(m, lab[j]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
     if (lane == 0 && m < li) {
@@ -1815,20 +1350,14 @@ static void launch_proj(cc_handle* h) {
 }
 
 void ccd_proj(cc_handle* h) {
-    if (h->dn_tc && h->prm.reserved0 != 16) {
+    if (h->dn_tc) {
         const int nkb = (int)((h->n + TC_K - 1) / TC_K);
         dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
         dim3 gp((unsigned)nkb, g.x);
         kd_prep_proj<<<gp, TC_THREADS, 0, h->stream>>>((int)h->n, (int)h->ld, nkb, h->Ap, h->abar, h->pre_B, h->sc);
-        kd_proj_tc2<<<g, TC_THREADS, TC2_SMEM, h->stream>>>((int)h->n, (int)h->ld, nkb, h->pre_S, h->pre_B, h->rs_S, h->Ap, h->U,
-                                                            h->X, h->mask, h->ubar, h->abar, h->A, h->sc,
-                                                            h->part + 0 * CC_MAXBLK * CC_NPART);
-        return;
-    }
-    if (h->dn_tc) {
-        dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
-        kd_proj_tc<<<g, TC_THREADS, TC_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->Sd, h->Ap, h->U, h->X, h->mask, h->ubar,
-                                                   h->abar, h->A, h->sc, h->part + 0 * CC_MAXBLK * CC_NPART);
+        kd_proj_tc3<<<g, TC_THREADS, F_SMEM, h->stream>>>((int)h->n, (int)h->ld, nkb, h->NB2d, h->Wd, h->pre_B, h->Ap, h->U, h->X,
+                                                          h->mask, h->ubar, h->abar, h->A, h->sc,
+                                                          h->part + 0 * CC_MAXBLK * CC_NPART);
         return;
     }
     if (!h->dn_big) launch_proj<4, 4>(h);
@@ -1844,48 +1373,36 @@ static void launch_pairs(cc_handle* h, const float* A, const float* Ap, int init
 }
 
 void ccd_pairs(cc_handle* h) {
-    if (h->dn_tc && h->prm.reserved0 != 8 && h->prm.reserved0 != 16) {
+    if (h->dn_tc) {
         const int ntile = (int)((h->n + TC_M - 1) / TC_M), nkb = (int)((h->ld + PK - 1) / PK), npad = ntile * TC_M;
         dim3 gp((unsigned)nkb, (unsigned)ntile);
         kd_prep_pairs<<<gp, TC_THREADS, 0, h->stream>>>((int)h->n, (int)h->ld, nkb, h->A, h->Ap, h->abar, h->pre_pairs,
                                                        h->nrm_part, npad, h->sc);
         kd_pairs_tc2<<<(unsigned)(ntile * (ntile + 1) / 2), TC_THREADS, PK2_SMEM, h->stream>>>(
-            (int)h->n, (int)h->ld, ntile, nkb, h->pre_pairs, h->nrm_part, npad, h->A, h->Ap, h->Sd, h->Wd, h->VNd, h->NB2d,
+            (int)h->n, (int)h->ld, ntile, nkb, h->pre_pairs, h->nrm_part, npad, h->A, h->Ap, h->Wd, h->NB2d,
             h->sc, h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, h->cond_outer);
-        return;
-    }
-    if (h->dn_tc && h->prm.reserved0 != 8) {
-        const int ntile = (int)((h->n + TC_M - 1) / TC_M);
-        kd_pairs_tc<<<(unsigned)(ntile * (ntile + 1) / 2), TC_THREADS, PK_SMEM, h->stream>>>(
-            (int)h->n, (int)h->ld, ntile, h->A, h->Ap, h->abar, h->Sd, h->Wd, h->VNd, h->NB2d, h->sc,
-            h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, h->cond_outer);
         return;
     }
     launch_pairs(h, h->A, h->Ap, 0);
 }
 
-static void launch_small(cc_handle* h, int init_only) {
-    if (!init_only && h->prm.reserved0 != 32) {
-        kd_small_ws<<<h->dn_small_grid, WS_THREADS, WS_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X,
-                                                                          h->mask, h->Wd, h->VNd, h->A, h->NB2d, h->sc,
-                                                                          h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi,
-                                                                          h->hist_d, h->cond_outer);
-        return;
-    }
-    kd_small<<<h->dn_small_grid, 256, SMALL_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X, h->mask,
-                                                      h->Wd, h->VNd, h->A, h->NB2d, h->sc, h->part + 3 * CC_MAXBLK * CC_NPART,
-                                                      h->hist_phi, h->hist_d, init_only ? 0 : h->cond_outer, init_only);
+static void launch_small(cc_handle* h) {
+    kd_small_ws<<<h->dn_small_grid, WS_THREADS, WS_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X,
+                                                                      h->mask, h->Wd, h->VNd, h->A, h->NB2d, h->sc,
+                                                                      h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi,
+                                                                      h->hist_d, h->cond_outer);
 }
 
 void ccd_edges(cc_handle* h, int init_only) {
-    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd,
-                                                   (h->dn_tc && h->prm.reserved0 == 0) ? (float*)nullptr : h->VNd, h->sc,
-                                                   h->part + 6 * CC_MAXBLK * CC_NPART, init_only, h->pre_S, h->rs_S,
-                                                   (int)((h->n + TC_K - 1) / TC_K));
+    kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc,
+                                                   h->part + 6 * CC_MAXBLK * CC_NPART, init_only);
 }
 
 void ccd_lab_hook(cc_handle* h, int* changed) {
-    kd_lab_hook<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->Sd, h->lab, changed);
+    if (h->dn_tc)
+        kd_lab_hook_nb<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->NB2d, h->Wd, h->dn_cthr, h->lab, changed);
+    else
+        kd_lab_hook<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->Sd, h->lab, changed);
 }
 
 // sizes, allocations and validation of the dense mode; W is copied.  Returns CC_* codes.
@@ -1894,24 +1411,22 @@ int ccd_setup(cc_handle* h, const float* W) {
     const int ntile = (int)((n + PT - 1) / PT);
     const long long ntp = (long long)ntile * (ntile + 1) / 2;
     h->dn_big = (n > 64 && h->ld >= 128) ? 1 : 0;
-    // tensor-core contraction when the tile shape pays (M = 128 rows) and rows of S are float4-aligned;
-    // prm.reserved0 = 4 forces the FFMA tiles (A/B comparison in tests and bench)
-    h->dn_tc = (n >= 128 && (n & 3) == 0 && h->prm.reserved0 != 4) ? 1 : 0;
+    // tensor-core path when the tile shape pays (M = 128 rows) and rows of the n x n matrices are float4-aligned; there the
+    // pair state is ||b|| alone (NB2d holds ||b||, S is implicit), elsewhere S and ||v|| are stored and kd_edges makes them
+    h->dn_tc = (n >= 128 && (n & 3) == 0) ? 1 : 0;
     if (h->dn_tc) {
-        cudaError_t ea = cudaFuncSetAttribute(kd_proj_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, TC_SMEM);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc, cudaFuncAttributeMaxDynamicSharedMemorySize, PK_SMEM);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_pairs_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, PK2_SMEM);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_proj_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, TC2_SMEM);
+        cudaError_t ea = cudaFuncSetAttribute(kd_pairs_tc2, cudaFuncAttributeMaxDynamicSharedMemorySize, PK2_SMEM);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(kd_proj_tc3, cudaFuncAttributeMaxDynamicSharedMemorySize, F_SMEM);
         if (ea != cudaSuccess) { cudaGetLastError(); h->dn_tc = 0; }
     }
     long long ks = (4LL * h->sms + ntp - 1) / ntp;
     const long long ksmax = (h->ld + 63) / 64;
     if (ks > ksmax) ks = ksmax;
     if (ks < 1) ks = 1;
-    if (h->dn_tc) ks = 1;                      // kd_pairs_tc walks all columns itself
+    if (h->dn_tc) ks = 1;                      // kd_pairs_tc2 walks all columns itself
     h->dn_ksplit = (int)ks;
     // n <= 64: the fused kernel; its slices are (CTA, column phase)
-    h->dn_small = (n <= SM_N && h->prm.reserved0 != 4) ? 1 : 0;
+    h->dn_small = n <= SM_N ? 1 : 0;
     if (h->dn_small) {
         const int nt4 = (int)((n + 3) / 4), ntiles = nt4 * (nt4 + 1) / 2;
         int cs = 256 / ntiles;
@@ -1919,10 +1434,9 @@ int ccd_setup(cc_handle* h, const float* W) {
         if (cs < 1) cs = 1;
         long long g = (h->ld + SM_C - 1) / SM_C;
         if (g > h->sms) g = h->sms;             // kd_small_ws: one 512-thread CTA per SM
-        if (cudaFuncSetAttribute(kd_small, cudaFuncAttributeMaxDynamicSharedMemorySize, SMALL_SMEM) != cudaSuccess ||
-            cudaFuncSetAttribute(kd_small_ws, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM) != cudaSuccess) {
+        if (cudaFuncSetAttribute(kd_small_ws, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM) != cudaSuccess) {
             cudaGetLastError();
-            snprintf(h->err, sizeof(h->err), "dense mode: cannot reserve %d bytes of shared memory for kd_small", SMALL_SMEM);
+            snprintf(h->err, sizeof(h->err), "dense mode: cannot reserve %d bytes of shared memory for kd_small_ws", WS_SMEM);
             return CC_ECUDA;
         }
         h->dn_small_cs = cs;
@@ -1935,12 +1449,11 @@ int ccd_setup(cc_handle* h, const float* W) {
         snprintf(h->err, sizeof(h->err), "dense mode: problem too large for this build (n=%lld, p=%lld)", (long long)n, (long long)h->p);
         return CC_EINVAL;
     }
-    float** mats[] = {&h->Wd, &h->Sd, &h->VNd};
-    for (float** m : mats) {
-        cudaError_t e = cc_dev_alloc((void**)m, (size_t)nn * sizeof(float), h->stream);
-        if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc n*n failed"); return CC_ENOMEM; }
-    }
-    cudaError_t e = cc_dev_alloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float), h->stream);
+    cudaError_t e = cc_dev_alloc((void**)&h->Wd, (size_t)nn * sizeof(float), h->stream);
+    if (e == cudaSuccess && !h->dn_tc) e = cc_dev_alloc((void**)&h->Sd, (size_t)nn * sizeof(float), h->stream);
+    if (e == cudaSuccess && !h->dn_tc) e = cc_dev_alloc((void**)&h->VNd, (size_t)nn * sizeof(float), h->stream);
+    if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc n*n failed"); return CC_ENOMEM; }
+    e = cc_dev_alloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->ubar, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->abar, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess && !h->dn_small) e = cc_dev_alloc((void**)&h->dbar, (size_t)h->ld * sizeof(float), h->stream);
@@ -1951,18 +1464,14 @@ int ccd_setup(cc_handle* h, const float* W) {
         const size_t ntile = (size_t)((n + TC_M - 1) / TC_M), nkb = (size_t)((h->ld + PK - 1) / PK);
         e = cc_dev_alloc((void**)&h->pre_pairs, ntile * nkb * PK_SIDE, h->stream);
         const size_t nkb32 = (size_t)((n + TC_K - 1) / TC_K), nct = (size_t)((h->ld + TC_N - 1) / TC_N);
-        if (e == cudaSuccess && h->prm.reserved0 != 16) {
-            e = cc_dev_alloc((void**)&h->pre_S, ntile * nkb32 * TC_SIDE, h->stream);
-            if (e == cudaSuccess) e = cudaMemsetAsync(h->pre_S, 0, ntile * nkb32 * TC_SIDE, h->stream);   // padding rows / columns stay 0
-            if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->pre_B, nct * nkb32 * TC_SIDE, h->stream);
-            if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->rs_S, (size_t)n * sizeof(float), h->stream);
-        }
+        if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->pre_B, nct * nkb32 * TC_SIDE, h->stream);
         if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->nrm_part, nkb * 3 * ntile * TC_M * sizeof(float), h->stream);
         if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
     }
     CC_CUDA(h, cudaMemcpyAsync(h->Wd, W, (size_t)nn * sizeof(float), cudaMemcpyDeviceToDevice, h->stream));
-    CC_CUDA(h, cudaMemsetAsync(h->Sd, 0, (size_t)nn * sizeof(float), h->stream));
-    CC_CUDA(h, cudaMemsetAsync(h->VNd, 0, (size_t)nn * sizeof(float), h->stream));
+    CC_CUDA(h, cudaMemsetAsync(h->NB2d, 0, (size_t)nn * ks * sizeof(float), h->stream));
+    if (h->Sd) CC_CUDA(h, cudaMemsetAsync(h->Sd, 0, (size_t)nn * sizeof(float), h->stream));
+    if (h->VNd) CC_CUDA(h, cudaMemsetAsync(h->VNd, 0, (size_t)nn * sizeof(float), h->stream));
     kd_check_w<<<h->grid_nodes, 256, 0, h->stream>>>((int)n, h->Wd, h->dflag);
     h->nnz = n * (n - 1);
     h->npairs = h->nnz / 2;
@@ -1995,15 +1504,19 @@ void ccd_sumw2(cc_handle* h) {
 void ccd_init_state(cc_handle* h) {
     const size_t bytes = (size_t)h->n * h->ld * sizeof(float);
     cudaMemcpyAsync(h->Ap, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
-    if (h->dn_small) launch_small(h, 1);
-    else launch_pairs(h, h->U, h->U, 1);
-    ccd_edges(h, 1);
+    launch_pairs(h, h->U, h->U, 1);            // ||u0_i - u0_j||^2 by direct differences (every dense path starts here)
+    if (h->dn_tc) {
+        kd_nb_sqrt<<<h->grid_nodes, 256, 0, h->stream>>>((long long)h->n * h->n, h->NB2d);
+        h->dn_cthr = 0.f;                      // threshold factor 0: s = 1 wherever ||b|| > 0
+    } else {
+        ccd_edges(h, 1);
+    }
     h->launches += 2;
 }
 
 void ccd_iteration(cc_handle* h) {
     if (h->dn_small) {
-        launch_small(h, 0);
+        launch_small(h);
         ccs_update_nodes(h);
         ccd_edges(h, 0);
         return;
@@ -2017,7 +1530,7 @@ void ccd_iteration(cc_handle* h) {
     }
     ccd_pairs(h);
     ccs_update_nodes(h);
-    ccd_edges(h, 0);
+    if (!h->dn_tc) ccd_edges(h, 0);            // the tensor-core path keeps ||b|| only: no pass over the n x n matrices
 }
 
 int ccd_solve_eager(cc_handle* h, int maxit) {
@@ -2034,7 +1547,7 @@ int ccd_solve_eager(cc_handle* h, int maxit) {
     return CC_OK;
 }
 
-// graph:  WHILE(outer){ kd_colsum1; kd_colsum2; kd_proj; kd_pairs; k_update; kd_edges }
+// graph:  WHILE(outer){ kd_colsum1; kd_colsum2; [kd_prep_proj;] kd_proj*; kd_dsum1; kd_dsum2; [kd_prep_pairs;] kd_pairs*; k_update; [kd_edges] }
 int ccd_build_graph(cc_handle* h) {
     if (h->gexec) return CC_OK;
     cudaStream_t cap;

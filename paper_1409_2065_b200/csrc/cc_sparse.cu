@@ -588,7 +588,7 @@ void ccs_apply_inv(cc_handle* h) {
 // cc_create: form Minv when n is small enough (the work space is released right away)
 int ccs_setup_inverse(cc_handle* h) {
     h->Minv = nullptr;
-    if (h->dense || h->n > CC_INV_NMAX || h->prm.reserved0 == 32) return CC_OK;
+    if (h->dense || h->n > CC_INV_NMAX) return CC_OK;
     const size_t n = (size_t)h->n;
     if (n * 128 * sizeof(float) > 48 * 1024) {
         cudaError_t ea = cudaFuncSetAttribute(k_apply_inv<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 128 * sizeof(float)));

@@ -193,22 +193,18 @@ __global__ void __launch_bounds__(256) kd_proj(int n, int ld, const float* __res
 
 // ---- the contraction S (A' - abar) on the 5th-generation tensor cores: common pieces ---------------------------
 // tcgen05.mma kind::tf32, M = 128 rows x N = 128 columns per CTA, fp32 accumulators in TMEM, K walked in blocks
-// of 32.  fp32 accuracy is kept with the 3xTF32 split: x = hi + lo with hi = x rounded to TF32 (10 mantissa bits)
+// of 16.  fp32 accuracy is kept with the 3xTF32 split: x = hi + lo with hi = x rounded to TF32 (10 mantissa bits)
 // and lo = x - hi rounded to TF32;  S A' ~= S_hi B_hi + S_hi B_lo + S_lo B_hi, three MMAs per K step into the same
 // accumulator (the dropped lo*lo term is 2^-22 relative).  Operands sit in shared memory in the canonical K-major
 // no-swizzle layout -- core matrices of 8 rows x 16 bytes, SBO between 8-row groups, LBO between K cores.
 // The tensor core's fp32 accumulation truncates; over K = n terms that is a systematic bias (measured: U drifts 5e-8
 // per MM iteration at n = 4096 against 2e-9 for FFMA, and the U update accumulates a bias by 1/kappa).  So the K blocks
-// rotate over FOUR TMEM accumulators (all 512 columns) and every TC_CH K blocks they are drained with tcgen05.ld into
-// fp32 registers (round-to-nearest adds) and restarted: no accumulator ever sums more than TC_CH / 4 K blocks (128 terms).
-constexpr int TC_M = 128, TC_N = 128, TC_K = 32;
+// rotate over FOUR TMEM accumulators (all 512 columns) and every F_CH K blocks they are drained with tcgen05.ld into
+// fp32 registers (round-to-nearest adds) and restarted: no accumulator ever sums more than F_CH / 4 K blocks (128 terms).
+constexpr int TC_M = 128, TC_N = 128;
 constexpr int TC_THREADS = 512, TC_WARPS = TC_THREADS / 32;
-constexpr int TC_CH = 16;                           // K blocks per accumulator chunk (512 terms)
-constexpr int TC_APASS = TC_M / (TC_WARPS * 4);        // A rows per thread (4 rows per warp and pass)
-constexpr int TC_BPASS = (TC_K / 4) / (TC_THREADS / 128);   // B K-cores per thread
 constexpr int TC_SBO = 128;                         // bytes between 8-row groups (one core matrix)
 constexpr int TC_LBO = (TC_M / 8) * 128 + 16;       // bytes between K cores; +16 spreads the staging stores over banks
-constexpr int TC_TILE = (TC_K / 4) * TC_LBO;        // bytes of one 128 x 32 operand tile
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -230,6 +226,8 @@ __device__ __forceinline__ void tc_mma(uint32_t tmem_d, uint64_t da, uint64_t db
         :: "r"(tmem_d), "l"(da), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
 }
 
+// try_wait suspends the waiting thread (up to a system-dependent time) instead of spinning: the warps that wait do not
+// take issue slots from the one lane that feeds the tensor core.
 __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
     for (int spin = 0; spin < (1 << 24); ++spin) {
         uint32_t ok;
@@ -239,12 +237,25 @@ __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity) {
     }
     return false;   // never hang the GPU: the caller raises cg_failed
 }
-
-__device__ __forceinline__ float rna_tf32(float x) {
-    uint32_t r;
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
-    return __uint_as_float(r);
+// the same for warps with slack (staging): back off between polls, so that a warp that waits leaves its scheduler to the
+// MMA-issuing lane (a single lane issuing ~10 instructions per MMA next to four spinning warps ran at ~190 cycles per MMA
+// where the tensor core takes 64)
+__device__ __forceinline__ bool mbar_wait_idle(uint32_t bar, uint32_t parity) {
+    for (int spin = 0; spin < (1 << 22); ++spin) {
+        uint32_t ok;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return true;
+        __nanosleep(100);
+    }
+    return false;
 }
+
+// Round to the nearest TF32 value (10 mantissa bits), ties away from zero -- what cvt.rna.tf32.f32 does.  ptxas emulates
+// that instruction on sm_100a with ~6 instructions (Inf / NaN handling included); for the finite numbers of this path the
+// integer form below is the same rounding in 2 (ncu: the staging loop of kd_proj_tc3 ran 194 instructions per thread and
+// K block, half of them these conversions, and was issue-bound with the tensor pipe 19 % busy).
+__device__ __forceinline__ float rna_tf32(float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u); }
 
 // x = hi + lo + O(2^-23 |x|), both parts exactly representable in TF32 and ROUNDED to nearest: truncating instead
 // (masking the low mantissa bits) biases every product the same way and the bias accumulates over the MM iterations
@@ -254,9 +265,26 @@ __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo) {
     lo = rna_tf32(x - hi);
 }
 
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+
 // ---- kd_prep_proj: the B operand (A' - abar)^T, split hi/lo ONCE per iteration, already in the tile layout (one
-// contiguous TC_SIDE block per column tile and K block), so that kd_proj_tc3 fetches it with one TMA bulk copy per K block
-constexpr int TC_SIDE = 2 * TC_TILE;                // hi + lo of one operand for one K block
+// contiguous F_SIDE block per column tile and K block), so that kd_proj_tc3 fetches it with one TMA bulk copy per K block
+
+// kd_proj_tc3's operands use the SWIZZLE_128B K-major layout (what a TMA tensor map with 128-byte swizzle writes): a K
+// block is 32 TF32 values = one 128-byte row per operand row; rows are stacked in 8-row atoms of 1024 bytes; inside an atom
+// the 16-byte chunk c of row r sits at chunk position c ^ (r % 8).  Descriptor: layout type 2, SBO = 1024 bytes between
+// 8-row groups, start address advanced by 32 bytes per K step of 8; tiles are 1024-byte aligned.  (The no-swizzle
+// core-matrix layout of the other tensor kernels fed the MMAs at ~190 cycles each in this kernel, operands resident:
+// measured with the staging and the TMA stubbed out.)
+constexpr int FK = 32;                               // K block of kd_proj_tc3: 32 columns of S = 4 MMA K steps
+constexpr int F_TILE = TC_M * FK * 4;                // bytes of one 128 x 32 operand tile (16 KB)
+constexpr int F_SIDE = 2 * F_TILE;                   // hi + lo
+constexpr int F_RAWT = TC_M * FK * 4;                // bytes of one raw fp32 tile of R, 128 rows x 32 columns, row-major
+__device__ __forceinline__ uint32_t sw128_off(int row, int chunk) { return (uint32_t)(row * 128 + ((chunk ^ (row & 7)) << 4)); }
 
 __global__ void __launch_bounds__(TC_THREADS) kd_prep_proj(int n, int ld, int nkb, const float* __restrict__ Ap,
                                                            const float* __restrict__ abar, uint8_t* __restrict__ Bpre,
@@ -264,71 +292,119 @@ __global__ void __launch_bounds__(TC_THREADS) kd_prep_proj(int n, int ld, int nk
     if (!sc->mm_active) return;
     count_launch(sc);
     const int kb = blockIdx.x, ct = blockIdx.y, tid = threadIdx.x;
-    const int nl = tid & 127, kc0 = tid >> 7, gc = ct * TC_N + nl;
+    const int nl = tid & 127, gc = ct * TC_N + nl;       // column of A' = a row of the N x K operand
     const bool ok = gc < ld;
     const float mean = ok ? __ldg(abar + gc) : 0.f;
-    uint8_t* base = Bpre + ((size_t)ct * nkb + kb) * TC_SIDE;
+    uint8_t* base = Bpre + ((size_t)ct * nkb + kb) * F_SIDE;
 #pragma unroll
-    for (int pass = 0; pass < TC_BPASS; ++pass) {
-        const int kc = kc0 + (TC_THREADS / 128) * pass;
+    for (int pass = 0; pass < 2; ++pass) {
+        const int kc = (tid >> 7) + 4 * pass;            // 16-byte chunk of the row: K indices 4 kc .. 4 kc + 3
         float v[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            const int gk = kb * TC_K + kc * 4 + q;
+            const int gk = kb * FK + kc * 4 + q;
             v[q] = (ok && gk < n) ? __ldg(Ap + (size_t)gk * ld + gc) - mean : 0.f;
         }
         float4 h, l;
         split_tf32(v[0], h.x, l.x); split_tf32(v[1], h.y, l.y); split_tf32(v[2], h.z, l.z); split_tf32(v[3], h.w, l.w);
-        const int off = kc * TC_LBO + (nl >> 3) * TC_SBO + (nl & 7) * 16;
+        const uint32_t off = sw128_off(nl, kc);
         *reinterpret_cast<float4*>(base + off) = h;
-        *reinterpret_cast<float4*>(base + TC_TILE + off) = l;
+        *reinterpret_cast<float4*>(base + F_TILE + off) = l;
     }
 }
 
-// The block soft-threshold factor of a pair from ||b|| and its threshold (||b|| <= thr gives
-// exactly 0, which covers b = 0).  On the tensor-core path S is never stored: the contraction (kd_proj_tc3), the pair
-// epilogue (kd_pairs_tc2) and the cluster read-out all recompute s_ij from the stored ||b_ij||, W_ij and the
-// threshold factor with THIS function, so they see bit-identical factors.
-__device__ __forceinline__ float shrink_factor(float nb, float thr) { return nb <= thr ? 0.f : 1.f - __fdividef(thr, nb); }
+// The block soft-threshold factor depends on a pair only through the ratio R = w / ||b||:
+//   s = max(0, 1 - thr / ||b||),  thr = (gamma d / rho) w  =>  s = max(0, 1 - cthr R),   ||b|| <= thr  <=>  cthr R >= 1.
+// On the tensor-core path the pair state is ||b|| (for the penalty and the next ||v||) and R; S is never stored: the
+// contraction (kd_proj_tc3), the pair epilogue (kd_pairs_tc2) and the cluster read-out recompute s_ij from R_ij and the
+// threshold factor with THESE functions, so they see bit-identical factors.  ||b|| = 0 gives R = FLT_MAX: fused for every
+// cthr > 0 (L88: b = 0 => v = 0), and s = 1 at the cold start's factor 0, where v = b = 0 anyway.
+__device__ __forceinline__ float pair_ratio(float w, float nb) { return nb > 0.f ? fminf(__fdividef(w, nb), 3.402823466e38f) : 3.402823466e38f; }
+__device__ __forceinline__ float shrink_ratio(float cthr, float R) {
+    const float x = cthr * R;
+    return x >= 1.f ? 0.f : 1.f - x;
+}
 
 // ---- kd_proj_tc3: shrink -> S tile -> S (A' - abar) in one kernel; S never reaches HBM ---------------
-// One CTA = 128 rows x 128 columns of S (A' - abar), K = all n columns of S walked in blocks of 32.  Per K block the
-// CTA's 512 threads read the 128 x 32 tiles of ||b|| and W (fp32, 8 lanes per 128-byte row segment), form
-// s = shrink_factor(||b||, cthr W), add the row sums of S (the flash-attention style running `l`), split s into TF32
-// hi + lo and store both in the tensor core's K-major core-matrix layout (two stages); the B operand (A' - abar)^T,
-// pre-split once per iteration by kd_prep_proj, arrives by TMA bulk copies (three stages, one K block ahead).  One thread
-// issues the 12 tcgen05.mma of the K block (3xTF32) after the CTA barrier.  Accumulators: four rotating 128-column TMEM
-// accumulators drained into fp32 registers every TC_CH K blocks (see the note on truncating accumulation above).
-// The loads of the next K block's ||b|| and W are in flight across the fence, the barrier and the MMA issue.
-constexpr int F_AST = 2, F_BST = 3;
-constexpr int F_SMEM = (F_AST + F_BST) * TC_SIDE + 1024;
+// One CTA = 128 rows x 128 columns of S (A' - abar), K = all n columns of S walked in blocks of FK = 32.  18 warps:
+//   warps 0-15 (staging)  thread = (row 32 (w % 4) + lane, 8 consecutive K indices w / 4).  Per K block its 32 bytes of
+//              R = w / ||b|| come in by cp.async, F_RAW K blocks deep; a thread fetches exactly what it will consume, so the
+//              ring needs no barrier, only cp.async.wait_group.  The thread clamps (Rc = min(R, 1 / cthr): S = 1 - cthr Rc),
+//              adds to the row sum (the flash-attention style running `l`), splits into TF32 hi + lo and writes both with
+//              tcgen05.st into TENSOR MEMORY: the A operand of the MMA lives in TMEM (lane = row, column = K index), in
+//              F_AST stages of 64 columns.  Each warp then arrives on the stage's `fullA` mbarrier.  Every F_CH K blocks the
+//              warps drain the two rotating accumulators into fp32 registers and arrive on `drained`.
+//   warp 16, one lane     waits fullA and the B operand's fullB, issues the 12 tcgen05.mma of the K block (3xTF32, A from
+//              TMEM, B from shared memory), commits freeA / freeB.
+//   warp 17, one lane     keeps the B ring filled: (A' - abar)^T, pre-split once per iteration by kd_prep_proj in the
+//              SWIZZLE_128B operand layout, one TMA bulk copy per K block.
+// Why A in TMEM: with both operands in shared memory a kind::tf32 MMA (M128 N128 K8) reads 4 + 4 KB of shared memory for 64
+// cycles of math -- all of the SM's 128 B/cycle -- and ran at ~190 cycles in this kernel whatever the layout (stub
+// experiments: no staging, no TMA, operands resident: still 190).  S is produced by threads anyway, so writing it to TMEM
+// costs nothing extra and halves the tensor core's shared-memory reads.
+// History (n = 8192, p = 256, us for the kernel): register prefetch of ||b|| and W one block ahead 454; TMA for B two blocks
+// ahead 657; cp.async for both operands, both TF32 splits in the loop 618 (194 instructions per thread and block: ptxas
+// emulates cvt.rna.tf32); integer rounding, B by TMA, MMA lane also a staging thread behind __syncthreads 482; dedicated
+// MMA warp, mbarrier hand-off 500; lean MMA lane (descriptor = base + constant) and separate TMA warp 400; K block 32 with
+// SWIZZLE_128B operands 295.
+constexpr int F_AST = 3, F_BST = 4, F_RAW = 4, F_CH = 16;
+constexpr int F_THREADS = TC_THREADS + 64;          // 16 staging warps + the MMA warp + the TMA warp
+constexpr int F_ACOL = 2 * TC_N;                     // TMEM columns 0 .. 255: two accumulators; from 256: the A stages
+constexpr int F_SMEM = F_BST * F_SIDE + F_RAW * F_RAWT + 1024;
 
-__global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc3(int n, int ld, int nkb, const float* __restrict__ NB,
-                                                      const float* __restrict__ W, const uint8_t* __restrict__ Bpre,
-                                                      const float* __restrict__ Ap, const float* __restrict__ U,
-                                                      const float* __restrict__ X, const uint8_t* __restrict__ mask,
-                                                      const float* __restrict__ ubar, const float* __restrict__ abar,
-                                                      float* __restrict__ A, cc_scal* sc, double* part) {
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const float (&v)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "r"(taddr), "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])),
+                    "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])),
+                    "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem descriptor]
+__device__ __forceinline__ void tc_mma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}\n"
+        :: "r"(tmem_d), "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+
+__global__ void __launch_bounds__(F_THREADS, 1) kd_proj_tc3(int n, int ld, int nkb, const float* __restrict__ Rm,
+                                                     const uint8_t* __restrict__ Bpre,
+                                                     const float* __restrict__ Ap, const float* __restrict__ U,
+                                                     const float* __restrict__ X, const uint8_t* __restrict__ mask,
+                                                     const float* __restrict__ ubar, const float* __restrict__ abar,
+                                                     float* __restrict__ A, cc_scal* sc, double* part) {
     if (!sc->mm_active) return;
     extern __shared__ uint8_t tc_smem_raw[];
-    __shared__ __align__(8) uint64_t fullB[F_BST], freeA[F_AST], mbar_acc;
+    __shared__ __align__(8) uint64_t fullA[F_AST], freeA[F_AST], fullB[F_BST], freeB[F_BST], mbar_acc, drained;
     __shared__ uint32_t tmem_base_s;
-    __shared__ float rs_s[TC_M];
+    __shared__ float rs_part[4][TC_M];
     __shared__ int fail_s;
-    uint8_t* sm = reinterpret_cast<uint8_t*>(((uintptr_t)tc_smem_raw + 1023) & ~(uintptr_t)1023);
-    uint8_t* smB = sm + (size_t)F_AST * TC_SIDE;
+    const uint32_t smB = (smem_u32(tc_smem_raw) + 1023u) & ~1023u;       // shared-space byte addresses from here on
+    const uint32_t smR = smB + F_BST * F_SIDE;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int It = blockIdx.y, Ct = blockIdx.x, i0 = It * TC_M, c0 = Ct * TC_N;
     const float cthr = sc->cthr;
     if (tid == 0) {
         fail_s = 0;
-        for (int b = 0; b < F_BST; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&fullB[b])));
-        for (int b = 0; b < F_AST; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&freeA[b])));
+        for (int b = 0; b < F_AST; ++b) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&fullA[b])), "r"(TC_WARPS));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&freeA[b])));
+        }
+        for (int b = 0; b < F_BST; ++b) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&fullB[b])));
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&freeB[b])));
+        }
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar_acc)));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&drained)), "r"(TC_WARPS));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(4 * TC_N));
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(512));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -340,114 +416,135 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc3(int n, int ld, int 
     float accr[TC_CPW];
 #pragma unroll
     for (int q = 0; q < TC_CPW; ++q) accr[q] = 0.f;
-    float rsum[TC_APASS];
-#pragma unroll
-    for (int q = 0; q < TC_APASS; ++q) rsum[q] = 0.f;
-    const uint8_t* srcB = Bpre + (size_t)Ct * nkb * TC_SIDE;
-    auto issue_B = [&](int kb) {      // one thread: TMA bulk copy of K block kb's B operand (hi + lo) into its stage
-        const int st = kb % F_BST;
-        const uint32_t bar = smem_u32(&fullB[st]);
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(TC_SIDE) : "memory");
-        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                     :: "r"(smem_u32(smB + (size_t)st * TC_SIDE)), "l"(srcB + (size_t)kb * TC_SIDE), "r"(TC_SIDE), "r"(bar) : "memory");
-    };
-    // staging role of a thread (fixed over the K loop): rows pass * 64 + warp * 4 + lane / 8, K core lane % 8
-    const int a_kc = lane & 7;
-    float4 vnb[TC_APASS], vw[TC_APASS];
-    auto load_block = [&](int k0) {
-#pragma unroll
-        for (int pass = 0; pass < TC_APASS; ++pass) {
-            const int gi = i0 + pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3), gk = k0 + a_kc * 4;
-            const bool ok = gi < n && gk < n;          // n is a multiple of 4 on this path: a quad is inside or outside
-            vnb[pass] = ok ? __ldg(reinterpret_cast<const float4*>(NB + (size_t)gi * n + gk)) : f4(0.f);
-            vw[pass] = ok ? __ldg(reinterpret_cast<const float4*>(W + (size_t)gi * n + gk)) : f4(0.f);
-        }
-    };
-    if (tid == 32 && nkb > 0) issue_B(0);
-    if (nkb > 0) load_block(0);
-    int nchunk_done = 0;
-    for (int kb = 0; kb < nkb; ++kb) {
-        const int stA = kb & 1;
-        uint8_t* a_hi = sm + (size_t)stA * TC_SIDE;
-        uint8_t* a_lo = a_hi + TC_TILE;
-        // the MMAs of K block kb - 2 are done: its A stage and its B stage (= the one block kb + 1 will use) are free
-        if (kb >= 2 && !mbar_wait(smem_u32(&freeA[stA]), (uint32_t)(((kb >> 1) - 1) & 1))) fail_s = 1;
-        if (tid == 32 && kb + 1 < nkb) issue_B(kb + 1);
-#pragma unroll
-        for (int pass = 0; pass < TC_APASS; ++pass) {
-            const int r = pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3);
-            const float4 nb4 = vnb[pass], w4 = vw[pass];
-            // out-of-range and diagonal entries have ||b|| = 0 <= thr: s = 0
-            const float s0 = shrink_factor(nb4.x, cthr * w4.x), s1 = shrink_factor(nb4.y, cthr * w4.y);
-            const float s2 = shrink_factor(nb4.z, cthr * w4.z), s3 = shrink_factor(nb4.w, cthr * w4.w);
-            rsum[pass] += (s0 + s1) + (s2 + s3);
-            float4 h, l;
-            split_tf32(s0, h.x, l.x); split_tf32(s1, h.y, l.y); split_tf32(s2, h.z, l.z); split_tf32(s3, h.w, l.w);
-            const int off = a_kc * TC_LBO + (r >> 3) * TC_SBO + (r & 7) * 16;
-            *reinterpret_cast<float4*>(a_hi + off) = h;
-            *reinterpret_cast<float4*>(a_lo + off) = l;
-        }
-        if (kb + 1 < nkb) load_block((kb + 1) * TC_K);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the tensor core
-        __syncthreads();
-        if (tid == 0) {
-            const int stB = kb % F_BST;
-            if (!mbar_wait(smem_u32(&fullB[stB]), (uint32_t)((kb / F_BST) & 1))) fail_s = 1;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const uint32_t sA = smem_u32(a_hi), sB = smem_u32(smB + (size_t)stB * TC_SIDE);
-            const uint32_t td = tmem_d + (uint32_t)((kb & 3) * TC_N);     // rotate over the four accumulators
-#pragma unroll
-            for (int ks = 0; ks < TC_K / 8; ++ks) {
-                const uint32_t koff = (uint32_t)(2 * ks * TC_LBO);
-                const uint64_t dah = tc_desc(sA + koff), dal = tc_desc(sA + TC_TILE + koff);
-                const uint64_t dbh = tc_desc(sB + koff), dbl = tc_desc(sB + TC_TILE + koff);
-                tc_mma(td, dah, dbh, idesc, ((kb % TC_CH) >= 4 || ks > 0) ? 1u : 0u);
-                tc_mma(td, dah, dbl, idesc, 1u);
-                tc_mma(td, dal, dbh, idesc, 1u);
+    if (warp == TC_WARPS + 1) {
+        // ===== TMA warp (one lane): keeps the B ring filled, up to F_BST K blocks ahead of the tensor core =====
+        if (lane == 0) {
+            const uint8_t* srcB = Bpre + (size_t)Ct * nkb * F_SIDE;
+            for (int kb = 0; kb < nkb; ++kb) {
+                const int st = kb % F_BST;
+                // the stage held block kb - F_BST: its MMAs must be complete
+                if (kb >= F_BST && !mbar_wait_idle(smem_u32(&freeB[st]), (uint32_t)((kb / F_BST - 1) & 1))) fail_s = 1;
+                const uint32_t bar = smem_u32(&fullB[st]);
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(F_SIDE) : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                             :: "r"(smB + (uint32_t)st * F_SIDE), "l"(srcB + (size_t)kb * F_SIDE), "r"(F_SIDE), "r"(bar) : "memory");
             }
-            asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&freeA[stA])) : "memory");
-            if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb)
-                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar_acc)) : "memory");
         }
-        if ((kb + 1) % TC_CH == 0 || kb + 1 == nkb) {      // chunk boundary: wait for the MMAs, drain, restart the accumulators
-            __syncwarp();
-            if (!mbar_wait(smem_u32(&mbar_acc), (uint32_t)(nchunk_done & 1))) fail_s = 1;
-            ++nchunk_done;
-            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            const int nacc = min(4, (kb % TC_CH) + 1);
-            for (int ac = 0; ac < nacc; ++ac)
-#pragma unroll
-                for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
-                    uint32_t v[16];
-                    const uint32_t taddr = tmem_d + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
-                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                                 : "r"(taddr));
-                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                    for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
+    } else if (warp == TC_WARPS) {
+        // ===== MMA warp (one lane).  A single thread issues about one instruction every few cycles, so this loop is kept
+        // lean: descriptors by adding constants to a per-stage base =====
+        if (lane == 0) {
+            // SWIZZLE_128B K-major descriptor: LBO unused (1), SBO = 1024 bytes, version 1, layout type 2
+            const uint64_t dconst = ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+            constexpr uint64_t LO = F_TILE >> 4;                 // hi -> lo tile, in descriptor units (16 bytes)
+            int ndrain = 0;
+            for (int kb = 0; kb < nkb; ++kb) {
+                const int stA = kb % F_AST, stB = kb % F_BST;
+                if (kb > 0 && kb % F_CH == 0) {      // the accumulators restart here: the staging warps must have drained them
+                    if (!mbar_wait(smem_u32(&drained), (uint32_t)(ndrain & 1))) fail_s = 1;
+                    ++ndrain;
                 }
-            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-            __syncthreads();
-        }
-    }
-    // row sums of S: 8 lanes hold one row's partial sums
+                if (!mbar_wait(smem_u32(&fullA[stA]), (uint32_t)((kb / F_AST) & 1))) fail_s = 1;
+                if (!mbar_wait(smem_u32(&fullB[stB]), (uint32_t)((kb / F_BST) & 1))) fail_s = 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t ta = tmem_d + (uint32_t)(F_ACOL + stA * 2 * FK);      // hi at ta, lo at ta + FK columns
+                const uint64_t db = dconst | (uint64_t)((smB + (uint32_t)stB * F_SIDE) >> 4);
+                const uint32_t td = tmem_d + (uint32_t)((kb & 1) * TC_N);            // rotate over the two accumulators
 #pragma unroll
-    for (int pass = 0; pass < TC_APASS; ++pass) {
-        float v = rsum[pass];
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        if ((lane & 7) == 0) rs_s[pass * (TC_WARPS * 4) + warp * 4 + (lane >> 3)] = v;
+                for (int ks = 0; ks < FK / 8; ++ks) {                        // 8 K indices: 8 TMEM columns of A, 32 bytes of B's row
+                    const uint64_t ko = (uint64_t)(2 * ks);
+                    tc_mma_ts(td, ta + 8 * ks, db + ko, idesc, ((kb % F_CH) >= 2 || ks > 0) ? 1u : 0u);
+                    tc_mma_ts(td, ta + 8 * ks, db + ko + LO, idesc, 1u);
+                    tc_mma_ts(td, ta + FK + 8 * ks, db + ko, idesc, 1u);
+                }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&freeA[stA])) : "memory");
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&freeB[stB])) : "memory");
+                if ((kb + 1) % F_CH == 0 || kb + 1 == nkb)
+                    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mbar_acc)) : "memory");
+            }
+        }
+    } else {
+        // ===== staging warps =====
+        const int row = (warp & 3) * 32 + lane, kq = warp >> 2, gir = i0 + row;     // TMEM lane quadrant of the warp, K octet
+        const uint32_t raw_off = (uint32_t)tid * 32u;
+        auto fetch = [&](int kb) {        // cp.async of this thread's 32 bytes of R for K block kb into ring slot kb % F_RAW
+            if (kb < nkb) {
+                const uint32_t dst = smR + (uint32_t)(kb % F_RAW) * F_RAWT + raw_off;
+#pragma unroll
+                for (int h2 = 0; h2 < 2; ++h2) {
+                    const int gk = kb * FK + kq * 8 + 4 * h2;
+                    const bool ok = gir < n && gk < n;       // n is a multiple of 4 on this path; outside: zero fill
+                    cp_async16(dst + 16 * h2, Rm + (ok ? (size_t)gir * n + gk : 0), ok ? 16 : 0);
+                }
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");     // one group per K block, empty past the end
+        };
+#pragma unroll
+        for (int k = 0; k < F_RAW - 1; ++k) fetch(k);
+        const float rcap = cthr > 0.f ? 1.f / cthr : 0.f;
+        const uint32_t tlane = tmem_d + ((uint32_t)((warp & 3) * 32) << 16);
+        float rsum = 0.f;
+        int nchunk_done = 0;
+        for (int kb = 0; kb < nkb; ++kb) {
+            const int st = kb % F_AST;
+            fetch(kb + F_RAW - 1);                                   // its slot held block kb - 1, which this thread has consumed
+            asm volatile("cp.async.wait_group %0;" :: "n"(F_RAW - 1) : "memory");   // block kb's chunks have landed
+            const uint32_t rp = smR + (uint32_t)(kb % F_RAW) * F_RAWT + raw_off;
+            const float4 r4 = lds128(rp), q4 = lds128(rp + 16);
+            // s = 1 - cthr min(R, 1 / cthr), and the rows of the B operand sum to zero over j (A' is centred by its column
+            // mean), so  S (A' - abar) = -cthr Rc (A' - abar)  with Rc = min(R, 1 / cthr):  the operand is Rc, one FMNMX per
+            // entry.  rowsum(S) = n - cthr rowsum(Rc).  Zero-filled entries (columns k >= n) contribute nothing; the diagonal
+            // (R = FLT_MAX) is clamped like a fused pair, and whatever factor it gets multiplies a'_i - a'_i = 0 in the sum
+            // the epilogue forms.  cthr = 0 (cold start): Rc = 0, S = 1.
+            float hi[8], lo[8];
+            const float rc[8] = {fminf(r4.x, rcap), fminf(r4.y, rcap), fminf(r4.z, rcap), fminf(r4.w, rcap),
+                                 fminf(q4.x, rcap), fminf(q4.y, rcap), fminf(q4.z, rcap), fminf(q4.w, rcap)};
+            rsum += ((rc[0] + rc[1]) + (rc[2] + rc[3])) + ((rc[4] + rc[5]) + (rc[6] + rc[7]));
+#pragma unroll
+            for (int q = 0; q < 8; ++q) split_tf32(rc[q], hi[q], lo[q]);
+            // the MMAs of K block kb - F_AST are done: this TMEM stage is free
+            if (kb >= F_AST && !mbar_wait_idle(smem_u32(&freeA[st]), (uint32_t)((kb / F_AST - 1) & 1))) fail_s = 1;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t ta = tlane + (uint32_t)(F_ACOL + st * 2 * FK + kq * 8);
+            tmem_st8(ta, hi);
+            tmem_st8(ta + FK, lo);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&fullA[st]));
+            if ((kb + 1) % F_CH == 0 || kb + 1 == nkb) {      // chunk boundary: wait for the MMAs, drain the accumulators
+                if (!mbar_wait_idle(smem_u32(&mbar_acc), (uint32_t)(nchunk_done & 1))) fail_s = 1;
+                ++nchunk_done;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const int nacc = min(2, (kb % F_CH) + 1);
+                for (int ac = 0; ac < nacc; ++ac)
+#pragma unroll
+                    for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
+                        uint32_t v[16];
+                        const uint32_t taddr = tlane + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
+                        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                                     : "r"(taddr));
+                        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                        for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
+                    }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&drained));
+            }
+        }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        rs_part[kq][row] = rsum;       // four K octets per row, added in a fixed order below
     }
     __syncthreads();
     // epilogue: warp w reads its rows (TMEM lanes 32 (w % 4) ..) and the column group w / 4:
     // a = u + [rowsum(S) (a' - abar) - S(A' - abar) - n (u - ubar)] / (n+1)      (closed-form projection, pin P3)
     const float inv = 1.f / (float)(n + 1), fn = (float)n;
     double red[2] = {0.0, 0.0};
-    const int row = (warp & 3) * 32 + lane, gi = i0 + row;
-    const float rs = rs_s[row];
+    const int row = (warp & 3) * 32 + lane, gi = warp < TC_WARPS ? i0 + row : n;     // the MMA and TMA warps have no rows
+    const float rs = (float)n - cthr * ((rs_part[0][row] + rs_part[1][row]) + (rs_part[2][row] + rs_part[3][row]));
 #pragma unroll
     for (int cb = (warp >> 2) * TC_CPW, h2 = 0; h2 < TC_CPW / 16; cb += 16, ++h2) {
         if (gi < n) {
@@ -457,8 +554,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc3(int n, int ld, int 
                 if (gc >= ld) continue;
                 const size_t o = (size_t)gi * ld + gc;
                 const float4 ap = ld4s(Ap + o) - ld4s(abar + gc), u = ld4s(U + o), ub = ld4s(ubar + gc);
-                const float4 sa = make_float4(accr[h2 * 16 + q4 * 4 + 0], accr[h2 * 16 + q4 * 4 + 1],
-                                              accr[h2 * 16 + q4 * 4 + 2], accr[h2 * 16 + q4 * 4 + 3]);
+                const float4 sa = make_float4(-cthr * accr[h2 * 16 + q4 * 4 + 0], -cthr * accr[h2 * 16 + q4 * 4 + 1],
+                                              -cthr * accr[h2 * 16 + q4 * 4 + 2], -cthr * accr[h2 * 16 + q4 * 4 + 3]);
                 // the two large terms (magnitude ~n) are combined in fp64
                 const float4 sg = make_float4((float)((double)rs * ap.x - sa.x), (float)((double)rs * ap.y - sa.y),
                                               (float)((double)rs * ap.z - sa.z), (float)((double)rs * ap.w - sa.w));
@@ -477,10 +574,10 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_proj_tc3(int n, int ld, int 
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(4 * TC_N));
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_d), "n"(512));
     if (tid == 0 && fail_s) sc->cg_failed = 2;
     double tot[2];
-    if (grid_reduce<2, TC_THREADS>(red, part, &sc->ticket[0], tot)) {
+    if (grid_reduce<2, F_THREADS>(red, part, &sc->ticket[0], tot)) {
         sc->dist2 = tot[0];
         sc->loss = tot[1];
         prof_mark(sc, 5);
@@ -509,8 +606,8 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                                                   float (*nrm)[3][TC_M], unsigned int (*flag_s)[4], float* svbuf,
                                                   const int* fail_p, const float* __restrict__ A,
                                                   const float* __restrict__ Ap, const float* __restrict__ W,
-                                                  float* NB, float cthr, cc_scal* sc, double* part, double* hist_phi,
-                                                  double* hist_d, cudaGraphConditionalHandle outer) {
+                                                  float* NB, float* __restrict__ Rm, float cthr, cc_scal* sc, double* part,
+                                                  double* hist_phi, double* hist_d, cudaGraphConditionalHandle outer) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // epilogue: warp w owns TMEM lanes 32 (w % 4) .. (its rows) and the 32-column group w / 4 of all four accumulators
     const int row = (warp & 3) * 32 + lane, gi = i0 + row, grp = warp >> 2;
@@ -522,8 +619,9 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
         const int cb = grp * 32 + half * 16;
         uint32_t g[4][16];
         // this row's 16 previous ||b|| (the pairs' state: v = s b', ||v|| = s ||b'||) and weights: eight float4 loads issued
-        // before the accumulators are read; the new ||b|| go to the same places afterwards (in-place: only this tile reads them)
-        float nbp[16], wq[16], nbrow[16];
+        // before the accumulators are read.  Afterwards nbp[] / wq[] are reused for the new ||b|| and the new ratios R, which
+        // go to the same places (in-place: only this tile reads them; ||b|| is kept for pairs i < j only, R on both sides)
+        float nbp[16], wq[16];
 #pragma unroll
         for (int q4 = 0; q4 < 4; ++q4) {
             const int gj = j0 + cb + q4 * 4;
@@ -547,17 +645,19 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
                 const int cl = cb + q, gj = j0 + cl;
-                if (gj >= n || (I == J && gi >= gj)) { nbrow[q] = 0.f; continue; }   // diagonal tiles: pairs i < j only, mirrored
+                if (gj >= n || (I == J && gi >= gj)) continue;     // diagonal tiles: pairs i < j only
                 const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
                 const size_t o = (size_t)gi * n + gj;
                 // the factor of v_m = s b' (L86), recomputed as kd_proj_tc3 did, and this pair's share of the penalty of Phi_m
-                const float sv = shrink_factor(nbp[q], cthr * wq[q]);
+                const float sv = shrink_ratio(cthr, pair_ratio(wq[q], nbp[q]));
                 red[1] += (double)(wq[q] * (sv * nbp[q]));
-                svbuf[row * TC_N + cl] = sv;
-                float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
+                svbuf[row * (TC_N + 1) + cl] = sv;      // stride 129: the 32 rows of a warp fall into 32 banks
+                const float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
                 // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
                 const float nbn = sqrtf(fmaxf(nb2, 0.f));
-                nbrow[q] = nbn;
+                const float rn = pair_ratio(wq[q], nbn);
+                nbp[q] = nbn;
+                wq[q] = rn;
                 if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
                     myflags |= 1u << (half * 16 + q);               // recomputed directly below
                 } else {
@@ -565,19 +665,21 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                     const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
                     const float om = 1.f - sv;
                     const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
-                    if (I == J) NB[o] = nbn;                       // diagonal tiles: guarded scalar stores (i < j only)
-                    NB[(size_t)gj * n + gi] = nbn;
+                    if (I == J) { NB[o] = nbn; Rm[o] = rn; }       // diagonal tiles: guarded scalar stores (i < j only)
+                    Rm[(size_t)gj * n + gi] = rn;
                     red[0] += (double)dv;
                 }
             }
             if (I != J) {
-                // off-diagonal tiles: this row's 16 values as four 16-byte stores (flagged entries are rewritten by the
-                // recompute phase, which runs after the barrier below)
+                // off-diagonal tiles: this row's 16 values as four 16-byte stores per array (flagged entries are rewritten by
+                // the recompute phase, which runs after the barrier below)
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4) {
                     const int gj = j0 + cb + q4 * 4;
-                    if (gj < n)
-                        st4(NB + (size_t)gi * n + gj, make_float4(nbrow[q4 * 4 + 0], nbrow[q4 * 4 + 1], nbrow[q4 * 4 + 2], nbrow[q4 * 4 + 3]));
+                    if (gj < n) {
+                        st4(NB + (size_t)gi * n + gj, make_float4(nbp[q4 * 4 + 0], nbp[q4 * 4 + 1], nbp[q4 * 4 + 2], nbp[q4 * 4 + 3]));
+                        st4(Rm + (size_t)gi * n + gj, make_float4(wq[q4 * 4 + 0], wq[q4 * 4 + 1], wq[q4 * 4 + 2], wq[q4 * 4 + 3]));
+                    }
                 }
             }
         }
@@ -596,7 +698,7 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                 m &= m - 1;
                 const int gj2 = j0 + gq * 32 + b;
                 const size_t o = (size_t)gi2 * n + gj2;
-                const float sv = svbuf[rr * TC_N + gq * 32 + b];
+                const float sv = svbuf[rr * (TC_N + 1) + gq * 32 + b];
                 float nbv = 0.f, dvv = 0.f;
                 for (int c = lane * 4; c < ld; c += 128) {
                     const float4 bb = ld4s(A + (size_t)gi2 * ld + c) - ld4s(A + (size_t)gj2 * ld + c);
@@ -611,9 +713,10 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
                     dvv += __shfl_xor_sync(0xffffffffu, dvv, of);
                 }
                 if (lane == 0) {
-                    const float nbn = sqrtf(nbv);
+                    const float nbn = sqrtf(nbv), rn = pair_ratio(__ldg(W + o), nbn);
                     NB[o] = nbn;
-                    NB[(size_t)gj2 * n + gi2] = nbn;
+                    Rm[o] = rn;
+                    Rm[(size_t)gj2 * n + gi2] = rn;
                     red[0] += (double)dvv;
                 }
             }
@@ -674,7 +777,7 @@ __global__ void __launch_bounds__(TC_THREADS) kd_prep_pairs(int n, int ld, int n
 __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int ntile, int nkb, const uint8_t* __restrict__ pre,
                                                        const float* __restrict__ nrm_part, int npad,
                                                        const float* __restrict__ A, const float* __restrict__ Ap,
-                                                       const float* __restrict__ W, float* NB, cc_scal* sc,
+                                                       const float* __restrict__ W, float* NB, float* __restrict__ Rm, cc_scal* sc,
                                                        double* part, double* hist_phi, double* hist_d,
                                                        cudaGraphConditionalHandle outer) {
     if (!sc->mm_active) return;
@@ -764,7 +867,7 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     __syncthreads();
     // every MMA is complete: the operand stages are free and serve as the 128 x 128 buffer of shrink factors
-    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, reinterpret_cast<float*>(sm), &fail_s, A, Ap, W, NB, cthr, sc, part,
+    pairs_tc_epilogue(n, ld, I, J, i0, j0, tmem_d, nrm, flag_s, reinterpret_cast<float*>(sm), &fail_s, A, Ap, W, NB, Rm, cthr, sc, part,
                       hist_phi, hist_d, outer);
 }
 
@@ -1113,7 +1216,7 @@ __global__ void __launch_bounds__(WS_THREADS, 1) kd_small_ws(int n, int ld, int 
 }
 
 // ---- kd_edges: block soft-threshold over the n x n matrices; the FFMA / n <= 64 paths only
-// (the tensor-core path never stores S: see shrink_factor)
+// (the tensor-core path never stores S: see shrink_ratio)
 __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, double* part,
                                                 int init_only) {
@@ -1166,11 +1269,14 @@ __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const floa
     }
 }
 
-// tensor-core path, cold start: the pair state is ||b|| itself (S4: V0 = D U0, so ||v|| = ||b|| and s = 1, which the
-// threshold factor 0 reproduces); kd_pairs wrote ||u0_i - u0_j||^2
-__global__ void kd_nb_sqrt(long long nn, float* __restrict__ NB) {
-    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += (long long)gridDim.x * blockDim.x)
-        NB[e] = sqrtf(NB[e]);
+// tensor-core path, cold start: the pair state is ||b|| and R = w / ||b|| (S4: V0 = D U0, so ||v|| = ||b|| and s = 1,
+// which the threshold factor 0 reproduces); kd_pairs wrote ||u0_i - u0_j||^2
+__global__ void kd_nb_init(long long nn, float* __restrict__ NB, const float* __restrict__ W, float* __restrict__ Rm) {
+    for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < nn; e += (long long)gridDim.x * blockDim.x) {
+        const float nb = sqrtf(NB[e]);
+        NB[e] = nb;
+        Rm[e] = pair_ratio(W[e], nb);
+    }
 }
 
 // dense-mode validation of W: symmetric, finite, > 0 off the diagonal
@@ -1205,15 +1311,15 @@ __global__ void kd_lab_hook(int n, const float* __restrict__ S, int* lab, int* c
     }
 }
 
-// the same on the tensor-core path, where S is implicit: s_ij = 0 iff ||b_ij|| <= cthr w_ij (shrink_factor's own test)
-__global__ void kd_lab_hook_nb(int n, const float* __restrict__ NB, const float* __restrict__ W, float cthr, int* lab, int* changed) {
+// the same on the tensor-core path, where S is implicit: s_ij = 0 iff cthr R_ij >= 1 (shrink_ratio's own test)
+__global__ void kd_lab_hook_r(int n, const float* __restrict__ Rm, float cthr, int* lab, int* changed) {
     const int i = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);   // one warp per row
     const int lane = threadIdx.x & 31;
     if (i >= n) return;
     const int li = lab[i];
     int m = li;
     for (int j = lane; j < n; j += 32)
-        if (j != i && shrink_factor(NB[(size_t)i * n + j], cthr * W[(size_t)i * n + j]) == 0.f) m = min(m, lab[j]);
+        if (j != i && shrink_ratio(cthr, Rm[(size_t)i * n + j]) == 0.f) m = min(m, lab[j]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m = min(m, __shfl_xor_sync(0xffffffffu, m, o));
     if (lane == 0 && m < li) {
@@ -1351,11 +1457,11 @@ static void launch_proj(cc_handle* h) {
 
 void ccd_proj(cc_handle* h) {
     if (h->dn_tc) {
-        const int nkb = (int)((h->n + TC_K - 1) / TC_K);
+        const int nkb = (int)((h->n + FK - 1) / FK);
         dim3 g((unsigned)((h->ld + TC_N - 1) / TC_N), (unsigned)((h->n + TC_M - 1) / TC_M));
         dim3 gp((unsigned)nkb, g.x);
         kd_prep_proj<<<gp, TC_THREADS, 0, h->stream>>>((int)h->n, (int)h->ld, nkb, h->Ap, h->abar, h->pre_B, h->sc);
-        kd_proj_tc3<<<g, TC_THREADS, F_SMEM, h->stream>>>((int)h->n, (int)h->ld, nkb, h->NB2d, h->Wd, h->pre_B, h->Ap, h->U, h->X,
+        kd_proj_tc3<<<g, F_THREADS, F_SMEM, h->stream>>>((int)h->n, (int)h->ld, nkb, h->Rd, h->pre_B, h->Ap, h->U, h->X,
                                                           h->mask, h->ubar, h->abar, h->A, h->sc,
                                                           h->part + 0 * CC_MAXBLK * CC_NPART);
         return;
@@ -1379,7 +1485,7 @@ void ccd_pairs(cc_handle* h) {
         kd_prep_pairs<<<gp, TC_THREADS, 0, h->stream>>>((int)h->n, (int)h->ld, nkb, h->A, h->Ap, h->abar, h->pre_pairs,
                                                        h->nrm_part, npad, h->sc);
         kd_pairs_tc2<<<(unsigned)(ntile * (ntile + 1) / 2), TC_THREADS, PK2_SMEM, h->stream>>>(
-            (int)h->n, (int)h->ld, ntile, nkb, h->pre_pairs, h->nrm_part, npad, h->A, h->Ap, h->Wd, h->NB2d,
+            (int)h->n, (int)h->ld, ntile, nkb, h->pre_pairs, h->nrm_part, npad, h->A, h->Ap, h->Wd, h->NB2d, h->Rd,
             h->sc, h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, h->cond_outer);
         return;
     }
@@ -1400,7 +1506,7 @@ void ccd_edges(cc_handle* h, int init_only) {
 
 void ccd_lab_hook(cc_handle* h, int* changed) {
     if (h->dn_tc)
-        kd_lab_hook_nb<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->NB2d, h->Wd, h->dn_cthr, h->lab, changed);
+        kd_lab_hook_r<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->Rd, h->dn_cthr, h->lab, changed);
     else
         kd_lab_hook<<<(unsigned)((h->n + 7) / 8), 256, 0, h->stream>>>((int)h->n, h->Sd, h->lab, changed);
 }
@@ -1463,8 +1569,9 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (h->dn_tc) {
         const size_t ntile = (size_t)((n + TC_M - 1) / TC_M), nkb = (size_t)((h->ld + PK - 1) / PK);
         e = cc_dev_alloc((void**)&h->pre_pairs, ntile * nkb * PK_SIDE, h->stream);
-        const size_t nkb32 = (size_t)((n + TC_K - 1) / TC_K), nct = (size_t)((h->ld + TC_N - 1) / TC_N);
-        if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->pre_B, nct * nkb32 * TC_SIDE, h->stream);
+        const size_t nkb16 = (size_t)((n + FK - 1) / FK), nct = (size_t)((h->ld + TC_N - 1) / TC_N);
+        if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->pre_B, nct * nkb16 * F_SIDE, h->stream);
+        if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->Rd, (size_t)nn * sizeof(float), h->stream);
         if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->nrm_part, nkb * 3 * ntile * TC_M * sizeof(float), h->stream);
         if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }
     }
@@ -1506,7 +1613,7 @@ void ccd_init_state(cc_handle* h) {
     cudaMemcpyAsync(h->Ap, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
     launch_pairs(h, h->U, h->U, 1);            // ||u0_i - u0_j||^2 by direct differences (every dense path starts here)
     if (h->dn_tc) {
-        kd_nb_sqrt<<<h->grid_nodes, 256, 0, h->stream>>>((long long)h->n * h->n, h->NB2d);
+        kd_nb_init<<<h->grid_nodes, 256, 0, h->stream>>>((long long)h->n * h->n, h->NB2d, h->Wd, h->Rd);
         h->dn_cthr = 0.f;                      // threshold factor 0: s = 1 wherever ||b|| > 0
     } else {
         ccd_edges(h, 1);

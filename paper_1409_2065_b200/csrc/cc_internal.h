@@ -87,14 +87,15 @@ struct cc_handle {
     float* dinv;                      // n: 1 / (1 + |N_i|)
     float* Minv;                      // n x n: (D^-1 (I+L))^-1 for n <= CC_INV_NMAX, else NULL (CG solver)
     // dense mode (complete graph): n x n matrices instead of the CSR arrays
-    float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices); tensor-core path: Wd and
-                                      // NB2d = ||b|| only (S and ||v|| are recomputed where they are used)
+    float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices); tensor-core path: Wd, NB2d =
+                                      // ||b|| (pairs i < j) and Rd only (S and ||v|| are recomputed where they are used)
     float *ubar, *abar;               // column means of U and A'
     float* dbar;                      // column means of A - U (dense mode; subtracted by k_update)
     double* colps;                    // partial column sums
     uint8_t* pre_pairs;               // kd_prep_pairs: TF32 hi/lo operand tiles in the tensor core's smem layout
     float* nrm_part;                  // per-K-block partial row norms
-    uint8_t* pre_B;                   // kd_proj_tc3's B operand (A' - abar)^T (by kd_prep_proj), hi/lo tiles
+    uint8_t* pre_B;                   // kd_proj_tc3's B operand (A' - abar)^T, TF32 hi/lo tiles in the operand layout (by kd_prep_proj)
+    float* Rd;                        // tensor-core path: R = w / ||b|| (n x n, both triangles): all the contraction needs to form S
     int dn_ksplit, dn_big, dn_tc, dn_small, dn_small_cs, dn_small_grid;
     float dn_cthr;                    // tensor-core path: the threshold factor gamma d / rho that defines the current implicit S
     // scalars

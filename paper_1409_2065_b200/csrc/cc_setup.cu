@@ -451,7 +451,7 @@ int ccu_min_margin(cc_handle* h, double* margin_out) {
 
 void ccu_free(cc_handle* h) {
     void* ptrs[] = {h->X, h->U, h->A, h->Ap, h->Z, h->R, h->Pv, h->Sv, h->Dl, h->Uc, h->mask, h->colmean, h->rowptr,
-                    h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Minv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->dbar, h->colps, h->pre_pairs, h->nrm_part, h->pre_B, h->sc, h->part,
+                    h->rowup, h->col, h->peer, h->w, h->s, h->vn, h->nb2, h->tmpE, h->dinv, h->Minv, h->Wd, h->Sd, h->VNd, h->NB2d, h->ubar, h->abar, h->dbar, h->colps, h->pre_pairs, h->nrm_part, h->pre_B, h->Rd, h->sc, h->part,
                     h->hist_phi, h->hist_d, h->dout, h->dflag, h->pt_nbpart, h->pt_spart, h->snapU, h->snapLab, h->lab, h->lab_flag, h->lab_rank, h->order, h->rowdesc};
     for (void* q : ptrs)
         cc_dev_free(q, h->stream);

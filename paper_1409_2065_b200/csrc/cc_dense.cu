@@ -813,6 +813,19 @@ __global__ void __launch_bounds__(TC_THREADS, 1) kd_pairs_tc2(int n, int ld, int
     const uint32_t tmem_d = tmem_base_s;
     const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) | ((uint32_t)(TC_M >> 4) << 24);
 
+    // The epilogue reads this tile of ||b|| and W (and writes ||b|| and R) once the MMAs are done; it was bound by the
+    // latency of those loads from DRAM (ncu: long-scoreboard stalls 10.8 per issue, issue slots 18 % busy).  The threads
+    // have nothing to do while the tensor core works, so they pull the tile's lines into L2 now: 128 rows x 512 bytes
+    // per array = 512 lines, one per thread and array.
+    {
+        const int pr = tid >> 2, pc = (tid & 3) * 32;
+        if (i0 + pr < n && j0 + pc < n) {
+            const size_t o = (size_t)(i0 + pr) * n + j0 + pc;
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(NB + o));
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(W + o));
+            asm volatile("prefetch.global.L2 [%0];" :: "l"(Rm + o));
+        }
+    }
     if (tid == 32) {
         // ===== producer: TMA bulk copies =====
         const uint8_t* srcI = pre + (size_t)I * nkb * PK_SIDE;

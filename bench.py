@@ -226,8 +226,11 @@ def impl_bytes(kernel, n, p, nnz, masked, dense=False):
         "k_cg_update": 6 * npb + 4 * n,                      # p, s, A, uc in; A, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
         "k_update": (5 * npb if dense else 8 * npb + 16 * nnz) + (n * p if masked else 0),
-        "kd_proj": (4 * npb if n <= 64 else 8 * n * n + 5 * npb) + (n * p if masked else 0),
-        "kd_pairs": 2 * npb + (n * n // 2) * 12 + 4 * n * n,
+        # n <= 64: the fused kernel streams U, A', X in and A out.  Tensor-core path (n >= 128): kd_proj_tc3 reads the ratio
+        # matrix R (n x n) + the pre-split B operand (2 np, re-read per row tile from L2) + 5 node arrays; kd_pairs_tc2 reads
+        # ||b||, R, W of the upper triangle and writes ||b|| (upper) and R (both triangles) + the pre-split operands
+        "kd_proj": (4 * npb if n <= 64 else 4 * n * n + 2 * npb + 5 * npb) + (n * p if masked else 0),
+        "kd_pairs": 3 * npb + (n * n // 2) * 12 + (n * n // 2) * 4 + 4 * n * n,
         "kd_edges": 16 * n * n,
     }[kernel]
 

@@ -120,6 +120,17 @@ int cc_knn_weights_geodesic(int64_t n, int64_t p, const float* X, const uint8_t*
 int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint8_t* mask, float phi, int32_t normalize,
                      float* W_out, void* stream);
 
+/* The same weights for callers that must not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): this entry point calls no cudaMalloc / cudaFree or any allocating routine.  The column slices'
+ * partial sums, which cc_dense_weights keeps in a temporary buffer, live in a static device array of 2 Mi floats (8 MB) that
+ * every GPU loading the library holds until the process exits.  A problem whose slices need more (n * n * slices floats,
+ * twice that with a mask; e.g. 52 x 200,000 fits with or without a mask, 64 x 200,000 with a mask does not) is rejected with CC_EINVAL and a message;
+ * problems with enough pair tiles to fill the GPU (n >= ~1100) use no scratch and are never rejected.  No normalisation
+ * (S8): scale the result yourself.  Results are bit-identical to cc_dense_weights with normalize = 0.
+ * ALL calls share the one array: calls that overlap on the GPU (other streams, threads) race -- serialise them.
+ * X, mask, W_out: DEVICE, as in cc_dense_weights.  Synchronises `stream`. */
+int cc_dense_weights_noalloc(int64_t n, int64_t p, const float* X, const uint8_t* mask, float phi, float* W_out, void* stream);
+
 /* Release the three arrays cc_knn_weights returned (NULLs are ignored). */
 void cc_free_graph(int64_t* rowptr, int32_t* col, float* w);
 

@@ -22,7 +22,7 @@ _lib = ctypes.CDLL(LIB_PATH)
 
 CC_OK, CC_EINVAL, CC_EGRAPH, CC_EMASK, CC_ENOMEM, CC_ECUDA, CC_ESTATE, CC_ENOCONV = 0, -1, -2, -3, -4, -5, -6, -7
 
-SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_knn_weights_composite", "cc_knn_weights_geodesic", "cc_dense_weights", "cc_graph_components",
+SYMBOLS = ("cc_default_params", "cc_knn_weights", "cc_knn_weights_composite", "cc_knn_weights_geodesic", "cc_dense_weights", "cc_dense_weights_noalloc", "cc_graph_components",
            "cc_smallest_connected_k", "cc_free_graph", "cc_create", "cc_solve", "cc_solve_continuation", "cc_path", "cc_path_continuation",
            "cc_get_U", "cc_get_projection", "cc_principal_components", "cc_clusters", "cc_get_history", "cc_get_stats", "cc_get_profile", "cc_reset_profile",
            "cc_reset", "cc_get_counts",
@@ -46,6 +46,7 @@ _lib.cc_knn_weights_composite.argtypes = [_i64, _i64, _vp, _vp, _i32, _vp, _P(ct
 _lib.cc_knn_weights_geodesic.argtypes = [_i64, _i64, _vp, _vp, _vp, ctypes.c_float, ctypes.c_float, _i32,
                                          ctypes.c_float, _i32, _P(_vp), _P(_vp), _P(_vp), _P(_i64), _vp]
 _lib.cc_dense_weights.argtypes = [_i64, _i64, _vp, _vp, ctypes.c_float, _i32, _vp, _vp]
+_lib.cc_dense_weights_noalloc.argtypes = [_i64, _i64, _vp, _vp, ctypes.c_float, _vp, _vp]
 _lib.cc_graph_components.argtypes = [_i64, _vp, _vp, _vp, _P(_i32), _vp]
 _lib.cc_smallest_connected_k.argtypes = [_i64, _i64, _vp, _vp, _i32, _P(_i32), _vp]
 _lib.cc_free_graph.argtypes = [_vp, _vp, _vp]
@@ -229,6 +230,12 @@ def cc_dense_weights(n, p, X, mask, phi, normalize=False):
     W = torch.empty(n, n, dtype=torch.float32, device=X.device)
     _check(_lib.cc_dense_weights(n, p, _ptr(X), _ptr(mask), phi, 1 if normalize else 0, _ptr(W), _stream()))
     return W
+
+
+def cc_dense_weights_noalloc(n, p, X, mask, phi, W_out):
+    """cc_dense_weights without any allocation: W_out is a caller-made (n, n) fp32 device tensor (see cc_b200.h)."""
+    _check(_lib.cc_dense_weights_noalloc(n, p, _ptr(X), _ptr(mask), phi, _ptr(W_out), _stream()))
+    return W_out
 
 
 def cc_graph_components(n, rowptr, col, labels_out):

@@ -1757,3 +1757,80 @@ extern "C" int cc_dense_weights(int64_t n, int64_t p, const float* X, const uint
     }
     return CC_OK;
 }
+
+// ---- cc_dense_weights_noalloc: the same weights with no allocation at all ----------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+// cc_dense_weights takes the column slices' partial sums from a cudaMalloc'ed buffer; here they live in a file-scope device
+// array of CC_NOALLOC_FLOATS floats (8 MB; every GPU that loads the library holds it until the process exits).
+// In host code the array's NAME is only a host-side stand-in, not a device address: its address is taken once per device
+// with cudaGetSymbolAddress (that device current) and the pointer is what the kernels get.
+// Every call shares the array (it keeps the last call's contents; nothing in it has to start at zero, because kd_weights
+// writes every entry kd_weights_fin reads), so calls that overlap on the GPU -- different streams, threads or processes of
+// one context -- RACE: serialise them.
+#define CC_NOALLOC_FLOATS (2u << 20)
+static __device__ __align__(256) float cc_noalloc_scratch[CC_NOALLOC_FLOATS];
+static float* cc_noalloc_ptr[64];     // per device: the array's device address (NULL = not looked up yet)
+
+extern "C" int cc_dense_weights_noalloc(int64_t n, int64_t p, const float* X, const uint8_t* mask, float phi, float* W_out,
+                                        void* stream) {
+    if (!X || !W_out || n < 2 || p < 1 || !(phi >= 0.f) || n > 46340) {
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights_noalloc: need n in [2, 46340], p >= 1, phi >= 0, non-NULL pointers");
+        return CC_EINVAL;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 148;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess || dev < 0 || dev >= 64) {
+        cudaGetLastError();
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights_noalloc: %s", e != cudaSuccess ? cudaGetErrorString(e) : "device ordinal >= 64");
+        return CC_ECUDA;
+    }
+    if (!cc_noalloc_ptr[dev]) {       // set-up, once per device, with that device current
+        float* ptr = nullptr;
+        e = cudaGetSymbolAddress((void**)&ptr, cc_noalloc_scratch);
+        if (e != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            return CC_ECUDA;
+        }
+        cc_noalloc_ptr[dev] = ptr;
+    }
+    float* part = cc_noalloc_ptr[dev];
+    // the slicing rule of cc_dense_weights, so that both entry points add the same partial sums in the same order
+    const int ntile = (int)((n + PT - 1) / PT);
+    const unsigned grid = (unsigned)(ntile * (ntile + 1) / 2);
+    long long ksplit = grid >= (unsigned)sms ? 1 : (2LL * sms + grid - 1) / grid;
+    const long long kmax = (p + 8LL * PCK - 1) / (8LL * PCK);
+    if (ksplit > kmax) ksplit = kmax;
+    if (ksplit <= 1) {                // enough pair tiles to fill the GPU: no scratch is used at all
+        if (mask) kd_weights<true><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)p, nullptr);
+        else kd_weights<false><<<grid, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)p, nullptr);
+    } else {
+        const long long cols = ((p + ksplit - 1) / ksplit + PCK - 1) / PCK * PCK;
+        ksplit = (p + cols - 1) / cols;
+        const unsigned long long need = (unsigned long long)ksplit * n * n * (mask ? 2 : 1);
+        if (need > CC_NOALLOC_FLOATS) {
+            snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights_noalloc: n=%lld, p=%lld%s needs %llu floats of scratch, the static "
+                     "array holds %u (8 MB): use cc_dense_weights", (long long)n, (long long)p, mask ? " with a mask" : "", need,
+                     (unsigned)CC_NOALLOC_FLOATS);
+            return CC_EINVAL;
+        }
+        const dim3 g2(grid, (unsigned)ksplit);
+        const unsigned gf = (unsigned)(((size_t)n * n + 255) / 256);
+        if (mask) {
+            kd_weights<true><<<g2, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)cols, part);
+            kd_weights_fin<true><<<gf, 256, 0, st>>>((int)n, (int)p, (int)ksplit, phi, part, W_out);
+        } else {
+            kd_weights<false><<<g2, 256, 0, st>>>((int)n, (int)p, ntile, phi, X, mask, W_out, (int)cols, part);
+            kd_weights_fin<false><<<gf, 256, 0, st>>>((int)n, (int)p, (int)ksplit, phi, part, W_out);
+        }
+    }
+    e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(cc_g_err, sizeof(cc_g_err), "cc_dense_weights_noalloc: %s", cudaGetErrorString(e));
+        return CC_ECUDA;
+    }
+    return CC_OK;
+}

@@ -21,6 +21,9 @@
 namespace {
 
 // ---- column means of two node arrays, deterministic two-stage ------------------------------------
+// Stage 1: slice sl of the rows, a thread per column (coalesced rows), up to 256 slices so that the two passes over the
+// node arrays fill the GPU (with 32 slices the grid was 64 CTAs and kd_colsum1 took 73 us per iteration at n = 8192,
+// p = 256, kd_dsum1 41 us).  Stage 2: a warp per column adds the slices -- lanes stride over them, then a fixed shuffle tree.
 __global__ void kd_colsum1(int n, int ld, int nslice, const float* __restrict__ U, const float* __restrict__ Ap,
                            double* __restrict__ ps, cc_scal* sc) {
     if (!sc->mm_active) return;
@@ -30,7 +33,14 @@ __global__ void kd_colsum1(int n, int ld, int nslice, const float* __restrict__ 
     if (c >= ld) return;
     const int r0 = (int)((long long)n * sl / nslice), r1 = (int)((long long)n * (sl + 1) / nslice);
     double su = 0.0, sa = 0.0;
-    for (int i = r0; i < r1; ++i) {
+    int i = r0;
+    for (; i + 4 <= r1; i += 4) {          // four rows in flight
+        const float u0 = U[(size_t)i * ld + c], u1 = U[(size_t)(i + 1) * ld + c], u2 = U[(size_t)(i + 2) * ld + c], u3 = U[(size_t)(i + 3) * ld + c];
+        const float a0 = Ap[(size_t)i * ld + c], a1 = Ap[(size_t)(i + 1) * ld + c], a2 = Ap[(size_t)(i + 2) * ld + c], a3 = Ap[(size_t)(i + 3) * ld + c];
+        su += (double)u0; su += (double)u1; su += (double)u2; su += (double)u3;
+        sa += (double)a0; sa += (double)a1; sa += (double)a2; sa += (double)a3;
+    }
+    for (; i < r1; ++i) {
         su += (double)U[(size_t)i * ld + c];
         sa += (double)Ap[(size_t)i * ld + c];
     }
@@ -38,19 +48,26 @@ __global__ void kd_colsum1(int n, int ld, int nslice, const float* __restrict__ 
     ps[((size_t)sl * 2 + 1) * ld + c] = sa;
 }
 
+__device__ __forceinline__ double warp_sum_slices(const double* __restrict__ p, size_t stride, int nslice, int lane) {
+    double v = 0.0;
+    for (int sl = lane; sl < nslice; sl += 32) v += p[(size_t)sl * stride];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
 __global__ void kd_colsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ ubar,
                            float* __restrict__ abar, cc_scal* sc) {
     if (!sc->mm_active) return;
     count_launch(sc);
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;    // a warp per column
     if (c >= ld) return;
-    double su = 0.0, sa = 0.0;
-    for (int sl = 0; sl < nslice; ++sl) {
-        su += ps[((size_t)sl * 2 + 0) * ld + c];
-        sa += ps[((size_t)sl * 2 + 1) * ld + c];
+    const double su = warp_sum_slices(ps + c, (size_t)2 * ld, nslice, lane);
+    const double sa = warp_sum_slices(ps + ld + c, (size_t)2 * ld, nslice, lane);
+    if (lane == 0) {
+        ubar[c] = (float)(su / n);
+        abar[c] = (float)(sa / n);
     }
-    ubar[c] = (float)(su / n);
-    abar[c] = (float)(sa / n);
 }
 
 // ---- kd_dsum: dbar_c = mean_i (a_ic - u_ic).  The projection satisfies 1'(A - U) = 0 exactly (1'L = 0); in fp32 the
@@ -65,18 +82,23 @@ __global__ void kd_dsum1(int n, int ld, int nslice, const float* __restrict__ A,
     if (c >= ld) return;
     const int r0 = (int)((long long)n * sl / nslice), r1 = (int)((long long)n * (sl + 1) / nslice);
     double s = 0.0;
-    for (int i = r0; i < r1; ++i) s += (double)(A[(size_t)i * ld + c] - U[(size_t)i * ld + c]);
+    int i = r0;
+    for (; i + 4 <= r1; i += 4) {
+        const float d0 = A[(size_t)i * ld + c] - U[(size_t)i * ld + c], d1 = A[(size_t)(i + 1) * ld + c] - U[(size_t)(i + 1) * ld + c];
+        const float d2 = A[(size_t)(i + 2) * ld + c] - U[(size_t)(i + 2) * ld + c], d3 = A[(size_t)(i + 3) * ld + c] - U[(size_t)(i + 3) * ld + c];
+        s += (double)d0; s += (double)d1; s += (double)d2; s += (double)d3;
+    }
+    for (; i < r1; ++i) s += (double)(A[(size_t)i * ld + c] - U[(size_t)i * ld + c]);
     ps[(size_t)sl * ld + c] = s;
 }
 
 __global__ void kd_dsum2(int n, int ld, int nslice, const double* __restrict__ ps, float* __restrict__ dbar, cc_scal* sc) {
     if (!sc->mm_active) return;
     count_launch(sc);
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    const int c = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
     if (c >= ld) return;
-    double s = 0.0;
-    for (int sl = 0; sl < nslice; ++sl) s += ps[(size_t)sl * ld + c];
-    dbar[c] = (float)(s / n);
+    const double s = warp_sum_slices(ps + c, (size_t)ld, nslice, lane);
+    if (lane == 0) dbar[c] = (float)(s / n);
 }
 
 // ---- kd_proj ---------------------------------------------------------------------------------------
@@ -1396,12 +1418,17 @@ __global__ void kd_wscale(long long nn, float* __restrict__ W, const double* __r
 // =============================================================================================
 // Host side
 // =============================================================================================
-static const int kSliceDense = 32;
+static const int kSliceDense = 256;      // most row slices of the column-sum kernels
+static int dense_slices(const cc_handle* h) {       // about 32 rows per slice
+    long long s = h->n / 32;
+    return (int)(s < 1 ? 1 : (s > kSliceDense ? kSliceDense : s));
+}
 
 void ccd_colmeans(cc_handle* h) {
-    dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)kSliceDense);
-    kd_colsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->U, h->Ap, h->colps, h->sc);
-    kd_colsum2<<<(unsigned)((h->ld + 127) / 128), 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->colps,
+    const int ns = dense_slices(h);
+    dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)ns);
+    kd_colsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, ns, h->U, h->Ap, h->colps, h->sc);
+    kd_colsum2<<<(unsigned)((h->ld + 7) / 8), 256, 0, h->stream>>>((int)h->n, (int)h->ld, ns, h->colps,
                                                                       h->ubar, h->abar, h->sc);
 }
 
@@ -1588,9 +1615,10 @@ void ccd_iteration(cc_handle* h) {
     ccd_colmeans(h);
     ccd_proj(h);
     {
-        dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)kSliceDense);
-        kd_dsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->A, h->U, h->colps, h->sc);
-        kd_dsum2<<<(unsigned)((h->ld + 127) / 128), 128, 0, h->stream>>>((int)h->n, (int)h->ld, kSliceDense, h->colps, h->dbar, h->sc);
+        const int ns = dense_slices(h);
+        dim3 g1((unsigned)((h->ld + 127) / 128), (unsigned)ns);
+        kd_dsum1<<<g1, 128, 0, h->stream>>>((int)h->n, (int)h->ld, ns, h->A, h->U, h->colps, h->sc);
+        kd_dsum2<<<(unsigned)((h->ld + 7) / 8), 256, 0, h->stream>>>((int)h->n, (int)h->ld, ns, h->colps, h->dbar, h->sc);
     }
     ccd_pairs(h);
     ccs_update_nodes(h);

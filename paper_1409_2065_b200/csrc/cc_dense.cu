@@ -1477,6 +1477,7 @@ void ccd_pairs(cc_handle* h) {
 }
 
 static void launch_small(cc_handle* h) {
+    if (h->dn_small_tc) { ccd_small_tc_launch(h); return; }
     kd_small_ws<<<h->dn_small_grid, WS_THREADS, WS_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X,
                                                                       h->mask, h->Wd, h->VNd, h->A, h->NB2d, h->sc,
                                                                       h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi,
@@ -1531,7 +1532,8 @@ int ccd_setup(cc_handle* h, const float* W) {
         }
         h->dn_small_cs = cs;
         h->dn_small_grid = (int)g;
-        h->dn_ksplit = (int)g * cs;
+        h->dn_small_tc = ccd_small_tc_setup(h);     // the tensor-core version (cc_small.cu) replaces the launch shape when it can run
+        h->dn_ksplit = h->dn_small_grid * h->dn_small_cs;
         ks = h->dn_ksplit;
     }
     const long long bproj = ((h->ld + 63) / 64) * ((n + 63) / 64);   // upper bound over the tile shapes used
@@ -1546,7 +1548,7 @@ int ccd_setup(cc_handle* h, const float* W) {
     e = cc_dev_alloc((void**)&h->NB2d, (size_t)nn * ks * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->ubar, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->abar, (size_t)h->ld * sizeof(float), h->stream);
-    if (e == cudaSuccess && !h->dn_small) e = cc_dev_alloc((void**)&h->dbar, (size_t)h->ld * sizeof(float), h->stream);
+    if (e == cudaSuccess && (!h->dn_small || h->dn_small_tc)) e = cc_dev_alloc((void**)&h->dbar, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess && h->dbar) e = cudaMemsetAsync(h->dbar, 0, (size_t)h->ld * sizeof(float), h->stream);
     if (e == cudaSuccess) e = cc_dev_alloc((void**)&h->colps, (size_t)kSliceDense * 2 * h->ld * sizeof(double), h->stream);
     if (e != cudaSuccess) { cudaGetLastError(); snprintf(h->err, sizeof(h->err), "dense mode: cudaMalloc failed"); return CC_ENOMEM; }

@@ -96,7 +96,8 @@ struct cc_handle {
     float* nrm_part;                  // per-K-block partial row norms
     uint8_t* pre_B;                   // kd_proj_tc3's B operand (A' - abar)^T, TF32 hi/lo tiles in the operand layout (by kd_prep_proj)
     float* Rd;                        // tensor-core path: R = w / ||b|| (n x n, both triangles): all the contraction needs to form S
-    int dn_ksplit, dn_big, dn_tc, dn_small, dn_small_cs, dn_small_grid;
+    int dn_ksplit, dn_big, dn_tc, dn_small, dn_small_cs, dn_small_grid, dn_small_tc;
+    unsigned long long dn_small_tm[4][16];          // kd_small_tc: the tensor maps of U, A', X, A (CUtensorMap, 128 bytes each)
     float dn_cthr;                    // tensor-core path: the threshold factor gamma d / rho that defines the current implicit S
     // scalars
     cc_scal* sc;                      // device
@@ -156,6 +157,10 @@ void ccd_lab_hook(cc_handle* h, int* changed);
 int ccd_solve_eager(cc_handle* h, int maxit);
 int ccd_build_graph(cc_handle* h);
 void ccs_update_nodes(cc_handle* h);  // k_update, node part only (dense mode)
+// ---- cc_small.cu (a9, n <= 64): the fused kernel with the contraction on the tensor cores
+int ccd_small_tc_setup(cc_handle* h);     // 1: use it (sets dn_small_cs, dn_small_grid); 0: not available
+int ccd_small_tc_maps(cc_handle* h);      // after the node arrays exist
+void ccd_small_tc_launch(cc_handle* h);
 
 // ---- cc_setup.cu ------------------------------------------------------------------------------------
 int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, const int64_t* rowptr,

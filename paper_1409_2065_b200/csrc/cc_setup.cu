@@ -397,6 +397,7 @@ int ccu_validate_and_build(cc_handle* h, const float* X, const uint8_t* mask, co
         CC_TRY(dmalloc(h, a, nl));
         CC_CUDA(h, cudaMemsetAsync(*a, 0, nl * sizeof(float), st));
     }
+    if (h->dense && h->dn_small_tc) CC_TRY(ccd_small_tc_maps(h));     // the TMA tensor maps of U, A', X, A
     CC_TRY(dmalloc(h, &h->s, (size_t)nnz_csr));
     CC_TRY(dmalloc(h, &h->vn, (size_t)nnz_csr));
     CC_TRY(dmalloc(h, &h->tmpE, (size_t)nnz_csr));

@@ -129,8 +129,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
     __shared__ __align__(8) uint64_t mma_done, xfull, full[ST_NBUF];
     __shared__ uint32_t tmem_base_s;
     __shared__ __align__(16) float rsS[ST_K];
-    __shared__ unsigned char t_ty[272], t_tx[272];      // pair tiles: 4 rows i (block ty) x 2 rows j (block tx)
-    __shared__ int ntiles_s, fail_s;
+    __shared__ int fail_s;
     const int tid = threadIdx.x, warp = tid >> 5;
     const int n4 = (n + 3) & ~3;
     // shared memory: [S operand | 2 data buffers {UA, P} | X buffer], every array 32 KB
@@ -142,17 +141,26 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
     float* xbuf = dbuf + (size_t)nbuf * 2 * bufsz;
     const uint32_t tx_bytes = (uint32_t)n * 4u * 128u;                  // one array of one chunk as the copy engine counts it
 
+    const int nchunks = (ld + ST_CN - 1) / ST_CN;
+    const int nmine = blockIdx.x < nchunks ? (nchunks - 1 - blockIdx.x) / gridDim.x + 1 : 0;   // chunks this CTA walks
     if (tid == 0) {
         fail_s = 0;
-        int k = 0;
-        const int nt4 = n4 >> 2;
-        for (int ty = 0; ty < nt4; ++ty)
-            for (int tx = 2 * ty; tx < 2 * nt4; ++tx) { t_ty[k] = (unsigned char)ty; t_tx[k] = (unsigned char)tx; ++k; }
-        ntiles_s = k;
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mma_done)));
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&xfull)));
         for (int b = 0; b < ST_NBUF; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&full[b])));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // the first chunks go to the copy engine at once (it writes rows < n only; the rest of this prologue touches other rows)
+        for (int kk = 0; kk < nbuf && kk < nmine; ++kk) {
+            const int c0 = (blockIdx.x + kk * gridDim.x) * ST_CN;
+            const uint32_t bar = smem_u32(&full[kk]), dst = smem_u32(dbuf + (size_t)kk * 2 * bufsz);
+            expect_tx(bar, 2u * tx_bytes);
+            small_issue_array(dst, &tmU, c0, bar);
+            small_issue_array(dst + bufsz * 4, &tmP, c0, bar);
+        }
+        if (nmine > 0) {
+            expect_tx(smem_u32(&xfull), tx_bytes);
+            small_issue_array(smem_u32(xbuf), &tmX, blockIdx.x * ST_CN, smem_u32(&xfull));
+        }
     }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(ST_TMEM));
@@ -175,30 +183,18 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
         sts32(bop + off, h);
         sts32(bop + ST_BOP / 2 + off, l);
     }
-    // the copy engine never writes rows >= n: zero once (the pair tiles read whole 4-row tiles)
-    for (int t = tid; t < (nbuf * 2 + 1) * bufsz; t += ST_THREADS) dbuf[t] = 0.f;      // (the X buffer follows the data buffers)
+    // the copy engine never writes rows >= n: zero once (the pair tiles read whole 4-row tiles, the column walks whole
+    // 8-row blocks); the X buffer follows the data buffers
+    {
+        const int padf = (ST_K - n) * 32;                               // floats to clear per column group
+        for (int t = tid; t < (nbuf * 2 + 1) * 4 * padf; t += ST_THREADS) dbuf[(t / padf) * ST_GRP + n * 32 + t % padf] = 0.f;
+    }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t tmem_d = tmem_base_s;
-    const int nchunks = (ld + ST_CN - 1) / ST_CN;
-    const int nmine = blockIdx.x < nchunks ? (nchunks - 1 - blockIdx.x) / gridDim.x + 1 : 0;   // chunks this CTA walks
     double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
-    // the first chunks go to the copy engine at once
-    if (tid == ST_PROJ)
-        for (int kk = 0; kk < nbuf && kk < nmine; ++kk) {
-            const int c0 = (blockIdx.x + kk * gridDim.x) * ST_CN;
-            const uint32_t bar = smem_u32(&full[kk]), dst = smem_u32(dbuf + (size_t)kk * 2 * bufsz);
-            expect_tx(bar, 2u * tx_bytes);
-            small_issue_array(dst, &tmU, c0, bar);
-            small_issue_array(dst + bufsz * 4, &tmP, c0, bar);
-        }
-    if (tid == 0 && nmine > 0) {
-        expect_tx(smem_u32(&xfull), tx_bytes);
-        small_issue_array(smem_u32(xbuf), &tmX, blockIdx.x * ST_CN, smem_u32(&xfull));
-    }
-
     if (tid < ST_PROJ) {
         // ================= projection role: thread = column c of the chunk = lane c of tensor memory =================
         const int c = tid;
@@ -353,12 +349,14 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
     }
 
     // ================= pair role (and, after the loop, everybody): tiles of 4 x 2 pairs, packed fp32 arithmetic =================
-    const int ntiles = ntiles_s;
+    const int nt2 = n4 >> 1, ntiles = (n4 >> 2) * ((n4 >> 2) + 1);      // row block ty owns the 2-row blocks tx = 2 ty .. nt2 - 1
     const bool pair_role = tid >= ST_PROJ;
     const int rt = tid - ST_PROJ;
     const bool pair_thread = pair_role && rt < ntiles * cs_per_tile;
     const int tile = pair_thread ? rt / cs_per_tile : 0, cph = pair_thread ? rt % cs_per_tile : 0;
-    const int ty = t_ty[tile], tx = t_tx[tile];           // rows 4 ty + a (a < 4) against rows 2 tx + b (b < 2)
+    int ty = 0, tx = tile;                                // rows 4 ty + a (a < 4) against rows 2 tx + b (b < 2)
+    while (tx >= nt2 - 2 * ty) { tx -= nt2 - 2 * ty; ++ty; }
+    tx += 2 * ty;
     f32x2 nb[4][2], dv[4][2];                             // (even columns, odd columns) partial sums
     if (pair_role) {
         float sv[4][2];

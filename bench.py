@@ -511,7 +511,7 @@ def run_ours(args):
     elif dense_small:
         # genotype-like: near the ridge: report against HBM (7 node arrays per iteration) and print the FP32 figure beside it
         v = per_kernel["kd_proj"]
-        roofline = {"bound": "hbm", "kernel": "kd_small_ws", "achieved": sweeps[top]["alg_gbs"], "peak": peak, "unit": "GB/s",
+        roofline = {"bound": "hbm", "kernel": "kd_small_tc", "achieved": sweeps[top]["alg_gbs"], "peak": peak, "unit": "GB/s",
                     "frac": sweeps[top]["frac"], "traffic": traffic, "l2_bytes": l2_bytes, "traffic_source": tsrc, "peak_source": peak_src,
                     "bytes_per_launch": sweeps[top]["bytes_per_launch"], "alg_tflops": v.get("alg_tflops"),
                     "frac_fp32_alu": v.get("alg_tflops", 0.0) / FP32_PEAK_TFLOPS, "per_iteration": per_iteration}

@@ -291,10 +291,15 @@ def test_cc_path_snapshots(B, torch_, oracle):
     B.cc_destroy(h)
 
 
-@pytest.mark.parametrize("name,kw,miss", [("genotype", dict(n=52, p=5001), 0.0), ("dense_weight", dict(n=37, p=130, n_clusters=3), 0.15)])
+@pytest.mark.parametrize("name,kw,miss", [("genotype", dict(n=52, p=5001), 0.0), ("dense_weight", dict(n=37, p=130, n_clusters=3), 0.15),
+                                          ("genotype", dict(n=64, p=1200), 0.0),       # the largest n: K = N = 64, 272 pair tiles, one column phase
+                                          ("genotype", dict(n=5, p=700), 0.0),         # one K step, 6 pair tiles
+                                          ("dense_weight", dict(n=61, p=333, n_clusters=4), 0.1),   # masked, ragged rows and columns
+                                          ("genotype", dict(n=20, p=40001), 0.0)])     # 313 chunks: every CTA walks 2-3, both buffers reused
 def test_dense_small_n_fused_kernel(B, torch_, oracle, name, kw, miss):
-    """n <= 64: the warp-specialised fused kernel (projection in the centred one-FFMA form, pairs by direct differences)
-    against the oracle, labels included, with and without missing entries."""
+    """n <= 64: the warp-specialised fused kernel kd_small_tc (contraction on tcgen05 in the centred form, operand and
+    accumulator in tensor memory, TMA tensor copies, pairs by direct differences in packed fp32) against the oracle, labels
+    included, with and without missing entries."""
     torch = torch_
     wl = synth.make(name, **kw)
     if miss > 0:

@@ -301,8 +301,9 @@ __device__ __forceinline__ float shrink_ratio(float cthr, float R) {
 //              ring needs no barrier, only cp.async.wait_group.  The thread clamps (Rc = min(R, 1 / cthr): S = 1 - cthr Rc),
 //              adds to the row sum (the flash-attention style running `l`), splits into TF32 hi + lo and writes both with
 //              tcgen05.st into TENSOR MEMORY: the A operand of the MMA lives in TMEM (lane = row, column = K index), in
-//              F_AST stages of 64 columns.  Each warp then arrives on the stage's `fullA` mbarrier.  Every F_CH K blocks the
-//              warps drain the two rotating accumulators into fp32 registers and arrive on `drained`.
+//              F_AST stages of 64 columns.  Each warp then arrives on the stage's `fullA` mbarrier.  A chunk of F_CH K blocks
+//              accumulates in one of two accumulators; a few K blocks into the next chunk (which runs in the other
+//              accumulator) the warps add the finished one to fp32 registers and arrive on its `drained` barrier.
 //   warp 16, one lane     waits fullA and the B operand's fullB, issues the 12 tcgen05.mma of the K block (3xTF32, A from
 //              TMEM, B from shared memory), commits freeA / freeB.
 //   warp 17, one lane     keeps the B ring filled: (A' - abar)^T, pre-split once per iteration by kd_prep_proj in the
@@ -315,7 +316,9 @@ __device__ __forceinline__ float shrink_ratio(float cthr, float R) {
 // ahead 657; cp.async for both operands, both TF32 splits in the loop 618 (194 instructions per thread and block: ptxas
 // emulates cvt.rna.tf32); integer rounding, B by TMA, MMA lane also a staging thread behind __syncthreads 482; dedicated
 // MMA warp, mbarrier hand-off 500; lean MMA lane (descriptor = base + constant) and separate TMA warp 400; K block 32 with
-// SWIZZLE_128B operands 295.
+// SWIZZLE_128B operands 295; accumulators ping-pong per chunk, drains pipelined 281 -> 266 (the tensor core used to idle at
+// every chunk boundary).  Stub with every wait removed (pure MMA issue): 115 us = 73 cycles per MMA; the rest is operand
+// feeding: the barrier hand-shake per K block, the B ring from L2 (2 GB per launch through L2), the staging arithmetic.
 constexpr int F_AST = 3, F_BST = 4, F_RAW = 4, F_CH = 16;
 constexpr int F_THREADS = TC_THREADS + 64;          // 16 staging warps + the MMA warp + the TMA warp
 constexpr int F_ACOL = 2 * TC_N;                     // TMEM columns 0 .. 255: two accumulators; from 256: the A stages
@@ -349,7 +352,7 @@ __global__ void __launch_bounds__(F_THREADS, 1) kd_proj_tc3(int n, int ld, int n
                                                      float* __restrict__ A, cc_scal* sc, double* part) {
     if (!sc->mm_active) return;
     extern __shared__ uint8_t tc_smem_raw[];
-    __shared__ __align__(8) uint64_t fullA[F_AST], freeA[F_AST], fullB[F_BST], freeB[F_BST], mbar_acc, drained;
+    __shared__ __align__(8) uint64_t fullA[F_AST], freeA[F_AST], fullB[F_BST], freeB[F_BST], mbar_acc, drained[2];
     __shared__ uint32_t tmem_base_s;
     __shared__ float rs_part[4][TC_M];
     __shared__ int fail_s;
@@ -369,7 +372,7 @@ __global__ void __launch_bounds__(F_THREADS, 1) kd_proj_tc3(int n, int ld, int n
             asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&freeB[b])));
         }
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mbar_acc)));
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&drained)), "r"(TC_WARPS));
+        for (int b = 0; b < 2; ++b) asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(smem_u32(&drained[b])), "r"(TC_WARPS));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 0) {
@@ -406,23 +409,23 @@ __global__ void __launch_bounds__(F_THREADS, 1) kd_proj_tc3(int n, int ld, int n
             // SWIZZLE_128B K-major descriptor: LBO unused (1), SBO = 1024 bytes, version 1, layout type 2
             const uint64_t dconst = ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
             constexpr uint64_t LO = F_TILE >> 4;                 // hi -> lo tile, in descriptor units (16 bytes)
-            int ndrain = 0;
             for (int kb = 0; kb < nkb; ++kb) {
-                const int stA = kb % F_AST, stB = kb % F_BST;
-                if (kb > 0 && kb % F_CH == 0) {      // the accumulators restart here: the staging warps must have drained them
-                    if (!mbar_wait(smem_u32(&drained), (uint32_t)(ndrain & 1))) fail_s = 1;
-                    ++ndrain;
-                }
+                const int stA = kb % F_AST, stB = kb % F_BST, ch = kb / F_CH;
+                // Chunk ch (F_CH K blocks) accumulates in accumulator ch % 2 while the staging warps drain the other one, so
+                // the tensor core does not idle at a chunk boundary (it did, ~3.7 us each, when both accumulators restarted
+                // together).  Before chunk ch >= 2 starts, the drain of chunk ch - 2 must be complete: one barrier per
+                // accumulator, one phase per two chunks -- a barrier cannot run ahead of this wait.
+                if (kb % F_CH == 0 && ch >= 2 && !mbar_wait(smem_u32(&drained[ch & 1]), (uint32_t)(((ch >> 1) - 1) & 1))) fail_s = 1;
                 if (!mbar_wait(smem_u32(&fullA[stA]), (uint32_t)((kb / F_AST) & 1))) fail_s = 1;
                 if (!mbar_wait(smem_u32(&fullB[stB]), (uint32_t)((kb / F_BST) & 1))) fail_s = 1;
                 asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
                 const uint32_t ta = tmem_d + (uint32_t)(F_ACOL + stA * 2 * FK);      // hi at ta, lo at ta + FK columns
                 const uint64_t db = dconst | (uint64_t)((smB + (uint32_t)stB * F_SIDE) >> 4);
-                const uint32_t td = tmem_d + (uint32_t)((kb & 1) * TC_N);            // rotate over the two accumulators
+                const uint32_t td = tmem_d + (uint32_t)((ch & 1) * TC_N);
 #pragma unroll
                 for (int ks = 0; ks < FK / 8; ++ks) {                        // 8 K indices: 8 TMEM columns of A, 32 bytes of B's row
                     const uint64_t ko = (uint64_t)(2 * ks);
-                    tc_mma_ts(td, ta + 8 * ks, db + ko, idesc, ((kb % F_CH) >= 2 || ks > 0) ? 1u : 0u);
+                    tc_mma_ts(td, ta + 8 * ks, db + ko, idesc, ((kb % F_CH) > 0 || ks > 0) ? 1u : 0u);
                     tc_mma_ts(td, ta + 8 * ks, db + ko + LO, idesc, 1u);
                     tc_mma_ts(td, ta + FK + 8 * ks, db + ko, idesc, 1u);
                 }
@@ -453,7 +456,27 @@ __global__ void __launch_bounds__(F_THREADS, 1) kd_proj_tc3(int n, int ld, int n
         const float rcap = cthr > 0.f ? 1.f / cthr : 0.f;
         const uint32_t tlane = tmem_d + ((uint32_t)((warp & 3) * 32) << 16);
         float rsum = 0.f;
-        int nchunk_done = 0;
+        int next_drain = 0;
+        const int last_chunk = (nkb - 1) / F_CH;
+        auto drain = [&](int ch) {      // chunk ch is complete in accumulator ch % 2: add it to the fp32 registers, free the accumulator
+            if (!mbar_wait_idle(smem_u32(&mbar_acc), (uint32_t)(ch & 1))) fail_s = 1;
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+#pragma unroll
+            for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
+                uint32_t v[16];
+                const uint32_t taddr = tlane + (uint32_t)((ch & 1) * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
+                asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                             : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                               "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                             : "r"(taddr));
+                asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+                for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&drained[ch & 1]));
+        };
         for (int kb = 0; kb < nkb; ++kb) {
             const int st = kb % F_AST;
             fetch(kb + F_RAW - 1);                                   // its slot held block kb - 1, which this thread has consumed
@@ -481,29 +504,11 @@ __global__ void __launch_bounds__(F_THREADS, 1) kd_proj_tc3(int n, int ld, int n
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(smem_u32(&fullA[st]));
-            if ((kb + 1) % F_CH == 0 || kb + 1 == nkb) {      // chunk boundary: wait for the MMAs, drain the accumulators
-                if (!mbar_wait_idle(smem_u32(&mbar_acc), (uint32_t)(nchunk_done & 1))) fail_s = 1;
-                ++nchunk_done;
-                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-                const int nacc = min(2, (kb % F_CH) + 1);
-                for (int ac = 0; ac < nacc; ++ac)
-#pragma unroll
-                    for (int h2 = 0; h2 < TC_CPW / 16; ++h2) {
-                        uint32_t v[16];
-                        const uint32_t taddr = tlane + (uint32_t)(ac * TC_N + (warp >> 2) * TC_CPW + h2 * 16);
-                        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                                     : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-                                       "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
-                                     : "r"(taddr));
-                        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-                        for (int q = 0; q < 16; ++q) accr[h2 * 16 + q] += __uint_as_float(v[q]);
-                    }
-                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&drained));
-            }
+            // the previous chunk's MMAs were issued F_AST K blocks ago at the latest: drain it now, a few blocks into this
+            // chunk, while the tensor core works on the other accumulator
+            if (kb % F_CH == F_AST + 1 && kb >= F_CH) drain(next_drain++);
         }
+        while (next_drain <= last_chunk) drain(next_drain++);
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         rs_part[kq][row] = rsum;       // four K octets per row, added in a fixed order below
     }

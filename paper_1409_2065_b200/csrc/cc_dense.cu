@@ -588,6 +588,13 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
     const float naI = nrm[0][0][row], aeI = nrm[0][1][row], neI = nrm[0][2][row];
     double red[2] = {0.0, 0.0};      // sum_{i<j} ||v - b||^2,  sum_{i<j} w ||v||
     unsigned int myflags = 0u;
+    // this thread's places: row gi of ||b|| and R (columns j0 ..), and column gi of R (rows j0 ..: the other triangle)
+    const size_t orow = (size_t)min(gi, n - 1) * n + j0;
+    float* const NBr = NB + orow;
+    float* const Rmr = Rm + orow;
+    float* const RmT = Rm + (size_t)j0 * n + gi;
+    const float* const Wr = W + orow;
+    const bool diag = I == J;
 #pragma unroll 1
     for (int half = 0; half < 2; ++half) {
         const int cb = grp * 32 + half * 16;
@@ -598,10 +605,9 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
         float nbp[16], wq[16];
 #pragma unroll
         for (int q4 = 0; q4 < 4; ++q4) {
-            const int gj = j0 + cb + q4 * 4;
-            const bool ok = gi < n && gj < n;
-            const float4 v = ok ? *reinterpret_cast<const float4*>(NB + (size_t)gi * n + gj) : f4(0.f);
-            const float4 u = ok ? __ldg(reinterpret_cast<const float4*>(W + (size_t)gi * n + gj)) : f4(0.f);
+            const bool ok = gi < n && j0 + cb + q4 * 4 < n;
+            const float4 v = ok ? *reinterpret_cast<const float4*>(NBr + cb + q4 * 4) : f4(0.f);
+            const float4 u = ok ? __ldg(reinterpret_cast<const float4*>(Wr + cb + q4 * 4)) : f4(0.f);
             nbp[q4 * 4 + 0] = v.x; nbp[q4 * 4 + 1] = v.y; nbp[q4 * 4 + 2] = v.z; nbp[q4 * 4 + 3] = v.w;
             wq[q4 * 4 + 0] = u.x; wq[q4 * 4 + 1] = u.y; wq[q4 * 4 + 2] = u.z; wq[q4 * 4 + 3] = u.w;
         }
@@ -616,43 +622,53 @@ __device__ __forceinline__ void pairs_tc_epilogue(int n, int ld, int I, int J, i
         }
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
         if (gi < n) {
+            // the 16 pairs' sums stay in fp32 here (16 terms) and join the fp64 totals once per half
+            float dvs = 0.f, pens = 0.f;
 #pragma unroll
             for (int q = 0; q < 16; ++q) {
-                const int cl = cb + q, gj = j0 + cl;
-                if (gj >= n || (I == J && gi >= gj)) continue;     // diagonal tiles: pairs i < j only
+                const int cl = cb + q;
+                // pairs of the tile that exist: column inside the matrix; diagonal tiles: i < j only
+                const bool live = j0 + cl < n && (!diag || row < cl);
                 const float naJ = nrm[1][0][cl], aeJ = nrm[1][1][cl], neJ = nrm[1][2][cl];
-                const size_t o = (size_t)gi * n + gj;
                 // the factor of v_m = s b' (L86), recomputed as kd_proj_tc3 did, and this pair's share of the penalty of Phi_m
                 const float sv = shrink_ratio(cthr, pair_ratio(wq[q], nbp[q]));
-                red[1] += (double)(wq[q] * (sv * nbp[q]));
-                svbuf[row * (TC_N + 1) + cl] = sv;      // stride 129: the 32 rows of a warp fall into 32 banks
+                const float pen = wq[q] * (sv * nbp[q]);
                 const float nb2 = naI + naJ - 2.f * __uint_as_float(g[0][q]);
-                // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold
-                const float nbn = sqrtf(fmaxf(nb2, 0.f));
+                // unflagged pairs have relative error <= 3e-7 / CC_RECOMP_REL = 3e-5 in ||b||^2, whatever the threshold.
+                // ||b|| = nb2 rsqrt(nb2): 2 ulp, one MUFU (the IEEE square root was a call on the slow path); the ratio R is
+                // formed from the stored ||b||, here and by every later reader, so the factors stay bit-identical
+                const float nb2c = fmaxf(nb2, 0.f);
+                const float nbn = nb2c > 0.f ? nb2c * rsqrtf(nb2c) : 0.f;
                 const float rn = pair_ratio(wq[q], nbn);
-                nbp[q] = nbn;
-                wq[q] = rn;
-                if (nb2 < CC_RECOMP_REL * (naI + naJ)) {
-                    myflags |= 1u << (half * 16 + q);               // recomputed directly below
-                } else {
-                    const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));
-                    const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
-                    const float om = 1.f - sv;
-                    const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
-                    if (I == J) { NB[o] = nbn; Rm[o] = rn; }       // diagonal tiles: guarded scalar stores (i < j only)
-                    Rm[(size_t)gj * n + gi] = rn;
-                    red[0] += (double)dv;
+                const bool flagged = nb2 < CC_RECOMP_REL * (naI + naJ);
+                const float bd = (aeI + aeJ) - (__uint_as_float(g[1][q]) + __uint_as_float(g[2][q]));
+                const float dd = fmaxf(neI + neJ - 2.f * __uint_as_float(g[3][q]), 0.f);
+                const float om = 1.f - sv;
+                const float dv = fmaxf(om * om * nb2 - 2.f * sv * om * bd + sv * sv * dd, 0.f);
+                if (live) {
+                    pens += pen;
+                    nbp[q] = nbn;
+                    wq[q] = rn;
+                    if (flagged) {
+                        myflags |= 1u << (half * 16 + q);               // recomputed directly below, with this factor
+                        svbuf[row * (TC_N + 1) + cl] = sv;              // stride 129: the 32 rows of a warp fall into 32 banks
+                    } else {
+                        dvs += dv;
+                        if (diag) { NBr[cl] = nbn; Rmr[cl] = rn; }      // diagonal tiles: guarded scalar stores (i < j only)
+                        RmT[(size_t)cl * n] = rn;
+                    }
                 }
             }
-            if (I != J) {
+            red[0] += (double)dvs;
+            red[1] += (double)pens;
+            if (!diag) {
                 // off-diagonal tiles: this row's 16 values as four 16-byte stores per array (flagged entries are rewritten by
                 // the recompute phase, which runs after the barrier below)
 #pragma unroll
                 for (int q4 = 0; q4 < 4; ++q4) {
-                    const int gj = j0 + cb + q4 * 4;
-                    if (gj < n) {
-                        st4(NB + (size_t)gi * n + gj, make_float4(nbp[q4 * 4 + 0], nbp[q4 * 4 + 1], nbp[q4 * 4 + 2], nbp[q4 * 4 + 3]));
-                        st4(Rm + (size_t)gi * n + gj, make_float4(wq[q4 * 4 + 0], wq[q4 * 4 + 1], wq[q4 * 4 + 2], wq[q4 * 4 + 3]));
+                    if (j0 + cb + q4 * 4 < n) {
+                        st4(NBr + cb + q4 * 4, make_float4(nbp[q4 * 4 + 0], nbp[q4 * 4 + 1], nbp[q4 * 4 + 2], nbp[q4 * 4 + 3]));
+                        st4(Rmr + cb + q4 * 4, make_float4(wq[q4 * 4 + 0], wq[q4 * 4 + 1], wq[q4 * 4 + 2], wq[q4 * 4 + 3]));
                     }
                 }
             }

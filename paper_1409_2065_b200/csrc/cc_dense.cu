@@ -964,257 +964,6 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
     }
 }
 
-// ---- kd_small: the whole pair/projection work of one iteration for n <= 64 (genotype shape) ---------------
-// All n rows of a chunk of 64 columns fit in shared memory together with S (n x n), so U and A' are read
-// once, A is written once, and projection, ||U-A||^2, loss, ||b||^2 and ||s b' - b||^2 are all formed from
-// shared memory.  A CTA walks chunks grid-stride and keeps its pair accumulators in registers; it writes
-// one slice of partial ||b||^2 per (CTA, column phase) at the end (kd_edges adds the slices in order).
-// Everything moves as float4 along the columns: one LDS.128 feeds 4 columns, so the projection runs at 2
-// shared loads per 32 arithmetic instructions (a thread = 4 rows x 4 columns, S broadcast as a float4 of
-// S^T) and the pairs at 16 loads per 320 (4 x 4 register tiles of pairs, only the tiles on or above the
-// diagonal, cs_per_tile threads per tile taking interleaved column quads).  Four barriers per chunk: load |
-// projection | exact-column-sum fix and store of A | pairs; the two column sums (mean of U, residual of
-// 1'(A-U)) are partial sums left in shared memory by the previous phase and added up by every thread that
-// needs them, in a fixed order.  History at 52 x 200,000: scalar shared loads, 8 barriers 330 us; float4 217 us.
-constexpr int SM_N = 64, SM_C = 64, SM_Q = SM_C / 4;
-
-// Column quad q of row r sits at float offset small_sw(r, q) of the row (row stride 64 floats): the quad index is
-// XORed with twice the row's 4-row tile index, so that the pair phase -- a quarter warp reads rows 4tx+a of four
-// consecutive tiles tx at two column quads -- hits 8 distinct 16-byte bank groups (a plain padded stride cannot:
-// rows 8 apart always collide), while a row's 16 quads stay a permutation of themselves.
-__device__ __forceinline__ int small_sw(int r, int q) { return (q ^ (((r >> 2) << 1) & 15)) << 2; }
-
-// ---- kd_small_ws: the same iteration, warp-specialised -------------------------------------------------------
-// kd_small alternates phases inside a CTA (load | projection | fix | pairs) and ncu showed a quarter of warp time
-// waiting at the phase barriers with issue slots 50 % busy.  Here one CTA of 512 threads per SM splits into two
-// roles that work on different chunks at the same time: threads 0..255 (projection role) load chunk k+1, project it
-// and write A while threads 256..511 (pair role) accumulate the pair norms of chunk k from the other shared-memory
-// buffer.  Hand-over by named barriers: FULL[b] (projection arrives, pairs wait), FREE[b] (pairs arrive, projection
-// waits before it overwrites buffer b two chunks later); the projection role keeps its own 256-thread barrier for its
-// internal steps.  Arithmetic, summation order and output slices are those of kd_small (same results bit for bit when
-// both use the same grid; the cold start still runs kd_small with init_only = 1).
-constexpr int WS_THREADS = 512;
-constexpr int WS_SMEM = (SM_N * (SM_N + 4) + 2 * 3 * SM_N * SM_C + 2 * 16 * SM_C) * (int)sizeof(float);
-
-__global__ void __launch_bounds__(WS_THREADS, 1) kd_small_ws(int n, int ld, int cs_per_tile, const float* __restrict__ S,
-                                                             const float* __restrict__ Ap, const float* __restrict__ U,
-                                                             const float* __restrict__ X, const uint8_t* __restrict__ mask,
-                                                             const float* __restrict__ W, const float* __restrict__ VN,
-                                                             float* __restrict__ A, float* __restrict__ NB2, cc_scal* sc,
-                                                             double* part, double* hist_phi, double* hist_d,
-                                                             cudaGraphConditionalHandle outer) {
-    if (!sc->mm_active) return;
-    constexpr int BAR_PROJ = 1, BAR_FULL = 2, BAR_FREE = 4;      // barrier 0 is __syncthreads
-    extern __shared__ __align__(16) float sm_small[];
-    float (*SsT)[SM_N + 4] = reinterpret_cast<float (*)[SM_N + 4]>(sm_small);
-    float (*bufs)[SM_C] = reinterpret_cast<float (*)[SM_C]>(sm_small + SM_N * (SM_N + 4));   // 2 x {Us, Ps, As}
-    float (*csum)[SM_C] = bufs + 2 * 3 * SM_N;
-    float (*dsum)[SM_C] = csum + 16;
-    __shared__ unsigned char t_ty[136], t_tx[136];
-    __shared__ int ntiles_s;
-    const int tid = threadIdx.x;
-    if (tid == 0) {
-        int k = 0;
-        const int nt4 = (n + 3) / 4;
-        for (int ty = 0; ty < nt4; ++ty)
-            for (int tx = ty; tx < nt4; ++tx) { t_ty[k] = (unsigned char)ty; t_tx[k] = (unsigned char)tx; ++k; }
-        ntiles_s = k;
-    }
-    for (int t = tid; t < SM_N * SM_N; t += WS_THREADS) {
-        const int i = t / SM_N, j = t % SM_N;
-        SsT[j][i] = (i < n && j < n) ? S[(size_t)i * n + j] : 0.f;
-    }
-    __syncthreads();
-    const bool pair_role = tid >= 256;
-    const int rt = tid & 255;
-    const int nchunks = (ld + SM_C - 1) / SM_C;
-    const int nmine = blockIdx.x < nchunks ? (nchunks - 1 - blockIdx.x) / gridDim.x + 1 : 0;   // chunks this CTA walks
-    double red[4] = {0.0, 0.0, 0.0, 0.0};   // ||U-A||^2, loss, sum ||v-b||^2, sum w ||v||
-    if (!pair_role) {
-        const float inv = 1.f / (float)(n + 1), fn = (float)n, rfn = 1.f / (float)n;
-        const int n4 = (n + 3) & ~3;
-        const int pq = rt & 15, prg = rt >> 4, i0r = prg * 4;
-        // sum_j s_ij (p_i - p_j) is evaluated as rowsum(S)_i p~_i - sum_j s_ij p~_j on rows centred by the column mean of
-        // U, p~ = p - ubar (A' is U up to O(d/rho), so p~ has the size of the spread between the rows, not of the data):
-        // one FFMA per (i, j, column) instead of a subtraction and an FFMA.  With n <= 64 terms the rounding error is
-        // ~n eps |p~|, the same order as that of the direct differences whenever some pair of the row is not fused.
-        float4 rsS = f4(0.f);
-        if (i0r < n)
-            for (int j = 0; j < n4; ++j) rsS = rsS + ld4s(&SsT[j][i0r]);
-        // rows prg, prg+16, prg+32, prg+48 of column quad pq of a chunk, held in registers one chunk ahead
-        float4 uu[4], pp[4];
-        auto fetch = [&](int k) {
-            const int c0 = (blockIdx.x + k * gridDim.x) * SM_C;
-            const bool in = c0 + pq * 4 < ld;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int r = prg + 16 * q;
-                const bool ok = r < n && in;
-                uu[q] = ok ? ld4s(U + (size_t)r * ld + c0 + pq * 4) : f4(0.f);
-                pp[q] = ok ? ld4s(Ap + (size_t)r * ld + c0 + pq * 4) : f4(0.f);
-            }
-        };
-        if (nmine > 0) fetch(0);
-        for (int k = 0; k < nmine; ++k) {
-            const int c0 = (blockIdx.x + k * gridDim.x) * SM_C;
-            float (*Us)[SM_C] = bufs + (k & 1) * 3 * SM_N;
-            float (*Ps)[SM_C] = Us + SM_N;
-            float (*As)[SM_C] = Ps + SM_N;
-            const bool inside = c0 + pq * 4 < ld;
-            if (k >= 2) named_sync(BAR_FREE + (k & 1), WS_THREADS);     // the pair role is done with this buffer
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int r = prg + 16 * q, o = small_sw(r, pq);
-                st4(&Us[r][o], uu[q]);
-                st4(&Ps[r][o], pp[q]);
-            }
-            st4(&csum[prg][pq * 4], (uu[0] + uu[1]) + (uu[2] + uu[3]));
-            // global loads that the rest of this iteration hides: the next chunk, and this chunk's data rows for the loss
-            if (k + 1 < nmine) fetch(k + 1);
-            float4 xq[4];
-            uchar4 mq[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int i = i0r + q;
-                const bool ok = i < n && inside;
-                xq[q] = ok ? ld4s(X + (size_t)i * ld + c0 + pq * 4) : f4(0.f);
-                mq[q] = (ok && mask) ? *reinterpret_cast<const uchar4*>(mask + (size_t)i * ld + c0 + pq * 4) : make_uchar4(1, 1, 1, 1);
-            }
-            named_sync(BAR_PROJ, 256);
-            float dua = 0.f, los = 0.f;
-            float4 dsl = f4(0.f);
-            if (i0r < n) {
-                float4 ub = ld4s(&csum[0][pq * 4]);
-#pragma unroll
-                for (int q = 1; q < 16; ++q) ub = ub + ld4s(&csum[q][pq * 4]);
-                ub = rfn * ub;                 // (a reciprocal multiply: the eight fp32 divisions per chunk sat on the critical role)
-                float4 pi[4], g[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) { pi[q] = ld4s(&Ps[i0r + q][small_sw(i0r, pq)]); g[q] = f4(0.f); }
-                for (int j4 = 0; j4 < n4; j4 += 4) {
-                    const int o = small_sw(j4, pq);
-#pragma unroll
-                    for (int jj = 0; jj < 4; ++jj) {
-                        const float4 pj = ld4s(&Ps[j4 + jj][o]) - ub;
-                        const float4 s4 = ld4s(&SsT[j4 + jj][i0r]);
-                        g[0] = fma4(-s4.x, pj, g[0]);
-                        g[1] = fma4(-s4.y, pj, g[1]);
-                        g[2] = fma4(-s4.z, pj, g[2]);
-                        g[3] = fma4(-s4.w, pj, g[3]);
-                    }
-                }
-                g[0] = fma4(rsS.x, pi[0] - ub, g[0]);
-                g[1] = fma4(rsS.y, pi[1] - ub, g[1]);
-                g[2] = fma4(rsS.z, pi[2] - ub, g[2]);
-                g[3] = fma4(rsS.w, pi[3] - ub, g[3]);
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const int i = i0r + q;
-                    if (i < n) {
-                        const float4 u = ld4s(&Us[i][small_sw(i0r, pq)]);
-                        float4 dl;
-                        dl.x = inv * (g[q].x - fn * (u.x - ub.x)); dl.y = inv * (g[q].y - fn * (u.y - ub.y));
-                        dl.z = inv * (g[q].z - fn * (u.z - ub.z)); dl.w = inv * (g[q].w - fn * (u.w - ub.w));
-                        const float4 a = u + dl;
-                        st4(&As[i][small_sw(i0r, pq)], a);
-                        dsl = dsl + (a - u);
-                        if (inside) {
-                            dua += dot4(dl, dl);
-                            float4 qx = xq[q] - u;
-                            const uchar4 mk = mq[q];
-                            qx.x = mk.x ? qx.x : 0.f; qx.y = mk.y ? qx.y : 0.f; qx.z = mk.z ? qx.z : 0.f; qx.w = mk.w ? qx.w : 0.f;
-                            los += dot4(qx, qx);
-                        }
-                    }
-                }
-            }
-            st4(&dsum[prg][pq * 4], dsl);
-            red[0] += (double)dua;
-            red[1] += (double)los;
-            named_sync(BAR_PROJ, 256);
-            if (i0r < n) {
-                float4 db = ld4s(&dsum[0][pq * 4]);
-#pragma unroll
-                for (int q = 1; q < 16; ++q) db = db + ld4s(&dsum[q][pq * 4]);
-                db = rfn * db;
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    const int i = i0r + q;
-                    float* as = &As[i][small_sw(i0r, pq)];
-                    const float4 a2 = i < n ? ld4s(as) - db : f4(0.f);
-                    st4(as, a2);
-                    if (i < n && inside) st4(A + (size_t)i * ld + c0 + pq * 4, a2);
-                }
-            }
-            named_arrive(BAR_FULL + (k & 1), WS_THREADS);
-        }
-    }
-    // pair role (and, after the loop, everybody): accumulators of the 4 x 4 tile of pairs
-    const int ntiles = ntiles_s;
-    const bool pair_thread = pair_role && rt < ntiles * cs_per_tile;
-    const int tile = pair_thread ? rt / cs_per_tile : 0, cph = rt % cs_per_tile;
-    const int ty = t_ty[tile], tx = t_tx[tile];
-    float nb[4][4], dv[4][4];
-    if (pair_role) {
-        float sv[4][4];
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int b = 0; b < 4; ++b) { sv[a][b] = SsT[tx * 4 + b][ty * 4 + a]; nb[a][b] = 0.f; dv[a][b] = 0.f; }
-        const int gy = (ty << 1) & 15, gx = (tx << 1) & 15;
-        for (int k = 0; k < nmine; ++k) {
-            float (*Ps)[SM_C] = bufs + (k & 1) * 3 * SM_N + SM_N;
-            float (*As)[SM_C] = Ps + SM_N;
-            named_sync(BAR_FULL + (k & 1), WS_THREADS);
-            if (pair_thread) {
-                for (int cq = cph; cq < SM_Q; cq += cs_per_tile) {
-                    const int oy = (cq ^ gy) << 2, ox = (cq ^ gx) << 2;
-                    float4 ai[4], aj[4], pi[4], pj[4];
-#pragma unroll
-                    for (int a = 0; a < 4; ++a) {
-                        ai[a] = ld4s(&As[ty * 4 + a][oy]); pi[a] = ld4s(&Ps[ty * 4 + a][oy]);
-                        aj[a] = ld4s(&As[tx * 4 + a][ox]); pj[a] = ld4s(&Ps[tx * 4 + a][ox]);
-                    }
-#pragma unroll
-                    for (int a = 0; a < 4; ++a)
-#pragma unroll
-                        for (int b = 0; b < 4; ++b) {
-                            const float4 bb = ai[a] - aj[b];
-                            const float4 dp = pi[a] - pj[b];
-                            const float4 tt = make_float4(fmaf(sv[a][b], dp.x, -bb.x), fmaf(sv[a][b], dp.y, -bb.y),
-                                                          fmaf(sv[a][b], dp.z, -bb.z), fmaf(sv[a][b], dp.w, -bb.w));
-                            nb[a][b] = fmaf(bb.w, bb.w, fmaf(bb.z, bb.z, fmaf(bb.y, bb.y, fmaf(bb.x, bb.x, nb[a][b]))));
-                            dv[a][b] = fmaf(tt.w, tt.w, fmaf(tt.z, tt.z, fmaf(tt.y, tt.y, fmaf(tt.x, tt.x, dv[a][b]))));
-                        }
-                }
-            }
-            if (k + 2 < nmine) named_arrive(BAR_FREE + (k & 1), WS_THREADS);
-        }
-    }
-    if (pair_thread) {
-        float* out = NB2 + (size_t)(blockIdx.x * cs_per_tile + cph) * n * n;
-#pragma unroll
-        for (int a = 0; a < 4; ++a)
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                const int gi = ty * 4 + a, gj = tx * 4 + b;
-                if (gi < n && gj < n && gi != gj) {
-                    out[(size_t)gi * n + gj] = nb[a][b];
-                    if (ty != tx) out[(size_t)gj * n + gi] = nb[a][b];
-                    if (gi < gj) {
-                        red[2] += (double)dv[a][b];
-                        if (blockIdx.x == 0 && cph == 0) red[3] += (double)(W[(size_t)gi * n + gj] * VN[(size_t)gi * n + gj]);
-                    }
-                }
-            }
-    }
-    double tot[4];
-    if (grid_reduce<4, WS_THREADS>(red, part, &sc->ticket[3], tot)) {
-        finish_iteration(sc, tot[0] + tot[2], tot[1], tot[3], hist_phi, hist_d, outer);
-        prof_mark(sc, 5);
-    }
-}
-
 // ---- kd_edges: block soft-threshold over the n x n matrices; the FFMA / n <= 64 paths only
 // (the tensor-core path never stores S: see shrink_ratio)
 __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
@@ -1497,13 +1246,7 @@ void ccd_pairs(cc_handle* h) {
     launch_pairs(h, h->A, h->Ap, 0);
 }
 
-static void launch_small(cc_handle* h) {
-    if (h->dn_small_tc) { ccd_small_tc_launch(h); return; }
-    kd_small_ws<<<h->dn_small_grid, WS_THREADS, WS_SMEM, h->stream>>>((int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, h->Ap, h->U, h->X,
-                                                                      h->mask, h->Wd, h->VNd, h->A, h->NB2d, h->sc,
-                                                                      h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi,
-                                                                      h->hist_d, h->cond_outer);
-}
+static void launch_small(cc_handle* h) { ccd_small_tc_launch(h); }      // cc_small.cu
 
 void ccd_edges(cc_handle* h, int init_only) {
     kd_edges<<<h->grid_nodes, 256, 0, h->stream>>>((int)h->n, h->dn_ksplit, h->NB2d, h->Wd, h->Sd, h->VNd, h->sc,
@@ -1537,23 +1280,11 @@ int ccd_setup(cc_handle* h, const float* W) {
     if (ks < 1) ks = 1;
     if (h->dn_tc) ks = 1;                      // kd_pairs_tc2 walks all columns itself
     h->dn_ksplit = (int)ks;
-    // n <= 64: the fused kernel; its slices are (CTA, column phase)
-    h->dn_small = n <= SM_N ? 1 : 0;
+    // n <= 64: the fused kernel kd_small_tc (cc_small.cu), which sets its own launch shape; its slices are (CTA, column
+    // phase).  Where it cannot run (no tensor-map encoder in the driver) the FFMA tiles above serve these shapes too.
+    h->dn_small = (n <= 64 && ccd_small_tc_setup(h)) ? 1 : 0;
+    h->dn_small_tc = h->dn_small;
     if (h->dn_small) {
-        const int nt4 = (int)((n + 3) / 4), ntiles = nt4 * (nt4 + 1) / 2;
-        int cs = 256 / ntiles;
-        if (cs > 4) cs = 4;
-        if (cs < 1) cs = 1;
-        long long g = (h->ld + SM_C - 1) / SM_C;
-        if (g > h->sms) g = h->sms;             // kd_small_ws: one 512-thread CTA per SM
-        if (cudaFuncSetAttribute(kd_small_ws, cudaFuncAttributeMaxDynamicSharedMemorySize, WS_SMEM) != cudaSuccess) {
-            cudaGetLastError();
-            snprintf(h->err, sizeof(h->err), "dense mode: cannot reserve %d bytes of shared memory for kd_small_ws", WS_SMEM);
-            return CC_ECUDA;
-        }
-        h->dn_small_cs = cs;
-        h->dn_small_grid = (int)g;
-        h->dn_small_tc = ccd_small_tc_setup(h);     // the tensor-core version (cc_small.cu) replaces the launch shape when it can run
         h->dn_ksplit = h->dn_small_grid * h->dn_small_cs;
         ks = h->dn_ksplit;
     }

@@ -54,6 +54,7 @@ struct cc_scal {
 
 // Per-block partial sums: up to CC_NPART doubles per block, CC_MAXBLK blocks.
 #define CC_INV_NMAX 384     // largest n whose projection uses the precomputed inverse (n x 128 floats of shared memory)
+#define CC_INVW_NMAX 4096   // ... and with at most 32 columns (all of uc in one CTA's shared memory): the inverse applied from L2
 #define CC_NPART 4
 #define CC_MAXBLK 16384
 
@@ -86,6 +87,7 @@ struct cc_handle {
     float* tmpE;                      // nnz scratch (diagnostics)
     float* dinv;                      // n: 1 / (1 + |N_i|)
     float* Minv;                      // n x n: (D^-1 (I+L))^-1 for n <= CC_INV_NMAX, else NULL (CG solver)
+    int inv_wide;                     // 1: Minv is applied by k_apply_inv_wide (n > CC_INV_NMAX, few columns)
     // dense mode (complete graph): n x n matrices instead of the CSR arrays
     float *Wd, *Sd, *VNd, *NB2d;      // weights, shrink factors, ||v||, ||b||^2 (dn_ksplit column-range slices); tensor-core path: Wd, NB2d =
                                       // ||b|| (pairs i < j) and Rd only (S and ||v|| are recomputed where they are used)

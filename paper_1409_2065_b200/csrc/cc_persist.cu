@@ -455,7 +455,7 @@ static size_t persist_smem(const cc_handle* h, int sw, int minv_in_smem) {
 // the inverse exists.  Leaves h->pt_slabs = 0 when the handle stays on the CUDA-graph path.
 int ccp_setup(cc_handle* h) {
     h->pt_slabs = 0;
-    if (h->dense || !h->Minv || !h->prm.use_graph || h->n > 65535) return CC_OK;
+    if (h->dense || !h->Minv || h->inv_wide || !h->prm.use_graph || h->n > CC_INV_NMAX) return CC_OK;
     int dev = 0, coop = 0, maxsm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) != cudaSuccess || !coop) {
         cudaGetLastError();

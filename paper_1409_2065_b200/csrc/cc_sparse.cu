@@ -279,6 +279,96 @@ __global__ void __launch_bounds__(1024) k_invert(int n, const int* __restrict__ 
     for (int t = tid; t < n * n; t += 1024) Minv[t] = (float)aug[(size_t)(t / n) * w2 + n + t % n];
 }
 
+// ---- the same inverse for a few thousand points and few columns (POPRES-like: 3000 x 10, k = 40: 19 CG sweeps of ~22 us
+// per MM iteration, every one of them launch- and reduction-bound) -----------------------------------------------------
+// In-place Gauss-Jordan in fp64 over the whole GPU, two launches per pivot: k_inv_pivot saves the scaled pivot row and
+// the pivot column of step k, k_inv_elim applies  a_ij <- a_ij - f_i r_j  (row k <- r, column k <- -f p).  The matrix
+// D^-1 (I + L) has a unit diagonal and is strictly diagonally dominant by rows: no pivoting.  n = 3000: 6000 launches,
+// 72 MB of work space (L2-resident), ~0.1 s once per handle.
+__global__ void k_inv_init(int n, const int* __restrict__ rowptr, const int* __restrict__ col, double* __restrict__ a) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const double dg = 1.0 + (double)(rowptr[i + 1] - rowptr[i]);
+        a[(size_t)i * n + i] = 1.0;
+        for (int e = rowptr[i]; e < rowptr[i + 1]; ++e) a[(size_t)i * n + col[e]] = -1.0 / dg;
+    }
+}
+__global__ void k_inv_pivot(int n, int k, const double* __restrict__ a, double* __restrict__ prow, double* __restrict__ fcol) {
+    const double p = 1.0 / a[(size_t)k * n + k];
+    for (int j = blockIdx.x * blockDim.x + threadIdx.x; j < n; j += gridDim.x * blockDim.x) {
+        prow[j] = j == k ? p : a[(size_t)k * n + j] * p;
+        fcol[j] = a[(size_t)j * n + k];
+    }
+}
+__global__ void __launch_bounds__(256) k_inv_elim(int n, int k, double* __restrict__ a, const double* __restrict__ prow,
+                                                  const double* __restrict__ fcol) {
+    const int j = blockIdx.x * 256 + threadIdx.x;
+    if (j >= n) return;
+    const double r = prow[j], p = prow[k];
+    for (int i = blockIdx.y; i < n; i += gridDim.y) {
+        const size_t o = (size_t)i * n + j;
+        const double f = fcol[i];
+        a[o] = i == k ? r : (j == k ? -f * p : a[o] - f * r);
+    }
+}
+__global__ void k_inv_store(long long nn, const double* __restrict__ a, float* __restrict__ Minv) {
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nn; t += (long long)gridDim.x * blockDim.x) Minv[t] = (float)a[t];
+}
+
+// A_i += sum_j Minv[i][j] uc_j for that shape: every CTA keeps ALL of uc (n rows of ld <= 32 floats, row stride ld + 1:
+// the lanes of a warp walk consecutive rows j) in shared memory and deals the rows i of Minv to its warps; a warp reads its
+// row of Minv once, coalesced (the matrix, 36 MB at n = 3000, lives in L2), and reduces the ld sums over its lanes.
+template <int LDW>
+__global__ void __launch_bounds__(512) k_apply_inv_wide(int n, int ld, const float* __restrict__ Minv, const float* __restrict__ Uc,
+                                                        float* __restrict__ A, cc_scal* sc) {
+    if (!sc->mm_active) return;
+    extern __shared__ float us[];                  // n x (ld + 1)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, rs = ld + 1;
+    const int q4 = ld >> 2;                         // ld is a multiple of 4: rows of uc as float4
+    for (int t = threadIdx.x; t < n * q4; t += 512) {
+        const int j = t / q4, c = (t - j * q4) * 4;
+        const float4 v = ld4s(Uc + (size_t)j * ld + c);
+        float* d = us + j * rs + c;
+        d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+    }
+    __syncthreads();
+    for (int i = blockIdx.x * 16 + warp; i < n; i += gridDim.x * 16) {
+        float acc[LDW];
+#pragma unroll
+        for (int c = 0; c < LDW; ++c) acc[c] = 0.f;
+        const float* mrow = Minv + (size_t)i * n;
+        for (int jb = lane; jb < n; jb += 32 * 8) {        // eight loads of the row in flight (the matrix comes from L2)
+            float m[8];
+#pragma unroll
+            for (int q = 0; q < 8; ++q) m[q] = jb + 32 * q < n ? __ldg(mrow + jb + 32 * q) : 0.f;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const float* u = us + min(jb + 32 * q, n - 1) * rs;
+#pragma unroll
+                for (int c = 0; c < LDW; ++c)
+                    if (c < ld) acc[c] = fmaf(m[q], u[c], acc[c]);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < LDW; ++c)
+#pragma unroll
+            for (int of = 16; of > 0; of >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], of);
+        // lane c owns column c of the row
+        float mine = 0.f;
+#pragma unroll
+        for (int c = 0; c < LDW; ++c)
+            if (lane == c) mine = acc[c];
+        if (lane < ld) A[(size_t)i * ld + lane] += mine;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&sc->ticket[5], 1u) == gridDim.x - 1) {
+            sc->ticket[5] = 0u;
+            prof_mark(sc, 2);      // charged to the k_cg_update slot: it takes the place of the CG loop
+        }
+    }
+}
+
 // A_i += sum_j Minv[i][j] uc_j.  One CTA per chunk of 128 columns: uc's chunk (n x 128) is staged in shared
 // memory once, each warp then produces rows i = w, w + 8, ...
 template <int DUMMY>
@@ -576,6 +666,15 @@ void ccs_rhs(cc_handle* h) {
 }
 
 void ccs_apply_inv(cc_handle* h) {
+    if (h->inv_wide) {
+        const size_t smem = (size_t)h->n * (h->ld + 1) * sizeof(float);
+        const int grid = h->sms < (int)((h->n + 15) / 16) ? h->sms : (int)((h->n + 15) / 16);   // one CTA per SM (shared memory)
+        if (h->ld <= 16)
+            k_apply_inv_wide<16><<<grid, 512, smem, h->stream>>>((int)h->n, (int)h->ld, h->Minv, h->Uc, h->A, h->sc);
+        else
+            k_apply_inv_wide<32><<<grid, 512, smem, h->stream>>>((int)h->n, (int)h->ld, h->Minv, h->Uc, h->A, h->sc);
+        return;
+    }
     const int nch = (int)((h->ld + 127) / 128);
     int split = (2 * h->sms + nch - 1) / nch;          // enough CTAs to fill the GPU: split the rows over blockIdx.y
     if (split > 8) split = 8;
@@ -588,8 +687,36 @@ void ccs_apply_inv(cc_handle* h) {
 // cc_create: form Minv when n is small enough (the work space is released right away)
 int ccs_setup_inverse(cc_handle* h) {
     h->Minv = nullptr;
-    if (h->dense || h->n > CC_INV_NMAX) return CC_OK;
+    h->inv_wide = 0;
+    if (h->dense) return CC_OK;
     const size_t n = (size_t)h->n;
+    if (h->n > CC_INV_NMAX) {
+        // a few thousand points, few columns: the dense inverse still pays (one product per MM iteration instead of ~20
+        // launch-bound CG sweeps) when all of uc fits in one CTA's shared memory and the matrix in L2
+        const size_t smem = n * (size_t)(h->ld + 1) * sizeof(float);
+        if (h->n > CC_INVW_NMAX || h->ld > 32 || smem > 200 * 1024) return CC_OK;
+        cudaError_t ea = cudaFuncSetAttribute(k_apply_inv_wide<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_apply_inv_wide<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (ea != cudaSuccess) { cudaGetLastError(); return CC_OK; }   // the CG solver
+        double *a = nullptr, *prow = nullptr;
+        CC_CUDA(h, cc_dev_alloc((void**)&a, n * n * sizeof(double), h->stream));
+        CC_CUDA(h, cc_dev_alloc((void**)&prow, 2 * n * sizeof(double), h->stream));
+        CC_CUDA(h, cc_dev_alloc((void**)&h->Minv, n * n * sizeof(float), h->stream));
+        CC_CUDA(h, cudaMemsetAsync(a, 0, n * n * sizeof(double), h->stream));
+        k_inv_init<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>((int)n, h->rowptr, h->col, a);
+        const dim3 ge((unsigned)((n + 255) / 256), (unsigned)(n < 64 ? n : 64));
+        for (int k = 0; k < (int)n; ++k) {
+            k_inv_pivot<<<(unsigned)((n + 255) / 256), 256, 0, h->stream>>>((int)n, k, a, prow, prow + n);
+            k_inv_elim<<<ge, 256, 0, h->stream>>>((int)n, k, a, prow, prow + n);
+        }
+        k_inv_store<<<h->grid_nodes, 256, 0, h->stream>>>((long long)(n * n), a, h->Minv);
+        CC_CUDA(h, cudaGetLastError());
+        cc_dev_free(prow, h->stream);
+        cc_dev_free(a, h->stream);
+        h->inv_wide = 1;
+        h->launches += 2 * (long long)n + 2;
+        return CC_OK;
+    }
     if (n * 128 * sizeof(float) > 48 * 1024) {
         cudaError_t ea = cudaFuncSetAttribute(k_apply_inv<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(n * 128 * sizeof(float)));
         if (ea != cudaSuccess) { cudaGetLastError(); return CC_OK; }   // fall back to the CG solver

@@ -388,50 +388,53 @@ __global__ void k_inv_store(long long nn, const double* __restrict__ a, float* _
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nn; t += (long long)gridDim.x * blockDim.x) Minv[t] = (float)a[t];
 }
 
-// A_i += sum_j Minv[i][j] uc_j for that shape: every CTA keeps ALL of uc (n rows of ld <= 32 floats, row stride ld + 1:
-// the lanes of a warp walk consecutive rows j) in shared memory and deals the rows i of Minv to its warps; a warp reads its
-// row of Minv once, coalesced (the matrix, 36 MB at n = 3000, lives in L2), and reduces the ld sums over its lanes.
-template <int LDW>
-__global__ void __launch_bounds__(512) k_apply_inv_wide(int n, int ld, const float* __restrict__ Minv, const float* __restrict__ Uc,
+// A_i += sum_j Minv[i][j] uc_j for that shape: every CTA keeps ALL of uc (n rows of Q float4, Q = ld / 4 <= 8) in shared
+// memory and deals the rows i of Minv to its warps; a warp reads its row of Minv once, coalesced (the matrix, 36 MB at
+// n = 3000, lives in L2), each lane takes the rows j = lane, lane + 32, ... of uc as 16-byte loads (row stride an odd number
+// of float4: eight consecutive rows fall into eight different bank groups), and the ld sums are reduced over the lanes.
+template <int Q>
+__global__ void __launch_bounds__(1024) k_apply_inv_wide(int n, int ld, const float* __restrict__ Minv, const float* __restrict__ Uc,
                                                         float* __restrict__ A, cc_scal* sc) {
     if (!sc->mm_active) return;
-    extern __shared__ float us[];                  // n x (ld + 1)
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, rs = ld + 1;
-    const int q4 = ld >> 2;                         // ld is a multiple of 4: rows of uc as float4
-    for (int t = threadIdx.x; t < n * q4; t += 512) {
-        const int j = t / q4, c = (t - j * q4) * 4;
-        const float4 v = ld4s(Uc + (size_t)j * ld + c);
-        float* d = us + j * rs + c;
-        d[0] = v.x; d[1] = v.y; d[2] = v.z; d[3] = v.w;
+    extern __shared__ float4 us4[];                // n x QS float4
+    constexpr int QS = Q | 1;                      // row stride in float4, odd
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int t = threadIdx.x; t < n * Q; t += 1024) {
+        const int j = t / Q, q = t - j * Q;
+        us4[j * QS + q] = ld4s(Uc + (size_t)j * ld + 4 * q);
     }
     __syncthreads();
-    for (int i = blockIdx.x * 16 + warp; i < n; i += gridDim.x * 16) {
-        float acc[LDW];
+    for (int i = blockIdx.x * 32 + warp; i < n; i += gridDim.x * 32) {
+        float4 acc[Q];
 #pragma unroll
-        for (int c = 0; c < LDW; ++c) acc[c] = 0.f;
+        for (int q = 0; q < Q; ++q) acc[q] = f4(0.f);
         const float* mrow = Minv + (size_t)i * n;
         for (int jb = lane; jb < n; jb += 32 * 8) {        // eight loads of the row in flight (the matrix comes from L2)
             float m[8];
 #pragma unroll
-            for (int q = 0; q < 8; ++q) m[q] = jb + 32 * q < n ? __ldg(mrow + jb + 32 * q) : 0.f;
+            for (int r = 0; r < 8; ++r) m[r] = jb + 32 * r < n ? __ldg(mrow + jb + 32 * r) : 0.f;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) {
-                const float* u = us + min(jb + 32 * q, n - 1) * rs;
+            for (int r = 0; r < 8; ++r) {
+                const float4* u = us4 + min(jb + 32 * r, n - 1) * QS;
 #pragma unroll
-                for (int c = 0; c < LDW; ++c)
-                    if (c < ld) acc[c] = fmaf(m[q], u[c], acc[c]);
+                for (int q = 0; q < Q; ++q) acc[q] = fma4(m[r], u[q], acc[q]);
             }
         }
 #pragma unroll
-        for (int c = 0; c < LDW; ++c)
+        for (int q = 0; q < Q; ++q)
 #pragma unroll
-            for (int of = 16; of > 0; of >>= 1) acc[c] += __shfl_xor_sync(0xffffffffu, acc[c], of);
-        // lane c owns column c of the row
-        float mine = 0.f;
+            for (int of = 16; of > 0; of >>= 1) {
+                acc[q].x += __shfl_xor_sync(0xffffffffu, acc[q].x, of);
+                acc[q].y += __shfl_xor_sync(0xffffffffu, acc[q].y, of);
+                acc[q].z += __shfl_xor_sync(0xffffffffu, acc[q].z, of);
+                acc[q].w += __shfl_xor_sync(0xffffffffu, acc[q].w, of);
+            }
+        // lane q owns quad q of the row
+        float4 mine = f4(0.f);
 #pragma unroll
-        for (int c = 0; c < LDW; ++c)
-            if (lane == c) mine = acc[c];
-        if (lane < ld) A[(size_t)i * ld + lane] += mine;
+        for (int q = 0; q < Q; ++q)
+            if (lane == q) mine = acc[q];
+        if (lane < Q) st4(A + (size_t)i * ld + 4 * lane, ld4s(A + (size_t)i * ld + 4 * lane) + mine);
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -440,6 +443,26 @@ __global__ void __launch_bounds__(512) k_apply_inv_wide(int n, int ld, const flo
             sc->ticket[5] = 0u;
             prof_mark(sc, 2);      // charged to the k_cg_update slot: it takes the place of the CG loop
         }
+    }
+}
+static size_t apply_wide_smem(const cc_handle* h) { return (size_t)h->n * (size_t)((h->ld / 4) | 1) * sizeof(float4); }
+template <int Q>
+static cudaError_t apply_wide_launch(cc_handle* h, int grid, bool only_attr) {
+    if (only_attr) return cudaFuncSetAttribute(k_apply_inv_wide<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)apply_wide_smem(h));
+    k_apply_inv_wide<Q><<<grid, 1024, apply_wide_smem(h), h->stream>>>((int)h->n, (int)h->ld, h->Minv, h->Uc, h->A, h->sc);
+    return cudaSuccess;
+}
+static cudaError_t apply_wide(cc_handle* h, bool only_attr) {
+    const int grid = h->sms < (int)((h->n + 31) / 32) ? h->sms : (int)((h->n + 31) / 32);   // one CTA per SM (shared memory)
+    switch ((int)(h->ld / 4)) {
+        case 1: return apply_wide_launch<1>(h, grid, only_attr);
+        case 2: return apply_wide_launch<2>(h, grid, only_attr);
+        case 3: return apply_wide_launch<3>(h, grid, only_attr);
+        case 4: return apply_wide_launch<4>(h, grid, only_attr);
+        case 5: return apply_wide_launch<5>(h, grid, only_attr);
+        case 6: return apply_wide_launch<6>(h, grid, only_attr);
+        case 7: return apply_wide_launch<7>(h, grid, only_attr);
+        default: return apply_wide_launch<8>(h, grid, only_attr);
     }
 }
 
@@ -741,12 +764,7 @@ void ccs_rhs(cc_handle* h) {
 
 void ccs_apply_inv(cc_handle* h) {
     if (h->inv_wide) {
-        const size_t smem = (size_t)h->n * (h->ld + 1) * sizeof(float);
-        const int grid = h->sms < (int)((h->n + 15) / 16) ? h->sms : (int)((h->n + 15) / 16);   // one CTA per SM (shared memory)
-        if (h->ld <= 16)
-            k_apply_inv_wide<16><<<grid, 512, smem, h->stream>>>((int)h->n, (int)h->ld, h->Minv, h->Uc, h->A, h->sc);
-        else
-            k_apply_inv_wide<32><<<grid, 512, smem, h->stream>>>((int)h->n, (int)h->ld, h->Minv, h->Uc, h->A, h->sc);
+        apply_wide(h, false);
         return;
     }
     const int nch = (int)((h->ld + 127) / 128);
@@ -767,11 +785,8 @@ int ccs_setup_inverse(cc_handle* h) {
     if (h->n > CC_INV_NMAX) {
         // a few thousand points, few columns: the dense inverse still pays (one product per MM iteration instead of ~20
         // launch-bound CG sweeps) when all of uc fits in one CTA's shared memory and the matrix in L2
-        const size_t smem = n * (size_t)(h->ld + 1) * sizeof(float);
-        if (h->n > CC_INVW_NMAX || h->ld > 32 || smem > 200 * 1024) return CC_OK;
-        cudaError_t ea = cudaFuncSetAttribute(k_apply_inv_wide<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_apply_inv_wide<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (ea != cudaSuccess) { cudaGetLastError(); return CC_OK; }   // the CG solver
+        if (h->n > CC_INVW_NMAX || h->ld > 32 || apply_wide_smem(h) > 200 * 1024) return CC_OK;
+        if (apply_wide(h, true) != cudaSuccess) { cudaGetLastError(); return CC_OK; }   // the CG solver
         double *a = nullptr, *wk = nullptr;           // wk: P (32 x 32), R' (32 x n), C (n x 32)
         CC_CUDA(h, cc_dev_alloc((void**)&a, n * n * sizeof(double), h->stream));
         CC_CUDA(h, cc_dev_alloc((void**)&wk, (CC_INVB * CC_INVB + 2 * CC_INVB * n) * sizeof(double), h->stream));

@@ -206,7 +206,8 @@ def sweep_bytes(n, p, nnz, masked, dense=False):
     npb, E = 4 * n * p, nnz // 2
     if dense and n <= 64:
         # genotype-like: read U, A', write A + read X, U, A, write U (SURVEY 8(d) "Dense path": 7 node arrays)
-        return {"a9_small": (7 * npb, ("kd_proj",)), "a4_edges": (16 * n * n, ("kd_edges",)), "a5_update": (4 * npb + n * p, ("k_update",))}
+        # (the block soft-threshold over the n x n matrices, a4, rides in k_update's launch: 16 n^2 bytes)
+        return {"a9_small": (7 * npb, ("kd_proj",)), "a5_update": (4 * npb + n * p + 16 * n * n, ("k_update",))}
     if dense:
         # dense-weight: W (n x n) once + ~10 node arrays per MM iteration; per kernel the n x n it must touch
         return {"a9_proj": (4 * n * n + 5 * npb, ("kd_proj",)), "a9_pairs": (4 * n * n // 2 + 2 * npb, ("kd_pairs",)),

@@ -964,7 +964,8 @@ __global__ void __launch_bounds__(256) kd_pairs(int n, int ld, int ntile, int ks
     }
 }
 
-// ---- kd_edges: block soft-threshold over the n x n matrices; the FFMA / n <= 64 paths only
+// ---- kd_edges: block soft-threshold over the n x n matrices; the FFMA / n <= 64 paths only, and
+// since late round 2 only their cold start (inside the iteration the same arithmetic rides in k_update's launch)
 // (the tensor-core path never stores S: see shrink_ratio)
 __global__ void __launch_bounds__(256, 4) kd_edges(int n, int ksplit, const float* __restrict__ NB2, const float* __restrict__ W,
                                                 float* __restrict__ S, float* __restrict__ VN, cc_scal* sc, double* part,
@@ -1362,8 +1363,7 @@ void ccd_init_state(cc_handle* h) {
 void ccd_iteration(cc_handle* h) {
     if (h->dn_small) {
         launch_small(h);
-        ccs_update_nodes(h);
-        ccd_edges(h, 0);
+        ccs_update_nodes(h, 1);                // the block soft-threshold over the n x n matrices rides along (kd_edges' work)
         return;
     }
     ccd_colmeans(h);
@@ -1375,8 +1375,7 @@ void ccd_iteration(cc_handle* h) {
         kd_dsum2<<<(unsigned)((h->ld + 7) / 8), 256, 0, h->stream>>>((int)h->n, (int)h->ld, ns, h->colps, h->dbar, h->sc);
     }
     ccd_pairs(h);
-    ccs_update_nodes(h);
-    if (!h->dn_tc) ccd_edges(h, 0);            // the tensor-core path keeps ||b|| only: no pass over the n x n matrices
+    ccs_update_nodes(h, h->dn_tc ? 0 : 1);     // the tensor-core path keeps ||b|| only: no pass over the n x n matrices
 }
 
 int ccd_solve_eager(cc_handle* h, int maxit) {
@@ -1393,7 +1392,7 @@ int ccd_solve_eager(cc_handle* h, int maxit) {
     return CC_OK;
 }
 
-// graph:  WHILE(outer){ kd_colsum1; kd_colsum2; [kd_prep_proj;] kd_proj*; kd_dsum1; kd_dsum2; [kd_prep_pairs;] kd_pairs*; k_update; [kd_edges] }
+// graph:  WHILE(outer){ kd_colsum1; kd_colsum2; [kd_prep_proj;] kd_proj*; kd_dsum1; kd_dsum2; [kd_prep_pairs;] kd_pairs*; k_update }   or   WHILE(outer){ kd_small_tc; k_update }
 int ccd_build_graph(cc_handle* h) {
     if (h->gexec) return CC_OK;
     cudaStream_t cap;

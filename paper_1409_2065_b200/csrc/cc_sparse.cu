@@ -649,8 +649,48 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
                                                         float* __restrict__ Z, float* __restrict__ Ap, float* __restrict__ Dl,
                                                         const float* __restrict__ dbar,
                                                         const float* __restrict__ w, const float* __restrict__ nb2,
-                                                        float* __restrict__ s, float* __restrict__ vn, cc_scal* sc) {
+                                                        float* __restrict__ s, float* __restrict__ vn, cc_scal* sc,
+                                                        const float* __restrict__ dNB2, int dksplit, const float* __restrict__ dW,
+                                                        float* __restrict__ dS, float* __restrict__ dVN, double* dpart) {
     if (!sc->mm_active) return;
+    if (dNB2) {
+        // dense mode with stored S (n < 128 or n not a multiple of 4): the block soft-threshold over the n x n matrices
+        // rides along here -- as a kernel of its own (kd_edges) it cost 12 us + a launch gap per
+        // iteration at 52 x 200,000, nearly all of it latency.  The slices of ||b||^2 are added in a fixed order.
+        const size_t nn = (size_t)n * n;
+        const float cthr = sc->cthr;
+        double pen[1] = {0.0};     // sum_{i<j} w ||v|| of the state written here = the penalty term of the next Phi
+        const bool warp_per = dksplit >= 32;
+        const int lane = threadIdx.x & 31;
+        const long long nwork = (long long)gridDim.x * (warp_per ? CC_THREADS / 32 : CC_THREADS);
+        for (long long e = warp_per ? (long long)blockIdx.x * (CC_THREADS / 32) + threadIdx.x / 32
+                                    : (long long)blockIdx.x * CC_THREADS + threadIdx.x;
+             e < (long long)nn; e += nwork) {
+            const int i = (int)(e / n), j = (int)(e % n);
+            float q = 0.f;
+            if (warp_per) {
+                for (int k = lane; k < dksplit; k += 32) q += dNB2[(size_t)k * nn + e];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+                if (lane) continue;
+            } else {
+                q = dNB2[e];
+                for (int k = 1; k < dksplit; ++k) q += dNB2[(size_t)k * nn + e];
+            }
+            float sn = 0.f, vnv = 0.f;
+            if (i != j) {
+                const float nb = sqrtf(q);
+                const float thr = cthr * dW[e];
+                sn = nb <= thr ? 0.f : 1.f - thr / nb;
+                vnv = sn * nb;
+            }
+            dS[e] = sn;
+            dVN[e] = vnv;
+            if (j > i) pen[0] += (double)(dW[e] * vnv);
+        }
+        double ptot[1];
+        if (grid_reduce<1>(pen, dpart, &sc->ticket[7], ptot)) sc->pen_next = ptot[0];
+    }
     const int gl = threadIdx.x & (G - 1);
     const long long ngroups = (long long)gridDim.x * (CC_THREADS / G);
     const long long items = (long long)n * nchunk;
@@ -841,13 +881,17 @@ void ccs_norm(cc_handle* h) {
 
 void ccs_update(cc_handle* h) {
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, (long long)h->nnz, h->X, h->mask,
-                  h->A, h->U, h->Minv ? (float*)nullptr : h->Z, h->Ap, h->Dl, (const float*)nullptr, h->w, h->nb2, h->s, h->vn, h->sc);
+                  h->A, h->U, h->Minv ? (float*)nullptr : h->Z, h->Ap, h->Dl, (const float*)nullptr, h->w, h->nb2, h->s, h->vn, h->sc,
+                  (const float*)nullptr, 0, (const float*)nullptr, (float*)nullptr, (float*)nullptr, (double*)nullptr);
 }
 
-void ccs_update_nodes(cc_handle* h) {
+void ccs_update_nodes(cc_handle* h, int with_edges) {
+    // with_edges: the dense paths that store S add their block soft-threshold (the work of kd_edges) to this launch
+    const float* nb = with_edges ? h->NB2d : nullptr;
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, 0LL, h->X, h->mask, h->A, h->U,
                   (float*)nullptr, h->Ap, (float*)nullptr, (const float*)h->dbar, (const float*)nullptr, (const float*)nullptr,
-                  (float*)nullptr, (float*)nullptr, h->sc);
+                  (float*)nullptr, (float*)nullptr, h->sc, nb, h->dn_ksplit, (const float*)h->Wd, h->Sd, h->VNd,
+                  h->part + 6 * CC_MAXBLK * CC_NPART);
 }
 
 void ccs_pair_norms(cc_handle* h, const float* V, float* out, float* s_out) {

@@ -124,6 +124,17 @@ def test_popres_like_low_p_large_k(B, torch_, oracle, phi):
     print("popres phi", phi, "clusters", [k for _, k in out])
 
 
+def test_popres_full_size_dense_inverse_from_l2(B, torch_, oracle):
+    """The POPRES-like configuration at its full size (3000 x 10, k = 40): a2 is the dense inverse formed once by the blocked
+    Gauss-Jordan and applied from L2 (k_apply_inv_wide); 94 pivot blocks, the last one ragged (3000 = 93 x 32 + 24)."""
+    wl = synth.make("popres")
+    assert wl.n == 3000 and wl.p == 10
+    prob = H.build_problem(oracle, wl)
+    gammas = [0.05, 1.0]
+    ref = H.oracle_path(oracle, prob, gammas, 40, proj_method=1)
+    _run_path(B, torch_, prob, gammas, 40, ref)
+
+
 def test_path_with_stop_rule_expression_masked(B, torch_, oracle):
     """cc_path with tol > 0 on a masked instance: per-gamma iteration counts (S3), labels and U follow the oracle."""
     torch = torch_

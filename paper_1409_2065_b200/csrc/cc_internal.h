@@ -127,7 +127,7 @@ struct cc_handle {
     unsigned long long prof_ns[8], prof_calls[8];   // accumulated over solves (cc_get_profile)
     int grid_nodes, grid_rows, grid_edges;   // launch sizes, fixed per handle (determinism)
     // persistent single-kernel solve (cc_persist.cu): 0 slabs = not used by this handle
-    int pt_slabs, pt_sw, pt_minv_smem, pt_prof;
+    int pt_slabs, pt_sw, pt_minv_smem, pt_prof;     // pt_minv_smem: the projection mode of k_mm_persist (0, 1, 2)
     size_t pt_smem;
     float* pt_nbpart;                 // pt_slabs x nnz partial squared norms
     double* pt_spart;                 // pt_slabs x 4 partial scalars

@@ -21,6 +21,7 @@
 
 #include "cc_device.cuh"
 #include "cc_internal.h"
+#include "cc_tc.cuh"
 
 namespace {
 
@@ -71,19 +72,46 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double (*sm)[PT_THREA
 
 struct pt_ctl {
     float cu, ca, cthr;
-    int stop;
+    int stop, fail;
 };
 
-template <bool MINV_SMEM>
+// MODE 0: the inverse stays in global memory; 1: transposed copy in shared memory, 4 x 8 register tiles (FFMA);
+// 2 (n <= 128): the inverse lives in TENSOR MEMORY for the whole solve (lane = row i, column = j, TF32 hi and lo) and the
+// projection of a slab is one tcgen05.mma tile per iteration: M = 128 rows, N = slab columns (padded to 16), K = n, 3xTF32;
+// phase 1a writes D^-1 r0 straight into the shared-memory operand (K-major, SWIZZLE_128B, hi and lo), the four warps that
+// own the TMEM lanes read the products back and add z.  (`expression`: 5.1 us of the 18.9 us iteration were the FFMA tiles.)
+constexpr int PT_KP = 128;                         // TMEM columns per plane of the inverse; the accumulator starts at 2 * PT_KP
+__device__ __forceinline__ void pt_mma_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}\n"
+        :: "r"(tmem_d), "r"(tmem_a), "l"(db), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void pt_tmem_st8(uint32_t taddr, const float (&v)[8]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+                 :: "r"(taddr), "r"(__float_as_uint(v[0])), "r"(__float_as_uint(v[1])), "r"(__float_as_uint(v[2])),
+                    "r"(__float_as_uint(v[3])), "r"(__float_as_uint(v[4])), "r"(__float_as_uint(v[5])),
+                    "r"(__float_as_uint(v[6])), "r"(__float_as_uint(v[7])) : "memory");
+}
+
+template <int MODE>
 __global__ void __launch_bounds__(PT_THREADS, 1)
 k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ rowptr, const int* __restrict__ rowup,
              const int* __restrict__ col, const int* __restrict__ peer, const float* __restrict__ w, float* s, float* vn,
              float* nb2, const float* __restrict__ dinv, const float* __restrict__ Minv, const float* __restrict__ X,
              const uint8_t* __restrict__ mask, float* U, float* A, float* Ap, cc_scal* sc, float* nbpart, double* spart,
              double* hist_phi, double* hist_d) {
-    extern __shared__ __align__(16) unsigned char pt_smem[];
+    constexpr bool MINV_SMEM = MODE == 1, PROJ_TC = MODE == 2;
+    extern __shared__ __align__(16) unsigned char pt_smem_raw[];
     __shared__ double red_s[3][PT_THREADS / 32];
     __shared__ pt_ctl ctl;
+    __shared__ __align__(8) uint64_t mma_done;
+    __shared__ uint32_t tmem_base_s;
+    // MODE 2: the operand of D^-1 r0 comes first (1024-byte aligned): {hi, lo} x ceil(n / 32) K chunks x NP rows x 128 bytes
+    const int NP = (sw + 15) & ~15, KCH = (n + 31) >> 5;
+    const uint32_t opb = PROJ_TC ? ((smem_u32(pt_smem_raw) + 1023u) & ~1023u) : 0u;
+    const uint32_t opsz = PROJ_TC ? (uint32_t)(2 * KCH * NP * 128) : 0u;
+    unsigned char* pt_smem = PROJ_TC ? pt_smem_raw + (opb - smem_u32(pt_smem_raw)) + opsz : pt_smem_raw;
     const int tid = threadIdx.x, c = blockIdx.x, nslab = gridDim.x;
     const int c0 = c * sw;
     const int wq = (min(sw, ld - c0)) >> 2;              // float4 quads of this slab (ld and sw are multiples of 4)
@@ -95,8 +123,8 @@ k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ ro
     float* Us = Xs + (size_t)n * rs_;
     float* Ps = Us + (size_t)n * rs_;                    // A' (the previous projection)
     float* As = Ps + (size_t)n * rs_;
-    float* Cs = As + (size_t)n * rs_;                    // D^-1 r0
-    float* ss = Cs + (size_t)n * rs_;                    // shrink factors, all directed entries
+    float* Cs = As + (size_t)n * rs_;                    // D^-1 r0 (MODE 2: not there, the operand takes its place)
+    float* ss = Cs + (PROJ_TC ? 0 : (size_t)n * rs_);    // shrink factors, all directed entries
     const int n4 = (n + 3) & ~3;
     float* Mv = ss + ((nnz + 3) & ~3);                   // Minv TRANSPOSED, n rows of n4 floats (rows i >= n of a column: 0), when it fits
     int* plist = reinterpret_cast<int*>(Mv + (MINV_SMEM ? (size_t)n * n4 : 0));   // upper entries (col > row), in order
@@ -111,6 +139,36 @@ k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ ro
     float* wps = vns + npairs;
 
     // ---- one-time loads
+    if (tid == 0) ctl.fail = 0;
+    if constexpr (PROJ_TC) {
+        if (tid == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(smem_u32(&mma_done)));
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        }
+        if (tid < 32) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_u32(&tmem_base_s)), "n"(512));
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+        }
+        for (uint32_t t = tid; t < opsz / 4; t += PT_THREADS)      // rows >= the slab's columns and K >= n stay zero for good
+            asm volatile("st.shared.f32 [%0], %1;" :: "r"(opb + 4u * t), "f"(0.f) : "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (tid < 128) {                                           // lane i of tensor memory = row i of the inverse
+            const uint32_t tl = tmem_base_s + ((uint32_t)((tid >> 5) * 32) << 16);
+            for (int j0 = 0; j0 < KCH * 32; j0 += 8) {
+                float hi[8], lo[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) {
+                    const float v = (tid < n && j0 + q < n) ? Minv[(size_t)tid * n + j0 + q] : 0.f;
+                    split_tf32(v, hi[q], lo[q]);
+                }
+                pt_tmem_st8(tl + j0, hi);
+                pt_tmem_st8(tl + PT_KP + j0, lo);
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        }
+    }
     for (int it = tid; it < n * wq; it += PT_THREADS) {
         const int i = it / wq, q = it - i * wq;
         const size_t g = (size_t)i * ld + c0 + 4 * q;
@@ -199,12 +257,73 @@ k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ ro
                 for (int b = 0; b < 4; ++b) acc = fma4(sv[b], api - pj[b], acc);
             }
             acc = acc - (api - ld4s(Us + o));
-            st4(Cs + o, dinv_s[i] * acc);
+            const float4 cv4 = dinv_s[i] * acc;
+            if constexpr (PROJ_TC) {
+                // element (column, j = i) of the operand: K chunk i / 32, row = column, 16-byte piece (i % 32) / 4 at position
+                // piece ^ (column % 8), word i % 4
+                const float cv[4] = {cv4.x, cv4.y, cv4.z, cv4.w};
+                const uint32_t kb = opb + (uint32_t)((i >> 5) * NP * 128 + (i & 3) * 4), pc = (uint32_t)((i & 31) >> 2);
+#pragma unroll
+                for (int e2 = 0; e2 < 4; ++e2) {
+                    const int colm = 4 * q + e2;
+                    float h2, l2;
+                    split_tf32(cv[e2], h2, l2);
+                    const uint32_t ad = kb + (uint32_t)(colm * 128) + ((pc ^ (uint32_t)(colm & 7)) << 4);
+                    asm volatile("st.shared.f32 [%0], %1;" :: "r"(ad), "f"(h2) : "memory");
+                    asm volatile("st.shared.f32 [%0], %1;" :: "r"(ad + (uint32_t)(KCH * NP * 128)), "f"(l2) : "memory");
+                }
+            } else {
+                st4(Cs + o, cv4);
+            }
+        }
+        if constexpr (PROJ_TC) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         }
         __syncthreads();
         lap(0);
         // ===== phase 1b: A = z + Minv (D^-1 r0), z = a'   (the projection, L90-L103, by the inverse formed once in cc_create)
-        if constexpr (MINV_SMEM) {
+        if constexpr (PROJ_TC) {
+            if (tid == 0) {
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t td = tmem_base_s + 2 * PT_KP;
+                const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(NP >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+                const uint64_t d0 = ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) | ((uint64_t)2 << 61);
+                const uint64_t dbh = d0 | (uint64_t)(opb >> 4), dbl = d0 | (uint64_t)((opb + (uint32_t)(KCH * NP * 128)) >> 4);
+                const int nks = (n + 7) >> 3;
+                for (int ks = 0; ks < nks; ++ks) {
+                    const uint64_t kb = (uint64_t)((ks >> 2) * ((NP * 128) >> 4) + (ks & 3) * 2);       // K chunk, then 32 bytes per step
+                    pt_mma_ts(td, tmem_base_s + 8 * ks, dbh + kb, idesc, ks > 0 ? 1u : 0u);
+                    pt_mma_ts(td, tmem_base_s + 8 * ks, dbl + kb, idesc, 1u);
+                    pt_mma_ts(td, tmem_base_s + PT_KP + 8 * ks, dbh + kb, idesc, 1u);
+                }
+                asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" :: "r"(smem_u32(&mma_done)) : "memory");
+            }
+            if (tid < 128) {
+                if (!mbar_wait(smem_u32(&mma_done), (uint32_t)(m & 1))) ctl.fail = 1;
+                asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+                const uint32_t tl = tmem_base_s + ((uint32_t)((tid >> 5) * 32) << 16) + 2 * PT_KP;
+                for (int cb = 0; cb < 4 * wq; cb += 16) {
+                    uint32_t v[16];
+                    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+                                   "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+                                 : "r"(tl + (uint32_t)cb));
+                    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                    if (tid < n) {
+#pragma unroll
+                        for (int q4 = 0; q4 < 4; ++q4) {
+                            if (cb + 4 * q4 < 4 * wq) {
+                                const int o = tid * rs_ + cb + 4 * q4;
+                                st4(As + o, ld4s(Ps + o) + make_float4(__uint_as_float(v[4 * q4]), __uint_as_float(v[4 * q4 + 1]),
+                                                                      __uint_as_float(v[4 * q4 + 2]), __uint_as_float(v[4 * q4 + 3])));
+                            }
+                        }
+                    }
+                }
+                asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            }
+        } else if constexpr (MINV_SMEM) {
             // register tile of 4 rows x 4 columns per thread; the sum over j is split over JS adjacent lanes (j = jp, jp + JS, ...)
             // and combined by a fixed shuffle tree, so that small problems still occupy the CTA.  Per j step: one 16-byte
             // load of D^-1 r0 and one of the transposed inverse for 16 FFMA (the one-row form was bound by shared-memory
@@ -422,6 +541,12 @@ k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ ro
         st4(Ap + g, ld4s(Ps + o));
         if (m > 0) st4(A + g, ld4s(As + o));
     }
+    if constexpr (PROJ_TC) {
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(tmem_base_s), "n"(512));
+        if (tid == 0 && ctl.fail) sc->cg_failed = 2;
+    }
     if (c == 0 && tid == 0) {
         sc->mm_iter = m;
         sc->dist2 = dist2_t; sc->loss = loss_t; sc->pen = pen_t;
@@ -441,14 +566,19 @@ k_mm_persist(int n, int ld, int sw, int rs_, int nnz, const int* __restrict__ ro
 // ---- host side -----------------------------------------------------------------------------------------------------
 static int persist_stride(int sw) { return ((sw >> 2) & 1) ? sw : sw + 4; }
 
-static size_t persist_smem(const cc_handle* h, int sw, int minv_in_smem) {
+// mode: 0 inverse in global memory, 1 transposed copy in shared memory, 2 inverse in tensor memory (n <= 128)
+static size_t persist_smem(const cc_handle* h, int sw, int mode) {
     const size_t n = (size_t)h->n, nnz = (size_t)h->nnz, rs = (size_t)persist_stride(sw);
-    size_t b = 5 * n * rs * sizeof(float) + ((nnz + 3) & ~(size_t)3) * sizeof(float);
-    if (minv_in_smem) b += n * ((n + 3) & ~(size_t)3) * sizeof(float);
+    size_t b = (mode == 2 ? 4 : 5) * n * rs * sizeof(float) + ((nnz + 3) & ~(size_t)3) * sizeof(float);
+    if (mode == 1) b += n * ((n + 3) & ~(size_t)3) * sizeof(float);
+    if (mode == 2) b += 1024 + 2 * ((n + 31) / 32) * (size_t)((sw + 15) & ~15) * 128;     // alignment + the operand of D^-1 r0
     b += (nnz / 2) * sizeof(int) + 2 * nnz * sizeof(unsigned short);
     if (h->mask) b += n * rs;
     if ((h->ld + sw - 1) / sw == 1) b += 3 * (nnz / 2) * sizeof(float);      // one slab: per-pair arrays
     return b + 16;
+}
+static const void* persist_fn(int mode) {
+    return mode == 2 ? (const void*)k_mm_persist<2> : mode == 1 ? (const void*)k_mm_persist<1> : (const void*)k_mm_persist<0>;
 }
 
 // Decide whether this handle runs the persistent kernel, and with which slab width.  Called once from cc_create after
@@ -472,25 +602,28 @@ int ccp_setup(cc_handle* h) {
     if (sw > ld) sw = ld;
     for (;; sw += 4) {            // shrink nothing: a wider slab only lowers the CTA count; stop when it cannot fit
         const int nslab = (int)((ld + sw - 1) / sw);
-        int minv_smem = 1;
-        size_t need = persist_smem(h, (int)sw, 1);
-        if (need > (size_t)maxsm) { minv_smem = 0; need = persist_smem(h, (int)sw, 0); }
+        int mode = (n <= 128 && sw <= 256) ? 2 : 1;
+        size_t need = persist_smem(h, (int)sw, mode);
+        if (need > (size_t)maxsm && mode == 2) { mode = 1; need = persist_smem(h, (int)sw, 1); }
+        if (need > (size_t)maxsm) { mode = 0; need = persist_smem(h, (int)sw, 0); }
         if (need > (size_t)maxsm) return CC_OK;            // does not fit at the narrowest admissible slab: graph path
         if (nslab > h->sms) { if (sw >= ld) return CC_OK; continue; }
-        const void* fn = minv_smem ? (const void*)k_mm_persist<true> : (const void*)k_mm_persist<false>;
+        const void* fn = persist_fn(mode);
         if (cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)need) != cudaSuccess) {
             cudaGetLastError();
             return CC_OK;
         }
         int occ = 0;
-        if ((minv_smem ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<true>, PT_THREADS, need)
-                       : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<false>, PT_THREADS, need)) != cudaSuccess || occ < 1) {
+        cudaError_t eo = mode == 2 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<2>, PT_THREADS, need)
+                       : mode == 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<1>, PT_THREADS, need)
+                                   : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_mm_persist<0>, PT_THREADS, need);
+        if (eo != cudaSuccess || occ < 1) {
             cudaGetLastError();
             return CC_OK;
         }
         h->pt_slabs = nslab;
         h->pt_sw = (int)sw;
-        h->pt_minv_smem = minv_smem;
+        h->pt_minv_smem = mode;
         h->pt_smem = need;
         break;
     }
@@ -505,7 +638,7 @@ int ccp_solve(cc_handle* h) {
     void* args[] = {&n, &ld, &sw, &rs, &nnz, &h->rowptr, &h->rowup, &h->col, &h->peer, &h->w, &h->s, &h->vn, &h->nb2,
                     &h->dinv, &h->Minv, &h->X, &h->mask, &h->U, &h->A, &h->Ap, &h->sc, &h->pt_nbpart, &h->pt_spart,
                     &h->hist_phi, &h->hist_d};
-    CC_CUDA(h, cudaLaunchCooperativeKernel(h->pt_minv_smem ? (const void*)k_mm_persist<true> : (const void*)k_mm_persist<false>, dim3((unsigned)h->pt_slabs), dim3(PT_THREADS), args,
+    CC_CUDA(h, cudaLaunchCooperativeKernel(persist_fn(h->pt_minv_smem), dim3((unsigned)h->pt_slabs), dim3(PT_THREADS), args,
                                            h->pt_smem, h->stream));
     return CC_OK;
 }

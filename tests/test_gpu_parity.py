@@ -135,6 +135,18 @@ def test_popres_full_size_dense_inverse_from_l2(B, torch_, oracle):
     _run_path(B, torch_, prob, gammas, 40, ref)
 
 
+@pytest.mark.parametrize("p,k", [(3, 12), (5, 20), (14, 16), (17, 10), (21, 10), (26, 10), (30, 8)])
+def test_dense_inverse_from_l2_every_width(B, torch_, oracle, p, k):
+    """k_apply_inv_wide has one instantiation per ld / 4 (ld = p rounded up to 4: 4, 8, 16, 20, 24, 28, 32 here; 12 is the
+    POPRES shape above): n = 450 > 384 points, so a2 is the blocked Gauss-Jordan inverse applied from L2 (15 pivot blocks,
+    the last of 2 rows)."""
+    wl = synth.make("popres", n=450, p=p, k=k, phi=2.0)
+    prob = H.build_problem(oracle, wl)
+    gammas = [0.05, 0.8]
+    ref = H.oracle_path(oracle, prob, gammas, 30, proj_method=1)
+    _run_path(B, torch_, prob, gammas, 30, ref)
+
+
 def test_path_with_stop_rule_expression_masked(B, torch_, oracle):
     """cc_path with tol > 0 on a masked instance: per-gamma iteration counts (S3), labels and U follow the oracle."""
     torch = torch_

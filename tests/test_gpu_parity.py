@@ -234,10 +234,15 @@ def test_graph_and_eager_launch_modes_are_bit_identical_and_deterministic(B, tor
     assert np.array_equal(outs[0], outs[2])
 
 
-@pytest.mark.parametrize("name,kw", [("tiny", {}), ("expression", dict(n=40, p=301)), ("expression", dict(n=100, p=2000))])
+@pytest.mark.parametrize("name,kw", [("tiny", {}), ("expression", dict(n=40, p=301)), ("expression", dict(n=100, p=2000)),
+                                     ("expression", dict(n=128, p=900)),     # the largest n of the tensor-core projection: K = M = 128
+                                     ("expression", dict(n=97, p=37)),       # one slab, ragged K (97 = 12 x 8 + 1) and N (40 -> 48)
+                                     ("expression", dict(n=129, p=600)),     # just above: the FFMA register tiles
+                                     ("expression", dict(n=12, p=5000))])    # K = 16 of which 12, wide slabs
 def test_persistent_kernel_and_stream_kernels_agree(B, torch_, oracle, name, kw):
     """Small n: cc_solve runs the whole MM loop as one persistent kernel (column slabs in shared memory, two grid
-    barriers per iteration); prm.use_graph = 0 drives the separate stream kernels from the host.  Different summation
+    barriers per iteration; for n <= 128 the projection by the inverse is one tcgen05 tile per slab, the inverse resident in
+    tensor memory); prm.use_graph = 0 drives the separate stream kernels from the host.  Different summation
     orders, same iteration: both within the tolerance of the oracle, and within 1e-5 of each other, labels equal."""
     torch = torch_
     wl = synth.make(name, **kw)

@@ -226,7 +226,8 @@ def impl_bytes(kernel, n, p, nnz, masked, dense=False):
         "k_cg_spmv": nnz * (row + 4) + 5 * npb + 4 * n,      # gather + own uc, p, s in; p, s out
         "k_cg_update": 6 * npb + 4 * n,                      # p, s, A, uc in; A, uc out
         "k_norm": (nnz // 2) * (2 * row + 28) + 4 * npb + (n * p if masked else 0) + 8 * n,
-        "k_update": (5 * npb if dense else 8 * npb + 16 * nnz) + (n * p if masked else 0),
+        # dense: A, U, X in, U and A' out -- n <= 64: no A' (the fused kernel reads A and dbar), + the n x n shrink
+        "k_update": ((4 * npb + 16 * n * n if n <= 64 else 5 * npb) if dense else 8 * npb + 16 * nnz) + (n * p if masked else 0),
         # n <= 64: the fused kernel streams U, A', X in and A out.  Tensor-core path (n >= 128): kd_proj_tc3 reads the ratio
         # matrix R (n x n) + the pre-split B operand (2 np, re-read per row tile from L2) + 5 node arrays; kd_pairs_tc2 reads
         # ||b||, R, W of the upper triangle and writes ||b|| (upper) and R (both triangles) + the pre-split operands

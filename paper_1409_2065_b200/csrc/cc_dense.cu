@@ -1350,6 +1350,10 @@ void ccd_sumw2(cc_handle* h) {
 void ccd_init_state(cc_handle* h) {
     const size_t bytes = (size_t)h->n * h->ld * sizeof(float);
     cudaMemcpyAsync(h->Ap, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
+    if (h->dn_small) {                         // this path keeps the previous projection as (A, dbar): A = U0, dbar = 0
+        cudaMemcpyAsync(h->A, h->U, bytes, cudaMemcpyDeviceToDevice, h->stream);
+        cudaMemsetAsync(h->dbar, 0, (size_t)h->ld * sizeof(float), h->stream);
+    }
     launch_pairs(h, h->U, h->U, 1);            // ||u0_i - u0_j||^2 by direct differences (every dense path starts here)
     if (h->dn_tc) {
         kd_nb_init<<<h->grid_nodes, 256, 0, h->stream>>>((long long)h->n * h->n, h->NB2d, h->Wd, h->Rd);
@@ -1363,7 +1367,8 @@ void ccd_init_state(cc_handle* h) {
 void ccd_iteration(cc_handle* h) {
     if (h->dn_small) {
         launch_small(h);
-        ccs_update_nodes(h, 1);                // the block soft-threshold over the n x n matrices rides along (kd_edges' work)
+        ccs_update_nodes(h, 1, 0);             // the block soft-threshold over the n x n matrices rides along (kd_edges' work);
+                                               // no A' = A - dbar is stored: kd_small_tc reads A and dbar
         return;
     }
     ccd_colmeans(h);
@@ -1375,7 +1380,7 @@ void ccd_iteration(cc_handle* h) {
         kd_dsum2<<<(unsigned)((h->ld + 7) / 8), 256, 0, h->stream>>>((int)h->n, (int)h->ld, ns, h->colps, h->dbar, h->sc);
     }
     ccd_pairs(h);
-    ccs_update_nodes(h, h->dn_tc ? 0 : 1);     // the tensor-core path keeps ||b|| only: no pass over the n x n matrices
+    ccs_update_nodes(h, h->dn_tc ? 0 : 1, 1);  // the tensor-core path keeps ||b|| only: no pass over the n x n matrices
 }
 
 int ccd_solve_eager(cc_handle* h, int maxit) {

@@ -158,7 +158,7 @@ void ccd_init_state(cc_handle* h);
 void ccd_lab_hook(cc_handle* h, int* changed);
 int ccd_solve_eager(cc_handle* h, int maxit);
 int ccd_build_graph(cc_handle* h);
-void ccs_update_nodes(cc_handle* h, int with_edges);  // k_update, node part (dense mode) [+ the block soft-threshold of the stored-S paths]
+void ccs_update_nodes(cc_handle* h, int with_edges, int store_ap);  // k_update, node part (dense mode) [+ the block soft-threshold of the stored-S paths]
 // ---- cc_small.cu (a9, n <= 64): the fused kernel with the contraction on the tensor cores
 int ccd_small_tc_setup(cc_handle* h);     // 1: use it (sets dn_small_cs, dn_small_grid); 0: not available
 int ccd_small_tc_maps(cc_handle* h);      // after the node arrays exist

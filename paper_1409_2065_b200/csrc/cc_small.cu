@@ -115,7 +115,7 @@ __device__ __forceinline__ void small_issue_array(uint32_t dst, const CUtensorMa
 }
 
 __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int cs_per_tile, const float* __restrict__ S,
-                                                             const __grid_constant__ CUtensorMap tmU, const __grid_constant__ CUtensorMap tmP,
+                                                             const __grid_constant__ CUtensorMap tmU,
                                                              const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmA,
                                                              const uint8_t* __restrict__ mask,
                                                              const float* __restrict__ W, const float* __restrict__ VN,
@@ -155,7 +155,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
             const uint32_t bar = smem_u32(&full[kk]), dst = smem_u32(dbuf + (size_t)kk * 2 * bufsz);
             expect_tx(bar, 2u * tx_bytes);
             small_issue_array(dst, &tmU, c0, bar);
-            small_issue_array(dst + bufsz * 4, &tmP, c0, bar);
+            small_issue_array(dst + bufsz * 4, &tmA, c0, bar);
         }
         if (nmine > 0) {
             expect_tx(smem_u32(&xfull), tx_bytes);
@@ -256,6 +256,11 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
             }
             if (!inside) los = 0.f;
             const float ub = su * rfn;
+            // The previous projection arrives as the array A this kernel wrote one iteration ago, whose residual column mean
+            // dbar k_update removed only in its own arithmetic (it no longer stores A' = A - dbar for this path: 41.6 MB per
+            // iteration at 52 x 200,000): a' - ubar = A - (ubar + dbar).  The pair role needs no correction at all -- a shift of
+            // a whole column cancels in a'_i - a'_j.
+            const float ubp = ub + (inside ? dbar[gc] : 0.f);
             // (2) p~ = a' - ubar split into TF32 hi + lo -> this thread's lane of tensor memory, 8 rows j per store
 #pragma unroll
             for (int ks = 0; ks < ST_K / 8; ++ks)
@@ -264,7 +269,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
 #pragma unroll
                     for (int q = 0; q < 8; ++q) pv[q] = lds32(uq[q] + ST_ARR * 4 + (ks * 8 + q) * 128);
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) split_tf32((inside && ks * 8 + q < n) ? pv[q] - ub : 0.f, hi[q], lo[q]);
+                    for (int q = 0; q < 8; ++q) split_tf32((inside && ks * 8 + q < n) ? pv[q] - ubp : 0.f, hi[q], lo[q]);
                     tmem_st8(tl + ST_K + ks * 8, hi);
                     tmem_st8(tl + 2 * ST_K + ks * 8, lo);
                 }
@@ -313,7 +318,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
 #pragma unroll
                     for (int q = 0; q < 16; ++q) {
                         const float u = u16[q];
-                        const float dlr = inv * fmaf(-fn, u - ub, fmaf(rs16[q], p16[q] - ub, -sa[q]));
+                        const float dlr = inv * fmaf(-fn, u - ub, fmaf(rs16[q], p16[q] - ubp, -sa[q]));
                         const float dl = (i0 + q < n && inside) ? dlr : 0.f;
                         const float a = u + dl;
                         u16[q] = a;
@@ -413,7 +418,7 @@ __global__ void __launch_bounds__(ST_THREADS, 1) kd_small_tc(int n, int ld, int 
                     const uint32_t bar = smem_u32(&full[b]), dst = smem_u32(As);
                     expect_tx(bar, 2u * tx_bytes);
                     small_issue_array(dst, &tmU, c0, bar);
-                    small_issue_array(dst + bufsz * 4, &tmP, c0, bar);
+                    small_issue_array(dst + bufsz * 4, &tmA, c0, bar);
                 }
             }
         }
@@ -499,7 +504,7 @@ int ccd_small_tc_setup(cc_handle* h) {
 int ccd_small_tc_maps(cc_handle* h) {
     static_assert(sizeof(CUtensorMap) == sizeof(h->dn_small_tm[0]), "tensor map storage");
     cc_encode_tiled_fn enc = small_tc_encoder();
-    const float* base[4] = {h->U, h->Ap, h->X, h->A};
+    const float* base[4] = {h->U, h->A, h->X, h->A};      // (slot 1 unused: the previous projection is read from A)
     for (int k = 0; k < 4; ++k) {
         CUtensorMap tm;
         if (enc == nullptr || !small_tc_map(enc, &tm, base[k], h->n, h->ld)) {
@@ -515,6 +520,6 @@ void ccd_small_tc_launch(cc_handle* h) {
     CUtensorMap tm[4];
     memcpy(tm, h->dn_small_tm, sizeof(tm));
     kd_small_tc<<<h->dn_small_grid, ST_THREADS, kSmallTcSmem, h->stream>>>(
-        (int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, tm[0], tm[1], tm[2], tm[3], h->mask, h->Wd, h->VNd, h->dbar, h->NB2d, h->sc,
+        (int)h->n, (int)h->ld, h->dn_small_cs, h->Sd, tm[0], tm[2], tm[3], h->mask, h->Wd, h->VNd, h->dbar, h->NB2d, h->sc,
         h->part + 3 * CC_MAXBLK * CC_NPART, h->hist_phi, h->hist_d, h->cond_outer);
 }

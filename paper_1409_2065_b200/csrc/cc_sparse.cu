@@ -717,7 +717,7 @@ __global__ void __launch_bounds__(CC_THREADS) k_update(int n, int ld, int nchunk
             st4(Z + oi, un + (dl + (dl - ld4s(Dl + oi))));
             st4(Dl + oi, dl);
         }
-        st4(Ap + oi, a);
+        if (Ap) st4(Ap + oi, a);       // (the n <= 64 dense path reads A and dbar instead)
     }
     const long long nthreads = (long long)gridDim.x * CC_THREADS;
     for (long long e = (long long)blockIdx.x * CC_THREADS + threadIdx.x; e < nnz; e += nthreads) {
@@ -885,12 +885,12 @@ void ccs_update(cc_handle* h) {
                   (const float*)nullptr, 0, (const float*)nullptr, (float*)nullptr, (float*)nullptr, (double*)nullptr);
 }
 
-void ccs_update_nodes(cc_handle* h, int with_edges) {
+void ccs_update_nodes(cc_handle* h, int with_edges, int store_ap) {
     // with_edges: the dense paths that store S add their block soft-threshold (the work of kd_edges) to this launch
     const float* nb = with_edges ? h->NB2d : nullptr;
     CC_DISPATCH_G(h, k_update, h->grid_rows, (int)h->n, (int)h->ld, h->nchunk, 0LL, h->X, h->mask, h->A, h->U,
-                  (float*)nullptr, h->Ap, (float*)nullptr, (const float*)h->dbar, (const float*)nullptr, (const float*)nullptr,
-                  (float*)nullptr, (float*)nullptr, h->sc, nb, h->dn_ksplit, (const float*)h->Wd, h->Sd, h->VNd,
+                  (float*)nullptr, store_ap ? h->Ap : (float*)nullptr, (float*)nullptr, (const float*)h->dbar, (const float*)nullptr,
+                  (const float*)nullptr, (float*)nullptr, (float*)nullptr, h->sc, nb, h->dn_ksplit, (const float*)h->Wd, h->Sd, h->VNd,
                   h->part + 6 * CC_MAXBLK * CC_NPART);
 }
 

@@ -69,6 +69,9 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-path", action="store_true", help="skip the full gamma-path wall time")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--continuation-study", default="",
+                    help="comma-separated stop tolerances (e.g. 1e-5,1e-6,1e-7): for each, the plain gamma path and the two staged "
+                         "kappa schedules are timed and their U compared with a path converged at tol 1e-9 (adds minutes)")
     ap.add_argument("--eager", action="store_true", help="plain stream launches instead of the CUDA graph (for ncu)")
     return ap.parse_args()
 
@@ -388,6 +391,41 @@ def run_ours(args):
                                 "wall_s": p0.elapsed_time(p1) / 1e3, "iters_total": int(sum(its_c)),
                                 "nclusters_first_mid_last": ks_c, "rel_dU_vs_plain_first_mid_last": dU}
         del Up, Uc
+        if args.continuation_study:
+            # distance to the converged path (S26 / section 6 table): the reference is the plain iteration at tol 1e-9
+            idx = sorted({ng // 4, ng // 2, (3 * ng) // 4, ng - 1})
+            B.cc_reset(h)
+            p0.record()
+            its_r, _ = B.cc_path(h, gam, 1e-9, 20000)
+            p1.record()
+            torch.cuda.synchronize()
+            ref_s = p0.elapsed_time(p1) / 1e3
+            Ur = [B.cc_get_U(h, g, torch.empty(n, wl.p, device=dev)) for g in idx]
+            Ut = torch.empty(n, wl.p, device=dev)
+
+            def errs():
+                out = []
+                for u, g in zip(Ur, idx):
+                    B.cc_get_U(h, g, Ut)
+                    out.append(float((Ut - u).norm() / u.norm().clamp_min(1e-30)))
+                return out
+            rows = []
+            for tol_s in args.continuation_study.split(","):
+                tol = float(tol_s)
+                row = {"tol": tol}
+                for name, run in (("plain", lambda: B.cc_path(h, gam, tol, 20000)),
+                                  ("staged_0.1_0.01", lambda: B.cc_path_continuation(h, gam, 0.1, 0.1, 200, tol, 20000)),
+                                  ("staged_1_0.1_0.01", lambda: B.cc_path_continuation(h, gam, 1.0, 0.1, 200, tol, 20000))):
+                    B.cc_reset(h)
+                    p0.record()
+                    its_x, _ = run()
+                    p1.record()
+                    torch.cuda.synchronize()
+                    row[name] = {"wall_s": p0.elapsed_time(p1) / 1e3, "iters_total": int(sum(its_x)), "rel_err_vs_converged": errs()}
+                rows.append(row)
+            path["continuation_study"] = {"gamma_indices": idx, "reference": {"tol": 1e-9, "maxit": 20000, "wall_s": ref_s,
+                                                                              "iters_total": int(sum(its_r))}, "rows": rows}
+            del Ur, Ut
     B.cc_destroy(h)
 
     # ---- e2e: host buffers -> cc_create -> cc_solve -> U back on the host, every step

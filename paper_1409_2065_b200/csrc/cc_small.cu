@@ -4,7 +4,9 @@
 // Complete graph, closed-form projection (PAPER.md L90-L103 with L = nI - 11', pin P3):
 //     a_i = u_i + [ rowsum(S)_i p~_i - sum_j s_ij p~_j - n (u_i - ubar) ] / (n+1),   p~ = a' - ubar,
 // then ||b_ij||^2 and ||s_ij b'_ij - b_ij||^2 for all pairs by direct differences (the fused / not-fused decision is taken on
-// ||b||, far below ||a|| for a pair about to fuse: no Gram trick).  U, A' and X are read once, A is written once.
+// ||b||, far below ||a|| for a pair about to fuse: no Gram trick).  U, the previous projection and X are read once, A is
+// written once.  The previous projection a' arrives as the array A of one iteration ago plus its residual column mean dbar
+// (a' = A - dbar: k_update removes dbar in its own arithmetic and stores no A' for this path).
 //
 // One 512-thread CTA per SM walks chunks of 128 columns; two roles work on different chunks at the same time:
 //   projection role, warps 0-3: thread = one column c of the chunk, so the column mean of U, the mean of A - U (the exact
@@ -13,17 +15,19 @@
 //     the 3xTF32 split (hi.hi + hi.lo + lo.hi).  Both the accumulator and the chunk operand live in TENSOR MEMORY, whose
 //     lane is the thread's column: the thread writes its own p~ (hi and lo) with tcgen05.st and reads its own results with
 //     tcgen05.ld -- no transposition, no shared-memory operand.  S (N x K, K-major, SWIZZLE_128B) is staged once per launch.
-//   pair role, warps 4-15: 4 x 4 register tiles of pairs on or above the diagonal, interleaved column quads.
-// Data movement is the copy engine's: a chunk of U, A' or X is four TMA tensor copies (32 columns x n rows each,
+//   pair role, warps 4-15: register tiles of 4 x 2 pairs on or above the diagonal blocks, interleaved column quads, packed
+//     fp32 arithmetic (FADD2 / FFMA2).
+// Data movement is the copy engine's: a chunk of U, A or X is four TMA tensor copies (32 columns x n rows each,
 // cp.async.bulk.tensor.2d, SWIZZLE_128B) completing on an mbarrier, and A leaves by four tensor stores -- 16 instructions
 // per chunk, issued by one lane.  A shared-memory array is [4 column groups][64 rows][128 bytes] with the 16-byte pieces of
 // row r at position piece ^ (r % 8): the projection role's column walks and the pair role's 16-byte reads of eight rows at
 // once are both conflict-free.  Columns beyond the matrix arrive as zeros (TMA's out-of-bounds fill) and are clipped on the
-// way out.  Chunks alternate between two {U -> A, A'} buffers: a pair warp refills a buffer as soon as its role has left it.
+// way out.  Chunks alternate between two {U -> A, A (previous)} buffers: a pair warp refills a buffer as soon as its role
+// has left it.
 // (History, 52 x 200,000: FFMA kernel kd_small_ws 182 us; tensor-core contraction with thread-issued loads 194-250 us --
 // the 26 cp.async + 13 LDG.128 per thread took 7 us per chunk to ISSUE next to twelve warps of LDS.128 traffic; one
 // cp.async.bulk per 512-byte row segment: 180 us, every bulk copy costs ~25 ns of its issuing warp, 208 of them per chunk.)
-// Per-(CTA, column phase) partial ||b||^2 go to NB2 slices; kd_edges adds them in order.
+// Per-(CTA, column phase) partial ||b||^2 go to NB2 slices; the edge section of k_update adds them in order.
 #include <cstdio>
 #include <cstring>
 

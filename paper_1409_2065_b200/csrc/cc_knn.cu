@@ -119,6 +119,10 @@ __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int kk, const fl
     __shared__ int qrow[TQ];
 
     const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    // The fp32 shortlist pass without a mask: packed arithmetic, and the two staged tiles TRANSPOSED ([column][row], row
+    // stride TQ + 4) with four CONSECUTIVE candidate rows per thread, so that a column costs two 16-byte shared loads
+    // instead of eight scalar ones (same footprint: PC x (TQ + 4) = TQ x (PC + 1) floats).
+    constexpr bool PACKED = sizeof(T) == 4 && !MASKED;
     const int q0 = blockIdx.x * TQ;
     const T big = knn_big<T>();
     for (int t = tid; t < TQ * kk; t += 256) { Ld[t] = big; Li[t] = -1; }
@@ -132,7 +136,6 @@ __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int kk, const fl
         for (int a = 0; a < 4; ++a)
 #pragma unroll
             for (int b = 0; b < 4; ++b) { acc[a][b] = (T)0; cnt[a][b] = 0.f; }
-        constexpr bool PACKED = sizeof(T) == 4 && !MASKED;          // the fp32 shortlist pass without a mask
         knn_f2 accp[4][2] = {{0ull, 0ull}, {0ull, 0ull}, {0ull, 0ull}, {0ull, 0ull}};
         for (int pc = 0; pc < p; pc += PC) {
             // stage PC columns of the query tile and of the candidate tile; values at missing entries are never read
@@ -146,13 +149,24 @@ __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int kk, const fl
                     Mq[r * (PC + 1) + c] = vi ? 1.f : 0.f;
                     Mc[r * (PC + 1) + c] = vj ? 1.f : 0.f;
                 }
-                Xq[r * (PC + 1) + c] = vi ? X[(size_t)gi * p + gc] : 0.f;
-                Xc[r * (PC + 1) + c] = vj ? X[(size_t)gj * p + gc] : 0.f;
+                if constexpr (PACKED) {
+                    Xq[c * (TQ + 4) + r] = vi ? X[(size_t)gi * p + gc] : 0.f;
+                    Xc[c * (TC + 4) + r] = vj ? X[(size_t)gj * p + gc] : 0.f;
+                } else {
+                    Xq[r * (PC + 1) + c] = vi ? X[(size_t)gi * p + gc] : 0.f;
+                    Xc[r * (PC + 1) + c] = vj ? X[(size_t)gj * p + gc] : 0.f;
+                }
             }
             __syncthreads();
 #pragma unroll
             for (int c = 0; c < PC; ++c) {
                 float xq[4], xc[4], mq[4], mc[4];
+                if constexpr (PACKED) {
+                    const float4 q4 = *reinterpret_cast<const float4*>(Xq + c * (TQ + 4) + ty * 4);
+                    const float4 c4 = *reinterpret_cast<const float4*>(Xc + c * (TC + 4) + tx * 4);
+                    xq[0] = q4.x; xq[1] = q4.y; xq[2] = q4.z; xq[3] = q4.w;
+                    xc[0] = c4.x; xc[1] = c4.y; xc[2] = c4.z; xc[3] = c4.w;
+                } else
 #pragma unroll
                 for (int a = 0; a < 4; ++a) {
                     xq[a] = Xq[(ty * 4 + a) * (PC + 1) + c];
@@ -218,10 +232,10 @@ __global__ void __launch_bounds__(256) k_knn_tile(int n, int p, int kk, const fl
                     else d = cnt[a][b] > 0.f ? d * (float)p / cnt[a][b] : big;
                 }
                 if (SIDE) {
-                    const int gi = qrow[ty * 4 + a], gj = c0 + tx + 16 * b;
+                    const int gi = qrow[ty * 4 + a], gj = c0 + (PACKED ? tx * 4 + b : tx + 16 * b);
                     if (gi >= 0 && gj < n && d < big) d = sd.alpha * sqrtf((float)d) + (1.f - sd.alpha) * side_dist(sd, gi, gj);
                 }
-                Dt[(ty * 4 + a) * (TC + 1) + tx + 16 * b] = d;
+                Dt[(ty * 4 + a) * (TC + 1) + (PACKED ? tx * 4 + b : tx + 16 * b)] = d;
             }
         __syncthreads();
         // selection: warp wq handles queries wq*8 .. wq*8+7; lanes look at candidates lane, lane+32
